@@ -1,0 +1,140 @@
+/*
+ * hpmc_oracle.h -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, serial, slow, obviously-correct CPU restatement of the checkerboard
+ * Metropolis sweep for hard shapes (arXiv:1509.04692, "HPMC"), written from the
+ * paper text (/root/reference/PAPER.md, cited below as P:<line>) and from the
+ * readings R1..R30 collected in DESIGN.md.
+ *
+ * Rules this file lives under:
+ *   - only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ *     --impl reference legs may load it;
+ *   - it shares no code, header, table or constant generator with the CUDA path
+ *     under paper_1509_04692_b200/csrc/ and neither includes the other;
+ *   - every overlap test is fp64; fp32 appears only where DESIGN.md pins a
+ *     bit-exact fp32 operation (cell_of, the translation fmaf, the wrap, the
+ *     grid shift) so that those integers/positions can be compared bit for bit;
+ *   - no blocking, fusion or reordering beyond what the algorithm states.
+ *
+ * Pins (tests/test_oracle_*.py, all `-m "not gpu"`): Philox known answers,
+ * closed-form contact distances, Sutherland-Hodgman clipping and Chebyshev-LP
+ * brute force for the SAT margins, GJK vs SAT sign, O(N^2) overlap counts, the
+ * all-N twin (O6), the zero-overlap invariant, dilute-limit acceptance closed
+ * form, colour independence (P4).  Acceptance/pressure VALUES for the
+ * pentagon and cube state points are "parity unpinned" against the paper (it
+ * prints none); see DESIGN.md.
+ */
+#ifndef HPMC_ORACLE_H
+#define HPMC_ORACLE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ORC_MAX_VERTS 32
+#define ORC_MAX_FACES 64
+#define ORC_MAX_EDGES 96
+
+#define ORC_KIND_DISK 0       /* disk (dim 2) or sphere (dim 3), "trivial" */
+#define ORC_KIND_POLYGON 1    /* convex polygon, CCW body-frame vertices */
+#define ORC_KIND_POLYHEDRON 2 /* convex polyhedron given by its vertices */
+
+typedef struct orc_shape orc_shape;
+typedef struct orc_sys orc_sys;
+
+typedef struct {
+    uint64_t trans_acc, trans_rej_overlap, trans_rej_cell;
+    uint64_t rot_acc, rot_rej_overlap;
+    uint64_t trials, sweeps;
+} orc_counters;
+
+/* O7 instrumentation, "early-exit serial order": candidates in
+ * ascending neighbour-cell order (dz, dy, dx loops) then ascending tag. */
+typedef struct {
+    uint64_t cand_scanned_full;  /* all candidates in the 3^d block, no early exit */
+    uint64_t sphere_pass_full;   /* of those, inside the circumsphere range          */
+    uint64_t cand_scanned_early; /* scanned until the first overlapping neighbour    */
+    uint64_t narrow_tests_early; /* narrow-phase tests until the first overlap       */
+} orc_work;
+
+typedef struct {
+    uint64_t compared;       /* trial slots compared                                 */
+    uint64_t marginal;       /* outcome differed, |m_min - eps_g| < tol: GPU adopted */
+    uint64_t hard_mismatch;  /* particle/type/leave-cell/non-marginal disagreement   */
+    int64_t first_bad_slot;  /* slot of the first hard mismatch, -1 if none          */
+    uint32_t first_bad_mine[2], first_bad_theirs[2];
+    double first_bad_mmin;
+} orc_follow_stats;
+
+/* ---- RNG (R3, R4) ------------------------------------------------------- */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+float orc_u01(uint32_t r);  /* (r>>8) * 2^-24 in [0,1)              */
+float orc_usym(uint32_t r); /* ((int)(r>>8) - 2^23) * 2^-23 in [-1,1) */
+
+/* ---- shapes and margins (O4) ------------------------------------------- */
+orc_shape* orc_shape_create(int dim, int kind, double diameter, int nverts, const double* verts);
+void orc_shape_destroy(orc_shape*);
+double orc_shape_dmax(const orc_shape*);
+int orc_shape_nfaces(const orc_shape*);
+int orc_shape_nedgedirs(const orc_shape*);
+void orc_shape_faces(const orc_shape*, double* normals3, double* offsets);
+/* margin m(A,B): r_ab = r_B - r_A (already minimum image), q = (w,x,y,z). */
+double orc_shape_margin(const orc_shape*, const double r_ab[3], const double qa[4], const double qb[4]);
+/* fp64 GJK boolean: 1 origin in interior of B (-) A, 0 disjoint, -1 undecided */
+int orc_shape_gjk(const orc_shape*, const double r_ab[3], const double qa[4], const double qb[4]);
+
+/* ---- system -------------------------------------------------------------- */
+orc_sys* orc_create(int dim, const double L[3], int kind, double diameter, int nverts,
+                    const double* verts, int64_t N, uint64_t seed);
+void orc_destroy(orc_sys*);
+const orc_shape* orc_sys_shape(const orc_sys*);
+int orc_set_moves(orc_sys*, double d, double a, int n_select);
+void orc_set_eps_guard(orc_sys*, double eps_g);
+void orc_set_state(orc_sys*, const float* pos4, const float* quat4);
+void orc_get_state(const orc_sys*, float* pos4, float* quat4);
+void orc_set_sweep_counter(orc_sys*, uint64_t t);
+uint64_t orc_get_sweep_counter(const orc_sys*);
+void orc_get_counters(const orc_sys*, orc_counters*);
+void orc_get_work(const orc_sys*, orc_work*);
+void orc_reset_counters(orc_sys*);
+/* n[3], w[3] (double), w_f[3], inv_w[3] (fp32 as used by cell_of), L_f[3] */
+void orc_get_grid(const orc_sys*, int32_t n[3], double w[3], float w_f[3], float inv_w[3], float L_f[3]);
+int64_t orc_num_cells(const orc_sys*);
+
+/* O3.1 / O3.2: grid shift and colour order of sweep t */
+void orc_sweep_header(const orc_sys*, uint64_t t, float shift[3], int32_t perm[8]);
+/* R13: pinned fp32 cell function, returns the linear cell id */
+int32_t orc_cell_of(const orc_sys*, const float x[3], const float shift[3]);
+/* O3.3: cell ids, CSR offsets (C+1), members ascending by tag (R8) */
+void orc_cell_list(const orc_sys*, const float shift[3], int32_t* cell_id, int32_t* cell_start,
+                   int32_t* members);
+
+/* One sweep (O3).  neighbour_mode 0 = 3^d cells, 1 = all N-1 particles (O6 twin).
+ * reverse_cells != 0 visits same-colour cells in descending id (P4 check).
+ * follow: GPU trace to lock-step against (O8) or NULL.  trace_out: 2 words per
+ * slot (cell*n_select+k) or NULL.  mmin_out: per-slot m_min (NaN if none) or NULL. */
+int orc_sweep(orc_sys*, int neighbour_mode, int reverse_cells, const uint32_t* follow, double follow_tol,
+              uint32_t* trace_out, double* mmin_out, orc_follow_stats* fs);
+int orc_sweeps(orc_sys*, int64_t n);
+
+/* mutation switches for O11-style checks (default all 0 = the real scheme) */
+void orc_set_mutations(orc_sys*, int no_shift, int fixed_colour_order, int no_leave_cell_reject);
+
+/* O11: textbook Metropolis, n_trials single-particle trials, own RNG tag */
+int orc_textbook_trials(orc_sys*, int64_t n_trials);
+
+/* O5: all N(N-1)/2 pairs, strict m < 0 */
+int64_t orc_count_overlaps_bruteforce(const orc_sys*);
+/* same count through the cell list (shift 0) */
+int64_t orc_count_overlaps_cells(const orc_sys*);
+/* smallest pair margin in the system through the cell list (diagnostic) */
+double orc_min_margin_cells(const orc_sys*);
+/* P4: min centre distance between particles of distinct same-colour cells */
+double orc_min_same_colour_distance(const orc_sys*, const float shift[3]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
