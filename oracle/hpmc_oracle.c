@@ -612,7 +612,9 @@ static double scan_candidates(orc_sys* s, int neighbour_mode, int64_t i, const f
     double qa[4], m_min = INFINITY;
     quat_to_double(qt, qa);
     int found = 0;
-    double dmax2 = sh->dmax * sh->dmax;
+    /* R16': the broad-phase range carries the guard band, so that "reject iff m < eps_g" (R15) also holds for
+     * pairs at centre distance d_max (touching disks; polygon vertices pointing at each other) */
+    double dmax2 = (sh->dmax + s->eps_g) * (sh->dmax + s->eps_g);
     if (neighbour_mode == 1) { /* O6 twin: all N-1 particles */
         for (int64_t j = 0; j < s->N; ++j) {
             if (j == i) continue;
