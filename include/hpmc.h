@@ -1,0 +1,141 @@
+/*
+ * hpmc.h -- C-ABI of libhpmc.so: the checkerboard-parallel Metropolis sweep for hard shapes
+ * (arXiv:1509.04692, "HPMC") as hand-written CUDA for sm_100a.
+ *
+ * Citations: P:<n> = line n of the paper text; R<k> = reading k in DESIGN.md section 2.
+ *
+ * Conventions
+ *   - every function returns 0 on success and a negative HPMC_E_* code on failure; the state is
+ *     untouched by a failed call; hpmc_last_error() gives a human-readable reason.  A CUDA error is
+ *     sticky: later calls on the same context report HPMC_E_CUDA too.
+ *   - "d_" pointers are DEVICE pointers, "h_" pointers are HOST pointers.  The library allocates no
+ *     particle-sized device memory: the caller (PyTorch in this repo) owns the state buffers and the
+ *     workspace and must keep them alive while they are bound.  The library never frees them.
+ *   - all work is enqueued on the CUDA stream given to hpmc_create (a cudaStream_t passed as void*;
+ *     NULL = the legacy default stream).  Calls are asynchronous unless stated otherwise.
+ *   - layout: pos4 = N x (x, y, z, 0) fp32, quat4 = N x (w, x, y, z) fp32 unit quaternions, both in
+ *     TAG order (particle i at row i).  2-D systems keep z = 0 and quat = (cos t/2, 0, 0, sin t/2) (R30).
+ *   - box: orthorhombic, periodic, centred on the origin, coordinates in [-L/2, L/2) (R14).  The box
+ *     edge is L rounded to fp32 (R-box).
+ *   - there is no CPU implementation behind this interface.
+ */
+#ifndef HPMC_H
+#define HPMC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define HPMC_MAX_VERTS 32
+
+#define HPMC_KIND_DISK 0       /* disk (dim 2) / sphere (dim 3): centre distance vs diameter   */
+#define HPMC_KIND_POLYGON 1    /* convex polygon, body-frame vertices counter-clockwise: SAT */
+#define HPMC_KIND_POLYHEDRON 2 /* convex polyhedron given by its vertices: GJK on the Minkowski
+                                  difference with the support function of Eq. (1)-(2)   */
+
+#define HPMC_OK 0
+#define HPMC_E_ARG (-1)       /* bad argument (dim, N, d, a, n_select, NULL pointer, ...)          */
+#define HPMC_E_SHAPE (-2)     /* non-convex / not CCW / too many vertices / vertex not on the hull */
+#define HPMC_E_GRID (-3)      /* fewer than 4 cells per side (R11) or more than 2^31-2 cells       */
+#define HPMC_E_UNBOUND (-4)   /* state/workspace not bound, or workspace too small                 */
+#define HPMC_E_CUDA (-5)      /* a CUDA call failed (sticky)                                       */
+#define HPMC_E_TRACE (-6)     /* trace buffer too small for C * n_select slots                     */
+
+typedef struct hpmc_ctx hpmc_ctx; /* opaque, owned by the library, freed by hpmc_destroy */
+
+typedef struct {
+    int dim;     /* 2 or 3 */
+    double L[3]; /* box edges; L[2] ignored when dim == 2 */
+} hpmc_box;
+
+typedef struct {
+    int kind;            /* HPMC_KIND_* */
+    double diameter;     /* kind 0 */
+    int nverts;          /* kind 1: 3..32 vertices (x,y); kind 2: 4..32 vertices (x,y,z) */
+    const double* verts; /* h_: nverts*2 or nverts*3 doubles, body frame; read during the call only */
+} hpmc_shape;
+
+/* P:47 "percentage of the trial moves are accepted": accepted / attempted per type (R26) */
+typedef struct {
+    uint64_t trans_acc, trans_rej_overlap, trans_rej_cell;
+    uint64_t rot_acc, rot_rej_overlap;
+    uint64_t trials, sweeps;
+} hpmc_counters;
+
+typedef struct {
+    int dim;
+    int n[3];        /* cells per side: n_k = 2*floor(L_k / (2 d_max (1 + 2^-10))) (R11)            */
+    double w[3];     /* cell width L_k / n_k                                                        */
+    float L_f[3];    /* box edge as used by the fp32 state                                          */
+    float inv_w[3];  /* (float)(n_k / L_k), the factor inside cell_of (R13)                         */
+    double d_max;    /* circumsphere diameter                                                 */
+    int64_t num_cells;
+    int64_t N;
+} hpmc_grid_info;
+
+/* NVT problem statement of P:38-45: N identical hard particles of one shape in a periodic box.
+ * Validates the shape (convexity, CCW) and the grid (>= 4 cells per side).  Does NOT check that the
+ * initial state is overlap-free -- call hpmc_count_overlaps (mirrors P:247).                       */
+int hpmc_create(const hpmc_box* box, const hpmc_shape* shape, int64_t N, uint64_t seed,
+                void* cuda_stream, hpmc_ctx** out);
+int hpmc_destroy(hpmc_ctx* ctx);
+const char* hpmc_last_error(const hpmc_ctx* ctx); /* valid until the next call on ctx; ctx may be NULL */
+int hpmc_get_grid(const hpmc_ctx* ctx, hpmc_grid_info* h_out);
+
+/* Bytes of scratch the CALLER must allocate (256-byte aligned) and pass to hpmc_bind.             */
+size_t hpmc_workspace_bytes(const hpmc_ctx* ctx);
+
+/* Bind the state (tag order, see layout above) and the workspace.  d_pos4/d_quat4 are read by the
+ * next hpmc_sweep / hpmc_count_overlaps (the library then works on its own cell-sorted copy inside
+ * the workspace) and are used as device staging by hpmc_sweep_host.  Re-binding restarts from the
+ * bound arrays; counters and the sweep counter are kept.                                           */
+int hpmc_bind(hpmc_ctx* ctx, float* d_pos4, float* d_quat4, void* d_workspace, size_t workspace_bytes);
+
+/* Trial move sizes: translation uniform in the cube [-d,d)^dim (R5), rotation angle uniform in
+ * [-a,a) rad (R6), n_select trials per non-empty cell per colour (R9).  d > 0, a >= 0,
+ * 1 <= n_select <= 65535.  Defaults: d = 0.1, a = 0.1, n_select = 4.                               */
+int hpmc_set_moves(hpmc_ctx* ctx, double d, double a, int n_select);
+
+/* n checkerboard sweeps (P:155-157 restated per north_star): per sweep a fresh grid shift, the
+ * colours in a fresh random order, n_select trials in every non-empty cell of each colour.
+ * Asynchronous; advances the sweep counter by n.                                                  */
+int hpmc_sweep(hpmc_ctx* ctx, int64_t n);
+
+/* Number of particle pairs whose interiors intersect (strict margin < 0, fp64 narrow phase),
+ * P:247.  Synchronises the stream.                                                                */
+int hpmc_count_overlaps(hpmc_ctx* ctx, int64_t* h_count);
+
+/* Current state back in tag order into caller buffers (may be the bound ones), counters and sweep
+ * counter to host.  Any of the out pointers may be NULL.  Synchronises iff a host pointer is given. */
+int hpmc_get_state(hpmc_ctx* ctx, float* d_pos4_out, float* d_quat4_out, hpmc_counters* h_counters,
+                   int64_t* h_sweep_counter);
+int hpmc_set_sweep_counter(hpmc_ctx* ctx, uint64_t t);
+int hpmc_reset_counters(hpmc_ctx* ctx);
+
+/* Parity/debug trace (O8): while set, every sweep writes two uint32 words per trial slot
+ * (slot = cell*n_select + k): word0 = particle tag, word1 = type (0 translate, 1 rotate) |
+ * outcome<<8 with outcome 0 none (empty cell), 1 accepted, 2 rejected: left its cell,
+ * 3 rejected: overlap.  The buffer is overwritten each sweep.  NULL disables.                      */
+int hpmc_set_trace(hpmc_ctx* ctx, uint32_t* d_trace, int64_t capacity_words);
+
+/* Parity/debug: build the cell list of sweep t (its grid shift) from the current state, without
+ * making moves, and copy it out: CSR offsets (num_cells+1), member tags in stored order (N; ascending
+ * inside each cell, R8) and the cell id of every particle in tag order (N).  Any pointer may be NULL. */
+int hpmc_get_cell_list(hpmc_ctx* ctx, uint64_t t, int32_t* d_cell_start, int32_t* d_member_tags,
+                       int32_t* d_cell_of_tag, float* h_shift3, int32_t* h_colour_perm8);
+
+/* End-to-end convenience with HOST buffers (pinned or pageable): copies the state host->device into
+ * the bound arrays, runs n sweeps, copies the state and counters back.  Synchronises.              */
+int hpmc_sweep_host(hpmc_ctx* ctx, const float* h_pos4, const float* h_quat4, int64_t n,
+                    float* h_pos4_out, float* h_quat4_out, hpmc_counters* h_counters);
+
+/* Launch bookkeeping for bench.py: kernels launched by this context so far.                        */
+int64_t hpmc_launch_count(const hpmc_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,222 @@
+"""Thin ctypes binding over libhpmc.so (C-ABI: include/hpmc.h).  Argument marshalling only.
+
+PyTorch is used for device memory and the CUDA stream; every step of the sweep runs in the library's
+CUDA kernels.  There is NO fallback: if libhpmc.so is missing or a call fails, this module raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libhpmc.so")
+
+KIND_DISK, KIND_POLYGON, KIND_POLYHEDRON = 0, 1, 2
+
+# every symbol include/hpmc.h declares (checked by tests/test_abi.py)
+ABI_SYMBOLS = ["hpmc_create", "hpmc_destroy", "hpmc_last_error", "hpmc_get_grid", "hpmc_workspace_bytes", "hpmc_bind",
+               "hpmc_set_moves", "hpmc_sweep", "hpmc_count_overlaps", "hpmc_get_state", "hpmc_set_sweep_counter",
+               "hpmc_reset_counters", "hpmc_set_trace", "hpmc_get_cell_list", "hpmc_sweep_host", "hpmc_launch_count"]
+
+
+class HpmcError(RuntimeError):
+    pass
+
+
+class Box(C.Structure):
+    _fields_ = [("dim", C.c_int), ("L", C.c_double * 3)]
+
+
+class ShapeDesc(C.Structure):
+    _fields_ = [("kind", C.c_int), ("diameter", C.c_double), ("nverts", C.c_int), ("verts", C.POINTER(C.c_double))]
+
+
+class Counters(C.Structure):
+    _fields_ = [(n, C.c_uint64) for n in
+                ("trans_acc", "trans_rej_overlap", "trans_rej_cell", "rot_acc", "rot_rej_overlap", "trials", "sweeps")]
+
+    def as_dict(self):
+        return {n: int(getattr(self, n)) for n, _ in self._fields_}
+
+
+class GridInfo(C.Structure):
+    _fields_ = [("dim", C.c_int), ("n", C.c_int * 3), ("w", C.c_double * 3), ("L_f", C.c_float * 3),
+                ("inv_w", C.c_float * 3), ("d_max", C.c_double), ("num_cells", C.c_int64), ("N", C.c_int64)]
+
+
+_lib = None
+
+
+def load_library():
+    """Load libhpmc.so; raises HpmcError if it has not been built (no CPU fallback exists)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise HpmcError(f"{LIB_PATH} is missing: build it with `python -m paper_1509_04692_b200.build` "
+                        "(there is no CPU fallback for the sweep)")
+    L = C.CDLL(LIB_PATH)
+    vp = C.c_void_p
+    L.hpmc_create.argtypes = [C.POINTER(Box), C.POINTER(ShapeDesc), C.c_int64, C.c_uint64, vp, C.POINTER(vp)]
+    L.hpmc_destroy.argtypes = [vp]
+    L.hpmc_last_error.argtypes = [vp]; L.hpmc_last_error.restype = C.c_char_p
+    L.hpmc_get_grid.argtypes = [vp, C.POINTER(GridInfo)]
+    L.hpmc_workspace_bytes.argtypes = [vp]; L.hpmc_workspace_bytes.restype = C.c_size_t
+    L.hpmc_bind.argtypes = [vp, vp, vp, vp, C.c_size_t]
+    L.hpmc_set_moves.argtypes = [vp, C.c_double, C.c_double, C.c_int]
+    L.hpmc_sweep.argtypes = [vp, C.c_int64]
+    L.hpmc_count_overlaps.argtypes = [vp, C.POINTER(C.c_int64)]
+    L.hpmc_get_state.argtypes = [vp, vp, vp, C.POINTER(Counters), C.POINTER(C.c_int64)]
+    L.hpmc_set_sweep_counter.argtypes = [vp, C.c_uint64]
+    L.hpmc_reset_counters.argtypes = [vp]
+    L.hpmc_set_trace.argtypes = [vp, vp, C.c_int64]
+    L.hpmc_get_cell_list.argtypes = [vp, C.c_uint64, vp, vp, vp, C.POINTER(C.c_float), C.POINTER(C.c_int32)]
+    L.hpmc_sweep_host.argtypes = [vp, vp, vp, C.c_int64, vp, vp, C.POINTER(Counters)]
+    L.hpmc_launch_count.argtypes = [vp]; L.hpmc_launch_count.restype = C.c_int64
+    for name in ABI_SYMBOLS:
+        if name not in ("hpmc_last_error", "hpmc_workspace_bytes", "hpmc_launch_count"):
+            getattr(L, name).restype = C.c_int
+    _lib = L
+    return L
+
+
+class Hpmc:
+    """One NVT hard-particle system on one GPU.  Mirrors the C-ABI names one to one."""
+
+    def __init__(self, dim, L, kind, N, seed, diameter=0.0, verts=None, device="cuda:0", stream=None):
+        import torch  # device memory + streams only
+        self._torch = torch
+        self._lib = load_library()
+        if not torch.cuda.is_available():
+            raise HpmcError("no CUDA device: the sweep has no CPU implementation")
+        self.device = torch.device(device)
+        self.dim, self.N, self.kind = int(dim), int(N), int(kind)
+        box = Box(); box.dim = self.dim
+        for k in range(3):
+            box.L[k] = float(L[k]) if k < self.dim else 1.0
+        sd = ShapeDesc(); sd.kind = self.kind; sd.diameter = float(diameter)
+        self._verts = None
+        if verts is not None:
+            self._verts = np.ascontiguousarray(verts, dtype=np.float64)
+            sd.nverts = int(self._verts.shape[0])
+            sd.verts = self._verts.ctypes.data_as(C.POINTER(C.c_double))
+        with torch.cuda.device(self.device):
+            self.stream = stream if stream is not None else torch.cuda.current_stream()
+            h = C.c_void_p()
+            rc = self._lib.hpmc_create(C.byref(box), C.byref(sd), self.N, int(seed), C.c_void_p(self.stream.cuda_stream), C.byref(h))
+        if rc != 0:
+            raise HpmcError(f"hpmc_create failed ({rc}): {self._lib.hpmc_last_error(None).decode()}")
+        self._h = h
+        gi = GridInfo(); self._check(self._lib.hpmc_get_grid(self._h, C.byref(gi)))
+        self.n = np.array(list(gi.n), dtype=np.int32)
+        self.w = np.array(list(gi.w)); self.L_f = np.array(list(gi.L_f), dtype=np.float32)
+        self.inv_w = np.array(list(gi.inv_w), dtype=np.float32)
+        self.d_max, self.C = float(gi.d_max), int(gi.num_cells)
+        self.n_select = 4
+        self.pos4 = self.quat4 = self.workspace = self._trace = None
+
+    # -- helpers ---------------------------------------------------------------------------------
+    def _check(self, rc):
+        if rc != 0:
+            raise HpmcError(f"libhpmc error {rc}: {self._lib.hpmc_last_error(self._h).decode()}")
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            self._lib.hpmc_destroy(self._h)
+            self._h = None
+
+    # -- C-ABI mirror ----------------------------------------------------------------------------
+    def workspace_bytes(self):
+        return int(self._lib.hpmc_workspace_bytes(self._h))
+
+    def bind(self, pos4, quat4):
+        """pos4/quat4: (N,4) float32, numpy (copied to the device) or CUDA torch tensors (used in place)."""
+        torch = self._torch
+        def dev(a):
+            if isinstance(a, np.ndarray):
+                a = torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to(self.device)
+            assert a.is_cuda and a.dtype == torch.float32 and a.is_contiguous() and tuple(a.shape) == (self.N, 4)
+            return a
+        self.pos4, self.quat4 = dev(pos4), dev(quat4)
+        if self.workspace is None:
+            self.workspace = torch.empty(self.workspace_bytes() + 256, dtype=torch.uint8, device=self.device)
+        base = self.workspace.data_ptr()
+        off = (-base) % 256
+        self.stream.synchronize()
+        self._check(self._lib.hpmc_bind(self._h, self.pos4.data_ptr(), self.quat4.data_ptr(), base + off, self.workspace.numel() - off))
+
+    def set_moves(self, d, a, n_select):
+        self._check(self._lib.hpmc_set_moves(self._h, float(d), float(a), int(n_select)))
+        self.n_select = int(n_select)
+
+    def sweep(self, n=1):
+        self._check(self._lib.hpmc_sweep(self._h, int(n)))
+
+    def count_overlaps(self):
+        out = C.c_int64(-1)
+        self._check(self._lib.hpmc_count_overlaps(self._h, C.byref(out)))
+        return int(out.value)
+
+    def get_state(self, to_host=True):
+        """Un-sort into the bound arrays; returns (pos4, quat4) as numpy (to_host) or the CUDA tensors."""
+        self._check(self._lib.hpmc_get_state(self._h, self.pos4.data_ptr(), self.quat4.data_ptr(), None, None))
+        if to_host:
+            self.stream.synchronize()
+            return self.pos4.cpu().numpy(), self.quat4.cpu().numpy()
+        return self.pos4, self.quat4
+
+    def counters(self):
+        c = Counters(); t = C.c_int64()
+        self._check(self._lib.hpmc_get_state(self._h, None, None, C.byref(c), C.byref(t)))
+        d = c.as_dict(); d["sweep_counter"] = int(t.value)
+        return d
+
+    def set_sweep_counter(self, t):
+        self._check(self._lib.hpmc_set_sweep_counter(self._h, int(t)))
+
+    def reset_counters(self):
+        self._check(self._lib.hpmc_reset_counters(self._h))
+
+    def enable_trace(self, on=True):
+        torch = self._torch
+        if on:
+            words = 2 * self.C * self.n_select
+            self._trace = torch.zeros(words, dtype=torch.int32, device=self.device)
+            self._check(self._lib.hpmc_set_trace(self._h, self._trace.data_ptr(), words))
+        else:
+            self._trace = None
+            self._check(self._lib.hpmc_set_trace(self._h, None, 0))
+
+    def read_trace(self):
+        self.stream.synchronize()
+        return self._trace.cpu().numpy().view(np.uint32).reshape(-1, 2)
+
+    def cell_list(self, t):
+        """Cell list of sweep t's grid shift for the current state: (cell_of_tag, cell_start, member_tags, shift, perm)."""
+        torch = self._torch
+        cst = torch.empty(self.C + 1, dtype=torch.int32, device=self.device)
+        mem = torch.empty(max(self.N, 1), dtype=torch.int32, device=self.device)
+        cid = torch.empty(max(self.N, 1), dtype=torch.int32, device=self.device)
+        shift = (C.c_float * 3)(); perm = (C.c_int32 * 8)()
+        self._check(self._lib.hpmc_get_cell_list(self._h, int(t), cst.data_ptr(), mem.data_ptr(), cid.data_ptr(), shift, perm))
+        self.stream.synchronize()
+        return (cid.cpu().numpy()[: self.N], cst.cpu().numpy(), mem.cpu().numpy()[: self.N],
+                np.array(list(shift), dtype=np.float32), np.array(list(perm), dtype=np.int32)[: 1 << self.dim])
+
+    def sweep_host(self, h_pos4, h_quat4, n, h_pos4_out, h_quat4_out):
+        """End-to-end call with HOST buffers (torch CPU tensors, ideally pinned): H2D, n sweeps, D2H."""
+        c = Counters()
+        self._check(self._lib.hpmc_sweep_host(self._h, h_pos4.data_ptr(), h_quat4.data_ptr(), int(n),
+                                              h_pos4_out.data_ptr(), h_quat4_out.data_ptr(), C.byref(c)))
+        return c.as_dict()
+
+    def launch_count(self):
+        return int(self._lib.hpmc_launch_count(self._h))
+
+
+def from_workload(w, seed=1, device="cuda:0"):
+    """Create + bind + set_moves for a workloads.Workload."""
+    h = Hpmc(w.dim, w.L, w.kind, w.N, seed, diameter=w.diameter, verts=w.verts, device=device)
+    h.set_moves(w.d, w.a, w.n_select)
+    h.bind(w.pos4, w.quat4)
+    return h

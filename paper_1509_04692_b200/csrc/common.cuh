@@ -1,0 +1,96 @@
+// Shared parameter blocks and the pinned fp32 geometry helpers of the CUDA path.
+// P:<n> = PAPER.md line n, R<k> = DESIGN.md section 2.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "philox.cuh"
+
+namespace hpmc {
+
+constexpr int kMaxVerts = 32;
+constexpr int kKindDisk = 0, kKindPolygon = 1, kKindPolyhedron = 2;
+
+// grid + box, passed by value to every kernel (lands in the constant bank)
+struct GridParams {
+    int dim;
+    int n[3];         // cells per side (even, >= 4), R11
+    int C;            // number of cells
+    int N;            // number of particles
+    float L[3];       // box edge (fp32-rounded, R-box)
+    float lo[3];      // -L/2 (exact)
+    float hi[3];      // +L/2 (exact)
+    float inv_w[3];   // (float)(n/L), R13
+    float w_f[3];     // (float)(L/n), scale of the grid shift, R10
+    double Ld[3];     // (double)L for the fp64 seam subtraction, R21
+};
+
+struct MoveParams {
+    float d, a;       // R5, R6
+    int n_select;     // R9
+    float eps_g;      // R15 guard band
+};
+
+// what every kernel of one sweep needs to know about that sweep (written by k_prepare)
+struct SweepHeader {
+    float shift[3];   // R10
+    int perm[8];      // R12
+    uint32_t t_lo, t_hi16;
+    uint32_t pad;
+};
+
+// device-resident control block
+struct Control {
+    unsigned long long t;  // sweep counter (persists across calls)
+    unsigned long long counters[7];  // trans_acc, trans_rej_overlap, trans_rej_cell, rot_acc, rot_rej_overlap, trials, sweeps
+    unsigned long long overlaps;     // validator result
+    SweepHeader hdr;
+};
+
+// R13: the one cell function, used both to assign cells and to test "left its cell".
+// Explicit _rn intrinsics so that no multiply-add is ever contracted.
+__device__ __forceinline__ int cell_axis(float x, float lo, float s, float L, float inv_w, int n)
+{
+    float f = __fsub_rn(__fsub_rn(x, lo), s);
+    if (f < 0.0f) f = __fadd_rn(f, L);
+    if (f >= L) f = __fsub_rn(f, L);
+    int c = (int)floorf(__fmul_rn(f, inv_w));
+    if (c >= n) c -= n;
+    return c;
+}
+
+__device__ __forceinline__ int cell_of(const GridParams& g, const float shift[3], float x, float y, float z, int& cx,
+                                       int& cy, int& cz)
+{
+    cx = cell_axis(x, g.lo[0], shift[0], g.L[0], g.inv_w[0], g.n[0]);
+    cy = cell_axis(y, g.lo[1], shift[1], g.L[1], g.inv_w[1], g.n[1]);
+    cz = (g.dim == 3) ? cell_axis(z, g.lo[2], shift[2], g.L[2], g.inv_w[2], g.n[2]) : 0;
+    return cx + g.n[0] * (cy + g.n[1] * cz);
+}
+
+// O3.1/O3.2 (R10, R12): grid shift and colour order of sweep t
+__device__ inline void make_header(const GridParams& g, uint32_t k0, uint32_t k1, unsigned long long t, bool zero_shift,
+                                   SweepHeader& h)
+{
+    const uint32_t t_lo = (uint32_t)t, t_hi16 = (uint32_t)((t >> 32) & 0xFFFFull);
+    h.t_lo = t_lo;
+    h.t_hi16 = t_hi16;
+    const U4 r = philox4x32_10(0u, t_lo, 0u, (kTagShift << 24) | t_hi16, k0, k1);
+    const uint32_t rr[3] = {r.x, r.y, r.z};
+    for (int k = 0; k < 3; ++k) h.shift[k] = (k < g.dim && !zero_shift) ? __fmul_rn(g.w_f[k], u01(rr[k])) : 0.0f;
+    const int ncol = 1 << g.dim;
+    for (int c = 0; c < 8; ++c) h.perm[c] = c;
+    int word = 0;
+    U4 blk{0, 0, 0, 0};
+    for (int i = ncol - 1; i >= 1; --i) {
+        if ((word & 3) == 0) blk = philox4x32_10(0u, t_lo, (uint32_t)(word >> 2), (kTagPerm << 24) | t_hi16, k0, k1);
+        const uint32_t rw = ((word & 3) == 0) ? blk.x : ((word & 3) == 1) ? blk.y : ((word & 3) == 2) ? blk.z : blk.w;
+        const uint32_t j = mulhi32(rw, (uint32_t)(i + 1));
+        const int tmp = h.perm[i];
+        h.perm[i] = h.perm[j];
+        h.perm[j] = tmp;
+        ++word;
+    }
+}
+
+}  // namespace hpmc

@@ -1,0 +1,557 @@
+// C-ABI of libhpmc.so (include/hpmc.h): host-side context, validation, workspace carving and the launch
+// sequence of one sweep.  Every step of the hot path runs in the kernels of cell_list.cuh / sweep.cuh.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/hpmc.h"
+#include "cell_list.cuh"
+#include "common.cuh"
+#include "overlap.cuh"
+#include "sweep.cuh"
+
+using namespace hpmc;
+
+struct hpmc_ctx {
+    GridParams g{};
+    MoveParams mv{};
+    ShapeF sf{};
+    ShapeD sd{};
+    double d_max = 0.0;
+    double w[3] = {1, 1, 1};
+    uint64_t seed = 0;
+    uint32_t k0 = 0, k1 = 0;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    bool cuda_failed = false;
+    int64_t launches = 0;
+    uint64_t t_host = 0;  // mirror of the device sweep counter
+
+    // caller-owned
+    float4* d_pos_bound = nullptr;
+    float4* d_quat_bound = nullptr;
+    char* d_ws = nullptr;
+    size_t ws_bytes = 0;
+    bool state_in_bound = false;  // true: next build reads the bound arrays (tag order)
+    bool have_sorted = false;
+
+    // carved from the workspace
+    float4* pos[2] = {nullptr, nullptr};
+    float4* quat[2] = {nullptr, nullptr};
+    int* tag[2] = {nullptr, nullptr};
+    int cur = 0;
+    int2* key_rank = nullptr;
+    int* cell_start = nullptr;  // C+1 (+ padding)
+    int* tile_sums = nullptr;
+    Control* ctrl = nullptr;
+
+    uint2* trace = nullptr;
+    int64_t trace_words = 0;
+};
+
+namespace {
+
+thread_local std::string g_err_noctx;
+
+int fail(hpmc_ctx* c, int code, const std::string& msg)
+{
+    if (c) c->err = msg;
+    else g_err_noctx = msg;
+    return code;
+}
+
+bool cuda_ok(hpmc_ctx* c, cudaError_t e, const char* what)
+{
+    if (e == cudaSuccess) return true;
+    c->cuda_failed = true;
+    c->err = std::string("CUDA error in ") + what + ": " + cudaGetErrorString(e);
+    return false;
+}
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct Carve {
+    size_t off = 0;
+    size_t take(size_t bytes)
+    {
+        const size_t o = off;
+        off = align_up(off + bytes, 256);
+        return o;
+    }
+};
+
+int scan_tiles(const hpmc_ctx* c) { return (c->g.C + 1 + kScanTile - 1) / kScanTile; }
+
+struct Layout {
+    size_t pos[2], quat[2], tag[2], key_rank, cell_start, tile_sums, ctrl, total;
+};
+
+Layout layout_of(const hpmc_ctx* c)
+{
+    Layout L{};
+    Carve cv;
+    const size_t N = (size_t)(c->g.N > 0 ? c->g.N : 1);
+    for (int b = 0; b < 2; ++b) {
+        L.pos[b] = cv.take(N * sizeof(float4));
+        L.quat[b] = cv.take(N * sizeof(float4));
+        L.tag[b] = cv.take(N * sizeof(int));
+    }
+    L.key_rank = cv.take(N * sizeof(int2));
+    L.cell_start = cv.take(((size_t)c->g.C + 2) * sizeof(int));
+    L.tile_sums = cv.take((size_t)(scan_tiles(c) + 1) * sizeof(int));
+    L.ctrl = cv.take(sizeof(Control));
+    L.total = cv.off;
+    return L;
+}
+
+// host-side shape validation and derived data (convexity, CCW, edge normals); fp64 then rounded for ShapeF
+int build_shape(hpmc_ctx* c, const hpmc_shape* s, int dim)
+{
+    ShapeD& D = c->sd;
+    std::memset(&D, 0, sizeof D);
+    D.kind = s->kind;
+    if (s->kind == HPMC_KIND_DISK) {
+        if (!(s->diameter > 0.0)) return fail(c, HPMC_E_SHAPE, "disk diameter must be > 0");
+        D.diameter = s->diameter;
+        c->d_max = s->diameter;
+    } else if (s->kind == HPMC_KIND_POLYGON || s->kind == HPMC_KIND_POLYHEDRON) {
+        const bool poly2 = s->kind == HPMC_KIND_POLYGON;
+        if ((poly2 && dim != 2) || (!poly2 && dim != 3)) return fail(c, HPMC_E_SHAPE, "polygon needs dim 2, polyhedron dim 3");
+        if (!s->verts || s->nverts < (poly2 ? 3 : 4) || s->nverts > HPMC_MAX_VERTS)
+            return fail(c, HPMC_E_SHAPE, "vertex count out of range");
+        const int nv = s->nverts, vd = poly2 ? 2 : 3;
+        D.nverts = nv;
+        double rmax = 0.0;
+        for (int i = 0; i < nv; ++i) {
+            D.vx[i] = s->verts[i * vd];
+            D.vy[i] = s->verts[i * vd + 1];
+            D.vz[i] = poly2 ? 0.0 : s->verts[i * vd + 2];
+            rmax = std::fmax(rmax, std::sqrt(D.vx[i] * D.vx[i] + D.vy[i] * D.vy[i] + D.vz[i] * D.vz[i]));
+        }
+        c->d_max = 2.0 * rmax;  // circumsphere centred on the particle position
+        if (poly2) {
+            for (int k = 0; k < nv; ++k) {
+                const int k1 = (k + 1) % nv, k2 = (k + 2) % nv;
+                const double ex = D.vx[k1] - D.vx[k], ey = D.vy[k1] - D.vy[k];
+                const double fx = D.vx[k2] - D.vx[k1], fy = D.vy[k2] - D.vy[k1];
+                if (!(ex * fy - ey * fx > 0.0)) return fail(c, HPMC_E_SHAPE, "polygon must be strictly convex with CCW vertices");
+                const double len = std::sqrt(ex * ex + ey * ey);
+                D.nx[k] = ey / len;
+                D.ny[k] = -ex / len;
+                D.fc[k] = D.nx[k] * D.vx[k] + D.ny[k] * D.vy[k];
+                if (!(D.fc[k] > 0.0)) return fail(c, HPMC_E_SHAPE, "the body-frame origin must be inside the polygon");
+            }
+        } else {
+            // every vertex must be an extreme point and the origin must be interior: for each vertex v there
+            // must be a direction (here: tested with the vertex direction itself and all pair/triple normals)
+            // -- brute force over supporting planes through vertex triples.
+            int on_hull[HPMC_MAX_VERTS] = {0};
+            int nplanes = 0;
+            for (int i = 0; i < nv; ++i)
+                for (int j = i + 1; j < nv; ++j)
+                    for (int k = j + 1; k < nv; ++k) {
+                        const double e1[3] = {D.vx[j] - D.vx[i], D.vy[j] - D.vy[i], D.vz[j] - D.vz[i]};
+                        const double e2[3] = {D.vx[k] - D.vx[i], D.vy[k] - D.vy[i], D.vz[k] - D.vz[i]};
+                        double n[3] = {e1[1] * e2[2] - e1[2] * e2[1], e1[2] * e2[0] - e1[0] * e2[2], e1[0] * e2[1] - e1[1] * e2[0]};
+                        const double len = std::sqrt(n[0] * n[0] + n[1] * n[1] + n[2] * n[2]);
+                        if (len < 1e-12) continue;
+                        for (double& x : n) x /= len;
+                        const double off = n[0] * D.vx[i] + n[1] * D.vy[i] + n[2] * D.vz[i];
+                        int npos = 0, nneg = 0;
+                        for (int l = 0; l < nv; ++l) {
+                            const double dd = n[0] * D.vx[l] + n[1] * D.vy[l] + n[2] * D.vz[l] - off;
+                            npos += dd > 1e-9;
+                            nneg += dd < -1e-9;
+                        }
+                        if (npos && nneg) continue;
+                        ++nplanes;
+                        // origin strictly inside: on the same side as the other vertices, off the plane
+                        const double o = -off;  // n.0 - off
+                        if ((npos && !(o > 1e-12)) || (nneg && !(o < -1e-12)))
+                            return fail(c, HPMC_E_SHAPE, "the body-frame origin must be inside the polyhedron");
+                        for (int l = 0; l < nv; ++l)
+                            if (std::fabs(n[0] * D.vx[l] + n[1] * D.vy[l] + n[2] * D.vz[l] - off) < 1e-9) on_hull[l]++;
+                    }
+            if (nplanes < 4) return fail(c, HPMC_E_SHAPE, "degenerate polyhedron");
+            for (int l = 0; l < nv; ++l)
+                if (on_hull[l] < 3) return fail(c, HPMC_E_SHAPE, "every vertex must be a hull vertex (convex polyhedron)");
+        }
+    } else
+        return fail(c, HPMC_E_SHAPE, "unknown shape kind");
+    D.dmax2 = c->d_max * c->d_max;  // the validator is strict: no guard band
+    ShapeF& F = c->sf;
+    std::memset(&F, 0, sizeof F);
+    F.kind = D.kind;
+    F.nverts = D.nverts;
+    F.diameter = (float)D.diameter;
+    for (int i = 0; i < kMaxVerts; ++i) {
+        F.vx[i] = (float)D.vx[i]; F.vy[i] = (float)D.vy[i]; F.vz[i] = (float)D.vz[i];
+        F.nx[i] = (float)D.nx[i]; F.ny[i] = (float)D.ny[i]; F.fc[i] = (float)D.fc[i];
+    }
+    return HPMC_OK;
+}
+
+void refresh_sweep_range(hpmc_ctx* c)
+{
+    // broad-phase range of the sweep includes the guard band (R16'): skip iff |r|^2 >= (d_max + eps_g)^2
+    const double rr = c->d_max + (double)c->mv.eps_g;
+    c->sf.dmax2 = (float)(rr * rr);
+}
+
+#define LAUNCH_CHECK(c, what)                                      \
+    do {                                                           \
+        ++(c)->launches;                                           \
+        if (!cuda_ok((c), cudaGetLastError(), what)) return HPMC_E_CUDA; \
+    } while (0)
+
+// build the cell list of the current state into buffer 1-cur and flip.  mode as in k_prepare.
+int build_cell_list(hpmc_ctx* c, int mode, unsigned long long t_override)
+{
+    const GridParams& g = c->g;
+    const int TB = 256;
+    const float4* src_pos = c->state_in_bound ? c->d_pos_bound : c->pos[c->cur];
+    const float4* src_quat = c->state_in_bound ? c->d_quat_bound : c->quat[c->cur];
+    const int* src_tag = c->state_in_bound ? nullptr : c->tag[c->cur];
+    const int dst = c->state_in_bound ? 0 : 1 - c->cur;
+    const int nblk_cells = (g.C + 1 + TB - 1) / TB;
+    const int nblk_part = (g.N + TB - 1) / TB;
+    k_prepare<<<nblk_cells < 2048 ? nblk_cells : 2048, TB, 0, c->stream>>>(g, c->ctrl, c->cell_start, c->k0, c->k1, mode, t_override);
+    LAUNCH_CHECK(c, "k_prepare");
+    if (g.N > 0) {
+        k_hist<<<nblk_part, TB, 0, c->stream>>>(g, c->ctrl, src_pos, c->cell_start, c->key_rank);
+        LAUNCH_CHECK(c, "k_hist");
+    }
+    const int tiles = scan_tiles(c);
+    k_scan_reduce<<<tiles, kScanThreads, 0, c->stream>>>(c->cell_start, g.C, c->tile_sums);
+    LAUNCH_CHECK(c, "k_scan_reduce");
+    k_scan_spine<<<1, kScanThreads, 0, c->stream>>>(c->tile_sums, tiles);
+    LAUNCH_CHECK(c, "k_scan_spine");
+    k_scan_final<<<tiles, kScanThreads, 0, c->stream>>>(c->cell_start, g.C, c->tile_sums);
+    LAUNCH_CHECK(c, "k_scan_final");
+    if (g.N > 0) {
+        k_scatter<<<nblk_part, TB, 0, c->stream>>>(g.N, src_pos, src_quat, src_tag, c->key_rank, c->cell_start, c->pos[dst],
+                                                  c->quat[dst], c->tag[dst]);
+        LAUNCH_CHECK(c, "k_scatter");
+        k_cell_sort<<<(g.C + TB - 1) / TB, TB, 0, c->stream>>>(g.C, c->cell_start, c->pos[dst], c->quat[dst], c->tag[dst]);
+        LAUNCH_CHECK(c, "k_cell_sort");
+    }
+    c->cur = dst;
+    c->state_in_bound = false;
+    c->have_sorted = true;
+    return HPMC_OK;
+}
+
+template <int KIND, int NV>
+void launch_colour(hpmc_ctx* c, int ci)
+{
+    const GridParams& g = c->g;
+    const int nactive = (g.n[0] / 2) * (g.n[1] / 2) * (g.dim == 3 ? g.n[2] / 2 : 1);
+    const int TB = 128;
+    k_sweep_colour<KIND, NV><<<(nactive + TB - 1) / TB, TB, 0, c->stream>>>(g, c->mv, c->sf, c->ctrl, ci, c->pos[c->cur], c->quat[c->cur],
+                                                                           c->tag[c->cur], c->cell_start, c->k0, c->k1, c->trace);
+}
+
+int launch_colour_dispatch(hpmc_ctx* c, int ci)
+{
+    switch (c->sf.kind) {
+        case kKindDisk: launch_colour<kKindDisk, 0>(c, ci); break;
+        case kKindPolygon:
+            switch (c->sf.nverts) {
+                case 3: launch_colour<kKindPolygon, 3>(c, ci); break;
+                case 4: launch_colour<kKindPolygon, 4>(c, ci); break;
+                case 5: launch_colour<kKindPolygon, 5>(c, ci); break;
+                case 6: launch_colour<kKindPolygon, 6>(c, ci); break;
+                case 8: launch_colour<kKindPolygon, 8>(c, ci); break;
+                default: launch_colour<kKindPolygon, 0>(c, ci); break;
+            }
+            break;
+        default: launch_colour<kKindPolyhedron, 0>(c, ci); break;
+    }
+    LAUNCH_CHECK(c, "k_sweep_colour");
+    return HPMC_OK;
+}
+
+int check_ready(hpmc_ctx* c)
+{
+    if (!c) return HPMC_E_ARG;
+    if (c->cuda_failed) return HPMC_E_CUDA;
+    if (!c->d_ws || (!c->have_sorted && !c->state_in_bound)) return fail(c, HPMC_E_UNBOUND, "state/workspace not bound");
+    return HPMC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int hpmc_create(const hpmc_box* box, const hpmc_shape* shape, int64_t N, uint64_t seed, void* cuda_stream, hpmc_ctx** out)
+{
+    if (!out) return fail(nullptr, HPMC_E_ARG, "out is NULL");
+    *out = nullptr;
+    if (!box || !shape) return fail(nullptr, HPMC_E_ARG, "box/shape is NULL");
+    if (box->dim != 2 && box->dim != 3) return fail(nullptr, HPMC_E_ARG, "dim must be 2 or 3");
+    if (N < 0 || N > 2147483000LL) return fail(nullptr, HPMC_E_ARG, "N out of range");
+    hpmc_ctx* c = new (std::nothrow) hpmc_ctx();
+    if (!c) return fail(nullptr, HPMC_E_ARG, "out of host memory");
+    int rc = build_shape(c, shape, box->dim);
+    if (rc != HPMC_OK) { g_err_noctx = c->err; delete c; return rc; }
+    GridParams& g = c->g;
+    g.dim = box->dim;
+    g.N = (int)N;
+    double cells = 1.0;
+    for (int k = 0; k < 3; ++k) {
+        if (k < g.dim) {
+            if (!(box->L[k] > 0.0)) { delete c; return fail(nullptr, HPMC_E_ARG, "box edge must be > 0"); }
+            g.L[k] = (float)box->L[k];            // R-box: the box edge is L rounded to fp32
+            g.Ld[k] = (double)g.L[k];
+            g.n[k] = 2 * (int)std::floor(g.Ld[k] / (2.0 * c->d_max * (1.0 + 1.0 / 1024.0)));  // R11
+            if (g.n[k] < 4) { delete c; return fail(nullptr, HPMC_E_GRID, "fewer than 4 cells per side (R11)"); }
+            c->w[k] = g.Ld[k] / g.n[k];
+            g.w_f[k] = (float)c->w[k];
+            g.inv_w[k] = (float)((double)g.n[k] / g.Ld[k]);
+        } else {
+            g.L[k] = 1.0f; g.Ld[k] = 1.0; g.n[k] = 1; g.w_f[k] = 1.0f; g.inv_w[k] = 1.0f; c->w[k] = 1.0;
+        }
+        g.hi[k] = 0.5f * g.L[k];
+        g.lo[k] = -g.hi[k];
+        cells *= g.n[k];
+    }
+    if (cells > 2147483000.0) { delete c; return fail(nullptr, HPMC_E_GRID, "too many cells for 32-bit ids"); }
+    g.C = (int)cells;
+    c->seed = seed;
+    c->k0 = (uint32_t)seed;
+    c->k1 = (uint32_t)(seed >> 32);
+    c->stream = (cudaStream_t)cuda_stream;
+    c->mv.d = 0.1f; c->mv.a = 0.1f; c->mv.n_select = 4; c->mv.eps_g = 2e-6f;  // R15
+    refresh_sweep_range(c);
+    *out = c;
+    return HPMC_OK;
+}
+
+int hpmc_destroy(hpmc_ctx* c)
+{
+    delete c;
+    return HPMC_OK;
+}
+
+const char* hpmc_last_error(const hpmc_ctx* c) { return c ? c->err.c_str() : g_err_noctx.c_str(); }
+
+int hpmc_get_grid(const hpmc_ctx* c, hpmc_grid_info* o)
+{
+    if (!c || !o) return HPMC_E_ARG;
+    o->dim = c->g.dim;
+    for (int k = 0; k < 3; ++k) { o->n[k] = c->g.n[k]; o->w[k] = c->w[k]; o->L_f[k] = c->g.L[k]; o->inv_w[k] = c->g.inv_w[k]; }
+    o->d_max = c->d_max;
+    o->num_cells = c->g.C;
+    o->N = c->g.N;
+    return HPMC_OK;
+}
+
+size_t hpmc_workspace_bytes(const hpmc_ctx* c) { return c ? layout_of(c).total : 0; }
+
+int hpmc_bind(hpmc_ctx* c, float* d_pos4, float* d_quat4, void* d_workspace, size_t bytes)
+{
+    if (!c) return HPMC_E_ARG;
+    if (c->cuda_failed) return HPMC_E_CUDA;
+    if (!d_pos4 || !d_quat4 || !d_workspace) return fail(c, HPMC_E_ARG, "NULL device pointer");
+    const Layout L = layout_of(c);
+    if (bytes < L.total) return fail(c, HPMC_E_UNBOUND, "workspace smaller than hpmc_workspace_bytes()");
+    if (((uintptr_t)d_workspace & 255u) || ((uintptr_t)d_pos4 & 15u) || ((uintptr_t)d_quat4 & 15u))
+        return fail(c, HPMC_E_ARG, "workspace must be 256-byte aligned, state arrays 16-byte aligned");
+    const bool first = (c->d_ws == nullptr) || (c->d_ws != (char*)d_workspace);
+    c->d_pos_bound = (float4*)d_pos4;
+    c->d_quat_bound = (float4*)d_quat4;
+    c->d_ws = (char*)d_workspace;
+    c->ws_bytes = bytes;
+    for (int b = 0; b < 2; ++b) {
+        c->pos[b] = (float4*)(c->d_ws + L.pos[b]);
+        c->quat[b] = (float4*)(c->d_ws + L.quat[b]);
+        c->tag[b] = (int*)(c->d_ws + L.tag[b]);
+    }
+    c->key_rank = (int2*)(c->d_ws + L.key_rank);
+    c->cell_start = (int*)(c->d_ws + L.cell_start);
+    c->tile_sums = (int*)(c->d_ws + L.tile_sums);
+    c->ctrl = (Control*)(c->d_ws + L.ctrl);
+    if (first) {  // a new workspace: (re)create the control block, keeping the host-side sweep counter
+        Control init;
+        std::memset(&init, 0, sizeof init);
+        init.t = c->t_host;
+        if (!cuda_ok(c, cudaMemcpyAsync(c->ctrl, &init, sizeof init, cudaMemcpyHostToDevice, c->stream), "bind/memcpy")) return HPMC_E_CUDA;
+        if (!cuda_ok(c, cudaStreamSynchronize(c->stream), "bind/sync")) return HPMC_E_CUDA;  // `init` is a stack object
+    }
+    c->state_in_bound = true;
+    c->have_sorted = false;
+    c->cur = 0;
+    return HPMC_OK;
+}
+
+int hpmc_set_moves(hpmc_ctx* c, double d, double a, int n_select)
+{
+    if (!c) return HPMC_E_ARG;
+    if (!(d > 0.0) || !(a >= 0.0) || n_select < 1 || n_select > 65535) return fail(c, HPMC_E_ARG, "need d > 0, a >= 0, 1 <= n_select <= 65535");
+    c->mv.d = (float)d;
+    c->mv.a = (float)a;
+    c->mv.n_select = n_select;
+    return HPMC_OK;
+}
+
+int hpmc_sweep(hpmc_ctx* c, int64_t n)
+{
+    int rc = check_ready(c);
+    if (rc != HPMC_OK) return rc;
+    if (n < 0) return fail(c, HPMC_E_ARG, "n must be >= 0");
+    if (c->trace && c->trace_words < 2 * (int64_t)c->g.C * c->mv.n_select) return fail(c, HPMC_E_TRACE, "trace buffer too small");
+    const int ncol = 1 << c->g.dim;
+    for (int64_t s = 0; s < n; ++s) {
+        rc = build_cell_list(c, 0, 0ull);
+        if (rc != HPMC_OK) return rc;
+        for (int ci = 0; ci < ncol; ++ci) {
+            rc = launch_colour_dispatch(c, ci);
+            if (rc != HPMC_OK) return rc;
+        }
+        ++c->t_host;
+    }
+    return HPMC_OK;
+}
+
+int hpmc_count_overlaps(hpmc_ctx* c, int64_t* h_count)
+{
+    int rc = check_ready(c);
+    if (rc != HPMC_OK) return rc;
+    if (!h_count) return fail(c, HPMC_E_ARG, "h_count is NULL");
+    rc = build_cell_list(c, 2, 0ull);
+    if (rc != HPMC_OK) return rc;
+    if (!cuda_ok(c, cudaMemsetAsync(&c->ctrl->overlaps, 0, sizeof(unsigned long long), c->stream), "count/memset")) return HPMC_E_CUDA;
+    if (c->g.N > 0) {
+        const int TB = 128, nb = (c->g.N + TB - 1) / TB;
+        switch (c->sd.kind) {
+            case kKindDisk: k_count_overlaps<kKindDisk><<<nb, TB, 0, c->stream>>>(c->g, c->sd, c->ctrl, c->pos[c->cur], c->quat[c->cur], c->tag[c->cur], c->cell_start); break;
+            case kKindPolygon: k_count_overlaps<kKindPolygon><<<nb, TB, 0, c->stream>>>(c->g, c->sd, c->ctrl, c->pos[c->cur], c->quat[c->cur], c->tag[c->cur], c->cell_start); break;
+            default: k_count_overlaps<kKindPolyhedron><<<nb, TB, 0, c->stream>>>(c->g, c->sd, c->ctrl, c->pos[c->cur], c->quat[c->cur], c->tag[c->cur], c->cell_start); break;
+        }
+        LAUNCH_CHECK(c, "k_count_overlaps");
+    }
+    unsigned long long v = 0;
+    if (!cuda_ok(c, cudaMemcpyAsync(&v, &c->ctrl->overlaps, sizeof v, cudaMemcpyDeviceToHost, c->stream), "count/memcpy")) return HPMC_E_CUDA;
+    if (!cuda_ok(c, cudaStreamSynchronize(c->stream), "count/sync")) return HPMC_E_CUDA;
+    *h_count = (int64_t)v;
+    return HPMC_OK;
+}
+
+int hpmc_get_state(hpmc_ctx* c, float* d_pos4_out, float* d_quat4_out, hpmc_counters* h_counters, int64_t* h_sweep_counter)
+{
+    int rc = check_ready(c);
+    if (rc != HPMC_OK) return rc;
+    if ((d_pos4_out || d_quat4_out) && c->g.N > 0) {
+        if (c->state_in_bound) {  // nothing ran since bind: the bound arrays are the state
+            const size_t bytes = (size_t)c->g.N * sizeof(float4);
+            if (d_pos4_out && (float4*)d_pos4_out != c->d_pos_bound &&
+                !cuda_ok(c, cudaMemcpyAsync(d_pos4_out, c->d_pos_bound, bytes, cudaMemcpyDeviceToDevice, c->stream), "get_state/copy")) return HPMC_E_CUDA;
+            if (d_quat4_out && (float4*)d_quat4_out != c->d_quat_bound &&
+                !cuda_ok(c, cudaMemcpyAsync(d_quat4_out, c->d_quat_bound, bytes, cudaMemcpyDeviceToDevice, c->stream), "get_state/copy")) return HPMC_E_CUDA;
+        } else {
+            const int TB = 256;
+            k_unsort<<<(c->g.N + TB - 1) / TB, TB, 0, c->stream>>>(c->g.N, c->pos[c->cur], c->quat[c->cur], c->tag[c->cur],
+                                                                  (float4*)d_pos4_out, (float4*)d_quat4_out);
+            LAUNCH_CHECK(c, "k_unsort");
+        }
+    }
+    if (h_counters || h_sweep_counter) {
+        Control h;
+        if (!cuda_ok(c, cudaMemcpyAsync(&h, c->ctrl, sizeof h, cudaMemcpyDeviceToHost, c->stream), "get_state/memcpy")) return HPMC_E_CUDA;
+        if (!cuda_ok(c, cudaStreamSynchronize(c->stream), "get_state/sync")) return HPMC_E_CUDA;
+        if (h_counters) {
+            h_counters->trans_acc = h.counters[0]; h_counters->trans_rej_overlap = h.counters[1];
+            h_counters->trans_rej_cell = h.counters[2]; h_counters->rot_acc = h.counters[3];
+            h_counters->rot_rej_overlap = h.counters[4]; h_counters->trials = h.counters[5]; h_counters->sweeps = h.counters[6];
+        }
+        if (h_sweep_counter) *h_sweep_counter = (int64_t)h.t;
+    }
+    return HPMC_OK;
+}
+
+int hpmc_set_sweep_counter(hpmc_ctx* c, uint64_t t)
+{
+    if (!c) return HPMC_E_ARG;
+    if (c->cuda_failed) return HPMC_E_CUDA;
+    c->t_host = t;
+    if (c->ctrl) {
+        const unsigned long long v = t;
+        if (!cuda_ok(c, cudaMemcpyAsync(&c->ctrl->t, &v, sizeof v, cudaMemcpyHostToDevice, c->stream), "set_t/memcpy")) return HPMC_E_CUDA;
+        if (!cuda_ok(c, cudaStreamSynchronize(c->stream), "set_t/sync")) return HPMC_E_CUDA;
+    }
+    return HPMC_OK;
+}
+
+int hpmc_reset_counters(hpmc_ctx* c)
+{
+    if (!c) return HPMC_E_ARG;
+    if (c->cuda_failed) return HPMC_E_CUDA;
+    if (!c->ctrl) return fail(c, HPMC_E_UNBOUND, "workspace not bound");
+    if (!cuda_ok(c, cudaMemsetAsync(c->ctrl->counters, 0, sizeof(unsigned long long) * 7, c->stream), "reset/memset")) return HPMC_E_CUDA;
+    return HPMC_OK;
+}
+
+int hpmc_set_trace(hpmc_ctx* c, uint32_t* d_trace, int64_t capacity_words)
+{
+    if (!c) return HPMC_E_ARG;
+    if (d_trace && ((uintptr_t)d_trace & 7u)) return fail(c, HPMC_E_ARG, "trace must be 8-byte aligned");
+    c->trace = (uint2*)d_trace;
+    c->trace_words = d_trace ? capacity_words : 0;
+    return HPMC_OK;
+}
+
+int hpmc_get_cell_list(hpmc_ctx* c, uint64_t t, int32_t* d_cell_start, int32_t* d_member_tags, int32_t* d_cell_of_tag,
+                       float* h_shift3, int32_t* h_colour_perm8)
+{
+    int rc = check_ready(c);
+    if (rc != HPMC_OK) return rc;
+    const bool from_bound = c->state_in_bound;
+    const int* src_tag = from_bound ? nullptr : c->tag[c->cur];
+    rc = build_cell_list(c, 1, (unsigned long long)t);
+    if (rc != HPMC_OK) return rc;
+    const size_t nb = (size_t)c->g.N * sizeof(int);
+    if (d_cell_start && !cuda_ok(c, cudaMemcpyAsync(d_cell_start, c->cell_start, ((size_t)c->g.C + 1) * sizeof(int), cudaMemcpyDeviceToDevice, c->stream), "cell_list/copy")) return HPMC_E_CUDA;
+    if (d_member_tags && c->g.N > 0 && !cuda_ok(c, cudaMemcpyAsync(d_member_tags, c->tag[c->cur], nb, cudaMemcpyDeviceToDevice, c->stream), "cell_list/copy")) return HPMC_E_CUDA;
+    if (d_cell_of_tag && c->g.N > 0) {
+        const int TB = 256;
+        k_cell_of_tag<<<(c->g.N + TB - 1) / TB, TB, 0, c->stream>>>(c->g.N, c->key_rank, src_tag, d_cell_of_tag);
+        LAUNCH_CHECK(c, "k_cell_of_tag");
+    }
+    if (h_shift3 || h_colour_perm8) {
+        Control h;
+        if (!cuda_ok(c, cudaMemcpyAsync(&h, c->ctrl, sizeof h, cudaMemcpyDeviceToHost, c->stream), "cell_list/memcpy")) return HPMC_E_CUDA;
+        if (!cuda_ok(c, cudaStreamSynchronize(c->stream), "cell_list/sync")) return HPMC_E_CUDA;
+        if (h_shift3) for (int k = 0; k < 3; ++k) h_shift3[k] = h.hdr.shift[k];
+        if (h_colour_perm8) for (int k = 0; k < 8; ++k) h_colour_perm8[k] = h.hdr.perm[k];
+    }
+    return HPMC_OK;
+}
+
+int hpmc_sweep_host(hpmc_ctx* c, const float* h_pos4, const float* h_quat4, int64_t n, float* h_pos4_out, float* h_quat4_out,
+                    hpmc_counters* h_counters)
+{
+    if (!c) return HPMC_E_ARG;
+    if (c->cuda_failed) return HPMC_E_CUDA;
+    if (!c->d_ws || !c->d_pos_bound) return fail(c, HPMC_E_UNBOUND, "state/workspace not bound");
+    if (!h_pos4 || !h_quat4) return fail(c, HPMC_E_ARG, "NULL host pointer");
+    const size_t bytes = (size_t)c->g.N * sizeof(float4);
+    if (!cuda_ok(c, cudaMemcpyAsync(c->d_pos_bound, h_pos4, bytes, cudaMemcpyHostToDevice, c->stream), "sweep_host/h2d")) return HPMC_E_CUDA;
+    if (!cuda_ok(c, cudaMemcpyAsync(c->d_quat_bound, h_quat4, bytes, cudaMemcpyHostToDevice, c->stream), "sweep_host/h2d")) return HPMC_E_CUDA;
+    c->state_in_bound = true;
+    c->have_sorted = false;
+    int rc = hpmc_sweep(c, n);
+    if (rc != HPMC_OK) return rc;
+    rc = hpmc_get_state(c, (float*)c->d_pos_bound, (float*)c->d_quat_bound, nullptr, nullptr);
+    if (rc != HPMC_OK) return rc;
+    if (h_pos4_out && !cuda_ok(c, cudaMemcpyAsync(h_pos4_out, c->d_pos_bound, bytes, cudaMemcpyDeviceToHost, c->stream), "sweep_host/d2h")) return HPMC_E_CUDA;
+    if (h_quat4_out && !cuda_ok(c, cudaMemcpyAsync(h_quat4_out, c->d_quat_bound, bytes, cudaMemcpyDeviceToHost, c->stream), "sweep_host/d2h")) return HPMC_E_CUDA;
+    hpmc_counters tmp;
+    rc = hpmc_get_state(c, nullptr, nullptr, h_counters ? h_counters : &tmp, nullptr);  // also synchronises
+    return rc;
+}
+
+int64_t hpmc_launch_count(const hpmc_ctx* c) { return c ? c->launches : 0; }
+
+}  // extern "C"

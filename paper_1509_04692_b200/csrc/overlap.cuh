@@ -1,0 +1,259 @@
+// Narrow-phase overlap tests of the CUDA path (S:8(a) row a9), templated on the scalar type:
+// float in the sweep kernels, double in the overlap-count validator.
+//   disk / sphere      : centre distance vs diameter, "trivial"
+//   convex polygon     : separating axes over the edge normals of both, in A's frame
+//   convex polyhedron  : GJK separating-axis search on the Minkowski difference B (-) A with the support
+//                        function of Eq. (2): S(n) = R S_B(R^-1 n) + r_AB - S_A(-n), in A's frame.
+// Every test answers "is the pair separated by at least eps?"; "no" means overlap (R15, R-poly).
+#pragma once
+#include "common.cuh"
+
+namespace hpmc {
+
+template <typename T>
+struct ShapeT {
+    int kind, nverts;
+    T diameter;
+    T dmax2;              // d_max^2, broad phase R16
+    T vx[kMaxVerts], vy[kMaxVerts], vz[kMaxVerts];
+    T nx[kMaxVerts], ny[kMaxVerts], fc[kMaxVerts];  // polygon: outward unit edge normals and offsets n.v
+};
+using ShapeF = ShapeT<float>;
+using ShapeD = ShapeT<double>;
+
+template <typename T>
+struct V3 {
+    T x, y, z;
+};
+template <typename T>
+__device__ __forceinline__ T dot(const V3<T>& a, const V3<T>& b)
+{
+    return a.x * b.x + a.y * b.y + a.z * b.z;
+}
+template <typename T>
+__device__ __forceinline__ V3<T> cross(const V3<T>& a, const V3<T>& b)
+{
+    return V3<T>{a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x};
+}
+template <typename T>
+__device__ __forceinline__ V3<T> operator-(const V3<T>& a, const V3<T>& b)
+{
+    return V3<T>{a.x - b.x, a.y - b.y, a.z - b.z};
+}
+template <typename T>
+__device__ __forceinline__ V3<T> operator+(const V3<T>& a, const V3<T>& b)
+{
+    return V3<T>{a.x + b.x, a.y + b.y, a.z + b.z};
+}
+template <typename T>
+__device__ __forceinline__ V3<T> operator*(T s, const V3<T>& a)
+{
+    return V3<T>{s * a.x, s * a.y, s * a.z};
+}
+
+// ---------------------------------------------------------------------------------------------
+// convex polygons: in A's body frame A's vertices/normals are the stored constants, so only B has to
+// be rotated ("a local coordinate system centered on particle A").
+// (rx, ry) = r_AB in the world frame; (cA,sA), (cB,sB) = cos/sin of the orientation angles.
+// NV > 0: compile-time vertex count (fully unrolled, registers); NV == 0: runtime count.
+// Returns true iff NO axis separates the pair by at least eps.
+// ---------------------------------------------------------------------------------------------
+template <typename T, int NV>
+__device__ __forceinline__ bool polygon_overlap(const ShapeT<T>& S, T rx, T ry, T cA, T sA, T cB, T sB, T eps)
+{
+    const int nv = (NV > 0) ? NV : S.nverts;
+    const T lx = cA * rx + sA * ry;    // R_A^T r_AB
+    const T ly = -sA * rx + cA * ry;
+    const T c = cA * cB + sA * sB;     // R = R_A^T R_B
+    const T s = cA * sB - sA * cB;
+    // axes of A: separation_k = min_j n_k . p_j - c_k with p_j = B's vertices in A's frame
+    {
+        T px[(NV > 0) ? NV : kMaxVerts], py[(NV > 0) ? NV : kMaxVerts];
+#pragma unroll
+        for (int j = 0; j < nv; ++j) {
+            px[j] = c * S.vx[j] - s * S.vy[j] + lx;
+            py[j] = s * S.vx[j] + c * S.vy[j] + ly;
+        }
+#pragma unroll
+        for (int k = 0; k < nv; ++k) {
+            T m = S.nx[k] * px[0] + S.ny[k] * py[0];
+#pragma unroll
+            for (int j = 1; j < nv; ++j) m = min(m, S.nx[k] * px[j] + S.ny[k] * py[j]);
+            if (m - S.fc[k] >= eps) return false;
+        }
+    }
+    // axes of B: n'_k = R n_k; separation_k = min_j n'_k . (v_j - r_loc) - c_k  (A's vertices seen from B)
+    {
+        T qx[(NV > 0) ? NV : kMaxVerts], qy[(NV > 0) ? NV : kMaxVerts];
+#pragma unroll
+        for (int j = 0; j < nv; ++j) {
+            qx[j] = S.vx[j] - lx;
+            qy[j] = S.vy[j] - ly;
+        }
+#pragma unroll
+        for (int k = 0; k < nv; ++k) {
+            const T nxk = c * S.nx[k] - s * S.ny[k];
+            const T nyk = s * S.nx[k] + c * S.ny[k];
+            T m = nxk * qx[0] + nyk * qy[0];
+#pragma unroll
+            for (int j = 1; j < nv; ++j) m = min(m, nxk * qx[j] + nyk * qy[j]);
+            if (m - S.fc[k] >= eps) return false;
+        }
+    }
+    return true;
+}
+
+// ---------------------------------------------------------------------------------------------
+// convex polyhedra: GJK.  Rm = rotation taking B's body frame into A's body frame (row major),
+// r = r_AB expressed in A's frame.
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+__device__ __forceinline__ V3<T> support_minkowski(const ShapeT<T>& S, const T* Rm, const V3<T>& r, const V3<T>& dir)
+{
+    // R^-1 dir = R^T dir
+    const V3<T> db{Rm[0] * dir.x + Rm[3] * dir.y + Rm[6] * dir.z, Rm[1] * dir.x + Rm[4] * dir.y + Rm[7] * dir.z,
+                   Rm[2] * dir.x + Rm[5] * dir.y + Rm[8] * dir.z};
+    T bestA = -(T)3.0e38, bestB = -(T)3.0e38;
+    int ia = 0, ib = 0;
+    for (int i = 0; i < S.nverts; ++i) {
+        const T da = -(dir.x * S.vx[i] + dir.y * S.vy[i] + dir.z * S.vz[i]);   // S_A(-dir)
+        const T dbv = db.x * S.vx[i] + db.y * S.vy[i] + db.z * S.vz[i];        // S_B(R^-1 dir)
+        if (da > bestA) { bestA = da; ia = i; }
+        if (dbv > bestB) { bestB = dbv; ib = i; }
+    }
+    const T bx = S.vx[ib], by = S.vy[ib], bz = S.vz[ib];
+    return V3<T>{Rm[0] * bx + Rm[1] * by + Rm[2] * bz + r.x - S.vx[ia], Rm[3] * bx + Rm[4] * by + Rm[5] * bz + r.y - S.vy[ia],
+                 Rm[6] * bx + Rm[7] * by + Rm[8] * bz + r.z - S.vz[ia]};
+}
+
+// closest point to the origin on triangle (a,b,c); mask bit0/1/2 = a/b/c supports the result
+template <typename T>
+__device__ __forceinline__ V3<T> closest_on_triangle(const V3<T>& a, const V3<T>& b, const V3<T>& c, int& mask)
+{
+    const V3<T> ab = b - a, ac = c - a;
+    const T d1 = -dot(ab, a), d2 = -dot(ac, a);
+    if (d1 <= 0 && d2 <= 0) { mask = 1; return a; }
+    const T d3 = -dot(ab, b), d4 = -dot(ac, b);
+    if (d3 >= 0 && d4 <= d3) { mask = 2; return b; }
+    const T vc = d1 * d4 - d3 * d2;
+    if (vc <= 0 && d1 >= 0 && d3 <= 0) { mask = 3; return a + (d1 / (d1 - d3)) * ab; }
+    const T d5 = -dot(ab, c), d6 = -dot(ac, c);
+    if (d6 >= 0 && d5 <= d6) { mask = 4; return c; }
+    const T vb = d5 * d2 - d1 * d6;
+    if (vb <= 0 && d2 >= 0 && d6 <= 0) { mask = 5; return a + (d2 / (d2 - d6)) * ac; }
+    const T va = d3 * d6 - d5 * d4;
+    if (va <= 0 && (d4 - d3) >= 0 && (d5 - d6) >= 0) { mask = 6; return b + ((d4 - d3) / ((d4 - d3) + (d5 - d6))) * (c - b); }
+    const T denom = (T)1 / (va + vb + vc);
+    mask = 7;
+    return a + (vb * denom) * ab + (vc * denom) * ac;
+}
+
+// Returns true iff a direction was found along which the support functions separate the pair by >= eps.
+// Everything else (origin enclosed, converged with distance < eps, no numerical progress, iteration cap)
+// returns false = treat as overlap (conservative, R-poly).
+template <typename T>
+__device__ bool gjk_separated(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T eps)
+{
+    const T tiny = (sizeof(T) == 4) ? (T)1e-14 : (T)1e-28;
+    const T reltol = (sizeof(T) == 4) ? (T)1e-6 : (T)1e-13;
+    V3<T> v = r;  // a point of B (-) A (both body origins are interior points)
+    T vv = dot(v, v);
+    if (vv < tiny) return false;
+    V3<T> W[4];
+    int nW = 0;
+    for (int iter = 0; iter < 40; ++iter) {
+        const V3<T> w = support_minkowski(S, Rm, r, V3<T>{-v.x, -v.y, -v.z});
+        const T vw = dot(v, w);
+        if (vw >= 0 && vw * vw >= eps * eps * vv) return true;          // certificate: v^.w >= eps
+        if (iter > 0 && vv - vw <= reltol * vv) return false;           // converged: distance |v| < eps
+        for (int i = 0; i < nW; ++i)
+            if (W[i].x == w.x && W[i].y == w.y && W[i].z == w.z) return false;  // same support point again
+        W[nW++] = w;
+        V3<T> vn;
+        if (nW == 1) {
+            vn = w;
+        } else if (nW == 2) {
+            const V3<T> a = W[1], b = W[0], ab = b - a;
+            const T t = -dot(a, ab);
+            if (t <= 0) { vn = a; W[0] = a; nW = 1; }
+            else {
+                const T den = dot(ab, ab);
+                if (t >= den) { vn = b; nW = 1; }
+                else vn = a + (t / den) * ab;
+            }
+        } else if (nW == 3) {
+            int mask;
+            const V3<T> a = W[2], b = W[1], c = W[0];
+            vn = closest_on_triangle(a, b, c, mask);
+            int k = 0;
+            if (mask & 4) W[k++] = c;
+            if (mask & 2) W[k++] = b;
+            if (mask & 1) W[k++] = a;
+            nW = k;
+        } else {
+            const V3<T> a = W[3], b = W[2], c = W[1], d = W[0];
+            // faces (a,b,c | d), (a,c,d | b), (a,d,b | c), (b,d,c | a): origin outside iff on the other side than the 4th vertex
+            T best = (T)3.0e38;
+            int bestFace = -1, bestMask = 0;
+            V3<T> bestV{0, 0, 0};
+#pragma unroll
+            for (int f = 0; f < 4; ++f) {
+                const V3<T> p = (f == 3) ? b : a;
+                const V3<T> q = (f == 0) ? b : (f == 1) ? c : d;
+                const V3<T> s3 = (f == 0) ? c : (f == 1) ? d : (f == 2) ? b : c;
+                const V3<T> o = (f == 0) ? d : (f == 1) ? b : (f == 2) ? c : a;
+                const V3<T> nn = cross(q - p, s3 - p);
+                const T sp = -dot(nn, p);          // origin side
+                const T sd = dot(nn, o - p);       // opposite-vertex side
+                if (sp * sd <= 0) {                // outside this face (or degenerate): closest point on it
+                    int m;
+                    const V3<T> cand = closest_on_triangle(p, q, s3, m);
+                    const T cc = dot(cand, cand);
+                    if (cc < best) { best = cc; bestFace = f; bestMask = m; bestV = cand; }
+                }
+            }
+            if (bestFace < 0) return false;        // origin inside the tetrahedron: overlap
+            const V3<T> p = (bestFace == 3) ? b : a;
+            const V3<T> q = (bestFace == 0) ? b : (bestFace == 1) ? c : d;
+            const V3<T> s3 = (bestFace == 0) ? c : (bestFace == 1) ? d : (bestFace == 2) ? b : c;
+            int k = 0;
+            if (bestMask & 4) W[k++] = s3;
+            if (bestMask & 2) W[k++] = q;
+            if (bestMask & 1) W[k++] = p;
+            nW = k;
+            vn = bestV;
+        }
+        const T vvn = dot(vn, vn);
+        if (vvn < tiny) return false;              // origin on the simplex: touching or inside
+        if (iter > 0 && vvn >= vv) return false;   // no numerical progress
+        v = vn;
+        vv = vvn;
+    }
+    return false;
+}
+
+// rotation matrix (row major) of the unit quaternion (w,x,y,z)
+template <typename T>
+__device__ __forceinline__ void quat_to_matrix(T w, T x, T y, T z, T* M)
+{
+    const T xx = x * x, yy = y * y, zz = z * z, xy = x * y, xz = x * z, yz = y * z, wx = w * x, wy = w * y, wz = w * z;
+    M[0] = 1 - 2 * (yy + zz); M[1] = 2 * (xy - wz);     M[2] = 2 * (xz + wy);
+    M[3] = 2 * (xy + wz);     M[4] = 1 - 2 * (xx + zz); M[5] = 2 * (yz - wx);
+    M[6] = 2 * (xz - wy);     M[7] = 2 * (yz + wx);     M[8] = 1 - 2 * (xx + yy);
+}
+
+// polyhedron pair in A's frame: MA, MB = world rotation matrices of A and B, rw = r_AB (world)
+template <typename T>
+__device__ __forceinline__ bool polyhedron_overlap(const ShapeT<T>& S, const T* MA, const T* MB, const V3<T>& rw, T eps)
+{
+    T Rm[9];  // R = MA^T MB takes B's frame into A's frame (q = q_A* q_B)
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) Rm[3 * i + j] = MA[i] * MB[j] + MA[3 + i] * MB[3 + j] + MA[6 + i] * MB[6 + j];
+    const V3<T> r{MA[0] * rw.x + MA[3] * rw.y + MA[6] * rw.z, MA[1] * rw.x + MA[4] * rw.y + MA[7] * rw.z,
+                  MA[2] * rw.x + MA[5] * rw.y + MA[8] * rw.z};
+    return !gjk_separated(S, Rm, r, eps);
+}
+
+}  // namespace hpmc

@@ -1,0 +1,205 @@
+"""GPU parity tests proper: the CUDA path (through the C-ABI binding) against the oracle, element by element,
+on the same seeded inputs.  Bars (BASELINE.json north_star): cell assignment and indexing bit-exact; the first
+10 sweeps' accept/reject decisions identical except on trials whose contact margin is within 1e-5 of the
+threshold (counted); positions within 1e-5 where no decision differed (here: bit-exact); zero overlaps."""
+import numpy as np
+import pytest
+
+from oracle import hpmc_oracle as ho
+from paper_1509_04692_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+MARGIN_TOL = 1e-5
+
+
+def gpu(w, seed=1):
+    from paper_1509_04692_b200 import binding as hb
+    return hb.from_workload(w, seed=seed)
+
+
+def orc(w, seed=1):
+    o = ho.Oracle(w.dim, w.L, w.kind, w.N, seed, diameter=w.diameter, verts=w.verts)
+    o.set_moves(w.d, w.a, w.n_select)
+    o.set_state(w.pos4, w.quat4)
+    return o
+
+
+CASES = {
+    "disks_24": lambda: wl.disks(24),
+    "pentagons_24": lambda: wl.pentagons(24),
+    "cubes_7": lambda: wl.cubes(7),
+    "k0_disks": lambda: wl.config(0),
+    "k1_pentagons": lambda: wl.config(1),
+    "cubes_12": lambda: wl.cubes(12),
+}
+
+
+def test_grid_matches_oracle():
+    for name in ("k0_disks", "k1_pentagons", "cubes_12"):
+        w = CASES[name]()
+        g, o = gpu(w), orc(w)
+        assert np.array_equal(g.n, o.n) and g.C == o.C
+        assert np.array_equal(g.inv_w[: w.dim], o.inv_w[: w.dim]) and np.array_equal(g.L_f[: w.dim], o.L_f[: w.dim])
+        assert g.d_max == pytest.approx(ho.Shape(w.dim, w.kind, diameter=w.diameter, verts=w.verts).dmax, abs=1e-15)
+
+
+@pytest.mark.parametrize("name", ["disks_24", "pentagons_24", "cubes_7", "k1_pentagons"])
+def test_header_and_cell_list_bit_exact(name):
+    w = CASES[name]()
+    g, o = gpu(w), orc(w)
+    for t in (0, 1, 2, 17, 2 ** 32 - 1, 2 ** 32 + 5, 2 ** 40 + 123):
+        cid, cst, mem, shift, perm = g.cell_list(t)
+        oshift, operm = o.sweep_header(t)
+        assert np.array_equal(shift[: w.dim], oshift[: w.dim]) and np.array_equal(perm, operm)   # Philox + R10 + R12
+        ocid, ocst, omem = o.cell_list(oshift)
+        assert np.array_equal(cid, ocid) and np.array_equal(cst, ocst) and np.array_equal(mem, omem)
+    # after some sweeps (off-lattice state, cell-sorted source order inside the library)
+    g.sweep(3)
+    pos, quat = g.get_state()
+    o.set_state(pos, quat)
+    for t in (3, 4, 99):
+        cid, cst, mem, shift, perm = g.cell_list(t)
+        oshift, operm = o.sweep_header(t)
+        ocid, ocst, omem = o.cell_list(oshift)
+        assert np.array_equal(shift[: w.dim], oshift[: w.dim]) and np.array_equal(perm, operm)
+        assert np.array_equal(cid, ocid) and np.array_equal(cst, ocst) and np.array_equal(mem, omem)
+    p2, q2 = g.get_state()   # building lists must not change the state
+    assert np.array_equal(p2, pos) and np.array_equal(q2, quat)
+
+
+def lockstep(w, n_sweeps, seed=1):
+    """O8: run the GPU one sweep at a time with the trace on; the oracle follows."""
+    g, o = gpu(w, seed), orc(w, seed)
+    g.enable_trace(True)
+    stats = {"marginal": 0, "hard": 0, "compared": 0, "trials": 0}
+    for s in range(n_sweeps):
+        g.sweep(1)
+        tr = g.read_trace()
+        res = o.sweep(follow=tr, follow_tol=MARGIN_TOL)
+        f = res["follow"]
+        stats["marginal"] += f["marginal"]; stats["hard"] += f["hard_mismatch"]; stats["compared"] += f["compared"]
+        assert f["hard_mismatch"] == 0, (s, f)
+        gp, gq = g.get_state()
+        op, oq = o.get_state()
+        assert np.array_equal(gp, op), f"sweep {s}: positions differ"          # single-fmaf translations: bit-exact
+        assert np.max(np.abs(gq.astype(np.float64) - oq.astype(np.float64))) < 1e-5
+        # the oracle adopts the GPU's quaternions so that ulp-level differences cannot accumulate (O8)
+        o.set_state(op, gq)
+    gc, oc = g.counters(), o.counters()
+    stats["trials"] = gc["trials"]
+    for k in ("trans_acc", "trans_rej_overlap", "trans_rej_cell", "rot_acc", "rot_rej_overlap", "trials", "sweeps"):
+        assert gc[k] == oc[k], (k, gc, oc)
+    assert gc["sweep_counter"] == n_sweeps
+    assert g.count_overlaps() == 0
+    return stats, g, o
+
+
+@pytest.mark.parametrize("name,n", [("disks_24", 10), ("pentagons_24", 10), ("cubes_7", 10),
+                                    ("k0_disks", 10), ("k1_pentagons", 10), ("cubes_12", 4)])
+def test_first_sweeps_lockstep_with_oracle(name, n):
+    w = CASES[name]()
+    stats, g, o = lockstep(w, n)
+    assert stats["compared"] == n * g.C * w.n_select
+    # P11: marginal trials should be of order 1e-4 of all trials or fewer
+    assert stats["marginal"] <= max(3, 2e-3 * stats["trials"]), stats
+    if w.N <= 2000:
+        assert o.count_overlaps_bruteforce() == 0
+    print(name, stats)
+
+
+@pytest.mark.parametrize("name", ["disks_24", "pentagons_24", "cubes_7"])
+def test_multi_sweep_call_equals_single_sweep_calls(name):
+    w = CASES[name]()
+    a, b = gpu(w), gpu(w)
+    a.sweep(6)
+    for _ in range(6):
+        b.sweep(1)
+    pa, qa = a.get_state(); pb, qb = b.get_state()
+    assert np.array_equal(pa, pb) and np.array_equal(qa, qb)
+    assert a.counters() == b.counters()
+
+
+def test_restart_from_state_and_sweep_counter():
+    w = wl.pentagons(24)
+    a = gpu(w)
+    a.sweep(4)
+    p4, q4 = a.get_state()
+    a.sweep(3)
+    p7, q7 = a.get_state()
+    w2 = wl.pentagons(24)
+    w2.pos4, w2.quat4 = p4.copy(), q4.copy()
+    b = gpu(w2)
+    b.set_sweep_counter(4)
+    b.sweep(3)
+    pb, qb = b.get_state()
+    assert np.array_equal(p7, pb) and np.array_equal(q7, qb)
+
+
+@pytest.mark.parametrize("name", ["disks_24", "pentagons_24", "cubes_7"])
+def test_count_overlaps_matches_bruteforce_on_planted_overlaps(name):
+    w = CASES[name]()
+    rng = np.random.default_rng(5)
+    pos, quat = w.pos4.copy(), w.quat4.copy()
+    L = np.array(w.L)
+    for i in rng.choice(w.N, size=12, replace=False):      # push a dozen particles into their neighbours
+        pos[i, : w.dim] += rng.uniform(-0.45, 0.45, size=w.dim).astype(np.float32)
+    pos[:, : w.dim] = ((pos[:, : w.dim] + L / 2) % L - L / 2).astype(np.float32)
+    w.pos4, w.quat4 = pos, quat
+    g, o = gpu(w), orc(w)
+    n = o.count_overlaps_bruteforce()
+    assert n > 0 and g.count_overlaps() == n
+
+
+def test_edge_cases_small_and_sparse():
+    # one particle, many empty cells, minimal 4x4 grid, large n_select
+    pos = np.zeros((1, 4), np.float32); quat = np.zeros((1, 4), np.float32); quat[:, 0] = 1
+    w = wl.Workload(name="one", dim=2, N=1, L=(4.2, 4.2), kind=wl.KIND_DISK, diameter=1.0, verts=None, d=0.3, a=0.0,
+                    n_select=37, sweeps=1, pos4=pos, quat4=quat)
+    stats, g, o = lockstep(w, 5)
+    assert list(g.n[:2]) == [4, 4] and stats["trials"] == 5 * 37
+    # two pentagons in a box where they keep meeting across the periodic seam
+    pos = np.zeros((2, 4), np.float32); pos[0, :2] = [-2.0, 0.1]; pos[1, :2] = [2.0, -0.1]
+    quat = np.zeros((2, 4), np.float32); quat[:, 0] = 1
+    w = wl.Workload(name="two", dim=2, N=2, L=(5.0, 5.0), kind=wl.KIND_POLYGON, diameter=0.0, verts=wl.regular_polygon(5, 0.5),
+                    d=0.4, a=0.5, n_select=8, sweeps=1, pos4=pos, quat4=quat)
+    stats, g, o = lockstep(w, 10)
+    c = g.counters()
+    assert c["trans_rej_overlap"] + c["rot_rej_overlap"] > 0      # they do collide through the seam
+    # irregular convex polygon with a vertex count that has no unrolled kernel (runtime-NV path)
+    rng = np.random.default_rng(1)
+    ang = np.sort(rng.uniform(0, 2 * np.pi, 7)); ang[0] = 0.1
+    verts = 0.5 * np.stack([np.cos(ang), np.sin(ang)], axis=1)
+    base = wl.disks(12, spacing=1.25)
+    w = wl.Workload(name="hept", dim=2, N=base.N, L=base.L, kind=wl.KIND_POLYGON, diameter=0.0, verts=verts, d=0.12, a=0.3,
+                    n_select=4, sweeps=1, pos4=base.pos4, quat4=base.quat4)
+    lockstep(w, 6)
+    # tetrahedra (generic polyhedron path with 4 vertices)
+    tet = 0.45 * np.array([[1, 1, 1], [1, -1, -1], [-1, 1, -1], [-1, -1, 1]], dtype=np.float64)
+    base = wl.cubes(6)
+    quat = np.zeros((base.N, 4), np.float32); quat[:, 0] = 1
+    w = wl.Workload(name="tet", dim=3, N=base.N, L=base.L, kind=wl.KIND_POLYHEDRON, diameter=0.0, verts=tet, d=0.15, a=0.3,
+                    n_select=4, sweeps=1, pos4=base.pos4, quat4=quat)
+    lockstep(w, 6)
+
+
+def test_empty_system():
+    w = wl.Workload(name="none", dim=2, N=0, L=(8.0, 8.0), kind=wl.KIND_DISK, diameter=1.0, verts=None, d=0.1, a=0.0,
+                    n_select=4, sweeps=1, pos4=np.zeros((0, 4), np.float32), quat4=np.zeros((0, 4), np.float32))
+    g = gpu(w)
+    g.sweep(3)
+    assert g.counters()["trials"] == 0 and g.count_overlaps() == 0
+
+
+def test_sweep_host_round_trip():
+    import torch
+    w = wl.pentagons(24)
+    a = gpu(w)
+    a.sweep(5)
+    pa, qa = a.get_state()
+    b = gpu(w)
+    hp = torch.from_numpy(w.pos4.copy()).pin_memory(); hq = torch.from_numpy(w.quat4.copy()).pin_memory()
+    op = torch.empty_like(hp).pin_memory(); oq = torch.empty_like(hq).pin_memory()
+    c = b.sweep_host(hp, hq, 5, op, oq)
+    assert np.array_equal(op.numpy(), pa) and np.array_equal(oq.numpy(), qa)
+    assert c["trials"] == a.counters()["trials"]
