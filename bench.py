@@ -1,0 +1,386 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the checkerboard Metropolis sweep (hpmc_sweep) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config k] [--impl reference]
+
+A "step" is ONE hpmc_sweep(1): grid shift + cell-list build + all 2^d colour passes (every S:8(a) row) over
+the whole synthetic system.  The default workload is BASELINE.json configs[2] (1 048 576 pentagons, the
+"GPU-saturating size" north_star quotes the metric on); configs[1] (4096 pentagons) is timed as well and
+reported under "also".  Prints ONE JSON line (rank 0).  See DESIGN.md section 8 for every definition.
+
+N > 1: the path does not shard in this build (one GPU per system, BASELINE.json north_star) -> N independent
+replicas with seeds 1..N, no data-path collective; `value` = trials of all replicas / max-over-ranks time.
+
+--impl reference: the oracle (oracle/, serial fp64 C) timed on the host cores; see DESIGN.md section 8.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_1509_04692_b200 import workloads as wl  # noqa: E402
+
+METRIC = "trial_moves_per_sec"
+UNIT = "trial moves/s"
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # SMs x FP32 lanes x 2 (FMA) x max SM clock
+HBM_FALLBACK_GBS = 6650.0                               # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
+
+# Algorithmic work per trial (tariff of SURVEY.md 8(d) x the oracle's O7 work counters on
+# the melted state of each workload).  flops per trial, and state bytes per particle.
+ALGO = {
+    # kind: (flops per trial, state bytes S per particle)
+    wl.KIND_DISK: (10 + 8 + 8 * 4.08, 16),
+    wl.KIND_POLYGON: (20 + 4 + 8 * 6.94 + 1.83 * 180.0, 32),
+    wl.KIND_POLYHEDRON: (35 + 6 + 11 * 68.0 + 8.12 * 1500.0, 32),
+}
+
+
+def algorithmic_bytes_per_sweep(w, C, accepted_per_sweep):
+    """B_sweep of SURVEY.md 8(d): N(32 + 2S + ncol S) + 16 C + S T_acc."""
+    S = ALGO[w.kind][1]
+    ncol = 1 << w.dim
+    return w.N * (32 + 2 * S + ncol * S) + 16 * C + S * accepted_per_sweep
+
+
+def colour_pass_bytes(w, C, accepted_per_sweep):
+    """Bytes one colour-pass launch must move: all state once + CSR offsets + accepted write-backs."""
+    S = ALGO[w.kind][1]
+    ncol = 1 << w.dim
+    return w.N * S + 8 * C / ncol + S * accepted_per_sweep / ncol
+
+
+def hbm_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured"
+        except Exception:
+            pass
+    return HBM_FALLBACK_GBS, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons sampled every 200 ms during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200",
+                                       "-i", str(index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        time.sleep(0.25)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def time_gpu(w, seed, device, steps, warmup, flush, dist_ctx):
+    """W untimed + K timed hpmc_sweep(1) steps on one replica; returns a dict of raw measurements."""
+    import torch
+    from paper_1509_04692_b200 import binding as hb
+    g = hb.from_workload(w, seed=seed, device=device)
+    assert g.count_overlaps() == 0, "initial state has overlaps"
+    g.sweep(w.warmup_sweeps)                       # melt the lattice (setup), untimed
+    stream = g.stream
+    fbuf = torch.empty(256 << 20, dtype=torch.uint8, device=device) if flush else None
+
+    def one_step():
+        if fbuf is not None:
+            fbuf.add_(1)                           # 256 MiB read+write > 126 MB L2: evicts the state
+        g.sweep(1)
+
+    for _ in range(max(warmup, 3)):
+        one_step()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    g.reset_counters()
+    g.set_profile(True)
+    l0 = g.launch_count()
+    dist_ctx.barrier(); torch.cuda.synchronize(device)
+    sampler = ClockSampler(torch.device(device).index or 0) if dist_ctx.rank == 0 else None
+    t_wall = time.perf_counter()
+    for s, e in ev:
+        if fbuf is not None:
+            fbuf.add_(1)
+        s.record(stream)
+        g.sweep(1)
+        e.record(stream)
+    torch.cuda.synchronize(device); dist_ctx.barrier()
+    t_wall = time.perf_counter() - t_wall
+    clocks = sampler.stop() if sampler else None
+    ms = float(sum(s.elapsed_time(e) for s, e in ev))
+    prof = g.get_profile(); g.set_profile(False)
+    c = g.counters()
+    launches = g.launch_count() - l0
+    assert g.count_overlaps() == 0, "overlaps after the timed window"
+    return dict(g=g, ms=ms, wall_s=t_wall, counters=c, prof=prof, launches=launches, clocks=clocks)
+
+
+def time_e2e(g, w, steps, device):
+    """The same step through hpmc_sweep_host: pinned HOST state in, one sweep, state + counters out."""
+    import torch
+    p, q = g.get_state()
+    hp = [torch.from_numpy(p.copy()).pin_memory(), torch.empty(w.N, 4).pin_memory()]
+    hq = [torch.from_numpy(q.copy()).pin_memory(), torch.empty(w.N, 4).pin_memory()]
+    g.sweep_host(hp[0], hq[0], 1, hp[1], hq[1])      # warm
+    g.reset_counters()
+    torch.cuda.synchronize(device)
+    t = time.perf_counter()
+    trials = 0
+    cur = 1
+    for _ in range(steps):
+        c = g.sweep_host(hp[cur], hq[cur], 1, hp[1 - cur], hq[1 - cur])
+        cur = 1 - cur
+    torch.cuda.synchronize(device)
+    t = time.perf_counter() - t
+    trials = c["trials"]                              # counters accumulate over the calls
+    nbytes = 2 * w.N * 16
+    return dict(seconds=t, trials=trials, h2d=nbytes, d2h=nbytes + 56)
+
+
+def oracle_rate(w_sample, sweeps, seed=1):
+    from oracle import hpmc_oracle as ho
+    o = ho.Oracle(w_sample.dim, w_sample.L, w_sample.kind, w_sample.N, seed, diameter=w_sample.diameter, verts=w_sample.verts)
+    o.set_moves(w_sample.d, w_sample.a, w_sample.n_select)
+    o.set_state(w_sample.pos4, w_sample.quat4)
+    t = time.perf_counter()
+    o.sweeps(sweeps)
+    t = time.perf_counter() - t
+    return o.counters()["trials"], t, o
+
+
+def sample_of(k, n_lat):
+    """A smaller system at the same state point (same lattice recipe, density, shape, moves) as config k."""
+    if k == 0:
+        return wl.disks(n_lat)
+    if k == 3:
+        return wl.cubes(n_lat)
+    return wl.pentagons(n_lat, name=f"pentagons_{n_lat * n_lat}_sample")
+
+
+class Dist:
+    def __init__(self, n):
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        self.on = self.world > 1
+        if self.on:
+            import torch
+            import torch.distributed as dist
+            torch.cuda.set_device(self.local)
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            dist.init_process_group("nccl", device_id=torch.device(f"cuda:{self.local}"))
+            self.dist = dist
+
+    def barrier(self):
+        if self.on:
+            self.dist.barrier()
+
+    def reduce(self, x, op):
+        if not self.on:
+            return x
+        import torch
+        t = torch.tensor([float(x)], dtype=torch.float64, device=f"cuda:{self.local}")
+        self.dist.all_reduce(t, op=getattr(self.dist.ReduceOp, op))
+        return float(t.item())
+
+    def close(self):
+        if self.on:
+            self.dist.destroy_process_group()
+
+
+def run_reference(args):
+    """The oracle as it stands on the host cores: each step = one oracle sweep of a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    k = args.config
+    full = wl.config(k) if k in (0, 1, 3) else None
+    total_steps = args.steps + args.warmup
+    # size the sample so that the whole run stays within ~2 minutes at the oracle's ~0.5 M pentagon trials/s
+    budget_trials = {0: 3.0e6, 1: 0.6e6, 2: 0.6e6, 3: 0.04e6, 4: 0.6e6}[k] * 100.0
+    per_step = budget_trials / total_steps
+    if k in (1, 2, 4):
+        n_full = {1: 64, 2: 1024, 4: 4096}[k]
+        n_lat = int(min(n_full, max(32, np.sqrt(per_step / 4.0)))) // 2 * 2
+        ws = sample_of(k, n_lat)
+    elif k == 0:
+        n_lat = int(min(64, max(16, np.sqrt(per_step / 4.0)))) // 2 * 2
+        ws = sample_of(0, n_lat)
+    else:
+        n_lat = int(min(32, max(6, (per_step / 1.3) ** (1.0 / 3.0))))
+        ws = sample_of(3, n_lat)
+    from oracle import hpmc_oracle as ho
+    o = ho.Oracle(ws.dim, ws.L, ws.kind, ws.N, 1, diameter=ws.diameter, verts=ws.verts)
+    o.set_moves(ws.d, ws.a, ws.n_select)
+    o.set_state(ws.pos4, ws.quat4)
+    o.sweeps(args.warmup)
+    o.reset_counters()
+    t = time.perf_counter()
+    o.sweeps(args.steps)
+    t = time.perf_counter() - t
+    trials = o.counters()["trials"]
+    v = trials / t
+    wname = wl.config(k).name if full is not None else {2: "k2_pentagons_1M", 4: "k4_pentagons_16M"}[k]
+    sample = f"{ws.name}: N={ws.N} particles at the state point of {wname}; {args.steps} oracle sweeps after {args.warmup} warm-up sweeps"
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wname, "sample": sample},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "particle_sweeps_per_sec": ws.N * args.steps / t}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--config", type=int, default=2, choices=[0, 1, 2, 3, 4])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-flush", action="store_true", help="do not evict L2 between steps (L2-resident number)")
+    ap.add_argument("--no-extras", action="store_true", help="skip e2e, cpu_baseline and the small-system line")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        args.steps = 20 if args.steps is None else args.steps
+        args.warmup = 5 if args.warmup is None else args.warmup
+        run_reference(args)
+        return
+    args.steps = {0: 500, 1: 500, 2: 200, 3: 200, 4: 30}[args.config] if args.steps is None else args.steps
+    args.warmup = {0: 50, 1: 50, 2: 20, 3: 20, 4: 5}[args.config] if args.warmup is None else args.warmup
+
+    import torch
+    from paper_1509_04692_b200 import build as hbuild
+    hbuild.build()                                   # no-op when the in-tree libhpmc.so is current
+    D = Dist(args.gpus)
+    device = f"cuda:{D.local}"
+    torch.cuda.set_device(D.local)
+    k = args.config
+    w = wl.config(k, seed=1 + D.rank)                # replica r: orientation seed and Philox seed 1 + r
+    flush = not args.no_flush
+    r = time_gpu(w, 1 + D.rank, device, args.steps, args.warmup, flush, D)
+    g = r["g"]
+    t_max = D.reduce(r["ms"], "MAX") * 1e-3
+    trials_all = D.reduce(r["counters"]["trials"], "SUM")
+    launches_all = D.reduce(r["launches"], "SUM")
+    value = trials_all / t_max
+    acc = r["counters"]["trans_acc"] + r["counters"]["rot_acc"]
+    trials = r["counters"]["trials"]
+
+    # roofline of the dominant kernel (the colour pass): DESIGN.md section 7
+    prof = r["prof"]
+    colour_ms = prof["colour_ms"] / max(prof["colour_n"], 1)
+    trials_per_launch = trials / max(prof["colour_n"], 1)
+    acc_per_sweep = acc / args.steps
+    hbm, hbm_src = hbm_peak()
+    bytes_launch = colour_pass_bytes(w, g.C, acc_per_sweep)
+    flops_launch = ALGO[w.kind][0] * trials_per_launch
+    t_hbm = bytes_launch / (hbm * 1e9)
+    t_alu = flops_launch / (FP32_PEAK_TFLOPS * 1e12)
+    if t_hbm >= t_alu:
+        roof = {"bound": "hbm", "achieved": bytes_launch / (colour_ms * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s"}
+    else:
+        roof = {"bound": "alu", "achieved": flops_launch / (colour_ms * 1e-3) / 1e12, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s"}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof.update({"traffic": None, "kernel": "k_sweep_colour", "avg_launch_ms": colour_ms, "launches_timed": prof["colour_n"],
+                 "peak_source": f"{hbm_src} hbm_gbs (MEASURED_PEAKS.json)" if roof["bound"] == "hbm" else "148 SM x 128 lanes x 2 x 1.965 GHz",
+                 "algorithmic_bytes_per_launch": bytes_launch, "algorithmic_flops_per_launch": flops_launch,
+                 "kernel_share_of_step": prof["colour_ms"] / r["ms"], "build_share_of_step": prof["build_ms"] / r["ms"],
+                 "sweep_frac": max(algorithmic_bytes_per_sweep(w, g.C, acc_per_sweep) / (hbm * 1e9),
+                                   ALGO[w.kind][0] * trials / args.steps / (FP32_PEAK_TFLOPS * 1e12)) / (r["ms"] * 1e-3 / args.steps)})
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "N": w.N, "cells": g.C, "n_select": w.n_select, "d": w.d, "a": w.a,
+                       "step": "one hpmc_sweep(1): shift + cell list + all colour passes",
+                       "melt_sweeps_before_warmup": w.warmup_sweeps,
+                       "l2": "flushed between steps (256 MiB read+write)" if flush else "not flushed (state L2-resident)",
+                       "parallelism": "1 gpu" if args.gpus == 1 else f"{args.gpus} independent replicas (no collective)",
+                       "notes": w.notes},
+            "particle_sweeps_per_sec": D.reduce(w.N, "SUM") * args.steps / t_max,
+            "acceptance": acc / max(trials, 1), "trials_per_step": trials / args.steps,
+            "gpu_launches": int(launches_all), "roofline": roof, "clocks": r["clocks"]}
+
+    if not args.no_extras:
+        e = time_e2e(g, w, min(args.steps, 20), device)
+        e_t = D.reduce(e["seconds"], "MAX")
+        e_trials = D.reduce(e["trials"], "SUM")
+        line["e2e"] = {"value": e_trials / e_t, "unit": UNIT, "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"],
+                       "steps": min(args.steps, 20), "call": "hpmc_sweep_host(n=1), pinned host buffers"}
+    del g, r
+    if not args.no_extras and D.rank == 0:
+        if args.gpus == 1:
+            # the oracle as it stands, one host thread, on a bounded sample of the same workload
+            n_lat = {0: 64, 1: 64, 2: 256, 3: 8, 4: 256}[k]
+            ws = sample_of(k, n_lat)
+            ns = {0: 100, 1: 100, 2: 40, 3: 20, 4: 40}[k]
+            tr, ts, _ = oracle_rate(ws, ns)
+            line["cpu_baseline"] = {"value": tr / ts, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": ts,
+                                    "host_cores_available": os.cpu_count(),
+                                    "sample": f"{ws.name}: N={ws.N} at the state point of {w.name}, {ns} sweeps from the lattice start"}
+        if k == 2:
+            # north_star also quotes 4096 pentagons: launch-bound, timed as hpmc_sweep(100) calls, L2-resident by size
+            w1 = wl.config(1)
+            from paper_1509_04692_b200 import binding as hb
+            g1 = hb.from_workload(w1, seed=1, device=device)
+            g1.sweep(w1.warmup_sweeps)
+            g1.reset_counters()
+            s, e2 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize(device)
+            s.record(g1.stream); g1.sweep(1000); e2.record(g1.stream)
+            torch.cuda.synchronize(device)
+            ms1 = s.elapsed_time(e2)
+            c1 = g1.counters()
+            assert g1.count_overlaps() == 0
+            line["also"] = {"k1_pentagons_4096": {"value": c1["trials"] / (ms1 * 1e-3), "unit": UNIT, "sweeps": 1000,
+                                                  "ms_per_sweep": ms1 / 1000, "particle_sweeps_per_sec": w1.N * 1000 / (ms1 * 1e-3),
+                                                  "l2": "state is 0.26 MB: resident by size"}}
+    if D.rank == 0:
+        print(json.dumps(line), flush=True)
+    D.close()
+
+
+if __name__ == "__main__":
+    main()

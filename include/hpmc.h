@@ -132,6 +132,13 @@ int hpmc_get_cell_list(hpmc_ctx* ctx, uint64_t t, int32_t* d_cell_start, int32_t
 int hpmc_sweep_host(hpmc_ctx* ctx, const float* h_pos4, const float* h_quat4, int64_t n,
                     float* h_pos4_out, float* h_quat4_out, hpmc_counters* h_counters);
 
+/* Per-kernel device timing for the roofline report (S:8(d)).  While on, CUDA events on the context's stream
+ * bracket every cell-list build (rows a1-a3) and every colour-pass launch (rows a4-a11).  hpmc_set_profile
+ * resets the sums; hpmc_get_profile synchronises and returns total milliseconds and number of bracketed
+ * regions per class since then.  Any out pointer may be NULL.                                          */
+int hpmc_set_profile(hpmc_ctx* ctx, int on);
+int hpmc_get_profile(hpmc_ctx* ctx, double* h_ms_build, int64_t* h_n_build, double* h_ms_colour, int64_t* h_n_colour);
+
 /* Launch bookkeeping for bench.py: kernels launched by this context so far.                        */
 int64_t hpmc_launch_count(const hpmc_ctx* ctx);
 

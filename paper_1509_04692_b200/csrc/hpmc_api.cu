@@ -5,6 +5,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "../../include/hpmc.h"
 #include "cell_list.cuh"
@@ -49,6 +50,15 @@ struct hpmc_ctx {
 
     uint2* trace = nullptr;
     int64_t trace_words = 0;
+
+    // optional per-kernel device timing (hpmc_set_profile): event pairs around the cell-list build (class 0)
+    // and around every colour-pass launch (class 1)
+    bool profile = false;
+    std::vector<cudaEvent_t> ev_pool;
+    std::vector<int> ev_class;     // one per recorded pair
+    size_t ev_used = 0;            // events handed out (2 per pair)
+    double prof_ms[2] = {0.0, 0.0};
+    int64_t prof_n[2] = {0, 0};
 };
 
 namespace {
@@ -200,6 +210,45 @@ void refresh_sweep_range(hpmc_ctx* c)
     c->sf.dmax2 = (float)(rr * rr);
 }
 
+// fold the recorded event pairs into the per-class sums (synchronises the stream)
+bool profile_fold(hpmc_ctx* c)
+{
+    if (c->ev_class.empty()) return true;
+    if (!cuda_ok(c, cudaStreamSynchronize(c->stream), "profile/sync")) return false;
+    for (size_t i = 0; i < c->ev_class.size(); ++i) {
+        float ms = 0.f;
+        if (!cuda_ok(c, cudaEventElapsedTime(&ms, c->ev_pool[2 * i], c->ev_pool[2 * i + 1]), "profile/elapsed")) return false;
+        c->prof_ms[c->ev_class[i]] += (double)ms;
+        c->prof_n[c->ev_class[i]] += 1;
+    }
+    c->ev_class.clear();
+    c->ev_used = 0;
+    return true;
+}
+
+struct ProfileScope {
+    hpmc_ctx* c;
+    bool on;
+    ProfileScope(hpmc_ctx* ctx, int cls) : c(ctx), on(ctx->profile && !ctx->cuda_failed)
+    {
+        if (!on) return;
+        if (c->ev_class.size() >= 4096) profile_fold(c);
+        while (c->ev_pool.size() < c->ev_used + 2) {
+            cudaEvent_t e;
+            if (cudaEventCreate(&e) != cudaSuccess) { on = false; return; }
+            c->ev_pool.push_back(e);
+        }
+        c->ev_class.push_back(cls);
+        cudaEventRecord(c->ev_pool[c->ev_used], c->stream);
+    }
+    ~ProfileScope()
+    {
+        if (!on) return;
+        cudaEventRecord(c->ev_pool[c->ev_used + 1], c->stream);
+        c->ev_used += 2;
+    }
+};
+
 #define LAUNCH_CHECK(c, what)                                      \
     do {                                                           \
         ++(c)->launches;                                           \
@@ -209,6 +258,7 @@ void refresh_sweep_range(hpmc_ctx* c)
 // build the cell list of the current state into buffer 1-cur and flip.  mode as in k_prepare.
 int build_cell_list(hpmc_ctx* c, int mode, unsigned long long t_override)
 {
+    ProfileScope prof(c, 0);
     const GridParams& g = c->g;
     const int TB = 256;
     const float4* src_pos = c->state_in_bound ? c->d_pos_bound : c->pos[c->cur];
@@ -249,12 +299,13 @@ void launch_colour(hpmc_ctx* c, int ci)
     const GridParams& g = c->g;
     const int nactive = (g.n[0] / 2) * (g.n[1] / 2) * (g.dim == 3 ? g.n[2] / 2 : 1);
     const int TB = 128;
-    k_sweep_colour<KIND, NV><<<(nactive + TB - 1) / TB, TB, 0, c->stream>>>(g, c->mv, c->sf, c->ctrl, ci, c->pos[c->cur], c->quat[c->cur],
+    k_sweep_colour<KIND, NV><<<(nactive + TB - 1) / TB, TB, 0, c->stream>>>(g, c->mv, c->sf, c->sd, c->ctrl, ci, c->pos[c->cur], c->quat[c->cur],
                                                                            c->tag[c->cur], c->cell_start, c->k0, c->k1, c->trace);
 }
 
 int launch_colour_dispatch(hpmc_ctx* c, int ci)
 {
+    ProfileScope prof(c, 1);
     switch (c->sf.kind) {
         case kKindDisk: launch_colour<kKindDisk, 0>(c, ci); break;
         case kKindPolygon:
@@ -331,6 +382,8 @@ int hpmc_create(const hpmc_box* box, const hpmc_shape* shape, int64_t N, uint64_
 
 int hpmc_destroy(hpmc_ctx* c)
 {
+    if (c)
+        for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return HPMC_OK;
 }
@@ -354,7 +407,7 @@ int hpmc_bind(hpmc_ctx* c, float* d_pos4, float* d_quat4, void* d_workspace, siz
 {
     if (!c) return HPMC_E_ARG;
     if (c->cuda_failed) return HPMC_E_CUDA;
-    if (!d_pos4 || !d_quat4 || !d_workspace) return fail(c, HPMC_E_ARG, "NULL device pointer");
+    if (((!d_pos4 || !d_quat4) && c->g.N > 0) || !d_workspace) return fail(c, HPMC_E_ARG, "NULL device pointer");
     const Layout L = layout_of(c);
     if (bytes < L.total) return fail(c, HPMC_E_UNBOUND, "workspace smaller than hpmc_workspace_bytes()");
     if (((uintptr_t)d_workspace & 255u) || ((uintptr_t)d_pos4 & 15u) || ((uintptr_t)d_quat4 & 15u))
@@ -550,6 +603,29 @@ int hpmc_sweep_host(hpmc_ctx* c, const float* h_pos4, const float* h_quat4, int6
     hpmc_counters tmp;
     rc = hpmc_get_state(c, nullptr, nullptr, h_counters ? h_counters : &tmp, nullptr);  // also synchronises
     return rc;
+}
+
+int hpmc_set_profile(hpmc_ctx* c, int on)
+{
+    if (!c) return HPMC_E_ARG;
+    if (c->cuda_failed) return HPMC_E_CUDA;
+    if (!profile_fold(c)) return HPMC_E_CUDA;
+    c->profile = on != 0;
+    c->prof_ms[0] = c->prof_ms[1] = 0.0;
+    c->prof_n[0] = c->prof_n[1] = 0;
+    return HPMC_OK;
+}
+
+int hpmc_get_profile(hpmc_ctx* c, double* h_ms_build, int64_t* h_n_build, double* h_ms_colour, int64_t* h_n_colour)
+{
+    if (!c) return HPMC_E_ARG;
+    if (c->cuda_failed) return HPMC_E_CUDA;
+    if (!profile_fold(c)) return HPMC_E_CUDA;
+    if (h_ms_build) *h_ms_build = c->prof_ms[0];
+    if (h_n_build) *h_n_build = c->prof_n[0];
+    if (h_ms_colour) *h_ms_colour = c->prof_ms[1];
+    if (h_n_colour) *h_n_colour = c->prof_n[1];
+    return HPMC_OK;
 }
 
 int64_t hpmc_launch_count(const hpmc_ctx* c) { return c ? c->launches : 0; }

@@ -148,26 +148,32 @@ __device__ __forceinline__ V3<T> closest_on_triangle(const V3<T>& a, const V3<T>
     return a + (vb * denom) * ab + (vc * denom) * ac;
 }
 
-// Returns true iff a direction was found along which the support functions separate the pair by >= eps.
-// Everything else (origin enclosed, converged with distance < eps, no numerical progress, iteration cap)
-// returns false = treat as overlap (conservative, R-poly).
+// GJK verdicts.  kGjkSeparated: a direction was found along which the support functions separate the pair by
+// >= eps (a certificate evaluated directly from the support points).  kGjkOverlap: the origin lies inside a
+// tetrahedron of Minkowski-difference points, farther than `deep` from each of its faces, so the interiors
+// intersect by at least `deep`.  kGjkUnsure: everything else (origin enclosed but close to a face, converged with
+// distance < eps, no numerical progress, repeated support point, iteration cap).  Near contact the GJK direction
+// v is the small difference of O(1) vectors, so in fp32 its relative error ~1e-7/|v| makes the certificate
+// unreliable for gaps below ~1e-3: the fp32 caller re-runs kGjkUnsure pairs in fp64 (mixed precision);
+// the fp64 caller treats kGjkUnsure as overlap (conservative, R-poly).
+constexpr int kGjkSeparated = 1, kGjkOverlap = 0, kGjkUnsure = -1;
 template <typename T>
-__device__ bool gjk_separated(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T eps)
+__device__ int gjk_classify(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T eps, T deep)
 {
     const T tiny = (sizeof(T) == 4) ? (T)1e-14 : (T)1e-28;
     const T reltol = (sizeof(T) == 4) ? (T)1e-6 : (T)1e-13;
     V3<T> v = r;  // a point of B (-) A (both body origins are interior points)
     T vv = dot(v, v);
-    if (vv < tiny) return false;
+    if (vv < tiny) return kGjkUnsure;
     V3<T> W[4];
     int nW = 0;
     for (int iter = 0; iter < 40; ++iter) {
         const V3<T> w = support_minkowski(S, Rm, r, V3<T>{-v.x, -v.y, -v.z});
         const T vw = dot(v, w);
-        if (vw >= 0 && vw * vw >= eps * eps * vv) return true;          // certificate: v^.w >= eps
-        if (iter > 0 && vv - vw <= reltol * vv) return false;           // converged: distance |v| < eps
+        if (vw >= 0 && vw * vw >= eps * eps * vv) return kGjkSeparated;   // certificate: v^.w >= eps
+        if (iter > 0 && vv - vw <= reltol * vv) return kGjkUnsure;           // converged: distance |v| < eps
         for (int i = 0; i < nW; ++i)
-            if (W[i].x == w.x && W[i].y == w.y && W[i].z == w.z) return false;  // same support point again
+            if (W[i].x == w.x && W[i].y == w.y && W[i].z == w.z) return kGjkUnsure;  // same support point again
         W[nW++] = w;
         V3<T> vn;
         if (nW == 1) {
@@ -196,6 +202,7 @@ __device__ bool gjk_separated(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T
             T best = (T)3.0e38;
             int bestFace = -1, bestMask = 0;
             V3<T> bestV{0, 0, 0};
+            T minIn = (T)3.0e38;   // min distance from the origin to the faces (when enclosed)
 #pragma unroll
             for (int f = 0; f < 4; ++f) {
                 const V3<T> p = (f == 3) ? b : a;
@@ -205,6 +212,8 @@ __device__ bool gjk_separated(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T
                 const V3<T> nn = cross(q - p, s3 - p);
                 const T sp = -dot(nn, p);          // origin side
                 const T sd = dot(nn, o - p);       // opposite-vertex side
+                const T nn2 = dot(nn, nn);
+                if (sp * sd > 0) minIn = min(minIn, fabs(sp) * rsqrt(nn2));
                 if (sp * sd <= 0) {                // outside this face (or degenerate): closest point on it
                     int m;
                     const V3<T> cand = closest_on_triangle(p, q, s3, m);
@@ -212,7 +221,7 @@ __device__ bool gjk_separated(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T
                     if (cc < best) { best = cc; bestFace = f; bestMask = m; bestV = cand; }
                 }
             }
-            if (bestFace < 0) return false;        // origin inside the tetrahedron: overlap
+            if (bestFace < 0) return (minIn > deep) ? kGjkOverlap : kGjkUnsure;   // origin inside the tetrahedron
             const V3<T> p = (bestFace == 3) ? b : a;
             const V3<T> q = (bestFace == 0) ? b : (bestFace == 1) ? c : d;
             const V3<T> s3 = (bestFace == 0) ? c : (bestFace == 1) ? d : (bestFace == 2) ? b : c;
@@ -224,12 +233,12 @@ __device__ bool gjk_separated(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T
             vn = bestV;
         }
         const T vvn = dot(vn, vn);
-        if (vvn < tiny) return false;              // origin on the simplex: touching or inside
-        if (iter > 0 && vvn >= vv) return false;   // no numerical progress
+        if (vvn < tiny) return kGjkUnsure;              // origin on the simplex: touching or inside
+        if (iter > 0 && vvn >= vv) return kGjkUnsure;   // no numerical progress
         v = vn;
         vv = vvn;
     }
-    return false;
+    return kGjkUnsure;
 }
 
 // rotation matrix (row major) of the unit quaternion (w,x,y,z)
@@ -242,9 +251,9 @@ __device__ __forceinline__ void quat_to_matrix(T w, T x, T y, T z, T* M)
     M[6] = 2 * (xz - wy);     M[7] = 2 * (yz + wx);     M[8] = 1 - 2 * (xx + yy);
 }
 
-// polyhedron pair in A's frame: MA, MB = world rotation matrices of A and B, rw = r_AB (world)
+// polyhedron pair in A's frame: MA, MB = world rotation matrices of A and B, rw = r_AB (world).  GJK verdict.
 template <typename T>
-__device__ __forceinline__ bool polyhedron_overlap(const ShapeT<T>& S, const T* MA, const T* MB, const V3<T>& rw, T eps)
+__device__ __forceinline__ int polyhedron_classify(const ShapeT<T>& S, const T* MA, const T* MB, const V3<T>& rw, T eps, T deep)
 {
     T Rm[9];  // R = MA^T MB takes B's frame into A's frame (q = q_A* q_B)
 #pragma unroll
@@ -253,7 +262,18 @@ __device__ __forceinline__ bool polyhedron_overlap(const ShapeT<T>& S, const T* 
         for (int j = 0; j < 3; ++j) Rm[3 * i + j] = MA[i] * MB[j] + MA[3 + i] * MB[3 + j] + MA[6 + i] * MB[6 + j];
     const V3<T> r{MA[0] * rw.x + MA[3] * rw.y + MA[6] * rw.z, MA[1] * rw.x + MA[4] * rw.y + MA[7] * rw.z,
                   MA[2] * rw.x + MA[5] * rw.y + MA[8] * rw.z};
-    return !gjk_separated(S, Rm, r, eps);
+    return gjk_classify(S, Rm, r, eps, deep);
+}
+
+// fp64 narrow phase from the raw fp32 state: normalised quaternions, exact separation rd (already minimum image)
+__device__ __noinline__ bool polyhedron_overlap_f64(const ShapeD& S, float4 qA, float4 qB, double rx, double ry, double rz, double eps)
+{
+    double MA[9], MB[9];
+    const double na = 1.0 / sqrt((double)qA.x * qA.x + (double)qA.y * qA.y + (double)qA.z * qA.z + (double)qA.w * qA.w);
+    const double nb = 1.0 / sqrt((double)qB.x * qB.x + (double)qB.y * qB.y + (double)qB.z * qB.z + (double)qB.w * qB.w);
+    quat_to_matrix<double>(qA.x * na, qA.y * na, qA.z * na, qA.w * na, MA);
+    quat_to_matrix<double>(qB.x * nb, qB.y * nb, qB.z * nb, qB.w * nb, MB);
+    return polyhedron_classify<double>(S, MA, MB, V3<double>{rx, ry, rz}, eps, 0.0) != kGjkSeparated;
 }
 
 }  // namespace hpmc

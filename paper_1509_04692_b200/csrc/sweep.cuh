@@ -22,6 +22,17 @@ __device__ __forceinline__ float min_image(float xj, float xt, float hi, double 
     return r;
 }
 
+constexpr float kGjkDeepF = 1e-4f;   // fp32 GJK "certainly overlapping" threshold (see overlap.cuh)
+
+// exact minimum-image separation in fp64 from the fp32 coordinates (fallback narrow phase only)
+__device__ __forceinline__ double min_image_d(float xj, float xt, double Ld)
+{
+    double rd = (double)xj - (double)xt;
+    if (rd > 0.5 * Ld) rd -= Ld;
+    else if (rd < -0.5 * Ld) rd += Ld;
+    return rd;
+}
+
 struct TrialState {
     float x, y, z;        // trial position (unwrapped)
     float qw, qx, qy, qz; // trial orientation
@@ -29,8 +40,8 @@ struct TrialState {
 
 // narrow phase of the trial particle A against neighbour B; r = r_B - r_A(trial), already minimum image
 template <int KIND, int NV>
-__device__ __forceinline__ bool narrow_overlap(const ShapeF& S, const TrialState& A, const float* MA, float rx, float ry,
-                                               float rz, const float4& qB, float eps)
+__device__ __forceinline__ bool narrow_overlap(const ShapeF& S, const ShapeD& SD, const TrialState& A, const float* MA, float rx,
+                                               float ry, float rz, const double* rd, const float4& qB, float eps)
 {
     if (KIND == kKindDisk) {
         return true;  // the broad phase already decided: |r|^2 < sigma^2
@@ -41,7 +52,10 @@ __device__ __forceinline__ bool narrow_overlap(const ShapeF& S, const TrialState
     } else {
         float MB[9];
         quat_to_matrix<float>(qB.x, qB.y, qB.z, qB.w, MB);
-        return polyhedron_overlap<float>(S, MA, MB, V3<float>{rx, ry, rz}, eps);
+        const int verdict = polyhedron_classify<float>(S, MA, MB, V3<float>{rx, ry, rz}, eps, kGjkDeepF);
+        if (verdict != kGjkUnsure) return verdict == kGjkOverlap;
+        // near contact: decide in fp64 from the raw fp32 state (mixed precision)
+        return polyhedron_overlap_f64(SD, make_float4(A.qw, A.qx, A.qy, A.qz), qB, rd[0], rd[1], rd[2], (double)eps);
     }
 }
 
@@ -49,7 +63,8 @@ __device__ __forceinline__ bool narrow_overlap(const ShapeF& S, const TrialState
 template <int KIND, int NV>
 __global__ void __launch_bounds__(128)
 k_sweep_colour(const __grid_constant__ GridParams g, const __grid_constant__ MoveParams mv,
-               const __grid_constant__ ShapeF S, Control* __restrict__ ctrl, int colour_index, float4* __restrict__ pos,
+               const __grid_constant__ ShapeF S, const __grid_constant__ ShapeD SD, Control* __restrict__ ctrl, int colour_index,
+               float4* __restrict__ pos,
                float4* __restrict__ quat, const int* __restrict__ tag, const int* __restrict__ cell_start, uint32_t k0,
                uint32_t k1, uint2* __restrict__ trace)
 {
@@ -149,7 +164,13 @@ k_sweep_colour(const __grid_constant__ GridParams g, const __grid_constant__ Mov
                                     if (rx * rx + ry * ry + rz * rz >= S.dmax2) continue;   // a8 circumsphere (R16)
                                     float4 qq = make_float4(1.f, 0.f, 0.f, 0.f);
                                     if (KIND != kKindDisk) qq = quat[q];
-                                    if (narrow_overlap<KIND, NV>(S, A, MA, rx, ry, rz, qq, mv.eps_g)) {
+                                    double rd[3] = {0.0, 0.0, 0.0};
+                                    if (KIND == kKindPolyhedron) {
+                                        rd[0] = min_image_d(xq.x, A.x, g.Ld[0]);
+                                        rd[1] = min_image_d(xq.y, A.y, g.Ld[1]);
+                                        rd[2] = min_image_d(xq.z, A.z, g.Ld[2]);
+                                    }
+                                    if (narrow_overlap<KIND, NV>(S, SD, A, MA, rx, ry, rz, rd, qq, mv.eps_g)) {
                                         overlap = true;
                                         break;
                                     }
@@ -245,7 +266,7 @@ k_count_overlaps(const __grid_constant__ GridParams g, const __grid_constant__ S
                             } else {
                                 double MB[9];
                                 quat_to_matrix<double>(w, x, y, z, MB);
-                                ov = polyhedron_overlap<double>(S, MA, MB, V3<double>{r[0], r[1], r[2]}, 0.0);
+                                ov = polyhedron_classify<double>(S, MA, MB, V3<double>{r[0], r[1], r[2]}, 0.0, 0.0) != kGjkSeparated;
                             }
                         }
                         if (ov) ++found;
