@@ -132,6 +132,12 @@ int hpmc_get_cell_list(hpmc_ctx* ctx, uint64_t t, int32_t* d_cell_start, int32_t
 int hpmc_sweep_host(hpmc_ctx* ctx, const float* h_pos4, const float* h_quat4, int64_t n,
                     float* h_pos4_out, float* h_quat4_out, hpmc_counters* h_counters);
 
+/* Tuning and test knobs; results never depend on them (only speed does).
+ *   "path"     0 = automatic, 1 = per-thread global-memory colour pass, 2 = shared-memory tile colour pass (2-D)
+ *   "tile_cap" upper limit on the particles a tile may stage; tiles above it take the per-thread path
+ *              (tests set 0 to force that fallback everywhere).                                              */
+int hpmc_set_option(hpmc_ctx* ctx, const char* name, int64_t value);
+
 /* Per-kernel device timing for the roofline report (S:8(d)).  While on, CUDA events on the context's stream
  * bracket every cell-list build (rows a1-a3) and every colour-pass launch (rows a4-a11).  hpmc_set_profile
  * resets the sums; hpmc_get_profile synchronises and returns total milliseconds and number of bracketed

@@ -16,7 +16,7 @@ KIND_DISK, KIND_POLYGON, KIND_POLYHEDRON = 0, 1, 2
 # every symbol include/hpmc.h declares (checked by tests/test_abi.py)
 ABI_SYMBOLS = ["hpmc_create", "hpmc_destroy", "hpmc_last_error", "hpmc_get_grid", "hpmc_workspace_bytes", "hpmc_bind",
                "hpmc_set_moves", "hpmc_sweep", "hpmc_count_overlaps", "hpmc_get_state", "hpmc_set_sweep_counter",
-               "hpmc_reset_counters", "hpmc_set_trace", "hpmc_get_cell_list", "hpmc_sweep_host", "hpmc_set_profile",
+               "hpmc_reset_counters", "hpmc_set_trace", "hpmc_get_cell_list", "hpmc_sweep_host", "hpmc_set_option", "hpmc_set_profile",
                "hpmc_get_profile", "hpmc_launch_count"]
 
 
@@ -73,6 +73,7 @@ def load_library():
     L.hpmc_set_trace.argtypes = [vp, vp, C.c_int64]
     L.hpmc_get_cell_list.argtypes = [vp, C.c_uint64, vp, vp, vp, C.POINTER(C.c_float), C.POINTER(C.c_int32)]
     L.hpmc_sweep_host.argtypes = [vp, vp, vp, C.c_int64, vp, vp, C.POINTER(Counters)]
+    L.hpmc_set_option.argtypes = [vp, C.c_char_p, C.c_int64]
     L.hpmc_set_profile.argtypes = [vp, C.c_int]
     L.hpmc_get_profile.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64), C.POINTER(C.c_double), C.POINTER(C.c_int64)]
     L.hpmc_launch_count.argtypes = [vp]; L.hpmc_launch_count.restype = C.c_int64
@@ -212,6 +213,9 @@ class Hpmc:
         self._check(self._lib.hpmc_sweep_host(self._h, h_pos4.data_ptr(), h_quat4.data_ptr(), int(n),
                                               h_pos4_out.data_ptr(), h_quat4_out.data_ptr(), C.byref(c)))
         return c.as_dict()
+
+    def set_option(self, name, value):
+        self._check(self._lib.hpmc_set_option(self._h, name.encode(), int(value)))
 
     def set_profile(self, on=True):
         self._check(self._lib.hpmc_set_profile(self._h, 1 if on else 0))

@@ -12,6 +12,7 @@
 #include "common.cuh"
 #include "overlap.cuh"
 #include "sweep.cuh"
+#include "sweep_tile2d.cuh"
 
 using namespace hpmc;
 
@@ -50,6 +51,10 @@ struct hpmc_ctx {
 
     uint2* trace = nullptr;
     int64_t trace_words = 0;
+
+    // tuning / test knobs (hpmc_set_option)
+    int opt_path = 0;                 // 0 auto, 1 per-thread global path, 2 tile path (2-D only)
+    int opt_tile_cap = 1 << 30;       // staging capacity limit of the tile kernel (tests force the overflow path)
 
     // optional per-kernel device timing (hpmc_set_profile): event pairs around the cell-list build (class 0)
     // and around every colour-pass launch (class 1)
@@ -141,6 +146,7 @@ int build_shape(hpmc_ctx* c, const hpmc_shape* s, int dim)
             rmax = std::fmax(rmax, std::sqrt(D.vx[i] * D.vx[i] + D.vy[i] * D.vy[i] + D.vz[i] * D.vz[i]));
         }
         c->d_max = 2.0 * rmax;  // circumsphere centred on the particle position
+        double r_in = 1e300;    // inscribed radius about the body origin = smallest face/edge offset
         if (poly2) {
             for (int k = 0; k < nv; ++k) {
                 const int k1 = (k + 1) % nv, k2 = (k + 2) % nv;
@@ -152,6 +158,7 @@ int build_shape(hpmc_ctx* c, const hpmc_shape* s, int dim)
                 D.ny[k] = -ex / len;
                 D.fc[k] = D.nx[k] * D.vx[k] + D.ny[k] * D.vy[k];
                 if (!(D.fc[k] > 0.0)) return fail(c, HPMC_E_SHAPE, "the body-frame origin must be inside the polygon");
+                r_in = std::fmin(r_in, D.fc[k]);
             }
         } else {
             // every vertex must be an extreme point and the origin must be interior: for each vertex v there
@@ -177,6 +184,7 @@ int build_shape(hpmc_ctx* c, const hpmc_shape* s, int dim)
                         }
                         if (npos && nneg) continue;
                         ++nplanes;
+                        r_in = std::fmin(r_in, std::fabs(off));
                         // origin strictly inside: on the same side as the other vertices, off the plane
                         const double o = -off;  // n.0 - off
                         if ((npos && !(o > 1e-12)) || (nneg && !(o < -1e-12)))
@@ -188,6 +196,8 @@ int build_shape(hpmc_ctx* c, const hpmc_shape* s, int dim)
             for (int l = 0; l < nv; ++l)
                 if (on_hull[l] < 3) return fail(c, HPMC_E_SHAPE, "every vertex must be a hull vertex (convex polyhedron)");
         }
+        const double din = std::fmax(0.0, 2.0 * r_in - 1e-5);
+        D.din2 = din * din;
     } else
         return fail(c, HPMC_E_SHAPE, "unknown shape kind");
     D.dmax2 = c->d_max * c->d_max;  // the validator is strict: no guard band
@@ -196,6 +206,7 @@ int build_shape(hpmc_ctx* c, const hpmc_shape* s, int dim)
     F.kind = D.kind;
     F.nverts = D.nverts;
     F.diameter = (float)D.diameter;
+    F.din2 = (float)D.din2;
     for (int i = 0; i < kMaxVerts; ++i) {
         F.vx[i] = (float)D.vx[i]; F.vy[i] = (float)D.vy[i]; F.vz[i] = (float)D.vz[i];
         F.nx[i] = (float)D.nx[i]; F.ny[i] = (float)D.ny[i]; F.fc[i] = (float)D.fc[i];
@@ -293,34 +304,55 @@ int build_cell_list(hpmc_ctx* c, int mode, unsigned long long t_override)
     return HPMC_OK;
 }
 
+constexpr int kTileTY = 4;   // warps per CTA of the 2-D tile kernel (tile = 32 x kTileTY active cells)
+
 template <int KIND, int NV>
-void launch_colour(hpmc_ctx* c, int ci)
+bool launch_colour(hpmc_ctx* c, int ci)
 {
     const GridParams& g = c->g;
+    if constexpr (KIND != kKindPolyhedron) {
+      if (g.dim == 2 && c->opt_path != 1) {
+        using TL = Tile2D<kTileTY>;
+        auto kern = k_sweep_tile2d<KIND, NV, kTileTY>;
+        static bool attr_set = false;   // per template instance
+        if (!attr_set) {
+            if (!cuda_ok(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TL::bytes), "tile/attr")) return false;
+            attr_set = true;
+        }
+        const int nax = g.n[0] / 2, nay = g.n[1] / 2;
+        const int tiles = ((nax + kTileW - 1) / kTileW) * ((nay + kTileTY - 1) / kTileTY);
+        kern<<<tiles, TL::NT, TL::bytes, c->stream>>>(g, c->mv, c->sf, c->sd, c->ctrl, ci, c->opt_tile_cap, c->pos[c->cur],
+                                                      c->quat[c->cur], c->tag[c->cur], c->cell_start, c->k0, c->k1, c->trace);
+        return true;
+      }
+    }
     const int nactive = (g.n[0] / 2) * (g.n[1] / 2) * (g.dim == 3 ? g.n[2] / 2 : 1);
     const int TB = 128;
     k_sweep_colour<KIND, NV><<<(nactive + TB - 1) / TB, TB, 0, c->stream>>>(g, c->mv, c->sf, c->sd, c->ctrl, ci, c->pos[c->cur], c->quat[c->cur],
                                                                            c->tag[c->cur], c->cell_start, c->k0, c->k1, c->trace);
+    return true;
 }
 
 int launch_colour_dispatch(hpmc_ctx* c, int ci)
 {
     ProfileScope prof(c, 1);
+    bool ok = true;
     switch (c->sf.kind) {
-        case kKindDisk: launch_colour<kKindDisk, 0>(c, ci); break;
+        case kKindDisk: ok = launch_colour<kKindDisk, 0>(c, ci); break;
         case kKindPolygon:
             switch (c->sf.nverts) {
-                case 3: launch_colour<kKindPolygon, 3>(c, ci); break;
-                case 4: launch_colour<kKindPolygon, 4>(c, ci); break;
-                case 5: launch_colour<kKindPolygon, 5>(c, ci); break;
-                case 6: launch_colour<kKindPolygon, 6>(c, ci); break;
-                case 8: launch_colour<kKindPolygon, 8>(c, ci); break;
-                default: launch_colour<kKindPolygon, 0>(c, ci); break;
+                case 3: ok = launch_colour<kKindPolygon, 3>(c, ci); break;
+                case 4: ok = launch_colour<kKindPolygon, 4>(c, ci); break;
+                case 5: ok = launch_colour<kKindPolygon, 5>(c, ci); break;
+                case 6: ok = launch_colour<kKindPolygon, 6>(c, ci); break;
+                case 8: ok = launch_colour<kKindPolygon, 8>(c, ci); break;
+                default: ok = launch_colour<kKindPolygon, 0>(c, ci); break;
             }
             break;
-        default: launch_colour<kKindPolyhedron, 0>(c, ci); break;
+        default: ok = launch_colour<kKindPolyhedron, 0>(c, ci); break;
     }
-    LAUNCH_CHECK(c, "k_sweep_colour");
+    if (!ok) return HPMC_E_CUDA;
+    LAUNCH_CHECK(c, "colour pass");
     return HPMC_OK;
 }
 
@@ -603,6 +635,21 @@ int hpmc_sweep_host(hpmc_ctx* c, const float* h_pos4, const float* h_quat4, int6
     hpmc_counters tmp;
     rc = hpmc_get_state(c, nullptr, nullptr, h_counters ? h_counters : &tmp, nullptr);  // also synchronises
     return rc;
+}
+
+int hpmc_set_option(hpmc_ctx* c, const char* name, int64_t value)
+{
+    if (!c || !name) return HPMC_E_ARG;
+    const std::string n(name);
+    if (n == "path") {
+        if (value < 0 || value > 2) return fail(c, HPMC_E_ARG, "path must be 0 (auto), 1 (per-thread) or 2 (tile)");
+        c->opt_path = (int)value;
+    } else if (n == "tile_cap") {
+        if (value < 0) return fail(c, HPMC_E_ARG, "tile_cap must be >= 0");
+        c->opt_tile_cap = value > (1 << 30) ? (1 << 30) : (int)value;
+    } else
+        return fail(c, HPMC_E_ARG, "unknown option");
+    return HPMC_OK;
 }
 
 int hpmc_set_profile(hpmc_ctx* c, int on)

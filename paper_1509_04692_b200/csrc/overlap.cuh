@@ -15,6 +15,8 @@ struct ShapeT {
     int kind, nverts;
     T diameter;
     T dmax2;              // d_max^2, broad phase R16
+    T din2;               // (2 r_in - 1e-5)^2: centres closer than this certainly overlap (r_in = inscribed radius about
+                          // the body origin); 0 for disks (the broad phase is the whole test)
     T vx[kMaxVerts], vy[kMaxVerts], vz[kMaxVerts];
     T nx[kMaxVerts], ny[kMaxVerts], fc[kMaxVerts];  // polygon: outward unit edge normals and offsets n.v
 };
@@ -101,6 +103,54 @@ __device__ __forceinline__ bool polygon_overlap(const ShapeT<T>& S, T rx, T ry, 
         }
     }
     return true;
+}
+
+// Branch-free variant for the dense narrow-phase pass of the tile kernel: the largest separation over the
+// same 2*nv axes with the same formulas as polygon_overlap: overlap <=> !(polygon_max_sep(...) >= eps).
+// No early exit: all lanes of a warp run the
+// same instruction stream (a warp finishes with its slowest lane anyway).
+template <typename T, int NV>
+__device__ __forceinline__ T polygon_max_sep(const ShapeT<T>& S, T rx, T ry, T cA, T sA, T cB, T sB)
+{
+    const int nv = (NV > 0) ? NV : S.nverts;
+    const T lx = cA * rx + sA * ry;
+    const T ly = -sA * rx + cA * ry;
+    const T c = cA * cB + sA * sB;
+    const T s = cA * sB - sA * cB;
+    T best = -(T)3.0e38;
+    {
+        T px[(NV > 0) ? NV : kMaxVerts], py[(NV > 0) ? NV : kMaxVerts];
+#pragma unroll
+        for (int j = 0; j < nv; ++j) {
+            px[j] = c * S.vx[j] - s * S.vy[j] + lx;
+            py[j] = s * S.vx[j] + c * S.vy[j] + ly;
+        }
+#pragma unroll
+        for (int k = 0; k < nv; ++k) {
+            T m = S.nx[k] * px[0] + S.ny[k] * py[0];
+#pragma unroll
+            for (int j = 1; j < nv; ++j) m = min(m, S.nx[k] * px[j] + S.ny[k] * py[j]);
+            best = max(best, m - S.fc[k]);
+        }
+    }
+    {
+        T qx[(NV > 0) ? NV : kMaxVerts], qy[(NV > 0) ? NV : kMaxVerts];
+#pragma unroll
+        for (int j = 0; j < nv; ++j) {
+            qx[j] = S.vx[j] - lx;
+            qy[j] = S.vy[j] - ly;
+        }
+#pragma unroll
+        for (int k = 0; k < nv; ++k) {
+            const T nxk = c * S.nx[k] - s * S.ny[k];
+            const T nyk = s * S.nx[k] + c * S.ny[k];
+            T m = nxk * qx[0] + nyk * qy[0];
+#pragma unroll
+            for (int j = 1; j < nv; ++j) m = min(m, nxk * qx[j] + nyk * qy[j]);
+            best = max(best, m - S.fc[k]);
+        }
+    }
+    return best;
 }
 
 // ---------------------------------------------------------------------------------------------

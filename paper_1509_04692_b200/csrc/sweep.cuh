@@ -59,28 +59,40 @@ __device__ __forceinline__ bool narrow_overlap(const ShapeF& S, const ShapeD& SD
     }
 }
 
-// v1 mapping: one thread per active cell.
-template <int KIND, int NV>
-__global__ void __launch_bounds__(128)
-k_sweep_colour(const __grid_constant__ GridParams g, const __grid_constant__ MoveParams mv,
-               const __grid_constant__ ShapeF S, const __grid_constant__ ShapeD SD, Control* __restrict__ ctrl, int colour_index,
-               float4* __restrict__ pos,
-               float4* __restrict__ quat, const int* __restrict__ tag, const int* __restrict__ cell_start, uint32_t k0,
-               uint32_t k1, uint2* __restrict__ trace)
+// Per-thread slow path: one thread makes the n_select trials of one active cell reading everything from global
+// memory.  Used for 3-D systems and as the overflow fallback of the 2-D tile kernel.
+struct CellCounters {
+    unsigned int tacc = 0, trov = 0, trcell = 0, racc = 0, rrov = 0, trials = 0;
+};
+
+__device__ __forceinline__ void flush_counters(Control* ctrl, CellCounters c)
 {
-    const SweepHeader& H = ctrl->hdr;
-    const int gamma = H.perm[colour_index];
-    const uint32_t t_lo = H.t_lo, t_hi16 = H.t_hi16;
-    const float shift[3] = {H.shift[0], H.shift[1], H.shift[2]};
+    // counters: warp reduce, one atomic per warp and counter
+    c.tacc = __reduce_add_sync(0xffffffffu, c.tacc);
+    c.trov = __reduce_add_sync(0xffffffffu, c.trov);
+    c.trcell = __reduce_add_sync(0xffffffffu, c.trcell);
+    c.racc = __reduce_add_sync(0xffffffffu, c.racc);
+    c.rrov = __reduce_add_sync(0xffffffffu, c.rrov);
+    c.trials = __reduce_add_sync(0xffffffffu, c.trials);
+    if ((threadIdx.x & 31) == 0 && c.trials) {
+        if (c.tacc) atomicAdd(&ctrl->counters[0], (unsigned long long)c.tacc);
+        if (c.trov) atomicAdd(&ctrl->counters[1], (unsigned long long)c.trov);
+        if (c.trcell) atomicAdd(&ctrl->counters[2], (unsigned long long)c.trcell);
+        if (c.racc) atomicAdd(&ctrl->counters[3], (unsigned long long)c.racc);
+        if (c.rrov) atomicAdd(&ctrl->counters[4], (unsigned long long)c.rrov);
+        atomicAdd(&ctrl->counters[5], (unsigned long long)c.trials);
+    }
+}
 
-    const int nax = g.n[0] >> 1, nay = g.n[1] >> 1, naz = (g.dim == 3) ? (g.n[2] >> 1) : 1;
-    const int nactive = nax * nay * naz;
-    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+template <int KIND, int NV>
+__device__ void sweep_cell_global(const GridParams& g, const MoveParams& mv, const ShapeF& S, const ShapeD& SD, int gamma,
+                                  uint32_t t_lo, uint32_t t_hi16, const float* shift, int cx, int cy, int cz,
+                                  float4* __restrict__ pos, float4* __restrict__ quat, const int* __restrict__ tag,
+                                  const int* __restrict__ cell_start, uint32_t k0, uint32_t k1, uint2* __restrict__ trace,
+                                  CellCounters& cc)
+{
     unsigned int c_tacc = 0, c_trov = 0, c_trcell = 0, c_racc = 0, c_rrov = 0, c_trials = 0;
-
-    if (idx < nactive) {
-        const int ix = idx % nax, iy = (idx / nax) % nay, iz = idx / (nax * nay);
-        const int cx = 2 * ix + (gamma & 1), cy = 2 * iy + ((gamma >> 1) & 1), cz = (g.dim == 3) ? 2 * iz + ((gamma >> 2) & 1) : 0;
+    {
         const int cell = cx + g.n[0] * (cy + g.n[1] * cz);
         const int start = cell_start[cell], nmem = cell_start[cell + 1] - start;
         const long long slot0 = (long long)cell * mv.n_select;
@@ -197,21 +209,31 @@ k_sweep_colour(const __grid_constant__ GridParams g, const __grid_constant__ Mov
             }
         }
     }
-    // counters: warp reduce, one atomic per warp and counter
-    c_tacc = __reduce_add_sync(0xffffffffu, c_tacc);
-    c_trov = __reduce_add_sync(0xffffffffu, c_trov);
-    c_trcell = __reduce_add_sync(0xffffffffu, c_trcell);
-    c_racc = __reduce_add_sync(0xffffffffu, c_racc);
-    c_rrov = __reduce_add_sync(0xffffffffu, c_rrov);
-    c_trials = __reduce_add_sync(0xffffffffu, c_trials);
-    if ((threadIdx.x & 31) == 0 && c_trials) {
-        if (c_tacc) atomicAdd(&ctrl->counters[0], (unsigned long long)c_tacc);
-        if (c_trov) atomicAdd(&ctrl->counters[1], (unsigned long long)c_trov);
-        if (c_trcell) atomicAdd(&ctrl->counters[2], (unsigned long long)c_trcell);
-        if (c_racc) atomicAdd(&ctrl->counters[3], (unsigned long long)c_racc);
-        if (c_rrov) atomicAdd(&ctrl->counters[4], (unsigned long long)c_rrov);
-        atomicAdd(&ctrl->counters[5], (unsigned long long)c_trials);
+    cc.tacc += c_tacc; cc.trov += c_trov; cc.trcell += c_trcell; cc.racc += c_racc; cc.rrov += c_rrov; cc.trials += c_trials;
+}
+
+// v1 mapping: one thread per active cell (any dimension).
+template <int KIND, int NV>
+__global__ void __launch_bounds__(128)
+k_sweep_colour(const __grid_constant__ GridParams g, const __grid_constant__ MoveParams mv,
+               const __grid_constant__ ShapeF S, const __grid_constant__ ShapeD SD, Control* __restrict__ ctrl, int colour_index,
+               float4* __restrict__ pos, float4* __restrict__ quat, const int* __restrict__ tag,
+               const int* __restrict__ cell_start, uint32_t k0, uint32_t k1, uint2* __restrict__ trace)
+{
+    const SweepHeader& H = ctrl->hdr;
+    const int gamma = H.perm[colour_index];
+    const float shift[3] = {H.shift[0], H.shift[1], H.shift[2]};
+    const int nax = g.n[0] >> 1, nay = g.n[1] >> 1, naz = (g.dim == 3) ? (g.n[2] >> 1) : 1;
+    const int nactive = nax * nay * naz;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    CellCounters cc;
+    if (idx < nactive) {
+        const int ix = idx % nax, iy = (idx / nax) % nay, iz = idx / (nax * nay);
+        const int cx = 2 * ix + (gamma & 1), cy = 2 * iy + ((gamma >> 1) & 1), cz = (g.dim == 3) ? 2 * iz + ((gamma >> 2) & 1) : 0;
+        sweep_cell_global<KIND, NV>(g, mv, S, SD, gamma, H.t_lo, H.t_hi16, shift, cx, cy, cz, pos, quat, tag, cell_start, k0, k1,
+                                    trace, cc);
     }
+    flush_counters(ctrl, cc);
 }
 
 // a12: count pairs (tag_p < tag_q) in 3^d neighbourhoods whose interiors intersect (strict, fp64).

@@ -120,6 +120,25 @@ def test_multi_sweep_call_equals_single_sweep_calls(name):
     assert a.counters() == b.counters()
 
 
+@pytest.mark.parametrize("name", ["disks_24", "pentagons_24", "k1_pentagons"])
+def test_colour_pass_variants_agree_bit_for_bit(name):
+    """The tile kernel, its overflow fallback (tile_cap=0) and the per-thread path make identical trajectories."""
+    w = CASES[name]()
+    ref = None
+    for opts in ({"path": 2}, {"path": 2, "tile_cap": 0}, {"path": 1}, {"path": 2, "tile_cap": 40}):
+        g = gpu(w)
+        for k, v in opts.items():
+            g.set_option(k, v)
+        g.enable_trace(True)
+        g.sweep(5)
+        out = (g.get_state(), g.counters(), g.read_trace().copy())
+        if ref is None:
+            ref = out
+        else:
+            assert np.array_equal(out[0][0], ref[0][0]) and np.array_equal(out[0][1], ref[0][1]), opts
+            assert out[1] == ref[1] and np.array_equal(out[2], ref[2]), opts
+
+
 def test_restart_from_state_and_sweep_counter():
     w = wl.pentagons(24)
     a = gpu(w)
