@@ -13,6 +13,7 @@
 #include "overlap.cuh"
 #include "sweep.cuh"
 #include "sweep_tile2d.cuh"
+#include "sweep_warp3d.cuh"
 
 using namespace hpmc;
 
@@ -327,6 +328,14 @@ bool launch_colour(hpmc_ctx* c, int ci)
       }
     }
     const int nactive = (g.n[0] / 2) * (g.n[1] / 2) * (g.dim == 3 ? g.n[2] / 2 : 1);
+    if constexpr (KIND != kKindPolygon) {
+        if (g.dim == 3 && c->opt_path != 1) {   // one warp per active cell, neighbourhood staged in shared memory
+            k_sweep_warp3d<KIND><<<(nactive + kW3Warps - 1) / kW3Warps, 32 * kW3Warps, 0, c->stream>>>(
+                g, c->mv, c->sf, c->sd, c->ctrl, ci, c->opt_tile_cap, c->pos[c->cur], c->quat[c->cur], c->tag[c->cur], c->cell_start,
+                c->k0, c->k1, c->trace);
+            return true;
+        }
+    }
     const int TB = 128;
     k_sweep_colour<KIND, NV><<<(nactive + TB - 1) / TB, TB, 0, c->stream>>>(g, c->mv, c->sf, c->sd, c->ctrl, ci, c->pos[c->cur], c->quat[c->cur],
                                                                            c->tag[c->cur], c->cell_start, c->k0, c->k1, c->trace);

@@ -38,6 +38,45 @@ struct TrialState {
     float qw, qx, qy, qz; // trial orientation
 };
 
+// a5 + a6: the trial pose of one move (R5-R7) and the leave-cell test (R13).  b0 = (select, type, ua, ub), uc = first
+// word of block 1 (3-D only).  Returns false iff a translation left `cell`.  One definition for every colour-pass
+// variant, so that they produce bit-identical trials.
+template <int KIND>
+__device__ __forceinline__ bool make_trial(const GridParams& g, const MoveParams& mv, const float* shift, int cell, int dim,
+                                           const U4& b0, uint32_t uc, const float4& xp, const float4& qp, TrialState& A, bool& rotate)
+{
+    rotate = (KIND != kKindDisk) && (b0.y >> 31);   // R7
+    A = TrialState{xp.x, xp.y, xp.z, qp.x, qp.y, qp.z, qp.w};
+    if (!rotate) {
+        A.x = __fmaf_rn(mv.d, usym(b0.z), xp.x);   // R5: one rounding per axis
+        A.y = __fmaf_rn(mv.d, usym(b0.w), xp.y);
+        if (dim == 3) A.z = __fmaf_rn(mv.d, usym(uc), xp.z);
+        int tx, ty, tz;
+        return cell_of(g, shift, A.x, A.y, A.z, tx, ty, tz) == cell;   // a6: same pinned cell function (R13)
+    }
+    if (dim == 2) {                                   // R6, 2-D: angle about z
+        float sn, cs;
+        sincosf(0.5f * __fmul_rn(mv.a, usym(b0.z)), &sn, &cs);
+        const float w = qp.x * cs - qp.w * sn, z = qp.x * sn + qp.w * cs;
+        const float inv = rsqrtf(w * w + z * z);
+        A.qw = w * inv; A.qx = 0.0f; A.qy = 0.0f; A.qz = z * inv;
+    } else {                                          // R6, 3-D: uniform axis, angle in [-a,a)
+        const float zz = usym(b0.z);
+        float sphi, cphi, sn, cs;
+        sincosf(6.283185307179586f * u01(b0.w), &sphi, &cphi);
+        const float rho = sqrtf(fmaxf(0.0f, 1.0f - zz * zz));
+        sincosf(0.5f * __fmul_rn(mv.a, usym(uc)), &sn, &cs);
+        const float dx = sn * rho * cphi, dy = sn * rho * sphi, dz = sn * zz, dw = cs;
+        const float w = qp.x * dw - qp.y * dx - qp.z * dy - qp.w * dz;   // q (x) dq
+        const float x = qp.x * dx + qp.y * dw + qp.z * dz - qp.w * dy;
+        const float y = qp.x * dy - qp.y * dz + qp.z * dw + qp.w * dx;
+        const float z = qp.x * dz + qp.y * dy - qp.z * dx + qp.w * dw;
+        const float inv = rsqrtf(w * w + x * x + y * y + z * z);
+        A.qw = w * inv; A.qx = x * inv; A.qy = y * inv; A.qz = z * inv;
+    }
+    return true;
+}
+
 // narrow phase of the trial particle A against neighbour B; r = r_B - r_A(trial), already minimum image
 template <int KIND, int NV>
 __device__ __forceinline__ bool narrow_overlap(const ShapeF& S, const ShapeD& SD, const TrialState& A, const float* MA, float rx,
@@ -108,39 +147,12 @@ __device__ void sweep_cell_global(const GridParams& g, const MoveParams& mv, con
                 if (g.dim == 3) uc = philox4x32_10((uint32_t)cell, t_lo, (uint32_t)k | (1u << 16), c3, k0, k1).x;
                 // a5: uniformly random member (R8), move type (R7)
                 const int p = start + (int)mulhi32(b0.x, (uint32_t)nmem);
-                const bool rotate = (KIND != kKindDisk) && (b0.y >> 31);
                 const float4 xp = pos[p];
                 const float4 qp = quat[p];
-                TrialState A{xp.x, xp.y, xp.z, qp.x, qp.y, qp.z, qp.w};
-                int outcome = 1;
+                TrialState A;
+                bool rotate;
+                int outcome = make_trial<KIND>(g, mv, shift, cell, g.dim, b0, uc, xp, qp, A, rotate) ? 1 : 2;   // a5, a6
                 ++c_trials;
-                if (!rotate) {
-                    A.x = __fmaf_rn(mv.d, usym(b0.z), xp.x);   // R5: one rounding per axis
-                    A.y = __fmaf_rn(mv.d, usym(b0.w), xp.y);
-                    if (g.dim == 3) A.z = __fmaf_rn(mv.d, usym(uc), xp.z);
-                    // a6: leave-cell reject with the same pinned cell function (R13)
-                    int tx, ty, tz;
-                    if (cell_of(g, shift, A.x, A.y, A.z, tx, ty, tz) != cell) outcome = 2;
-                } else if (g.dim == 2) {                          // R6, 2-D: angle about z
-                    float sn, cs;
-                    sincosf(0.5f * __fmul_rn(mv.a, usym(b0.z)), &sn, &cs);
-                    const float w = qp.x * cs - qp.w * sn, z = qp.x * sn + qp.w * cs;
-                    const float inv = rsqrtf(w * w + z * z);
-                    A.qw = w * inv; A.qx = 0.0f; A.qy = 0.0f; A.qz = z * inv;
-                } else {                                          // R6, 3-D: uniform axis, angle in [-a,a)
-                    const float zz = usym(b0.z);
-                    float sphi, cphi, sn, cs;
-                    sincosf(6.283185307179586f * u01(b0.w), &sphi, &cphi);
-                    const float rho = sqrtf(fmaxf(0.0f, 1.0f - zz * zz));
-                    sincosf(0.5f * __fmul_rn(mv.a, usym(uc)), &sn, &cs);
-                    const float dx = sn * rho * cphi, dy = sn * rho * sphi, dz = sn * zz, dw = cs;
-                    const float w = qp.x * dw - qp.y * dx - qp.z * dy - qp.w * dz;   // q (x) dq
-                    const float x = qp.x * dx + qp.y * dw + qp.z * dz - qp.w * dy;
-                    const float y = qp.x * dy - qp.y * dz + qp.z * dw + qp.w * dx;
-                    const float z = qp.x * dz + qp.y * dy - qp.z * dx + qp.w * dw;
-                    const float inv = rsqrtf(w * w + x * x + y * y + z * z);
-                    A.qw = w * inv; A.qx = x * inv; A.qy = y * inv; A.qz = z * inv;
-                }
                 if (outcome == 1) {
                     // orientation data of the trial particle, computed once per trial
                     float MA[9];

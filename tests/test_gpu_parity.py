@@ -32,7 +32,16 @@ CASES = {
     "k0_disks": lambda: wl.config(0),
     "k1_pentagons": lambda: wl.config(1),
     "cubes_12": lambda: wl.cubes(12),
+    "spheres_8": lambda: spheres(8),
 }
+
+
+def spheres(n_lat):
+    """3-D hard spheres (KIND_DISK in a 3-D box) on the cube lattice of wl.cubes: diameter 1, spacing 1.25."""
+    base = wl.cubes(n_lat)
+    q = np.zeros((base.N, 4), np.float32); q[:, 0] = 1
+    return wl.Workload(name=f"spheres_{n_lat}", dim=3, N=base.N, L=base.L, kind=wl.KIND_DISK, diameter=1.0, verts=None, d=0.2,
+                       a=0.0, n_select=4, sweeps=1, pos4=base.pos4, quat4=q)
 
 
 def test_grid_matches_oracle():
@@ -95,7 +104,7 @@ def lockstep(w, n_sweeps, seed=1):
     return stats, g, o
 
 
-@pytest.mark.parametrize("name,n", [("disks_24", 10), ("pentagons_24", 10), ("cubes_7", 10),
+@pytest.mark.parametrize("name,n", [("disks_24", 10), ("pentagons_24", 10), ("cubes_7", 10), ("spheres_8", 10),
                                     ("k0_disks", 10), ("k1_pentagons", 10), ("cubes_12", 4)])
 def test_first_sweeps_lockstep_with_oracle(name, n):
     w = CASES[name]()
@@ -120,12 +129,14 @@ def test_multi_sweep_call_equals_single_sweep_calls(name):
     assert a.counters() == b.counters()
 
 
-@pytest.mark.parametrize("name", ["disks_24", "pentagons_24", "k1_pentagons"])
+@pytest.mark.parametrize("name", ["disks_24", "pentagons_24", "k1_pentagons", "cubes_7", "spheres_8"])
 def test_colour_pass_variants_agree_bit_for_bit(name):
-    """The tile kernel, its overflow fallback (tile_cap=0) and the per-thread path make identical trajectories."""
+    """The staged kernels (2-D tile, 3-D warp-per-cell), their overflow fallbacks (tile_cap=0 everywhere, a small
+    tile_cap on some tiles/cells) and the per-thread path make identical trajectories."""
     w = CASES[name]()
     ref = None
-    for opts in ({"path": 2}, {"path": 2, "tile_cap": 0}, {"path": 1}, {"path": 2, "tile_cap": 40}):
+    some = 40 if w.dim == 2 else (84 if w.kind == wl.KIND_POLYHEDRON else 50)   # a capacity only some tiles/cells exceed
+    for opts in ({"path": 2}, {"path": 2, "tile_cap": 0}, {"path": 1}, {"path": 2, "tile_cap": some}):
         g = gpu(w)
         for k, v in opts.items():
             g.set_option(k, v)
