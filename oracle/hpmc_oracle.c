@@ -303,6 +303,58 @@ double orc_shape_margin(const orc_shape* s, const double r_ab[3], const double q
     return m;
 }
 
+/* O9 ("histogram of scale factors s that cause two neighboring particles to overlap"): the scale
+ * lambda* of the separation vector at which the pair first touches.  With the O4 axis set,
+ * m(lambda r) = max_n [lambda n.r - H_n], H_n = h_A(n) + h_B(-n) > 0, so the pair overlaps iff
+ * lambda < lambda* = min over axes with n.r > 0 of H_n / (n.r).  Disks: lambda* = sigma / |r|.
+ * A pair overlaps after a uniform compression of all separations by (1 - s) iff s > 1 - lambda*. */
+static void touch_axis(const double nhat[3], const double r_ab[3], double (*wa)[3], double (*wb)[3], int nv, double* best)
+{
+    double nr = dot3(nhat, r_ab);
+    if (nr <= 0.0) return;
+    double neg[3] = {-nhat[0], -nhat[1], -nhat[2]};
+    double lam = (support_height(wa, nv, nhat) + support_height(wb, nv, neg)) / nr;
+    if (lam < *best) *best = lam;
+}
+
+double orc_shape_touch_scale(const orc_shape* s, const double r_ab[3], const double qa[4], const double qb[4])
+{
+    if (s->kind == ORC_KIND_DISK) return s->diameter / norm3(r_ab);
+    double wa[ORC_MAX_VERTS][3], wb[ORC_MAX_VERTS][3];
+    int nv = s->nverts;
+    for (int i = 0; i < nv; ++i) {
+        quat_rotate(qa, s->verts[i], wa[i]);
+        quat_rotate(qb, s->verts[i], wb[i]);
+    }
+    double best = INFINITY;
+    for (int f = 0; f < s->nfaces; ++f) {
+        double na[3], nb[3];
+        quat_rotate(qa, s->face_n[f], na);
+        quat_rotate(qb, s->face_n[f], nb);
+        for (int c = 0; c < 3; ++c) nb[c] = -nb[c];
+        touch_axis(na, r_ab, wa, wb, nv, &best);
+        touch_axis(nb, r_ab, wa, wb, nv, &best);
+    }
+    if (s->kind == ORC_KIND_POLYHEDRON) {
+        for (int i = 0; i < s->nedgedirs; ++i) {
+            double ea[3];
+            quat_rotate(qa, s->edge_d[i], ea);
+            for (int j = 0; j < s->nedgedirs; ++j) {
+                double eb[3], n[3];
+                quat_rotate(qb, s->edge_d[j], eb);
+                cross3(ea, eb, n);
+                double len = norm3(n);
+                if (len < 1e-9) continue;
+                for (int c = 0; c < 3; ++c) n[c] /= len;
+                touch_axis(n, r_ab, wa, wb, nv, &best);
+                for (int c = 0; c < 3; ++c) n[c] = -n[c];
+                touch_axis(n, r_ab, wa, wb, nv, &best);
+            }
+        }
+    }
+    return best;
+}
+
 /* ---- fp64 GJK boolean on the Minkowski difference B (-) A, support by Eq. (1) P:97 ---- */
 typedef struct { double (*wa)[3]; double (*wb)[3]; int nv; const double* r; } gjk_ctx;
 
@@ -917,6 +969,56 @@ int64_t orc_count_overlaps_cells(const orc_sys* s)
     return c;
 }
 double orc_min_margin_cells(const orc_sys* s) { return cells_pair_scan(s, NULL); }
+
+/* O9: histogram of s = 1 - lambda* over all pairs i<j of the current state with 0 <= s < s_max, nbins equal
+ * bins.  Pairs are found in the 5^d cells around each particle (|r| < d_max / (1 - s_max) can reach two cells
+ * away), which needs >= 5 cells per side; returns -1 otherwise, else the number of pairs binned. */
+int64_t orc_scale_histogram(const orc_sys* s, double s_max, int nbins, uint64_t* hist)
+{
+    for (int k = 0; k < s->dim; ++k)
+        if (s->n[k] < 5) return -1;
+    if (!(s_max > 0.0 && s_max < 0.1) || nbins < 1) return -1;
+    float shift[3] = {0.0f, 0.0f, 0.0f};
+    int32_t* cid = (int32_t*)malloc(sizeof(int32_t) * (size_t)(s->N > 0 ? s->N : 1));
+    int32_t* mem = (int32_t*)malloc(sizeof(int32_t) * (size_t)(s->N > 0 ? s->N : 1));
+    int32_t* cst = (int32_t*)malloc(sizeof(int32_t) * (size_t)(s->C + 1));
+    orc_cell_list(s, shift, cid, cst, mem);
+    for (int b = 0; b < nbins; ++b) hist[b] = 0;
+    int64_t binned = 0;
+    double range = s->shape->dmax / (1.0 - s_max), range2 = range * range;
+    int zr = (s->dim == 3) ? 2 : 0;
+    for (int64_t i = 0; i < s->N; ++i) {
+        int64_t cell = cid[i];
+        int32_t cx = (int32_t)(cell % s->n[0]), cy = (int32_t)((cell / s->n[0]) % s->n[1]);
+        int32_t cz = (int32_t)(cell / ((int64_t)s->n[0] * s->n[1]));
+        double qa[4];
+        quat_to_double(&s->quat[4 * i], qa);
+        for (int dz = -zr; dz <= zr; ++dz)
+            for (int dy = -2; dy <= 2; ++dy)
+                for (int dx = -2; dx <= 2; ++dx) {
+                    int32_t nx = ((cx + dx) % s->n[0] + s->n[0]) % s->n[0];
+                    int32_t ny = ((cy + dy) % s->n[1] + s->n[1]) % s->n[1];
+                    int32_t nz = ((cz + dz) % s->n[2] + s->n[2]) % s->n[2];
+                    int32_t nc = nx + s->n[0] * (ny + s->n[1] * nz);
+                    for (int32_t p = cst[nc]; p < cst[nc + 1]; ++p) {
+                        int64_t j = mem[p];
+                        if (j <= i) continue;
+                        double r[3], qb[4];
+                        min_image(s, &s->pos[4 * j], &s->pos[4 * i], r);
+                        if (dot3(r, r) >= range2) continue;
+                        quat_to_double(&s->quat[4 * j], qb);
+                        double sc = 1.0 - orc_shape_touch_scale(s->shape, r, qa, qb);
+                        if (sc < 0.0 || sc >= s_max) continue;
+                        int b = (int)(sc / s_max * nbins);
+                        if (b >= nbins) b = nbins - 1;
+                        hist[b]++;
+                        ++binned;
+                    }
+                }
+    }
+    free(cid); free(mem); free(cst);
+    return binned;
+}
 
 /* P4: smallest centre distance between particles that sit in DIFFERENT cells of the SAME colour */
 double orc_min_same_colour_distance(const orc_sys* s, const float shift[3])

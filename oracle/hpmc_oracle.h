@@ -82,6 +82,8 @@ int orc_shape_nedgedirs(const orc_shape*);
 void orc_shape_faces(const orc_shape*, double* normals3, double* offsets);
 /* margin m(A,B): r_ab = r_B - r_A (already minimum image), q = (w,x,y,z). */
 double orc_shape_margin(const orc_shape*, const double r_ab[3], const double qa[4], const double qb[4]);
+/* O9: scale lambda* of r_ab at which the pair first touches (overlap iff lambda < lambda*), from the O4 axis set */
+double orc_shape_touch_scale(const orc_shape*, const double r_ab[3], const double qa[4], const double qb[4]);
 /* fp64 GJK boolean: 1 origin in interior of B (-) A, 0 disjoint, -1 undecided */
 int orc_shape_gjk(const orc_shape*, const double r_ab[3], const double qa[4], const double qb[4]);
 
@@ -131,6 +133,8 @@ int64_t orc_count_overlaps_bruteforce(const orc_sys*);
 int64_t orc_count_overlaps_cells(const orc_sys*);
 /* smallest pair margin in the system through the cell list (diagnostic) */
 double orc_min_margin_cells(const orc_sys*);
+/* O9: histogram of s = 1 - lambda* in [0, s_max) over all pairs of the current state (5^d cell search) */
+int64_t orc_scale_histogram(const orc_sys*, double s_max, int nbins, uint64_t* hist);
 /* P4: min centre distance between particles of distinct same-colour cells */
 double orc_min_same_colour_distance(const orc_sys*, const float shift[3]);
 

@@ -60,6 +60,8 @@ def lib():
     L.orc_shape_faces.argtypes = [vp, dp, dp]
     L.orc_shape_margin.argtypes = [vp, dp, dp, dp]; L.orc_shape_margin.restype = C.c_double
     L.orc_shape_gjk.argtypes = [vp, dp, dp, dp]; L.orc_shape_gjk.restype = C.c_int
+    L.orc_shape_touch_scale.argtypes = [vp, dp, dp, dp]; L.orc_shape_touch_scale.restype = C.c_double
+    L.orc_scale_histogram.argtypes = [vp, C.c_double, C.c_int, C.POINTER(C.c_uint64)]; L.orc_scale_histogram.restype = C.c_int64
     L.orc_create.argtypes = [C.c_int, dp, C.c_int, C.c_double, C.c_int, dp, C.c_int64, C.c_uint64]
     L.orc_create.restype = vp
     L.orc_destroy.argtypes = [vp]
@@ -161,6 +163,12 @@ class Shape:
         r = np.zeros(3); r[:len(r_ab)] = r_ab
         a = np.ascontiguousarray(qa, dtype=np.float64); b = np.ascontiguousarray(qb, dtype=np.float64)
         return lib().orc_shape_margin(self._h, _dp(r), _dp(a), _dp(b))
+
+    def touch_scale(self, r_ab, qa, qb):
+        """O9: lambda* such that the pair at separation lambda * r_ab overlaps iff lambda < lambda*."""
+        r = np.zeros(3); r[:len(r_ab)] = r_ab
+        a = np.ascontiguousarray(qa, dtype=np.float64); b = np.ascontiguousarray(qb, dtype=np.float64)
+        return lib().orc_shape_touch_scale(self._h, _dp(r), _dp(a), _dp(b))
 
     def gjk(self, r_ab, qa, qb):
         r = np.zeros(3); r[:len(r_ab)] = r_ab
@@ -273,6 +281,13 @@ class Oracle:
 
     def count_overlaps_cells(self):
         return int(lib().orc_count_overlaps_cells(self._h))
+
+    def scale_histogram(self, s_max=0.02, nbins=40):
+        """O9: counts of pairs whose touch scale s = 1 - lambda* falls in each of nbins bins on [0, s_max)."""
+        h = np.zeros(nbins, dtype=np.uint64)
+        n = lib().orc_scale_histogram(self._h, float(s_max), int(nbins), h.ctypes.data_as(C.POINTER(C.c_uint64)))
+        assert n >= 0, "scale_histogram needs >= 5 cells per side"
+        return h
 
     def min_margin_cells(self):
         return float(lib().orc_min_margin_cells(self._h))

@@ -1,0 +1,83 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (default options):
+configs[2] (1 048 576 pentagons) and configs[4] (16 777 216 pentagons).
+
+The oracle replays whole sweeps of the full system (O8 lock-step: every trial slot compared, 4.2 M / 67 M slots
+per sweep), then properties that hold at any size are checked after more sweeps: zero overlaps, counters that
+add up, trials = n_select x non-empty cells, the traced and untraced runs bit-identical.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import hpmc_oracle as ho
+from paper_1509_04692_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+def _lockstep_full(k, n_lock, n_more):
+    from paper_1509_04692_b200 import binding as hb
+    w = wl.config(k)
+    g = hb.from_workload(w, seed=1)
+    o = ho.Oracle(w.dim, w.L, w.kind, w.N, 1, diameter=w.diameter, verts=w.verts)
+    o.set_moves(w.d, w.a, w.n_select)
+    o.set_state(w.pos4, w.quat4)
+    assert g.count_overlaps() == 0
+    # cell list of sweep 0: ids, CSR and member order bit-exact
+    cid, cst, mem, shift, perm = g.cell_list(0)
+    oshift, operm = o.sweep_header(0)
+    ocid, ocst, omem = o.cell_list(oshift)
+    assert np.array_equal(shift[:2], oshift[:2]) and np.array_equal(perm, operm)
+    assert np.array_equal(cid, ocid) and np.array_equal(cst, ocst) and np.array_equal(mem, omem)
+    del cid, cst, mem, ocid, ocst, omem
+    g.enable_trace(True)
+    marginal = trials = 0
+    for s in range(n_lock):
+        g.sweep(1)
+        f = o.sweep(follow=g.read_trace(), follow_tol=1e-5)["follow"]
+        assert f["hard_mismatch"] == 0, (k, s, f)
+        assert f["compared"] == g.C * w.n_select
+        marginal += f["marginal"]
+        gp, gq = g.get_state()
+        op, oq = o.get_state()
+        assert np.array_equal(gp, op), f"config {k} sweep {s}: positions differ"
+        assert np.max(np.abs(gq - oq)) < 1e-5
+        o.set_state(op, gq)
+    gc, oc = g.counters(), o.counters()
+    for key in ("trans_acc", "trans_rej_overlap", "trans_rej_cell", "rot_acc", "rot_rej_overlap", "trials", "sweeps"):
+        assert gc[key] == oc[key], (key, gc, oc)
+    trials = gc["trials"]
+    assert marginal <= max(3, 2e-4 * trials), (marginal, trials)       # P11
+    # untraced run of the same sweeps: bit-identical state (the trace changes nothing)
+    g2 = hb.from_workload(w, seed=1)
+    g2.sweep(n_lock)
+    p2, q2 = g2.get_state()
+    assert np.array_equal(p2, gp) and np.array_equal(q2, gq) and g2.counters() == gc
+    del g, o, gp, gq, op, oq
+    # properties at any size, after more sweeps in the timed configuration
+    g2.reset_counters()
+    for s in range(n_more):
+        cst = g2.cell_list(n_lock + s)[1]
+        nonempty = int(np.count_nonzero(np.diff(cst)))
+        c0 = g2.counters()["trials"]
+        g2.sweep(1)
+        assert g2.counters()["trials"] - c0 == w.n_select * nonempty
+    c = g2.counters()
+    assert c["trials"] == c["trans_acc"] + c["trans_rej_overlap"] + c["trans_rej_cell"] + c["rot_acc"] + c["rot_rej_overlap"]
+    assert c["sweep_counter"] == n_lock + n_more
+    assert g2.count_overlaps() == 0
+    p, q = g2.get_state()
+    half = np.float32(0.5) * np.float32(w.L[0])
+    assert np.all(p[:, :2] >= -half) and np.all(p[:, :2] < half) and np.all(p[:, 2:] == 0)
+    assert np.all(q[:, 1:3] == 0) and np.max(np.abs(np.sum(q.astype(np.float64) ** 2, axis=1) - 1)) < 1e-6
+    print(f"config {k}: {trials} trials locked to the oracle, {marginal} marginal")
+
+
+def test_config2_pentagons_1M_lockstep_and_invariants():
+    _lockstep_full(2, 3, 5)
+
+
+@pytest.mark.skipif(os.environ.get("HPMC_SKIP_16M") == "1", reason="HPMC_SKIP_16M=1")
+def test_config4_pentagons_16M_lockstep_and_invariants():
+    _lockstep_full(4, 1, 2)
