@@ -197,37 +197,6 @@ def sample_of(k, n_lat):
     return wl.pentagons(n_lat, name=f"pentagons_{n_lat * n_lat}_sample")
 
 
-class Dist:
-    def __init__(self, n):
-        self.world = int(os.environ.get("WORLD_SIZE", "1"))
-        self.rank = int(os.environ.get("RANK", "0"))
-        self.local = int(os.environ.get("LOCAL_RANK", "0"))
-        self.on = self.world > 1
-        if self.on:
-            import torch
-            import torch.distributed as dist
-            torch.cuda.set_device(self.local)
-            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-            dist.init_process_group("nccl", device_id=torch.device(f"cuda:{self.local}"))
-            self.dist = dist
-
-    def barrier(self):
-        if self.on:
-            self.dist.barrier()
-
-    def reduce(self, x, op):
-        if not self.on:
-            return x
-        import torch
-        t = torch.tensor([float(x)], dtype=torch.float64, device=f"cuda:{self.local}")
-        self.dist.all_reduce(t, op=getattr(self.dist.ReduceOp, op))
-        return float(t.item())
-
-    def close(self):
-        if self.on:
-            self.dist.destroy_process_group()
-
-
 def run_reference(args):
     """The oracle as it stands on the host cores: each step = one oracle sweep of a bounded sample of the workload."""
     rank = int(os.environ.get("RANK", "0"))
@@ -293,18 +262,17 @@ def main():
     import torch
     from paper_1509_04692_b200 import build as hbuild
     hbuild.build()                                   # no-op when the in-tree libhpmc.so is current
-    D = Dist(args.gpus)
+    from paper_1509_04692_b200.replicas import Replicas
+    D = Replicas("nccl")
     device = f"cuda:{D.local}"
     torch.cuda.set_device(D.local)
     k = args.config
-    w = wl.config(k, seed=1 + D.rank)                # replica r: orientation seed and Philox seed 1 + r
+    w = wl.config(k, seed=D.seed)                    # replica r: orientation seed and Philox seed 1 + r
     flush = not args.no_flush
-    r = time_gpu(w, 1 + D.rank, device, args.steps, args.warmup, flush, D)
+    r = time_gpu(w, D.seed, device, args.steps, args.warmup, flush, D)
     g = r["g"]
-    t_max = D.reduce(r["ms"], "MAX") * 1e-3
-    trials_all = D.reduce(r["counters"]["trials"], "SUM")
+    value, trials_all, t_max = D.aggregate(r["counters"]["trials"], r["ms"] * 1e-3)
     launches_all = D.reduce(r["launches"], "SUM")
-    value = trials_all / t_max
     acc = r["counters"]["trans_acc"] + r["counters"]["rot_acc"]
     trials = r["counters"]["trials"]
 
