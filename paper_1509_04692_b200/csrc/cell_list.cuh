@@ -128,8 +128,9 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_final(int* __restrict__ c
     }
 }
 
-// second half of a3: scatter into the cell-sorted SoA.  src_tag == nullptr: source is in tag order.
-__global__ void k_scatter(int N, const float4* __restrict__ src_pos, const float4* __restrict__ src_quat,
+// second half of a3: scatter into the cell-sorted SoA.  src_tag == nullptr: source is the caller's tag-order pos4/quat4;
+// otherwise the source is the other sorted buffer (2-D: poses only).
+__global__ void k_scatter(int N, int dim, const float4* __restrict__ src_pos, const float4* __restrict__ src_quat,
                           const int* __restrict__ src_tag, const int2* __restrict__ key_rank,
                           const int* __restrict__ cell_start, float4* __restrict__ dst_pos, float4* __restrict__ dst_quat,
                           int* __restrict__ dst_tag)
@@ -138,13 +139,22 @@ __global__ void k_scatter(int N, const float4* __restrict__ src_pos, const float
     if (p >= N) return;
     const int2 kr = key_rank[p];
     const int dst = cell_start[kr.x] + kr.y;
-    dst_pos[dst] = src_pos[p];
-    dst_quat[dst] = src_quat[p];
+    const float4 P = src_pos[p];
+    if (dim == 2) {
+        if (src_tag) dst_pos[dst] = P;
+        else {
+            const float4 Q = src_quat[p];
+            dst_pos[dst] = make_float4(P.x, P.y, Q.x, Q.w);
+        }
+    } else {
+        dst_pos[dst] = P;
+        dst_quat[dst] = src_quat[p];
+    }
     dst_tag[dst] = src_tag ? src_tag[p] : p;
 }
 
 // R8: members of a cell in ascending tag, whatever order the atomics produced
-__global__ void k_cell_sort(int C, const int* __restrict__ cell_start, float4* __restrict__ pos, float4* __restrict__ quat,
+__global__ void k_cell_sort(int C, int dim, const int* __restrict__ cell_start, float4* __restrict__ pos, float4* __restrict__ quat,
                             int* __restrict__ tag)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
@@ -154,28 +164,32 @@ __global__ void k_cell_sort(int C, const int* __restrict__ cell_start, float4* _
         const int ti = tag[i];
         int j = i - 1;
         if (tag[j] <= ti) continue;
-        const float4 pi = pos[i], qi = quat[i];
+        const float4 pi = pos[i];
+        float4 qi = pi;
+        if (dim == 3) qi = quat[i];
         while (j >= s && tag[j] > ti) {
             tag[j + 1] = tag[j];
             pos[j + 1] = pos[j];
-            quat[j + 1] = quat[j];
+            if (dim == 3) quat[j + 1] = quat[j];
             --j;
         }
         tag[j + 1] = ti;
         pos[j + 1] = pi;
-        quat[j + 1] = qi;
+        if (dim == 3) quat[j + 1] = qi;
     }
 }
 
 // a13: back to tag order
-__global__ void k_unsort(int N, const float4* __restrict__ pos, const float4* __restrict__ quat, const int* __restrict__ tag,
+__global__ void k_unsort(int N, int dim, const float4* __restrict__ pos, const float4* __restrict__ quat, const int* __restrict__ tag,
                          float4* __restrict__ out_pos, float4* __restrict__ out_quat)
 {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= N) return;
     const int t = tag[p];
-    if (out_pos) out_pos[t] = pos[p];
-    if (out_quat) out_quat[t] = quat[p];
+    float4 x, q;
+    load_state(dim, pos, quat, p, x, q);
+    if (out_pos) out_pos[t] = x;
+    if (out_quat) out_quat[t] = q;
 }
 
 // debug: cell id of every particle in tag order, from the (cell, rank) pairs of the last build

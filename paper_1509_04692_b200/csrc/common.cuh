@@ -47,6 +47,29 @@ struct Control {
     SweepHeader hdr;
 };
 
+// Cell-sorted state.  3-D: pos = (x, y, z, 0) and quat = (w, x, y, z), two arrays.  2-D: ONE array of
+// poses (x, y, qw, qz) in `pos` (R30: z = 0 and qx = qy = 0 always), `quat` is not allocated -- half the bytes per particle.
+__device__ __forceinline__ void load_state(int dim, const float4* __restrict__ pos, const float4* __restrict__ quat, int i,
+                                           float4& x, float4& q)
+{
+    const float4 P = pos[i];
+    if (dim == 2) {
+        x = make_float4(P.x, P.y, 0.0f, 0.0f);
+        q = make_float4(P.z, 0.0f, 0.0f, P.w);
+    } else {
+        x = P;
+        q = quat[i];
+    }
+}
+
+__device__ __forceinline__ void store_state(int dim, float4* __restrict__ pos, float4* __restrict__ quat, int i, const float4& x,
+                                            const float4& q, bool rotated)
+{
+    if (dim == 2) pos[i] = make_float4(x.x, x.y, q.x, q.w);
+    else if (!rotated) pos[i] = x;
+    else quat[i] = q;
+}
+
 // R13: the one cell function, used both to assign cells and to test "left its cell".
 // Explicit _rn intrinsics so that no multiply-add is ever contracted.
 __device__ __forceinline__ int cell_axis(float x, float lo, float s, float L, float inv_w, int n)

@@ -56,6 +56,7 @@ struct hpmc_ctx {
     // tuning / test knobs (hpmc_set_option)
     int opt_path = 0;                 // 0 auto, 1 per-thread global path, 2 tile path (2-D only)
     int opt_tile_cap = 1 << 30;       // staging capacity limit of the tile kernel (tests force the overflow path)
+    int opt_tile_shape = 0;           // 0 = by grid size, 1..4 = fixed (see pick_tile_shape)
 
     // optional per-kernel device timing (hpmc_set_profile): event pairs around the cell-list build (class 0)
     // and around every colour-pass launch (class 1)
@@ -111,7 +112,7 @@ Layout layout_of(const hpmc_ctx* c)
     const size_t N = (size_t)(c->g.N > 0 ? c->g.N : 1);
     for (int b = 0; b < 2; ++b) {
         L.pos[b] = cv.take(N * sizeof(float4));
-        L.quat[b] = cv.take(N * sizeof(float4));
+        L.quat[b] = cv.take(c->g.dim == 3 ? N * sizeof(float4) : 0);   // 2-D keeps one pose array
         L.tag[b] = cv.take(N * sizeof(int));
     }
     L.key_rank = cv.take(N * sizeof(int2));
@@ -293,10 +294,10 @@ int build_cell_list(hpmc_ctx* c, int mode, unsigned long long t_override)
     k_scan_final<<<tiles, kScanThreads, 0, c->stream>>>(c->cell_start, g.C, c->tile_sums);
     LAUNCH_CHECK(c, "k_scan_final");
     if (g.N > 0) {
-        k_scatter<<<nblk_part, TB, 0, c->stream>>>(g.N, src_pos, src_quat, src_tag, c->key_rank, c->cell_start, c->pos[dst],
+        k_scatter<<<nblk_part, TB, 0, c->stream>>>(g.N, g.dim, src_pos, src_quat, src_tag, c->key_rank, c->cell_start, c->pos[dst],
                                                   c->quat[dst], c->tag[dst]);
         LAUNCH_CHECK(c, "k_scatter");
-        k_cell_sort<<<(g.C + TB - 1) / TB, TB, 0, c->stream>>>(g.C, c->cell_start, c->pos[dst], c->quat[dst], c->tag[dst]);
+        k_cell_sort<<<(g.C + TB - 1) / TB, TB, 0, c->stream>>>(g.C, g.dim, c->cell_start, c->pos[dst], c->quat[dst], c->tag[dst]);
         LAUNCH_CHECK(c, "k_cell_sort");
     }
     c->cur = dst;
@@ -305,27 +306,49 @@ int build_cell_list(hpmc_ctx* c, int mode, unsigned long long t_override)
     return HPMC_OK;
 }
 
-constexpr int kTileTY = 4;   // warps per CTA of the 2-D tile kernel (tile = 32 x kTileTY active cells)
+template <int KIND, int NV, int WARPS, int R>
+bool launch_tile2d(hpmc_ctx* c, int ci)
+{
+    using TL = Tile2D<WARPS, R>;
+    const GridParams& g = c->g;
+    auto kern = k_sweep_tile2d<KIND, NV, WARPS, R>;
+    static bool attr_set = false;   // per template instance
+    if (!attr_set) {
+        if (!cuda_ok(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TL::bytes), "tile/attr")) return false;
+        attr_set = true;
+    }
+    const int nax = g.n[0] / 2, nay = g.n[1] / 2;
+    const int tiles = ((nax + kTileW - 1) / kTileW) * ((nay + TL::TH - 1) / TL::TH);
+    kern<<<tiles, TL::NT, TL::bytes, c->stream>>>(g, c->mv, c->sf, c->sd, c->ctrl, ci, c->opt_tile_cap, c->pos[c->cur], c->tag[c->cur],
+                                                  c->cell_start, c->k0, c->k1, c->trace);
+    return true;
+}
+
+// tile shapes (warps per CTA, rows of 32 active cells per warp); "tile_shape" option, 0 = by grid size
+int pick_tile_shape(const hpmc_ctx* c)
+{
+    if (c->opt_tile_shape) return c->opt_tile_shape;
+    const int nax = c->g.n[0] / 2, nay = c->g.n[1] / 2;
+    const long long cols = (nax + kTileW - 1) / kTileW;
+    if (cols * ((nay + 15) / 16) >= 3 * 148) return 1;   // 8 warps x 2 rows
+    if (cols * ((nay + 7) / 8) >= 2 * 148) return 2;     // 4 warps x 2 rows
+    if (cols * ((nay + 3) / 4) >= 148) return 3;         // 4 warps x 1 row
+    return 4;                                            // 2 warps x 1 row
+}
 
 template <int KIND, int NV>
 bool launch_colour(hpmc_ctx* c, int ci)
 {
     const GridParams& g = c->g;
     if constexpr (KIND != kKindPolyhedron) {
-      if (g.dim == 2 && c->opt_path != 1) {
-        using TL = Tile2D<kTileTY>;
-        auto kern = k_sweep_tile2d<KIND, NV, kTileTY>;
-        static bool attr_set = false;   // per template instance
-        if (!attr_set) {
-            if (!cuda_ok(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TL::bytes), "tile/attr")) return false;
-            attr_set = true;
+        if (g.dim == 2 && c->opt_path != 1) {
+            switch (pick_tile_shape(c)) {
+                case 1: return launch_tile2d<KIND, NV, 8, 2>(c, ci);
+                case 2: return launch_tile2d<KIND, NV, 4, 2>(c, ci);
+                case 3: return launch_tile2d<KIND, NV, 4, 1>(c, ci);
+                default: return launch_tile2d<KIND, NV, 2, 1>(c, ci);
+            }
         }
-        const int nax = g.n[0] / 2, nay = g.n[1] / 2;
-        const int tiles = ((nax + kTileW - 1) / kTileW) * ((nay + kTileTY - 1) / kTileTY);
-        kern<<<tiles, TL::NT, TL::bytes, c->stream>>>(g, c->mv, c->sf, c->sd, c->ctrl, ci, c->opt_tile_cap, c->pos[c->cur],
-                                                      c->quat[c->cur], c->tag[c->cur], c->cell_start, c->k0, c->k1, c->trace);
-        return true;
-      }
     }
     const int nactive = (g.n[0] / 2) * (g.n[1] / 2) * (g.dim == 3 ? g.n[2] / 2 : 1);
     if constexpr (KIND != kKindPolygon) {
@@ -546,7 +569,7 @@ int hpmc_get_state(hpmc_ctx* c, float* d_pos4_out, float* d_quat4_out, hpmc_coun
                 !cuda_ok(c, cudaMemcpyAsync(d_quat4_out, c->d_quat_bound, bytes, cudaMemcpyDeviceToDevice, c->stream), "get_state/copy")) return HPMC_E_CUDA;
         } else {
             const int TB = 256;
-            k_unsort<<<(c->g.N + TB - 1) / TB, TB, 0, c->stream>>>(c->g.N, c->pos[c->cur], c->quat[c->cur], c->tag[c->cur],
+            k_unsort<<<(c->g.N + TB - 1) / TB, TB, 0, c->stream>>>(c->g.N, c->g.dim, c->pos[c->cur], c->quat[c->cur], c->tag[c->cur],
                                                                   (float4*)d_pos4_out, (float4*)d_quat4_out);
             LAUNCH_CHECK(c, "k_unsort");
         }
@@ -656,6 +679,9 @@ int hpmc_set_option(hpmc_ctx* c, const char* name, int64_t value)
     } else if (n == "tile_cap") {
         if (value < 0) return fail(c, HPMC_E_ARG, "tile_cap must be >= 0");
         c->opt_tile_cap = value > (1 << 30) ? (1 << 30) : (int)value;
+    } else if (n == "tile_shape") {
+        if (value < 0 || value > 4) return fail(c, HPMC_E_ARG, "tile_shape must be 0 (auto) or 1..4");
+        c->opt_tile_shape = (int)value;
     } else
         return fail(c, HPMC_E_ARG, "unknown option");
     return HPMC_OK;

@@ -38,6 +38,26 @@ struct TrialState {
     float qw, qx, qy, qz; // trial orientation
 };
 
+// sin and cos of the half rotation angle h, |h| <= a/2.  For a <= 1 rad (every config: a = 0.1) the Taylor series to
+// h^9 / h^10 is exact to fp32 rounding (next terms < 1.3e-11) and costs a dozen FMAs instead of sincosf's range reduction.
+__device__ __forceinline__ void small_sincos(float h, float a, float& sn, float& cs)
+{
+    if (a <= 1.0f) {
+        const float h2 = __fmul_rn(h, h);
+        float ps = __fmaf_rn(h2, 2.7557319e-6f, -1.9841270e-4f);
+        ps = __fmaf_rn(h2, ps, 8.3333333e-3f);
+        ps = __fmaf_rn(h2, ps, -1.6666667e-1f);
+        sn = __fmaf_rn(__fmul_rn(h, h2), ps, h);
+        float pc = __fmaf_rn(h2, -2.7557319e-7f, 2.4801587e-5f);
+        pc = __fmaf_rn(h2, pc, -1.3888889e-3f);
+        pc = __fmaf_rn(h2, pc, 4.1666667e-2f);
+        pc = __fmaf_rn(h2, pc, -0.5f);
+        cs = __fmaf_rn(h2, pc, 1.0f);
+    } else {
+        sincosf(h, &sn, &cs);
+    }
+}
+
 // a5 + a6: the trial pose of one move (R5-R7) and the leave-cell test (R13).  b0 = (select, type, ua, ub), uc = first
 // word of block 1 (3-D only).  Returns false iff a translation left `cell`.  One definition for every colour-pass
 // variant, so that they produce bit-identical trials.
@@ -56,7 +76,7 @@ __device__ __forceinline__ bool make_trial(const GridParams& g, const MoveParams
     }
     if (dim == 2) {                                   // R6, 2-D: angle about z
         float sn, cs;
-        sincosf(0.5f * __fmul_rn(mv.a, usym(b0.z)), &sn, &cs);
+        small_sincos(0.5f * __fmul_rn(mv.a, usym(b0.z)), mv.a, sn, cs);
         const float w = qp.x * cs - qp.w * sn, z = qp.x * sn + qp.w * cs;
         const float inv = rsqrtf(w * w + z * z);
         A.qw = w * inv; A.qx = 0.0f; A.qy = 0.0f; A.qz = z * inv;
@@ -147,8 +167,8 @@ __device__ void sweep_cell_global(const GridParams& g, const MoveParams& mv, con
                 if (g.dim == 3) uc = philox4x32_10((uint32_t)cell, t_lo, (uint32_t)k | (1u << 16), c3, k0, k1).x;
                 // a5: uniformly random member (R8), move type (R7)
                 const int p = start + (int)mulhi32(b0.x, (uint32_t)nmem);
-                const float4 xp = pos[p];
-                const float4 qp = quat[p];
+                float4 xp, qp;
+                load_state(g.dim, pos, quat, p, xp, qp);
                 TrialState A;
                 bool rotate;
                 int outcome = make_trial<KIND>(g, mv, shift, cell, g.dim, b0, uc, xp, qp, A, rotate) ? 1 : 2;   // a5, a6
@@ -181,13 +201,13 @@ __device__ void sweep_cell_global(const GridParams& g, const MoveParams& mv, con
                                 const int qs = cell_start[row + nx], qe = cell_start[row + nx + 1];
                                 for (int q = qs; q < qe; ++q) {
                                     if (q == p) continue;
-                                    const float4 xq = pos[q];
+                                    const float4 xq = pos[q];   // 2-D: the pose (x, y, qw, qz)
                                     const float rx = min_image(xq.x, A.x, g.hi[0], g.Ld[0]);
                                     const float ry = min_image(xq.y, A.y, g.hi[1], g.Ld[1]);
                                     const float rz = (g.dim == 3) ? min_image(xq.z, A.z, g.hi[2], g.Ld[2]) : 0.0f;
                                     if (rx * rx + ry * ry + rz * rz >= S.dmax2) continue;   // a8 circumsphere (R16)
                                     float4 qq = make_float4(1.f, 0.f, 0.f, 0.f);
-                                    if (KIND != kKindDisk) qq = quat[q];
+                                    if (KIND != kKindDisk) qq = (g.dim == 2) ? make_float4(xq.z, 0.f, 0.f, xq.w) : quat[q];
                                     double rd[3] = {0.0, 0.0, 0.0};
                                     if (KIND == kKindPolyhedron) {
                                         rd[0] = min_image_d(xq.x, A.x, g.Ld[0]);
@@ -209,8 +229,7 @@ __device__ void sweep_cell_global(const GridParams& g, const MoveParams& mv, con
                     if (x >= g.hi[0]) x = __fsub_rn(x, g.L[0]); else if (x < g.lo[0]) x = __fadd_rn(x, g.L[0]);
                     if (y >= g.hi[1]) y = __fsub_rn(y, g.L[1]); else if (y < g.lo[1]) y = __fadd_rn(y, g.L[1]);
                     if (g.dim == 3) { if (z >= g.hi[2]) z = __fsub_rn(z, g.L[2]); else if (z < g.lo[2]) z = __fadd_rn(z, g.L[2]); }
-                    if (!rotate) pos[p] = make_float4(x, y, z, xp.w);
-                    else quat[p] = make_float4(A.qw, A.qx, A.qy, A.qz);
+                    store_state(g.dim, pos, quat, p, make_float4(x, y, z, xp.w), make_float4(A.qw, A.qx, A.qy, A.qz), rotate);
                     if (rotate) ++c_racc; else ++c_tacc;
                 } else if (outcome == 2) {
                     ++c_trcell;
@@ -260,8 +279,8 @@ k_count_overlaps(const __grid_constant__ GridParams g, const __grid_constant__ S
     unsigned int found = 0;
     if (p < g.N) {
         const float shift[3] = {ctrl->hdr.shift[0], ctrl->hdr.shift[1], ctrl->hdr.shift[2]};
-        const float4 xp = pos[p];
-        const float4 qp = quat[p];
+        float4 xp, qp;
+        load_state(g.dim, pos, quat, p, xp, qp);
         const int tp = tag[p];
         int cx, cy, cz;
         cell_of(g, shift, xp.x, xp.y, xp.z, cx, cy, cz);
@@ -281,7 +300,8 @@ k_count_overlaps(const __grid_constant__ GridParams g, const __grid_constant__ S
                     const int c2 = nx + g.n[0] * (ny + g.n[1] * nz);
                     for (int q = cell_start[c2]; q < cell_start[c2 + 1]; ++q) {
                         if (tag[q] <= tp) continue;
-                        const float4 xq = pos[q];
+                        float4 xq, qq;
+                        load_state(g.dim, pos, quat, q, xq, qq);
                         double r[3] = {(double)xq.x - (double)xp.x, (double)xq.y - (double)xp.y, (double)xq.z - (double)xp.z};
                         for (int k = 0; k < g.dim; ++k) {
                             if (r[k] > 0.5 * g.Ld[k]) r[k] -= g.Ld[k];
@@ -292,7 +312,6 @@ k_count_overlaps(const __grid_constant__ GridParams g, const __grid_constant__ S
                         if (d2 >= S.dmax2) continue;
                         bool ov = true;
                         if (KIND != kKindDisk) {
-                            const float4 qq = quat[q];
                             const double nq = sqrt((double)qq.x * qq.x + (double)qq.y * qq.y + (double)qq.z * qq.z + (double)qq.w * qq.w);
                             const double w = qq.x / nq, x = qq.y / nq, y = qq.z / nq, z = qq.w / nq;
                             if (KIND == kKindPolygon) {

@@ -1,24 +1,28 @@
-// 2-D colour pass, tile version (S:8(a) rows a4-a11).
+// 2-D colour pass, tile version v3 (S:8(a) rows a4-a11).
 //
-// One CTA = a tile of 32 x TY active cells of the current colour (one warp per row of 32 active cells, one lane
-// per cell).  The CTA first stages every particle of the (2*32+1) x (2*TY+1) cell region around its tile into
-// shared memory as compact float4 (x, y, qw, qz) with coalesced loads (a7: "neighbour gather staged in shared
-// memory").  After that the warps are independent: active cells of one colour never share a neighbour cell's
-// *writes* (their 3x3 blocks only overlap in inactive cells), so everything below the staging
-// barrier is warp-synchronous:
+// One CTA = a tile of 32 x (WARPS*R) active cells of the current colour.  The CTA stages every pose of the
+// (2*32+1) x (2*WARPS*R+1) cell region around its tile into shared memory (a7: "neighbour gather staged in shared
+// memory").  Cells of a row are contiguous in the cell-sorted pose array, so a region row is one contiguous run
+// (two at the periodic wrap): 2*RH segment copies, fully coalesced, and a local CSR of 16-bit offsets.
 //
-//   A  every lane generates trial k of its cell (Philox -> member, move type, displacement; leave-cell test
-//      with the pinned cell function), runs the circumsphere broad phase over the three staged row runs of its
-//      3x3 block and turns the hits into a bit mask; centres closer than the inscribed-disk bound are decided
-//      on the spot.  The warp packs all (lane, neighbour) hits into a per-warp queue in shared memory.
-//   B  the queue is drained densely: lane e takes entry e, e+32, ... and runs the branch-free separating-axis
-//      test; an overlap sets the owner's flag.  This is the paper's block queue at warp scope:
-//      lanes no longer idle while one neighbour of one trial is in its narrow phase.
-//   C  owners read their flag, accepted moves are written to the staged copy (so trial k+1 of the cell sees it)
-//      and to global memory.
+// After the staging barrier the warps are independent (active cells of one colour never read each other's writes,
+// P:21).  A warp owns R rows of 32 active cells.  It first compacts its NON-EMPTY cells (ballot/popc) so that
+// every lane of every round has work, then for each of the n_select trial rounds:
 //
-// A tile whose region holds more particles than the staging capacity falls back to the per-thread global
-// path (sweep_cell_global); results are identical.
+//   A  each lane takes up to R cells in turn: Philox block -> member, move type, trial pose (a0, a5), leave-cell test
+//      with the pinned cell function (a6), circumsphere broad phase over the three staged row runs of the cell's 3x3
+//      block (a8); centres inside the inscribed-disk bound reject on the spot; the remaining hits are appended to the
+//      warp's queue in shared memory (a10) as (owner slot, neighbour).
+//   B  the queue (~60 R entries) is drained densely, one entry per lane: branch-free separating-axis test (a9); an
+//      overlap sets the owner's flag.  This is the paper's block queue at warp scope: lanes do not idle
+//      while one neighbour of one trial is in its narrow phase, and R cells per lane keep the last
+//      32-entry batch from running nearly empty.
+//   C  owners read their flag; accepted poses go to the staged copy (trial k+1 of the cell sees them) and to global
+//      memory (a11).
+//
+// Only tiles whose region touches the periodic seam use the fp64 minimum image (R21): elsewhere every compared pair is
+// closer than 2w <= L/2 and the plain fp32 difference is the same number.  A tile whose region holds more particles
+// than the staging capacity falls back to the per-thread global path (sweep_cell_global); results are identical.
 #pragma once
 #include "common.cuh"
 #include "overlap.cuh"
@@ -26,263 +30,319 @@
 
 namespace hpmc {
 
-constexpr int kTileW = 32;                    // active cells per tile row = lanes of a warp
-constexpr int kRegionW = 2 * kTileW + 1;      // staged cells per region row
-constexpr int kCapPerCell = 2;                // staging capacity in particles per region cell (pentagon fluid: ~1)
-constexpr int kWarpQueueCap = 160;            // narrow-phase queue entries per warp and trial round
+constexpr int kTileW = 32;   // active cells per tile row = lanes of a warp
 
-template <int TY>
+template <int WARPS, int R>
 struct Tile2D {
-    static constexpr int NT = 32 * TY;
-    static constexpr int RH = 2 * TY + 1;
-    static constexpr int NCELLS = kRegionW * RH;
-    static constexpr int CAP = kCapPerCell * NCELLS;
-    static constexpr int CPT = (NCELLS + NT - 1) / NT;   // region cells per thread while staging
+    static constexpr int NT = 32 * WARPS;
+    static constexpr int TH = WARPS * R;                 // active rows per tile
+    static constexpr int RW = 2 * kTileW + 1;            // staged cells per region row
+    static constexpr int RH = 2 * TH + 1;                // staged region rows
+    static constexpr int NCELLS = RW * RH;
+    static constexpr int CAP = (NCELLS * 5 / 4 + 63) / 64 * 64;   // staged poses (pentagon fluid: ~1.0 per cell)
+    static constexpr int NSEG = 2 * RH;                  // contiguous runs: two per region row (periodic wrap in x)
+    static constexpr int QCAP = 96 * R;                  // narrow-phase queue entries per warp and trial round
+    static constexpr int SLOTS = 32 * R;                 // trial slots per warp and round
+    static_assert(NSEG + 1 <= NT, "one thread per segment");
+    static_assert(CAP < 65536, "16-bit local offsets");
     // shared-memory carve (bytes)
     static constexpr size_t off_pose = 0;
     static constexpr size_t off_trial = off_pose + sizeof(float4) * CAP;
-    static constexpr size_t off_gidx = off_trial + sizeof(float4) * NT;
-    static constexpr size_t off_lstart = off_gidx + sizeof(int) * CAP;
-    static constexpr size_t off_queue = off_lstart + sizeof(int) * (NCELLS + 1);
-    static constexpr size_t off_wsum = off_queue + sizeof(unsigned) * TY * kWarpQueueCap;
-    static constexpr size_t off_flag = off_wsum + sizeof(int) * CPT * TY;
-    static constexpr size_t bytes = off_flag + sizeof(unsigned) * NT;
+    static constexpr size_t off_queue = off_trial + sizeof(float4) * SLOTS * WARPS;
+    static constexpr size_t off_seg_g = off_queue + sizeof(unsigned) * QCAP * WARPS;
+    static constexpr size_t off_seg_l = off_seg_g + sizeof(int) * NSEG;
+    static constexpr size_t off_qcount = off_seg_l + sizeof(int) * (NSEG + 1);
+    static constexpr size_t off_lstart = off_qcount + sizeof(int) * WARPS;
+    static constexpr size_t off_flag = off_lstart + ((sizeof(unsigned short) * (NCELLS + 1) + 15) / 16) * 16;
+    static constexpr size_t off_act = off_flag + SLOTS * WARPS;
+    static constexpr size_t bytes = off_act + SLOTS * WARPS;
 };
 
 // narrow phase of trial pose A against staged pose B, both (x, y, qw, qz); true = overlap (R15 guard band)
 template <int KIND, int NV>
-__device__ __forceinline__ bool pair_overlap_2d(const GridParams& g, const ShapeF& S, const float4& A, const float4& B, float eps)
+__device__ __forceinline__ bool pair_overlap_2d(const GridParams& g, const ShapeF& S, const float4& A, const float4& B, float eps, bool seam)
 {
-    const float rx = min_image(B.x, A.x, g.hi[0], g.Ld[0]);
-    const float ry = min_image(B.y, A.y, g.hi[1], g.Ld[1]);
+    float rx = B.x - A.x, ry = B.y - A.y;
+    if (seam) {
+        rx = min_image(B.x, A.x, g.hi[0], g.Ld[0]);
+        ry = min_image(B.y, A.y, g.hi[1], g.Ld[1]);
+    }
     if (KIND == kKindDisk) return rx * rx + ry * ry < S.dmax2;
     const float cA = A.z * A.z - A.w * A.w, sA = 2.0f * A.z * A.w;   // cos t = w^2 - z^2, sin t = 2wz (R30)
     const float cB = B.z * B.z - B.w * B.w, sB = 2.0f * B.z * B.w;
     return !(polygon_max_sep<float, NV>(S, rx, ry, cA, sA, cB, sB) >= eps);
 }
 
-template <int KIND, int NV, int TY>
-__global__ void __launch_bounds__(32 * TY)
+// out-of-line copy for the rare direct evaluations (queue overflow, > 32 candidates): keeps the hot loop's code small
+template <int KIND, int NV>
+__device__ __noinline__ bool pair_overlap_2d_cold(const GridParams& g, const ShapeF& S, float4 A, float4 B, float eps)
+{
+    return pair_overlap_2d<KIND, NV>(g, S, A, B, eps, true);
+}
+
+template <int KIND, int NV, int WARPS, int R>
+__global__ void __launch_bounds__(32 * WARPS)
 k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ MoveParams mv, const __grid_constant__ ShapeF S,
                const __grid_constant__ ShapeD SD, Control* __restrict__ ctrl, int colour_index, int cap_limit,
-               float4* __restrict__ pos, float4* __restrict__ quat, const int* __restrict__ tag,
-               const int* __restrict__ cell_start, uint32_t k0, uint32_t k1, uint2* __restrict__ trace)
+               float4* __restrict__ pose, const int* __restrict__ tag, const int* __restrict__ cell_start, uint32_t k0,
+               uint32_t k1, uint2* __restrict__ trace)
 {
-    using TL = Tile2D<TY>;
+    using TL = Tile2D<WARPS, R>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    float4* sm_pose = reinterpret_cast<float4*>(smem_raw + TL::off_pose);     // staged (x, y, qw, qz)
-    float4* sm_trial = reinterpret_cast<float4*>(smem_raw + TL::off_trial);   // trial pose of every lane
-    int* sm_gidx = reinterpret_cast<int*>(smem_raw + TL::off_gidx);           // global (cell-sorted) index
-    int* sm_lstart = reinterpret_cast<int*>(smem_raw + TL::off_lstart);       // local CSR over region cells
+    float4* sm_pose = reinterpret_cast<float4*>(smem_raw + TL::off_pose);       // staged (x, y, qw, qz)
+    float4* sm_trial = reinterpret_cast<float4*>(smem_raw + TL::off_trial);     // trial pose of every slot
     unsigned* sm_queue = reinterpret_cast<unsigned*>(smem_raw + TL::off_queue);
-    int* sm_wsum = reinterpret_cast<int*>(smem_raw + TL::off_wsum);
-    unsigned* sm_flag = reinterpret_cast<unsigned*>(smem_raw + TL::off_flag);
+    int* sm_seg_g = reinterpret_cast<int*>(smem_raw + TL::off_seg_g);           // global start of each segment
+    int* sm_seg_l = reinterpret_cast<int*>(smem_raw + TL::off_seg_l);           // local start of each segment (+ total)
+    int* sm_qcount = reinterpret_cast<int*>(smem_raw + TL::off_qcount);
+    unsigned short* sm_lstart = reinterpret_cast<unsigned short*>(smem_raw + TL::off_lstart);   // local CSR over region cells
+    unsigned char* sm_flag = smem_raw + TL::off_flag;
+    unsigned char* sm_act = smem_raw + TL::off_act;
 
     const SweepHeader& H = ctrl->hdr;
     const int gamma = H.perm[colour_index];
     const uint32_t t_lo = H.t_lo, t_hi16 = H.t_hi16;
     const float shift[3] = {H.shift[0], H.shift[1], 0.0f};
     const int gx = gamma & 1, gy = (gamma >> 1) & 1;
-    const int nax = g.n[0] >> 1, nay = g.n[1] >> 1;
+    const int n0 = g.n[0], n1 = g.n[1];
+    const int nax = n0 >> 1, nay = n1 >> 1;
     const int tiles_x = (nax + kTileW - 1) / kTileW;
     const int tx = blockIdx.x % tiles_x, ty = blockIdx.x / tiles_x;
-    const int ix0 = tx * kTileW, iy0 = ty * TY;
+    const int ix0 = tx * kTileW, iy0 = ty * TL::TH;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    // region = cells [cx0-1, cx0-1+RW) x [cy0-1, cy0-1+RHv), clipped to what the valid active cells of the tile need
+    // region = cells [cx0-1, cx0-1+RW) x [cy0-1, cy0-1+RHv) (unwrapped), clipped to what the valid active cells need
     const int cx0 = 2 * ix0 + gx, cy0 = 2 * iy0 + gy;
-    const int RW = 2 * min(kTileW, nax - ix0) + 1, RHv = 2 * min(TY, nay - iy0) + 1;
+    const int RW = 2 * min(kTileW, nax - ix0) + 1, RHv = 2 * min(TL::TH, nay - iy0) + 1;
     const int ncells = RW * RHv;
+    int xs = cx0 - 1;                       // first region column, wrapped
+    xs += (xs < 0) ? n0 : 0;
+    const int split = min(RW, n0 - xs);     // columns before the periodic wrap in x
+    // the region touches the seam iff it contains cell n-1 (which holds coordinates near both box edges) or wraps
+    const bool seam = (cx0 - 1 < 0) || (cx0 - 1 + RW - 1 >= n0 - 1) || (cy0 - 1 < 0) || (cy0 - 1 + RHv - 1 >= n1 - 1);
 
-    // ---- staging: region cell counts -> local CSR (prefix sum) -> coalesced copy ------------------------------
-    int cs[TL::CPT], cnt[TL::CPT], inc[TL::CPT];
-#pragma unroll
-    for (int j = 0; j < TL::CPT; ++j) {
-        const int lc = j * TL::NT + tid;
-        cs[j] = 0; cnt[j] = 0;
-        if (lc < ncells) {
-            const int ry = lc / RW, rx = lc - ry * RW;
-            int cx = cx0 - 1 + rx, cy = cy0 - 1 + ry;
-            cx += (cx < 0) ? g.n[0] : 0; cx -= (cx >= g.n[0]) ? g.n[0] : 0;
-            cy += (cy < 0) ? g.n[1] : 0; cy -= (cy >= g.n[1]) ? g.n[1] : 0;
-            const int c = cx + g.n[0] * cy;
-            cs[j] = cell_start[c];
-            cnt[j] = cell_start[c + 1] - cs[j];
+    // ---- staging 1: the contiguous runs of the region rows -------------------------------------------------------
+    if (tid < TL::NSEG) {
+        const int ry = tid >> 1, second = tid & 1;
+        int gb = 0, len = 0;
+        if (ry < RHv) {
+            int cy = cy0 - 1 + ry;
+            cy += (cy < 0) ? n1 : 0;
+            cy -= (cy >= n1) ? n1 : 0;
+            const int first = second ? 0 : xs, ncol = second ? RW - split : split;
+            if (ncol > 0) {
+                gb = cell_start[cy * n0 + first];
+                len = cell_start[cy * n0 + first + ncol] - gb;
+            }
         }
-        int v = cnt[j];
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int n = __shfl_up_sync(0xffffffffu, v, o);
-            if (lane >= o) v += n;
-        }
-        inc[j] = v;
-        if (lane == 31) sm_wsum[j * TY + warp] = v;
+        sm_seg_g[tid] = gb;
+        sm_seg_l[tid] = len;
     }
     __syncthreads();
-    int run = 0, mybase[TL::CPT];
+    if (warp == 0) {   // exclusive scan of the segment lengths
+        int carry = 0;
 #pragma unroll
-    for (int j = 0; j < TL::CPT; ++j)
+        for (int b = 0; b < (TL::NSEG + 31) / 32; ++b) {
+            const int i = b * 32 + lane;
+            const int v = (i < TL::NSEG) ? sm_seg_l[i] : 0;
+            int inc = v;
 #pragma unroll
-        for (int w = 0; w < TY; ++w) {
-            if (w == warp) mybase[j] = run;
-            run += sm_wsum[j * TY + w];
+            for (int o = 1; o < 32; o <<= 1) {
+                const int n = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += n;
+            }
+            __syncwarp();
+            if (i < TL::NSEG) sm_seg_l[i] = carry + inc - v;
+            carry += __shfl_sync(0xffffffffu, inc, 31);
         }
-    const int ntot = run;
+        if (lane == 0) sm_seg_l[TL::NSEG] = carry;
+    }
+    __syncthreads();
+    const int ntot = sm_seg_l[TL::NSEG];
     const bool staged = ntot <= min(cap_limit, TL::CAP);   // block-uniform
-    const bool valid = (ix0 + lane < nax) && (iy0 + warp < nay);
-    const int cx = cx0 + 2 * lane, cy = cy0 + 2 * warp;     // this lane's active cell
     CellCounters cc;
 
     if (!staged) {
         // overflow: more particles around this tile than the staging buffers hold -> per-thread global path
-        if (valid)
-            sweep_cell_global<KIND, NV>(g, mv, S, SD, gamma, t_lo, t_hi16, shift, cx, cy, 0, pos, quat, tag, cell_start, k0, k1,
-                                        trace, cc);
+#pragma unroll 1
+        for (int j = 0; j < R; ++j) {
+            const int ay = warp * R + j;
+            if (ix0 + lane < nax && iy0 + ay < nay)
+                sweep_cell_global<KIND, NV>(g, mv, S, SD, gamma, t_lo, t_hi16, shift, cx0 + 2 * lane, cy0 + 2 * ay, 0, pose, nullptr, tag,
+                                            cell_start, k0, k1, trace, cc);
+        }
         flush_counters(ctrl, cc);
         return;
     }
 
-#pragma unroll
-    for (int j = 0; j < TL::CPT; ++j) {
-        const int lc = j * TL::NT + tid;
-        if (lc < ncells) {
-            const int l0 = mybase[j] + inc[j] - cnt[j];
-            sm_lstart[lc] = l0;
-            for (int m = 0; m < cnt[j]; ++m) {
-                const int gi = cs[j] + m;
-                const float4 P = pos[gi];
-                float4 Q = make_float4(1.f, 0.f, 0.f, 0.f);
-                if (KIND != kKindDisk) Q = quat[gi];
-                sm_pose[l0 + m] = make_float4(P.x, P.y, Q.x, Q.w);
-                sm_gidx[l0 + m] = gi;
-            }
-        }
+    // ---- staging 2: local CSR (16-bit) and the poses, coalesced ---------------------------------------------------
+    for (int lc = tid; lc < ncells; lc += TL::NT) {
+        const int ry = lc / RW, rx = lc - ry * RW;
+        int cy = cy0 - 1 + ry;
+        cy += (cy < 0) ? n1 : 0;
+        cy -= (cy >= n1) ? n1 : 0;
+        const int second = rx >= split;
+        const int cx = second ? rx - split : xs + rx;
+        const int seg = 2 * ry + second;
+        sm_lstart[lc] = (unsigned short)(cell_start[cy * n0 + cx] - sm_seg_g[seg] + sm_seg_l[seg]);
     }
-    if (tid == 0) sm_lstart[ncells] = ntot;
+    if (tid == 0) sm_lstart[ncells] = (unsigned short)ntot;
+    for (int seg = warp; seg < 2 * RHv; seg += WARPS) {
+        const int gb = sm_seg_g[seg], lb = sm_seg_l[seg], len = sm_seg_l[seg + 1] - lb;
+        for (int e = lane; e < len; e += 32) sm_pose[lb + e] = pose[gb + e];
+    }
     __syncthreads();
 
-    // ---- per-lane constants: own cell and the three row runs of its 3x3 block (local indices) -----------------
-    const int cell = cx + g.n[0] * cy;
-    const long long slot0 = (long long)cell * mv.n_select;
-    int own_s = 0, nmem = 0, rs[3] = {0, 0, 0}, re[3] = {0, 0, 0};
-    if (valid) {
-        const int rxl = 2 * lane + 1, ryl = 2 * warp + 1;
-        const int lc = ryl * RW + rxl;
-        own_s = sm_lstart[lc];
-        nmem = sm_lstart[lc + 1] - own_s;
+    // ---- this warp's non-empty active cells, compacted: sm_act[slot] = j*32 + lane of the cell ---------------------
+    unsigned char* my_act = sm_act + warp * TL::SLOTS;
+    unsigned char* my_flag = sm_flag + warp * TL::SLOTS;
+    float4* my_trial = sm_trial + warp * TL::SLOTS;
+    unsigned* my_queue = sm_queue + warp * TL::QCAP;
+    int n_act = 0;
 #pragma unroll
-        for (int dy = 0; dy < 3; ++dy) {
-            const int row = (ryl + dy - 1) * RW + rxl;
-            rs[dy] = sm_lstart[row - 1];
-            re[dy] = sm_lstart[row + 2];
+    for (int j = 0; j < R; ++j) {
+        const int ay = warp * R + j;
+        const bool valid = (ix0 + lane < nax) && (iy0 + ay < nay);
+        int nmem = 0;
+        if (valid) {
+            const int lc = (2 * ay + 1) * RW + 2 * lane + 1;
+            nmem = (int)sm_lstart[lc + 1] - (int)sm_lstart[lc];
+            if (nmem == 0 && trace) {
+                const long long slot0 = (long long)((cx0 + 2 * lane) + n0 * (cy0 + 2 * ay)) * mv.n_select;
+                for (int k = 0; k < mv.n_select; ++k) trace[slot0 + k] = make_uint2(0u, 0u);
+            }
         }
+        const unsigned bal = __ballot_sync(0xffffffffu, nmem > 0);
+        if (nmem > 0) my_act[n_act + __popc(bal & ((1u << lane) - 1u))] = (unsigned char)(j * 32 + lane);
+        n_act += __popc(bal);
     }
-    const bool act = valid && nmem > 0;
-    if (valid && !act && trace)
-        for (int k = 0; k < mv.n_select; ++k) trace[slot0 + k] = make_uint2(0u, 0u);
-    const int n0 = re[0] - rs[0], n01 = n0 + (re[1] - rs[1]);
-    unsigned* my_queue = sm_queue + warp * kWarpQueueCap;
+    __syncwarp();
+    const int nrounds = (n_act + 31) >> 5;
     const uint32_t c3 = (kTagTrial << 24) | ((uint32_t)gamma << 16) | t_hi16;
 
     for (int k = 0; k < mv.n_select; ++k) {
-        // ---- phase A: trial generation (a0, a5, a6) + broad phase (a8) --------------------------------------
-        int p = 0, outcome = 0;
-        bool rotate = false, own_ov = false;
-        float4 T = make_float4(0.f, 0.f, 1.f, 0.f);
-        unsigned mask = 0u;
-        if (act) {
-            const U4 b0 = philox4x32_10((uint32_t)cell, t_lo, (uint32_t)k, c3, k0, k1);
-            p = own_s + (int)mulhi32(b0.x, (uint32_t)nmem);                 // R8
-            rotate = (KIND != kKindDisk) && (b0.y >> 31);                    // R7
-            const float4 P = sm_pose[p];
-            T = P;
-            outcome = 1;
-            ++cc.trials;
-            if (!rotate) {
-                T.x = __fmaf_rn(mv.d, usym(b0.z), P.x);                      // R5
-                T.y = __fmaf_rn(mv.d, usym(b0.w), P.y);
-                int tcx, tcy, tcz;
-                if (cell_of(g, shift, T.x, T.y, 0.0f, tcx, tcy, tcz) != cell) outcome = 2;   // a6, R13
-            } else {                                                         // R6, 2-D
-                float sn, cs_;
-                sincosf(0.5f * __fmul_rn(mv.a, usym(b0.z)), &sn, &cs_);
-                const float w = P.z * cs_ - P.w * sn, z = P.z * sn + P.w * cs_;
-                const float inv = rsqrtf(w * w + z * z);
-                T.z = w * inv;
-                T.w = z * inv;
-            }
-            if (outcome == 1) {
-                int bit = 0;
+        if (lane == 0) sm_qcount[warp] = 0;
+        __syncwarp();
+        // per-slot state kept in registers between phases A and C: member index | rotate<<16 | outcome<<17 | sure<<19
+        unsigned st[R];
+        // ---- phase A: trial generation (a0, a5, a6) + broad phase (a8) + queue fill (a10) ------------------------
 #pragma unroll
-                for (int dy = 0; dy < 3; ++dy) {
-                    for (int q = rs[dy]; q < re[dy]; ++q, ++bit) {
-                        if (q == p) continue;
-                        const float4 B = sm_pose[q];
-                        const float rx = min_image(B.x, T.x, g.hi[0], g.Ld[0]);
-                        const float ry = min_image(B.y, T.y, g.hi[1], g.Ld[1]);
-                        const float d2 = rx * rx + ry * ry;
-                        if (d2 >= S.dmax2) continue;                          // a8 circumsphere (R16)
-                        if (KIND == kKindDisk || d2 < S.din2) own_ov = true;  // inside the inscribed-disk bound
-                        else if (bit < 32) mask |= 1u << bit;
-                        else if (!own_ov) own_ov = pair_overlap_2d<KIND, NV>(g, S, T, B, mv.eps_g);   // > 32 candidates
+        for (int s = 0; s < R; ++s) {
+            st[s] = 0u;
+            if (s < nrounds) {
+                const int slot = s * 32 + lane;
+                if (slot < n_act) {
+                    const int id = my_act[slot];
+                    const int ay = warp * R + (id >> 5), al = id & 31;
+                    const int rxl = 2 * al + 1, ryl = 2 * ay + 1;
+                    const int cell = (cx0 + 2 * al) + n0 * (cy0 + 2 * ay);
+                    const int lc = ryl * RW + rxl;
+                    const int own_s = sm_lstart[lc], nmem = (int)sm_lstart[lc + 1] - own_s;
+                    const U4 b0 = philox4x32_10((uint32_t)cell, t_lo, (uint32_t)k, c3, k0, k1);
+                    const int p = own_s + (int)mulhi32(b0.x, (uint32_t)nmem);                 // R8
+                    const float4 P = sm_pose[p];
+                    TrialState A;
+                    bool rotate;
+                    const bool inside = make_trial<KIND>(g, mv, shift, cell, 2, b0, 0u, make_float4(P.x, P.y, 0.f, 0.f),
+                                                         make_float4(P.z, 0.f, 0.f, P.w), A, rotate);
+                    const float4 T = make_float4(A.x, A.y, A.qw, A.qz);
+                    my_trial[slot] = T;
+                    my_flag[slot] = 0;
+                    unsigned outcome = inside ? 1u : 2u;
+                    ++cc.trials;
+                    bool sure = false;
+                    if (inside) {
+                        unsigned mask = 0u;
+                        int bit = 0;
+                        int rs[3], re[3];
+#pragma unroll
+                        for (int dy = 0; dy < 3; ++dy) {
+                            const int row = (ryl + dy - 1) * RW + rxl;
+                            rs[dy] = sm_lstart[row - 1];
+                            re[dy] = sm_lstart[row + 2];
+                        }
+#pragma unroll
+                        for (int dy = 0; dy < 3; ++dy) {
+                            for (int q = rs[dy]; q < re[dy]; ++q, ++bit) {
+                                if (q == p) continue;
+                                const float4 B = sm_pose[q];
+                                float rx = B.x - T.x, ry = B.y - T.y;
+                                if (seam) {
+                                    rx = min_image(B.x, T.x, g.hi[0], g.Ld[0]);
+                                    ry = min_image(B.y, T.y, g.hi[1], g.Ld[1]);
+                                }
+                                const float d2 = rx * rx + ry * ry;
+                                if (d2 >= S.dmax2) continue;                          // a8 circumsphere (R16)
+                                if (KIND == kKindDisk || d2 < S.din2) sure = true;    // inside the inscribed-disk bound
+                                else if (bit < 32) mask |= 1u << bit;
+                                else if (!sure) sure = pair_overlap_2d_cold<KIND, NV>(g, S, T, B, mv.eps_g);   // > 32 candidates
+                            }
+                        }
+                        if (KIND != kKindDisk && !sure && mask) {                     // early exit otherwise
+                            int at = atomicAdd(&sm_qcount[warp], __popc(mask));
+                            const int n_0 = re[0] - rs[0], n_01 = n_0 + (re[1] - rs[1]);
+                            while (mask) {
+                                const int b = __ffs(mask) - 1;
+                                mask &= mask - 1u;
+                                const int q = (b < n_0) ? rs[0] + b : (b < n_01) ? rs[1] + (b - n_0) : rs[2] + (b - n_01);
+                                if (at < TL::QCAP) my_queue[at] = ((unsigned)slot << 16) | (unsigned)q;
+                                else if (!sure) sure = pair_overlap_2d_cold<KIND, NV>(g, S, T, sm_pose[q], mv.eps_g);   // queue full
+                                ++at;
+                            }
+                        }
                     }
+                    st[s] = (unsigned)p | (rotate ? 1u << 16 : 0u) | (outcome << 17) | (sure ? 1u << 19 : 0u);
                 }
-                if (own_ov) mask = 0u;                                        // early exit
             }
         }
+        __syncwarp();
+        // ---- phase B: dense narrow phase (a9) --------------------------------------------------------------------------
         if (KIND != kKindDisk) {
-            // pack the hits of all lanes into the warp queue (a10)
-            const int c = __popc(mask);
-            int incl = c;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int n = __shfl_up_sync(0xffffffffu, incl, o);
-                if (lane >= o) incl += n;
-            }
-            const int total = __shfl_sync(0xffffffffu, incl, 31);
-            int slot = incl - c;
-            sm_trial[tid] = T;
-            sm_flag[tid] = 0u;
-            while (mask) {
-                const int b = __ffs(mask) - 1;
-                mask &= mask - 1u;
-                const int q = (b < n0) ? rs[0] + b : (b < n01) ? rs[1] + (b - n0) : rs[2] + (b - n01);
-                if (slot < kWarpQueueCap) my_queue[slot] = ((unsigned)lane << 24) | (unsigned)q;
-                else if (!own_ov) own_ov = pair_overlap_2d<KIND, NV>(g, S, T, sm_pose[q], mv.eps_g);   // queue full
-                ++slot;
-            }
-            __syncwarp();
-            // ---- phase B: dense narrow phase (a9) -----------------------------------------------------------
-            const int nq = min(total, kWarpQueueCap);
+            const int nq = min(sm_qcount[warp], TL::QCAP);
             for (int e = lane; e < nq; e += 32) {
                 const unsigned ent = my_queue[e];
-                const int o = (int)(ent >> 24), q = (int)(ent & 0xffffffu);
-                if (pair_overlap_2d<KIND, NV>(g, S, sm_trial[(warp << 5) + o], sm_pose[q], mv.eps_g)) sm_flag[(warp << 5) + o] = 1u;
+                const int o = (int)(ent >> 16), q = (int)(ent & 0xffffu);
+                if (pair_overlap_2d<KIND, NV>(g, S, my_trial[o], sm_pose[q], mv.eps_g, seam)) my_flag[o] = 1;
             }
             __syncwarp();
-            if (sm_flag[tid]) own_ov = true;
         }
-        // ---- phase C: accept / write back (a11) ---------------------------------------------------------------
-        if (act) {
-            if (outcome == 1 && own_ov) outcome = 3;
-            if (outcome == 1) {
-                if (!rotate) {
-                    float x = T.x, y = T.y;
-                    if (x >= g.hi[0]) x = __fsub_rn(x, g.L[0]); else if (x < g.lo[0]) x = __fadd_rn(x, g.L[0]);
-                    if (y >= g.hi[1]) y = __fsub_rn(y, g.L[1]); else if (y < g.lo[1]) y = __fadd_rn(y, g.L[1]);
-                    T.x = x; T.y = y;
-                    pos[sm_gidx[p]] = make_float4(x, y, 0.0f, 0.0f);
-                    ++cc.tacc;
+        // ---- phase C: accept / write back (a11) ---------------------------------------------------------------------------
+#pragma unroll
+        for (int s = 0; s < R; ++s) {
+            const unsigned outcome0 = (st[s] >> 17) & 3u;
+            if (outcome0 != 0u) {
+                const int slot = s * 32 + lane;
+                const int p = (int)(st[s] & 0xffffu);
+                const bool rotate = (st[s] >> 16) & 1u;
+                unsigned outcome = outcome0;
+                if (outcome == 1u && (((st[s] >> 19) & 1u) || my_flag[slot])) outcome = 3u;
+                const int id = my_act[slot];
+                const int ay = warp * R + (id >> 5), al = id & 31;
+                const int ryl = 2 * ay + 1, rxl = 2 * al + 1;
+                const int seg = 2 * ryl + (rxl >= split ? 1 : 0);
+                const int gi = sm_seg_g[seg] + (p - sm_seg_l[seg]);
+                if (outcome == 1u) {
+                    float4 T = my_trial[slot];
+                    if (!rotate) {
+                        float x = T.x, y = T.y;
+                        if (x >= g.hi[0]) x = __fsub_rn(x, g.L[0]); else if (x < g.lo[0]) x = __fadd_rn(x, g.L[0]);
+                        if (y >= g.hi[1]) y = __fsub_rn(y, g.L[1]); else if (y < g.lo[1]) y = __fadd_rn(y, g.L[1]);
+                        T.x = x; T.y = y;
+                        ++cc.tacc;
+                    } else {
+                        ++cc.racc;
+                    }
+                    pose[gi] = T;
+                    sm_pose[p] = T;
+                } else if (outcome == 2u) {
+                    ++cc.trcell;
                 } else {
-                    quat[sm_gidx[p]] = make_float4(T.z, 0.0f, 0.0f, T.w);
-                    ++cc.racc;
+                    if (rotate) ++cc.rrov; else ++cc.trov;
                 }
-                sm_pose[p] = T;
-            } else if (outcome == 2) {
-                ++cc.trcell;
-            } else {
-                if (rotate) ++cc.rrov; else ++cc.trov;
+                if (trace) {
+                    const long long slot0 = (long long)((cx0 + 2 * al) + n0 * (cy0 + 2 * ay)) * mv.n_select;
+                    trace[slot0 + k] = make_uint2((uint32_t)tag[gi], (rotate ? 1u : 0u) | (outcome << 8));
+                }
             }
-            if (trace) trace[slot0 + k] = make_uint2((uint32_t)tag[sm_gidx[p]], (rotate ? 1u : 0u) | ((uint32_t)outcome << 8));
         }
         __syncwarp();
     }

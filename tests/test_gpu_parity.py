@@ -136,7 +136,8 @@ def test_colour_pass_variants_agree_bit_for_bit(name):
     w = CASES[name]()
     ref = None
     some = 40 if w.dim == 2 else (84 if w.kind == wl.KIND_POLYHEDRON else 50)   # a capacity only some tiles/cells exceed
-    for opts in ({"path": 2}, {"path": 2, "tile_cap": 0}, {"path": 1}, {"path": 2, "tile_cap": some}):
+    shapes = [{"tile_shape": k} for k in (1, 2, 3, 4)] if w.dim == 2 else []   # every 2-D tile shape
+    for opts in [{"path": 2}, {"path": 2, "tile_cap": 0}, {"path": 1}, {"path": 2, "tile_cap": some}] + shapes:
         g = gpu(w)
         for k, v in opts.items():
             g.set_option(k, v)
