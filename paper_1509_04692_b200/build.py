@@ -22,7 +22,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_source():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + ["-o", LIB] + SOURCES
+    fast = ["-DHPMC_FAST_BUILD"] if os.environ.get("HPMC_FAST_BUILD") == "1" else []   # development: fewer unrolled polygon sizes
+    cmd = [nvcc] + NVCC_FLAGS + fast + ["-o", LIB] + SOURCES
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode != 0:
         print(res.stdout)

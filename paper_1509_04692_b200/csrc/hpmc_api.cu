@@ -306,12 +306,12 @@ int build_cell_list(hpmc_ctx* c, int mode, unsigned long long t_override)
     return HPMC_OK;
 }
 
-template <int KIND, int NV, int WARPS, int R>
+template <int KIND, int NV, int WARPS, int R, int MINB>
 bool launch_tile2d(hpmc_ctx* c, int ci)
 {
     using TL = Tile2D<WARPS, R>;
     const GridParams& g = c->g;
-    auto kern = k_sweep_tile2d<KIND, NV, WARPS, R>;
+    auto kern = k_sweep_tile2d<KIND, NV, WARPS, R, MINB>;
     static bool attr_set = false;   // per template instance
     if (!attr_set) {
         if (!cuda_ok(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TL::bytes), "tile/attr")) return false;
@@ -343,10 +343,13 @@ bool launch_colour(hpmc_ctx* c, int ci)
     if constexpr (KIND != kKindPolyhedron) {
         if (g.dim == 2 && c->opt_path != 1) {
             switch (pick_tile_shape(c)) {
-                case 1: return launch_tile2d<KIND, NV, 8, 2>(c, ci);
-                case 2: return launch_tile2d<KIND, NV, 4, 2>(c, ci);
-                case 3: return launch_tile2d<KIND, NV, 4, 1>(c, ci);
-                default: return launch_tile2d<KIND, NV, 2, 1>(c, ci);
+                case 1: return launch_tile2d<KIND, NV, 8, 2, 2>(c, ci);
+                case 2: return launch_tile2d<KIND, NV, 4, 2, 4>(c, ci);
+                case 3: return launch_tile2d<KIND, NV, 4, 1, 5>(c, ci);
+                case 5: return launch_tile2d<KIND, NV, 4, 1, 8>(c, ci);
+                case 6: return launch_tile2d<KIND, NV, 8, 1, 3>(c, ci);
+                case 7: return launch_tile2d<KIND, NV, 4, 1, 6>(c, ci);
+                default: return launch_tile2d<KIND, NV, 2, 1, 8>(c, ci);
             }
         }
     }
@@ -373,11 +376,13 @@ int launch_colour_dispatch(hpmc_ctx* c, int ci)
         case kKindDisk: ok = launch_colour<kKindDisk, 0>(c, ci); break;
         case kKindPolygon:
             switch (c->sf.nverts) {
+#ifndef HPMC_FAST_BUILD
                 case 3: ok = launch_colour<kKindPolygon, 3>(c, ci); break;
                 case 4: ok = launch_colour<kKindPolygon, 4>(c, ci); break;
-                case 5: ok = launch_colour<kKindPolygon, 5>(c, ci); break;
                 case 6: ok = launch_colour<kKindPolygon, 6>(c, ci); break;
                 case 8: ok = launch_colour<kKindPolygon, 8>(c, ci); break;
+#endif
+                case 5: ok = launch_colour<kKindPolygon, 5>(c, ci); break;
                 default: ok = launch_colour<kKindPolygon, 0>(c, ci); break;
             }
             break;
@@ -680,7 +685,7 @@ int hpmc_set_option(hpmc_ctx* c, const char* name, int64_t value)
         if (value < 0) return fail(c, HPMC_E_ARG, "tile_cap must be >= 0");
         c->opt_tile_cap = value > (1 << 30) ? (1 << 30) : (int)value;
     } else if (n == "tile_shape") {
-        if (value < 0 || value > 4) return fail(c, HPMC_E_ARG, "tile_shape must be 0 (auto) or 1..4");
+        if (value < 0 || value > 7) return fail(c, HPMC_E_ARG, "tile_shape must be 0 (auto) or 1..7");
         c->opt_tile_shape = (int)value;
     } else
         return fail(c, HPMC_E_ARG, "unknown option");

@@ -47,7 +47,7 @@ struct Tile2D {
     static_assert(CAP < 65536, "16-bit local offsets");
     // shared-memory carve (bytes)
     static constexpr size_t off_pose = 0;
-    static constexpr size_t off_trial = off_pose + sizeof(float4) * CAP;
+    static constexpr size_t off_trial = off_pose + sizeof(float4) * (CAP + 4);   // + 4: the predicated candidate slots may read past the end
     static constexpr size_t off_queue = off_trial + sizeof(float4) * SLOTS * WARPS;
     static constexpr size_t off_seg_g = off_queue + sizeof(unsigned) * QCAP * WARPS;
     static constexpr size_t off_seg_l = off_seg_g + sizeof(int) * NSEG;
@@ -80,8 +80,8 @@ __device__ __noinline__ bool pair_overlap_2d_cold(const GridParams& g, const Sha
     return pair_overlap_2d<KIND, NV>(g, S, A, B, eps, true);
 }
 
-template <int KIND, int NV, int WARPS, int R>
-__global__ void __launch_bounds__(32 * WARPS)
+template <int KIND, int NV, int WARPS, int R, int MINB>
+__global__ void __launch_bounds__(32 * WARPS, MINB)
 k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ MoveParams mv, const __grid_constant__ ShapeF S,
                const __grid_constant__ ShapeD SD, Control* __restrict__ ctrl, int colour_index, int cap_limit,
                float4* __restrict__ pose, const int* __restrict__ tag, const int* __restrict__ cell_start, uint32_t k0,
@@ -251,39 +251,53 @@ k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
                     ++cc.trials;
                     bool sure = false;
                     if (inside) {
+                        // a8: the three row runs of the 3x3 block hold <= 4 poses each in all but rare cases: 12 fixed,
+                        // predicated candidate slots (bit 4*dy + j), no data-dependent loop in the common path
                         unsigned mask = 0u;
-                        int bit = 0;
-                        int rs[3], re[3];
+                        int rs[3];
+                        bool extra = false;
 #pragma unroll
                         for (int dy = 0; dy < 3; ++dy) {
                             const int row = (ryl + dy - 1) * RW + rxl;
-                            rs[dy] = sm_lstart[row - 1];
-                            re[dy] = sm_lstart[row + 2];
-                        }
+                            const int qs = sm_lstart[row - 1], n = (int)sm_lstart[row + 2] - qs;
+                            rs[dy] = qs;
+                            extra |= n > 4;
 #pragma unroll
-                        for (int dy = 0; dy < 3; ++dy) {
-                            for (int q = rs[dy]; q < re[dy]; ++q, ++bit) {
-                                if (q == p) continue;
-                                const float4 B = sm_pose[q];
+                            for (int j = 0; j < 4; ++j) {
+                                const int q = qs + j;
+                                const float4 B = sm_pose[q];        // the pose buffer is padded by 4: q < ntot + 4
                                 float rx = B.x - T.x, ry = B.y - T.y;
                                 if (seam) {
                                     rx = min_image(B.x, T.x, g.hi[0], g.Ld[0]);
                                     ry = min_image(B.y, T.y, g.hi[1], g.Ld[1]);
                                 }
                                 const float d2 = rx * rx + ry * ry;
-                                if (d2 >= S.dmax2) continue;                          // a8 circumsphere (R16)
-                                if (KIND == kKindDisk || d2 < S.din2) sure = true;    // inside the inscribed-disk bound
-                                else if (bit < 32) mask |= 1u << bit;
-                                else if (!sure) sure = pair_overlap_2d_cold<KIND, NV>(g, S, T, B, mv.eps_g);   // > 32 candidates
+                                const bool hit = (j < n) && (q != p) && (d2 < S.dmax2);       // R16
+                                if (hit) mask |= 1u << (4 * dy + j);
+                                if (hit && (KIND == kKindDisk || d2 < S.din2)) sure = true;  // inside the inscribed-disk bound
+                            }
+                        }
+                        if (extra) {   // a row run with more than 4 poses: the rest one by one
+#pragma unroll 1
+                            for (int dy = 0; dy < 3; ++dy) {
+                                const int row = (ryl + dy - 1) * RW + rxl;
+                                for (int q = rs[dy] + 4; q < (int)sm_lstart[row + 2] && !sure; ++q) {
+                                    if (q == p) continue;
+                                    const float4 B = sm_pose[q];
+                                    const float rx = min_image(B.x, T.x, g.hi[0], g.Ld[0]), ry = min_image(B.y, T.y, g.hi[1], g.Ld[1]);
+                                    const float d2 = rx * rx + ry * ry;
+                                    if (d2 >= S.dmax2) continue;
+                                    sure = (KIND == kKindDisk || d2 < S.din2) ? true : pair_overlap_2d_cold<KIND, NV>(g, S, T, B, mv.eps_g);
+                                }
                             }
                         }
                         if (KIND != kKindDisk && !sure && mask) {                     // early exit otherwise
                             int at = atomicAdd(&sm_qcount[warp], __popc(mask));
-                            const int n_0 = re[0] - rs[0], n_01 = n_0 + (re[1] - rs[1]);
                             while (mask) {
                                 const int b = __ffs(mask) - 1;
                                 mask &= mask - 1u;
-                                const int q = (b < n_0) ? rs[0] + b : (b < n_01) ? rs[1] + (b - n_0) : rs[2] + (b - n_01);
+                                const int dy = b >> 2;
+                                const int q = ((dy == 0) ? rs[0] : (dy == 1) ? rs[1] : rs[2]) + (b & 3);
                                 if (at < TL::QCAP) my_queue[at] = ((unsigned)slot << 16) | (unsigned)q;
                                 else if (!sure) sure = pair_overlap_2d_cold<KIND, NV>(g, S, T, sm_pose[q], mv.eps_g);   // queue full
                                 ++at;
