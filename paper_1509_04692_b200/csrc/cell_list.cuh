@@ -27,7 +27,7 @@ __global__ void k_prepare(const __grid_constant__ GridParams g, Control* __restr
         ctrl->hdr = h;
         if (mode == 0) {
             ctrl->t = t + 1ull;
-            ctrl->counters[6] += 1ull;
+            ctrl->sweeps += 1ull;
         }
     }
 }

@@ -39,10 +39,17 @@ struct SweepHeader {
     uint32_t pad;
 };
 
+constexpr int kCounterSets = 128;
+
 // device-resident control block
 struct Control {
     unsigned long long t;  // sweep counter (persists across calls)
-    unsigned long long counters[7];  // trans_acc, trans_rej_overlap, trans_rej_cell, rot_acc, rot_rej_overlap, trials, sweeps
+    unsigned long long sweeps;
+    // trans_acc, trans_rej_overlap, trans_rej_cell, rot_acc, rot_rej_overlap, trials (+2 pad): kCounterSets replicas, one
+    // 64-byte line each.  Every warp of a colour pass adds its tallies to the replica picked by its CTA index: thousands of
+    // same-address atomics per launch would otherwise serialise in one L2 slice (measured: ~40 us per launch on 1M
+    // pentagons).  Readers sum the replicas.
+    unsigned long long counters[kCounterSets][8];
     unsigned long long overlaps;     // validator result
     SweepHeader hdr;
 };

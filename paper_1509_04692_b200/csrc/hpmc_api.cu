@@ -31,6 +31,7 @@ struct hpmc_ctx {
     bool cuda_failed = false;
     int64_t launches = 0;
     uint64_t t_host = 0;  // mirror of the device sweep counter
+    Control h_ctrl{};     // host landing buffer for the control block
 
     // caller-owned
     float4* d_pos_bound = nullptr;
@@ -330,9 +331,7 @@ int pick_tile_shape(const hpmc_ctx* c)
     if (c->opt_tile_shape) return c->opt_tile_shape;
     const int nax = c->g.n[0] / 2, nay = c->g.n[1] / 2;
     const long long cols = (nax + kTileW - 1) / kTileW;
-    if (cols * ((nay + 15) / 16) >= 3 * 148) return 1;   // 8 warps x 2 rows
-    if (cols * ((nay + 7) / 8) >= 2 * 148) return 2;     // 4 warps x 2 rows
-    if (cols * ((nay + 3) / 4) >= 148) return 3;         // 4 warps x 1 row
+    if (cols * ((nay + 3) / 4) >= 2 * 148) return 5;     // 4 warps x 1 row, 64 registers: 8 CTAs per SM
     return 4;                                            // 2 warps x 1 row
 }
 
@@ -496,7 +495,7 @@ int hpmc_bind(hpmc_ctx* c, float* d_pos4, float* d_quat4, void* d_workspace, siz
     c->tile_sums = (int*)(c->d_ws + L.tile_sums);
     c->ctrl = (Control*)(c->d_ws + L.ctrl);
     if (first) {  // a new workspace: (re)create the control block, keeping the host-side sweep counter
-        Control init;
+        Control& init = c->h_ctrl;
         std::memset(&init, 0, sizeof init);
         init.t = c->t_host;
         if (!cuda_ok(c, cudaMemcpyAsync(c->ctrl, &init, sizeof init, cudaMemcpyHostToDevice, c->stream), "bind/memcpy")) return HPMC_E_CUDA;
@@ -580,13 +579,16 @@ int hpmc_get_state(hpmc_ctx* c, float* d_pos4_out, float* d_quat4_out, hpmc_coun
         }
     }
     if (h_counters || h_sweep_counter) {
-        Control h;
+        Control& h = c->h_ctrl;
         if (!cuda_ok(c, cudaMemcpyAsync(&h, c->ctrl, sizeof h, cudaMemcpyDeviceToHost, c->stream), "get_state/memcpy")) return HPMC_E_CUDA;
         if (!cuda_ok(c, cudaStreamSynchronize(c->stream), "get_state/sync")) return HPMC_E_CUDA;
         if (h_counters) {
-            h_counters->trans_acc = h.counters[0]; h_counters->trans_rej_overlap = h.counters[1];
-            h_counters->trans_rej_cell = h.counters[2]; h_counters->rot_acc = h.counters[3];
-            h_counters->rot_rej_overlap = h.counters[4]; h_counters->trials = h.counters[5]; h_counters->sweeps = h.counters[6];
+            unsigned long long sum[6] = {0, 0, 0, 0, 0, 0};
+            for (int r = 0; r < kCounterSets; ++r)
+                for (int k = 0; k < 6; ++k) sum[k] += h.counters[r][k];
+            h_counters->trans_acc = sum[0]; h_counters->trans_rej_overlap = sum[1];
+            h_counters->trans_rej_cell = sum[2]; h_counters->rot_acc = sum[3];
+            h_counters->rot_rej_overlap = sum[4]; h_counters->trials = sum[5]; h_counters->sweeps = h.sweeps;
         }
         if (h_sweep_counter) *h_sweep_counter = (int64_t)h.t;
     }
@@ -611,7 +613,7 @@ int hpmc_reset_counters(hpmc_ctx* c)
     if (!c) return HPMC_E_ARG;
     if (c->cuda_failed) return HPMC_E_CUDA;
     if (!c->ctrl) return fail(c, HPMC_E_UNBOUND, "workspace not bound");
-    if (!cuda_ok(c, cudaMemsetAsync(c->ctrl->counters, 0, sizeof(unsigned long long) * 7, c->stream), "reset/memset")) return HPMC_E_CUDA;
+    if (!cuda_ok(c, cudaMemsetAsync(&c->ctrl->sweeps, 0, sizeof(unsigned long long) * (1 + 8 * kCounterSets), c->stream), "reset/memset")) return HPMC_E_CUDA;
     return HPMC_OK;
 }
 
@@ -642,7 +644,7 @@ int hpmc_get_cell_list(hpmc_ctx* c, uint64_t t, int32_t* d_cell_start, int32_t* 
         LAUNCH_CHECK(c, "k_cell_of_tag");
     }
     if (h_shift3 || h_colour_perm8) {
-        Control h;
+        Control& h = c->h_ctrl;
         if (!cuda_ok(c, cudaMemcpyAsync(&h, c->ctrl, sizeof h, cudaMemcpyDeviceToHost, c->stream), "cell_list/memcpy")) return HPMC_E_CUDA;
         if (!cuda_ok(c, cudaStreamSynchronize(c->stream), "cell_list/sync")) return HPMC_E_CUDA;
         if (h_shift3) for (int k = 0; k < 3; ++k) h_shift3[k] = h.hdr.shift[k];

@@ -134,12 +134,13 @@ __device__ __forceinline__ void flush_counters(Control* ctrl, CellCounters c)
     c.rrov = __reduce_add_sync(0xffffffffu, c.rrov);
     c.trials = __reduce_add_sync(0xffffffffu, c.trials);
     if ((threadIdx.x & 31) == 0 && c.trials) {
-        if (c.tacc) atomicAdd(&ctrl->counters[0], (unsigned long long)c.tacc);
-        if (c.trov) atomicAdd(&ctrl->counters[1], (unsigned long long)c.trov);
-        if (c.trcell) atomicAdd(&ctrl->counters[2], (unsigned long long)c.trcell);
-        if (c.racc) atomicAdd(&ctrl->counters[3], (unsigned long long)c.racc);
-        if (c.rrov) atomicAdd(&ctrl->counters[4], (unsigned long long)c.rrov);
-        atomicAdd(&ctrl->counters[5], (unsigned long long)c.trials);
+        unsigned long long* set = ctrl->counters[(blockIdx.x * 7u + (threadIdx.x >> 5)) & (kCounterSets - 1)];
+        if (c.tacc) atomicAdd(&set[0], (unsigned long long)c.tacc);
+        if (c.trov) atomicAdd(&set[1], (unsigned long long)c.trov);
+        if (c.trcell) atomicAdd(&set[2], (unsigned long long)c.trcell);
+        if (c.racc) atomicAdd(&set[3], (unsigned long long)c.racc);
+        if (c.rrov) atomicAdd(&set[4], (unsigned long long)c.rrov);
+        atomicAdd(&set[5], (unsigned long long)c.trials);
     }
 }
 
