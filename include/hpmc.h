@@ -136,8 +136,10 @@ int hpmc_sweep_host(hpmc_ctx* ctx, const float* h_pos4, const float* h_quat4, in
  *   "path"     0 = automatic, 1 = per-thread global-memory colour pass, 2 = shared-memory tile colour pass (2-D)
  *   "tile_cap" upper limit on the particles a tile may stage; tiles above it take the per-thread path
  *              (tests set 0 to force that fallback everywhere).
- *   "tile_shape" 2-D tile kernel shape: 0 = chosen by grid size, 1 = 8 warps x 2 rows of 32 active cells per warp,
- *              2 = 4 x 2, 3 = 4 x 1, 4 = 2 x 1.                                                              */
+ *   "tile_shape" 2-D tile kernel shape: 0 = chosen by grid size, 1..7 = fixed (warps per CTA x rows of 32 active cells per
+ *              warp x minimum CTAs per SM; see pick_tile_shape in hpmc_api.cu).
+ *   "graph"    1 (default): hpmc_sweep(n >= 3) replays a captured CUDA graph of two sweeps; 0: plain launches.
+ *              Needs a real stream: contexts created on the legacy default stream (NULL) always use plain launches.  */
 int hpmc_set_option(hpmc_ctx* ctx, const char* name, int64_t value);
 
 /* Per-kernel device timing for the roofline report (S:8(d)).  While on, CUDA events on the context's stream

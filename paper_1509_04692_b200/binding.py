@@ -105,7 +105,8 @@ class Hpmc:
             sd.nverts = int(self._verts.shape[0])
             sd.verts = self._verts.ctypes.data_as(C.POINTER(C.c_double))
         with torch.cuda.device(self.device):
-            self.stream = stream if stream is not None else torch.cuda.current_stream()
+            # a stream of our own: the legacy default stream cannot be captured into a CUDA graph
+            self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
             h = C.c_void_p()
             rc = self._lib.hpmc_create(C.byref(box), C.byref(sd), self.N, int(seed), C.c_void_p(self.stream.cuda_stream), C.byref(h))
         if rc != 0:
@@ -141,9 +142,11 @@ class Hpmc:
                 a = torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to(self.device)
             assert a.is_cuda and a.dtype == torch.float32 and a.is_contiguous() and tuple(a.shape) == (self.N, 4)
             return a
-        self.pos4, self.quat4 = dev(pos4), dev(quat4)
-        if self.workspace is None:
-            self.workspace = torch.empty(self.workspace_bytes() + 256, dtype=torch.uint8, device=self.device)
+        torch.cuda.current_stream(self.device).synchronize()      # caller's tensors are ready
+        with torch.cuda.stream(self.stream):                       # every torch op on the state runs on OUR stream
+            self.pos4, self.quat4 = dev(pos4), dev(quat4)
+            if self.workspace is None:
+                self.workspace = torch.empty(self.workspace_bytes() + 256, dtype=torch.uint8, device=self.device)
         base = self.workspace.data_ptr()
         off = (-base) % 256
         self.stream.synchronize()
@@ -164,8 +167,8 @@ class Hpmc:
     def get_state(self, to_host=True):
         """Un-sort into the bound arrays; returns (pos4, quat4) as numpy (to_host) or the CUDA tensors."""
         self._check(self._lib.hpmc_get_state(self._h, self.pos4.data_ptr(), self.quat4.data_ptr(), None, None))
+        self.stream.synchronize()
         if to_host:
-            self.stream.synchronize()
             return self.pos4.cpu().numpy(), self.quat4.cpu().numpy()
         return self.pos4, self.quat4
 
@@ -185,7 +188,9 @@ class Hpmc:
         torch = self._torch
         if on:
             words = 2 * self.C * self.n_select
-            self._trace = torch.zeros(words, dtype=torch.int32, device=self.device)
+            with torch.cuda.stream(self.stream):
+                self._trace = torch.zeros(words, dtype=torch.int32, device=self.device)
+            self.stream.synchronize()
             self._check(self._lib.hpmc_set_trace(self._h, self._trace.data_ptr(), words))
         else:
             self._trace = None
@@ -198,9 +203,10 @@ class Hpmc:
     def cell_list(self, t):
         """Cell list of sweep t's grid shift for the current state: (cell_of_tag, cell_start, member_tags, shift, perm)."""
         torch = self._torch
-        cst = torch.empty(self.C + 1, dtype=torch.int32, device=self.device)
-        mem = torch.empty(max(self.N, 1), dtype=torch.int32, device=self.device)
-        cid = torch.empty(max(self.N, 1), dtype=torch.int32, device=self.device)
+        with torch.cuda.stream(self.stream):
+            cst = torch.empty(self.C + 1, dtype=torch.int32, device=self.device)
+            mem = torch.empty(max(self.N, 1), dtype=torch.int32, device=self.device)
+            cid = torch.empty(max(self.N, 1), dtype=torch.int32, device=self.device)
         shift = (C.c_float * 3)(); perm = (C.c_int32 * 8)()
         self._check(self._lib.hpmc_get_cell_list(self._h, int(t), cst.data_ptr(), mem.data_ptr(), cid.data_ptr(), shift, perm))
         self.stream.synchronize()

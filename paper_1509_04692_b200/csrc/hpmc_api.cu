@@ -57,7 +57,12 @@ struct hpmc_ctx {
     // tuning / test knobs (hpmc_set_option)
     int opt_path = 0;                 // 0 auto, 1 per-thread global path, 2 tile path (2-D only)
     int opt_tile_cap = 1 << 30;       // staging capacity limit of the tile kernel (tests force the overflow path)
-    int opt_tile_shape = 0;           // 0 = by grid size, 1..4 = fixed (see pick_tile_shape)
+    int opt_tile_shape = 0;           // 0 = by grid size, 1..7 = fixed (see pick_tile_shape)
+    int opt_graph = 1;                // 1: hpmc_sweep(n >= 3) replays a captured two-sweep CUDA graph
+
+    // CUDA graph of two consecutive sweeps (the ping-pong buffers return to where they started), one per parity of `cur`
+    cudaGraphExec_t graph_exec[2] = {nullptr, nullptr};
+    int64_t graph_launches = 0;       // kernels inside one replay
 
     // optional per-kernel device timing (hpmc_set_profile): event pairs around the cell-list build (class 0)
     // and around every colour-pass launch (class 1)
@@ -392,6 +397,27 @@ int launch_colour_dispatch(hpmc_ctx* c, int ci)
     return HPMC_OK;
 }
 
+// one sweep: shift + cell list + the colours in the sweep's random order (S:8(a) rows a0-a11)
+int sweep_once(hpmc_ctx* c)
+{
+    int rc = build_cell_list(c, 0, 0ull);
+    if (rc != HPMC_OK) return rc;
+    const int ncol = 1 << c->g.dim;
+    for (int ci = 0; ci < ncol; ++ci) {
+        rc = launch_colour_dispatch(c, ci);
+        if (rc != HPMC_OK) return rc;
+    }
+    ++c->t_host;
+    return HPMC_OK;
+}
+
+// anything the captured launches depend on changed: pointers, move sizes, options, trace
+void graph_reset(hpmc_ctx* c)
+{
+    for (int b = 0; b < 2; ++b)
+        if (c->graph_exec[b]) { cudaGraphExecDestroy(c->graph_exec[b]); c->graph_exec[b] = nullptr; }
+}
+
 int check_ready(hpmc_ctx* c)
 {
     if (!c) return HPMC_E_ARG;
@@ -450,8 +476,10 @@ int hpmc_create(const hpmc_box* box, const hpmc_shape* shape, int64_t N, uint64_
 
 int hpmc_destroy(hpmc_ctx* c)
 {
-    if (c)
+    if (c) {
+        graph_reset(c);
         for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+    }
     delete c;
     return HPMC_OK;
 }
@@ -480,6 +508,7 @@ int hpmc_bind(hpmc_ctx* c, float* d_pos4, float* d_quat4, void* d_workspace, siz
     if (bytes < L.total) return fail(c, HPMC_E_UNBOUND, "workspace smaller than hpmc_workspace_bytes()");
     if (((uintptr_t)d_workspace & 255u) || ((uintptr_t)d_pos4 & 15u) || ((uintptr_t)d_quat4 & 15u))
         return fail(c, HPMC_E_ARG, "workspace must be 256-byte aligned, state arrays 16-byte aligned");
+    graph_reset(c);
     const bool first = (c->d_ws == nullptr) || (c->d_ws != (char*)d_workspace);
     c->d_pos_bound = (float4*)d_pos4;
     c->d_quat_bound = (float4*)d_quat4;
@@ -511,6 +540,7 @@ int hpmc_set_moves(hpmc_ctx* c, double d, double a, int n_select)
 {
     if (!c) return HPMC_E_ARG;
     if (!(d > 0.0) || !(a >= 0.0) || n_select < 1 || n_select > 65535) return fail(c, HPMC_E_ARG, "need d > 0, a >= 0, 1 <= n_select <= 65535");
+    graph_reset(c);
     c->mv.d = (float)d;
     c->mv.a = (float)a;
     c->mv.n_select = n_select;
@@ -523,15 +553,41 @@ int hpmc_sweep(hpmc_ctx* c, int64_t n)
     if (rc != HPMC_OK) return rc;
     if (n < 0) return fail(c, HPMC_E_ARG, "n must be >= 0");
     if (c->trace && c->trace_words < 2 * (int64_t)c->g.C * c->mv.n_select) return fail(c, HPMC_E_TRACE, "trace buffer too small");
-    const int ncol = 1 << c->g.dim;
-    for (int64_t s = 0; s < n; ++s) {
-        rc = build_cell_list(c, 0, 0ull);
-        if (rc != HPMC_OK) return rc;
-        for (int ci = 0; ci < ncol; ++ci) {
-            rc = launch_colour_dispatch(c, ci);
+    int64_t s = 0;
+    // Launch-bound systems (config 1: 11 launches of a few microseconds per sweep): replay a captured graph of two
+    // sweeps.  The sweep counter, header and counters live on the device, so the replay needs no new arguments.
+    if (c->opt_graph && c->stream != nullptr && !c->trace && !c->profile && n >= 3) {   // the legacy default stream cannot be captured
+        if (c->state_in_bound || !c->graph_exec[c->cur]) {   // one plain sweep first: sorted copy exists, kernels are loaded
+            rc = sweep_once(c);
             if (rc != HPMC_OK) return rc;
+            ++s;
         }
-        ++c->t_host;
+        if (!c->graph_exec[c->cur] && n - s >= 2) {
+            const int64_t l0 = c->launches;
+            cudaGraph_t graph = nullptr;
+            if (!cuda_ok(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal), "graph/begin")) return HPMC_E_CUDA;
+            rc = sweep_once(c);
+            if (rc == HPMC_OK) rc = sweep_once(c);
+            const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+            c->t_host -= (rc == HPMC_OK) ? 2 : 0;   // captured, not run
+            if (rc != HPMC_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+            if (!cuda_ok(c, e, "graph/end")) return HPMC_E_CUDA;
+            c->graph_launches = c->launches - l0;
+            c->launches = l0;
+            const cudaError_t ei = cudaGraphInstantiate(&c->graph_exec[c->cur], graph, 0);
+            cudaGraphDestroy(graph);
+            if (!cuda_ok(c, ei, "graph/instantiate")) return HPMC_E_CUDA;
+        }
+        while (n - s >= 2 && c->graph_exec[c->cur]) {
+            if (!cuda_ok(c, cudaGraphLaunch(c->graph_exec[c->cur], c->stream), "graph/launch")) return HPMC_E_CUDA;
+            c->launches += c->graph_launches;
+            c->t_host += 2;
+            s += 2;
+        }
+    }
+    for (; s < n; ++s) {
+        rc = sweep_once(c);
+        if (rc != HPMC_OK) return rc;
     }
     return HPMC_OK;
 }
@@ -621,6 +677,7 @@ int hpmc_set_trace(hpmc_ctx* c, uint32_t* d_trace, int64_t capacity_words)
 {
     if (!c) return HPMC_E_ARG;
     if (d_trace && ((uintptr_t)d_trace & 7u)) return fail(c, HPMC_E_ARG, "trace must be 8-byte aligned");
+    graph_reset(c);
     c->trace = (uint2*)d_trace;
     c->trace_words = d_trace ? capacity_words : 0;
     return HPMC_OK;
@@ -680,7 +737,10 @@ int hpmc_set_option(hpmc_ctx* c, const char* name, int64_t value)
 {
     if (!c || !name) return HPMC_E_ARG;
     const std::string n(name);
-    if (n == "path") {
+    graph_reset(c);
+    if (n == "graph") {
+        c->opt_graph = value != 0;
+    } else if (n == "path") {
         if (value < 0 || value > 2) return fail(c, HPMC_E_ARG, "path must be 0 (auto), 1 (per-thread) or 2 (tile)");
         c->opt_path = (int)value;
     } else if (n == "tile_cap") {

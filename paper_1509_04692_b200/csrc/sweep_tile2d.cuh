@@ -31,6 +31,7 @@
 namespace hpmc {
 
 constexpr int kTileW = 32;   // active cells per tile row = lanes of a warp
+constexpr int kRowSlots = 5; // predicated broad-phase slots per row run of 3 cells (a run holds more in ~0.1 % of the cases)
 
 template <int WARPS, int R>
 struct Tile2D {
@@ -47,7 +48,7 @@ struct Tile2D {
     static_assert(CAP < 65536, "16-bit local offsets");
     // shared-memory carve (bytes)
     static constexpr size_t off_pose = 0;
-    static constexpr size_t off_trial = off_pose + sizeof(float4) * (CAP + 4);   // + 4: the predicated candidate slots may read past the end
+    static constexpr size_t off_trial = off_pose + sizeof(float4) * (CAP + 8);   // + 8: the predicated candidate slots may read past the end
     static constexpr size_t off_queue = off_trial + sizeof(float4) * SLOTS * WARPS;
     static constexpr size_t off_seg_g = off_queue + sizeof(unsigned) * QCAP * WARPS;
     static constexpr size_t off_seg_l = off_seg_g + sizeof(int) * NSEG;
@@ -175,21 +176,22 @@ k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
     }
 
     // ---- staging 2: local CSR (16-bit) and the poses, coalesced ---------------------------------------------------
-    for (int lc = tid; lc < ncells; lc += TL::NT) {
-        const int ry = lc / RW, rx = lc - ry * RW;
+    for (int ry = warp; ry < RHv; ry += WARPS) {   // one region row per warp at a time: no index division, coalesced
         int cy = cy0 - 1 + ry;
         cy += (cy < 0) ? n1 : 0;
         cy -= (cy >= n1) ? n1 : 0;
-        const int second = rx >= split;
-        const int cx = second ? rx - split : xs + rx;
-        const int seg = 2 * ry + second;
-        sm_lstart[lc] = (unsigned short)(cell_start[cy * n0 + cx] - sm_seg_g[seg] + sm_seg_l[seg]);
+        const int* row_start = cell_start + cy * n0;
+        const int g0 = sm_seg_g[2 * ry], g1 = sm_seg_g[2 * ry + 1];
+        const int l0 = sm_seg_l[2 * ry], l1 = sm_seg_l[2 * ry + 1], l2 = sm_seg_l[2 * ry + 2];
+        for (int rx = lane; rx < RW; rx += 32) {
+            const bool second = rx >= split;
+            const int cx = second ? rx - split : xs + rx;
+            sm_lstart[ry * RW + rx] = (unsigned short)(row_start[cx] - (second ? g1 : g0) + (second ? l1 : l0));
+        }
+        for (int e = lane; e < l1 - l0; e += 32) sm_pose[l0 + e] = pose[g0 + e];
+        for (int e = lane; e < l2 - l1; e += 32) sm_pose[l1 + e] = pose[g1 + e];
     }
     if (tid == 0) sm_lstart[ncells] = (unsigned short)ntot;
-    for (int seg = warp; seg < 2 * RHv; seg += WARPS) {
-        const int gb = sm_seg_g[seg], lb = sm_seg_l[seg], len = sm_seg_l[seg + 1] - lb;
-        for (int e = lane; e < len; e += 32) sm_pose[lb + e] = pose[gb + e];
-    }
     __syncthreads();
 
     // ---- this warp's non-empty active cells, compacted: sm_act[slot] = j*32 + lane of the cell ---------------------
@@ -251,8 +253,8 @@ k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
                     ++cc.trials;
                     bool sure = false;
                     if (inside) {
-                        // a8: the three row runs of the 3x3 block hold <= 4 poses each in all but rare cases: 12 fixed,
-                        // predicated candidate slots (bit 4*dy + j), no data-dependent loop in the common path
+                        // a8: the three row runs of the 3x3 block hold <= kRowSlots poses each in all but rare cases: fixed,
+                        // predicated candidate slots (bit kRowSlots*dy + j), no data-dependent loop in the common path
                         unsigned mask = 0u;
                         int rs[3];
                         bool extra = false;
@@ -261,11 +263,11 @@ k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
                             const int row = (ryl + dy - 1) * RW + rxl;
                             const int qs = sm_lstart[row - 1], n = (int)sm_lstart[row + 2] - qs;
                             rs[dy] = qs;
-                            extra |= n > 4;
+                            extra |= n > kRowSlots;
 #pragma unroll
-                            for (int j = 0; j < 4; ++j) {
+                            for (int j = 0; j < kRowSlots; ++j) {
                                 const int q = qs + j;
-                                const float4 B = sm_pose[q];        // the pose buffer is padded by 4: q < ntot + 4
+                                const float4 B = sm_pose[q];        // the pose buffer is padded: q < ntot + kRowSlots
                                 float rx = B.x - T.x, ry = B.y - T.y;
                                 if (seam) {
                                     rx = min_image(B.x, T.x, g.hi[0], g.Ld[0]);
@@ -273,15 +275,15 @@ k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
                                 }
                                 const float d2 = rx * rx + ry * ry;
                                 const bool hit = (j < n) && (q != p) && (d2 < S.dmax2);       // R16
-                                if (hit) mask |= 1u << (4 * dy + j);
+                                if (hit) mask |= 1u << (kRowSlots * dy + j);
                                 if (hit && (KIND == kKindDisk || d2 < S.din2)) sure = true;  // inside the inscribed-disk bound
                             }
                         }
-                        if (extra) {   // a row run with more than 4 poses: the rest one by one
+                        if (extra) {   // a row run with more than kRowSlots poses: the rest one by one
 #pragma unroll 1
                             for (int dy = 0; dy < 3; ++dy) {
                                 const int row = (ryl + dy - 1) * RW + rxl;
-                                for (int q = rs[dy] + 4; q < (int)sm_lstart[row + 2] && !sure; ++q) {
+                                for (int q = rs[dy] + kRowSlots; q < (int)sm_lstart[row + 2] && !sure; ++q) {
                                     if (q == p) continue;
                                     const float4 B = sm_pose[q];
                                     const float rx = min_image(B.x, T.x, g.hi[0], g.Ld[0]), ry = min_image(B.y, T.y, g.hi[1], g.Ld[1]);
@@ -296,8 +298,8 @@ k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
                             while (mask) {
                                 const int b = __ffs(mask) - 1;
                                 mask &= mask - 1u;
-                                const int dy = b >> 2;
-                                const int q = ((dy == 0) ? rs[0] : (dy == 1) ? rs[1] : rs[2]) + (b & 3);
+                                const int dy = (b >= 2 * kRowSlots) ? 2 : (b >= kRowSlots) ? 1 : 0;
+                                const int q = ((dy == 0) ? rs[0] : (dy == 1) ? rs[1] - kRowSlots : rs[2] - 2 * kRowSlots) + b;
                                 if (at < TL::QCAP) my_queue[at] = ((unsigned)slot << 16) | (unsigned)q;
                                 else if (!sure) sure = pair_overlap_2d_cold<KIND, NV>(g, S, T, sm_pose[q], mv.eps_g);   // queue full
                                 ++at;
