@@ -7,38 +7,37 @@
 
 namespace hpmc {
 
-constexpr int kScanThreads = 256;
-constexpr int kScanItems = 8;
+constexpr int kScanThreads = 512;
+constexpr int kScanItems = 16;
 constexpr int kScanTile = kScanThreads * kScanItems;
 
-// mode 0: header of the device sweep counter t, then t++ and sweeps++   (a real sweep)
-// mode 1: header of t_override, nothing advanced                         (debug cell list)
-// mode 2: zero shift, nothing advanced                                   (validator)
-__global__ void k_prepare(const __grid_constant__ GridParams g, Control* __restrict__ ctrl, int* __restrict__ counts,
-                          uint32_t k0, uint32_t k1, int mode, unsigned long long t_override)
-{
-    const int stride = gridDim.x * blockDim.x;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i <= g.C; i += stride) counts[i] = 0;
-    if (blockIdx.x == 0 && threadIdx.x == 0) {
-        const unsigned long long t = (mode == 0) ? ctrl->t : t_override;
-        SweepHeader h;
-        make_header(g, k0, k1, t, mode == 2, h);
-        h.pad = 0;
-        ctrl->hdr = h;
-        if (mode == 0) {
-            ctrl->t = t + 1ull;
-            ctrl->sweeps += 1ull;
-        }
-    }
-}
+// Three launches build the cell list of a sweep:
+//   k_hist          header (a0, a1) + cell id and arrival rank of every particle (a2, first half of a3)
+//   k_scan          single-pass exclusive scan of the per-cell counts (decoupled look-back), zeroes the counts for the
+//                   next build, advances the sweep counter
+//   k_scatter_sort  scatter into the cell-sorted SoA; the last particle to arrive in a cell puts the cell's members in
+//                   ascending tag order (R8)
+// mode 0: header of the device sweep counter t; k_scan then does t++ and sweeps++   (a real sweep)
+// mode 1: header of t_override, nothing advanced                                     (debug cell list)
+// mode 2: zero shift, nothing advanced                                               (validator)
 
-// a2 + first half of a3: cell id and slot inside the cell (arrival order; made canonical by k_cell_sort)
-__global__ void k_hist(const __grid_constant__ GridParams g, const Control* __restrict__ ctrl,
-                       const float4* __restrict__ pos, int* __restrict__ counts, int2* __restrict__ key_rank)
+// a0-a2 + first half of a3.  Every block derives the same header from the (unchanged) sweep counter; block 0 stores it for
+// the kernels that follow.  `counts` is all zero on entry (bind, then k_scan after every use).
+__global__ void k_hist(const __grid_constant__ GridParams g, Control* __restrict__ ctrl, const float4* __restrict__ pos,
+                       int* __restrict__ counts, int2* __restrict__ key_rank, uint32_t k0, uint32_t k1, int mode,
+                       unsigned long long t_override)
 {
+    __shared__ SweepHeader sh;
+    if (threadIdx.x == 0) {
+        const unsigned long long t = (mode == 0) ? ctrl->t : t_override;
+        make_header(g, k0, k1, t, mode == 2, sh);
+        sh.pad = 0;
+        if (blockIdx.x == 0) ctrl->hdr = sh;
+    }
+    __syncthreads();
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= g.N) return;
-    const float shift[3] = {ctrl->hdr.shift[0], ctrl->hdr.shift[1], ctrl->hdr.shift[2]};
+    const float shift[3] = {sh.shift[0], sh.shift[1], sh.shift[2]};
     const float4 x = pos[p];
     int cx, cy, cz;
     const int c = cell_of(g, shift, x.x, x.y, x.z, cx, cy, cz);
@@ -76,69 +75,108 @@ __device__ __forceinline__ int block_exclusive_scan(int v, int& total)
     return offset + inc - v;
 }
 
-// scan pass 1: per-tile totals
-__global__ void __launch_bounds__(kScanThreads) k_scan_reduce(const int* __restrict__ counts, int n, int* __restrict__ tile_sums)
+// tile state of the single-pass scan: value (low 32 bits) | epoch << 34 | status << 32; status 1 = tile aggregate,
+// 2 = inclusive prefix.  The epoch makes words of earlier launches invalid without clearing the array.
+__device__ __forceinline__ unsigned long long scan_pack(unsigned int value, unsigned int status, unsigned long long epoch)
 {
-    const int base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
-    int s = 0;
-#pragma unroll
-    for (int i = 0; i < kScanItems; ++i)
-        if (base + i < n) s += counts[base + i];
-    int total;
-    block_exclusive_scan(s, total);
-    if (threadIdx.x == 0) tile_sums[blockIdx.x] = total;
+    return (unsigned long long)value | ((unsigned long long)status << 32) | (epoch << 34);
 }
 
-// scan pass 2: exclusive scan of the tile totals by ONE block
-__global__ void __launch_bounds__(kScanThreads) k_scan_spine(int* __restrict__ tile_sums, int ntiles)
+// second quarter of a3: cell_start[i] = sum of counts[0..i) for i = 0..n (n = C: the grand total), one pass.
+// Tiles take tickets so that every predecessor of a tile is already resident (no deadlock in the look-back).
+__global__ void __launch_bounds__(kScanThreads)
+k_scan(int* __restrict__ counts, int n, int* __restrict__ cell_start, unsigned long long* __restrict__ tile_state,
+       Control* __restrict__ ctrl, int ntiles, int mode)
 {
-    __shared__ int carry_s;
-    if (threadIdx.x == 0) carry_s = 0;
+    __shared__ int s_tile;
+    __shared__ int s_prefix;
+    __shared__ unsigned long long s_epoch;
+    if (threadIdx.x == 0) {
+        s_epoch = ctrl->scan_epoch;                       // read BEFORE taking the ticket (see the last tile below)
+        s_tile = (int)atomicAdd(&ctrl->scan_ticket, 1u);
+    }
     __syncthreads();
-    for (int base = 0; base < ntiles; base += kScanThreads) {
-        const int i = base + threadIdx.x;
-        const int v = (i < ntiles) ? tile_sums[i] : 0;
-        int total;
-        const int ex = block_exclusive_scan(v, total);
-        const int carry = carry_s;
-        if (i < ntiles) tile_sums[i] = carry + ex;
-        __syncthreads();
-        if (threadIdx.x == 0) carry_s = carry + total;
-        __syncthreads();
-    }
-}
-
-// scan pass 3: in-place exclusive scan of each tile plus its offset; element n (= C) receives the grand total
-__global__ void __launch_bounds__(kScanThreads) k_scan_final(int* __restrict__ counts, int n, const int* __restrict__ tile_sums)
-{
-    const int base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
-    int v[kScanItems];
-    int s = 0;
+    const int tile = s_tile;
+    const unsigned long long epoch = s_epoch & 0x3fffffffull;
+    // warp w owns 32*kScanItems consecutive counts; item k of lane l is element k*32 + l of that chunk: every load and
+    // store is one coalesced 128-byte line per warp
+    __shared__ int s_wsum[kScanThreads / 32];
+    const int lane_ = threadIdx.x & 31, warp_ = threadIdx.x >> 5;
+    const int wbase = tile * kScanTile + warp_ * (32 * kScanItems) + lane_;
+    int v[kScanItems], ex[kScanItems];
 #pragma unroll
-    for (int i = 0; i < kScanItems; ++i) {
-        v[i] = (base + i < n) ? counts[base + i] : 0;
-        s += v[i];
+    for (int k = 0; k < kScanItems; ++k) {
+        const int idx = wbase + 32 * k;
+        v[k] = (idx <= n) ? counts[idx] : 0;
     }
-    int total;
-    int run = block_exclusive_scan(s, total) + tile_sums[blockIdx.x];
+    int carry = 0;
 #pragma unroll
-    for (int i = 0; i < kScanItems; ++i) {
-        if (base + i <= n) counts[base + i] = run;   // index n gets the total (all later v are 0)
-        run += v[i];
+    for (int k = 0; k < kScanItems; ++k) {
+        const int idx = wbase + 32 * k;
+        if (idx <= n) counts[idx] = 0;                    // ready for the next build
+        const int inc = warp_inclusive_scan(v[k]);
+        ex[k] = carry + inc - v[k];
+        carry += __shfl_sync(0xffffffffu, inc, 31);
+    }
+    if (lane_ == 0) s_wsum[warp_] = carry;
+    __syncthreads();
+    int woff = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < kScanThreads / 32; ++w) {
+        const int t = s_wsum[w];
+        if (w < warp_) woff += t;
+        total += t;
+    }
+    if (threadIdx.x < 32) {                               // warp 0: publish, look back 32 tiles at a time
+        volatile unsigned long long* st = tile_state;
+        const int lane = threadIdx.x;
+        int prefix = 0;
+        if (lane == 0) st[tile] = scan_pack((unsigned)total, tile == 0 ? 2u : 1u, epoch);
+        for (int j = tile - 1; j >= 0; j -= 32) {
+            const int idx = j - lane;
+            unsigned long long w = scan_pack(0u, 2u, epoch);          // before tile 0: an inclusive prefix of zero
+            if (idx >= 0)
+                do { w = st[idx]; } while ((w >> 34) != epoch || ((w >> 32) & 3ull) == 0ull);
+            const unsigned incl = __ballot_sync(0xffffffffu, ((w >> 32) & 3ull) == 2ull);
+            const int first = incl ? __ffs(incl) - 1 : 31;            // nearest tile that already knows its inclusive prefix
+            prefix += __reduce_add_sync(0xffffffffu, lane <= first ? (int)(unsigned int)w : 0);
+            if (incl) break;
+        }
+        if (lane == 0) {
+            if (tile != 0) st[tile] = scan_pack((unsigned)(prefix + total), 2u, epoch);
+            s_prefix = prefix;
+            if (tile == ntiles - 1) {                     // every other tile has already read the epoch and its ticket
+                ctrl->scan_ticket = 0u;
+                ctrl->scan_epoch = (epoch + 1ull) & 0x3fffffffull;
+                if (mode == 0) {
+                    ctrl->t += 1ull;
+                    ctrl->sweeps += 1ull;
+                }
+            }
+        }
+    }
+    __syncthreads();
+    const int off = s_prefix + woff;
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        const int idx = wbase + 32 * k;
+        if (idx <= n) cell_start[idx] = off + ex[k];
     }
 }
 
 // second half of a3: scatter into the cell-sorted SoA.  src_tag == nullptr: source is the caller's tag-order pos4/quat4;
-// otherwise the source is the other sorted buffer (2-D: poses only).
-__global__ void k_scatter(int N, int dim, const float4* __restrict__ src_pos, const float4* __restrict__ src_quat,
-                          const int* __restrict__ src_tag, const int2* __restrict__ key_rank,
-                          const int* __restrict__ cell_start, float4* __restrict__ dst_pos, float4* __restrict__ dst_quat,
-                          int* __restrict__ dst_tag)
+// otherwise the source is the other sorted buffer (2-D: poses only).  In a cell with several members the LAST particle to
+// arrive (counted in `arrived`, which it resets) sorts the members by tag (R8), whatever order the atomics produced.
+__global__ void k_scatter_sort(int N, int dim, const float4* __restrict__ src_pos, const float4* __restrict__ src_quat,
+                               const int* __restrict__ src_tag, const int2* __restrict__ key_rank,
+                               const int* __restrict__ cell_start, int* __restrict__ arrived, float4* dst_pos, float4* dst_quat,
+                               int* dst_tag)
 {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= N) return;
     const int2 kr = key_rank[p];
-    const int dst = cell_start[kr.x] + kr.y;
+    const int s = cell_start[kr.x], cnt = cell_start[kr.x + 1] - s;
+    const int dst = s + kr.y;
     const float4 P = src_pos[p];
     if (dim == 2) {
         if (src_tag) dst_pos[dst] = P;
@@ -151,31 +189,28 @@ __global__ void k_scatter(int N, int dim, const float4* __restrict__ src_pos, co
         dst_quat[dst] = src_quat[p];
     }
     dst_tag[dst] = src_tag ? src_tag[p] : p;
-}
-
-// R8: members of a cell in ascending tag, whatever order the atomics produced
-__global__ void k_cell_sort(int C, int dim, const int* __restrict__ cell_start, float4* __restrict__ pos, float4* __restrict__ quat,
-                            int* __restrict__ tag)
-{
-    const int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= C) return;
-    const int s = cell_start[c], e = cell_start[c + 1];
-    for (int i = s + 1; i < e; ++i) {
-        const int ti = tag[i];
+    if (cnt < 2) return;
+    __threadfence();
+    if (atomicAdd(&arrived[kr.x], 1) != cnt - 1) return;
+    __threadfence();
+    arrived[kr.x] = 0;
+    // insertion sort of the cell by tag; loads bypass L1 (other SMs wrote these lines during this kernel)
+    for (int i = s + 1; i < s + cnt; ++i) {
+        const int ti = __ldcg(&dst_tag[i]);
         int j = i - 1;
-        if (tag[j] <= ti) continue;
-        const float4 pi = pos[i];
+        if (__ldcg(&dst_tag[j]) <= ti) continue;
+        const float4 pi = __ldcg(&dst_pos[i]);
         float4 qi = pi;
-        if (dim == 3) qi = quat[i];
-        while (j >= s && tag[j] > ti) {
-            tag[j + 1] = tag[j];
-            pos[j + 1] = pos[j];
-            if (dim == 3) quat[j + 1] = quat[j];
+        if (dim == 3) qi = __ldcg(&dst_quat[i]);
+        while (j >= s && __ldcg(&dst_tag[j]) > ti) {
+            dst_tag[j + 1] = __ldcg(&dst_tag[j]);
+            dst_pos[j + 1] = __ldcg(&dst_pos[j]);
+            if (dim == 3) dst_quat[j + 1] = __ldcg(&dst_quat[j]);
             --j;
         }
-        tag[j + 1] = ti;
-        pos[j + 1] = pi;
-        if (dim == 3) quat[j + 1] = qi;
+        dst_tag[j + 1] = ti;
+        dst_pos[j + 1] = pi;
+        if (dim == 3) dst_quat[j + 1] = qi;
     }
 }
 

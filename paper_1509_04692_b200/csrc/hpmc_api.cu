@@ -48,7 +48,9 @@ struct hpmc_ctx {
     int cur = 0;
     int2* key_rank = nullptr;
     int* cell_start = nullptr;  // C+1 (+ padding)
-    int* tile_sums = nullptr;
+    int* counts = nullptr;      // per-cell histogram, all zero between builds
+    int* arrived = nullptr;     // per-cell arrival counter of k_scatter_sort, all zero between builds
+    unsigned long long* tile_state = nullptr;   // look-back words of k_scan
     Control* ctrl = nullptr;
 
     uint2* trace = nullptr;
@@ -108,7 +110,7 @@ struct Carve {
 int scan_tiles(const hpmc_ctx* c) { return (c->g.C + 1 + kScanTile - 1) / kScanTile; }
 
 struct Layout {
-    size_t pos[2], quat[2], tag[2], key_rank, cell_start, tile_sums, ctrl, total;
+    size_t pos[2], quat[2], tag[2], key_rank, cell_start, counts, arrived, tile_state, ctrl, total;
 };
 
 Layout layout_of(const hpmc_ctx* c)
@@ -123,7 +125,9 @@ Layout layout_of(const hpmc_ctx* c)
     }
     L.key_rank = cv.take(N * sizeof(int2));
     L.cell_start = cv.take(((size_t)c->g.C + 2) * sizeof(int));
-    L.tile_sums = cv.take((size_t)(scan_tiles(c) + 1) * sizeof(int));
+    L.counts = cv.take(((size_t)c->g.C + 2) * sizeof(int));
+    L.arrived = cv.take(((size_t)c->g.C + 2) * sizeof(int));
+    L.tile_state = cv.take((size_t)(scan_tiles(c) + 1) * sizeof(unsigned long long));
     L.ctrl = cv.take(sizeof(Control));
     L.total = cv.off;
     return L;
@@ -284,27 +288,16 @@ int build_cell_list(hpmc_ctx* c, int mode, unsigned long long t_override)
     const float4* src_quat = c->state_in_bound ? c->d_quat_bound : c->quat[c->cur];
     const int* src_tag = c->state_in_bound ? nullptr : c->tag[c->cur];
     const int dst = c->state_in_bound ? 0 : 1 - c->cur;
-    const int nblk_cells = (g.C + 1 + TB - 1) / TB;
     const int nblk_part = (g.N + TB - 1) / TB;
-    k_prepare<<<nblk_cells < 2048 ? nblk_cells : 2048, TB, 0, c->stream>>>(g, c->ctrl, c->cell_start, c->k0, c->k1, mode, t_override);
-    LAUNCH_CHECK(c, "k_prepare");
-    if (g.N > 0) {
-        k_hist<<<nblk_part, TB, 0, c->stream>>>(g, c->ctrl, src_pos, c->cell_start, c->key_rank);
-        LAUNCH_CHECK(c, "k_hist");
-    }
+    k_hist<<<nblk_part > 0 ? nblk_part : 1, TB, 0, c->stream>>>(g, c->ctrl, src_pos, c->counts, c->key_rank, c->k0, c->k1, mode, t_override);
+    LAUNCH_CHECK(c, "k_hist");
     const int tiles = scan_tiles(c);
-    k_scan_reduce<<<tiles, kScanThreads, 0, c->stream>>>(c->cell_start, g.C, c->tile_sums);
-    LAUNCH_CHECK(c, "k_scan_reduce");
-    k_scan_spine<<<1, kScanThreads, 0, c->stream>>>(c->tile_sums, tiles);
-    LAUNCH_CHECK(c, "k_scan_spine");
-    k_scan_final<<<tiles, kScanThreads, 0, c->stream>>>(c->cell_start, g.C, c->tile_sums);
-    LAUNCH_CHECK(c, "k_scan_final");
+    k_scan<<<tiles, kScanThreads, 0, c->stream>>>(c->counts, g.C, c->cell_start, c->tile_state, c->ctrl, tiles, mode);
+    LAUNCH_CHECK(c, "k_scan");
     if (g.N > 0) {
-        k_scatter<<<nblk_part, TB, 0, c->stream>>>(g.N, g.dim, src_pos, src_quat, src_tag, c->key_rank, c->cell_start, c->pos[dst],
-                                                  c->quat[dst], c->tag[dst]);
-        LAUNCH_CHECK(c, "k_scatter");
-        k_cell_sort<<<(g.C + TB - 1) / TB, TB, 0, c->stream>>>(g.C, g.dim, c->cell_start, c->pos[dst], c->quat[dst], c->tag[dst]);
-        LAUNCH_CHECK(c, "k_cell_sort");
+        k_scatter_sort<<<nblk_part, TB, 0, c->stream>>>(g.N, g.dim, src_pos, src_quat, src_tag, c->key_rank, c->cell_start, c->arrived,
+                                                       c->pos[dst], c->quat[dst], c->tag[dst]);
+        LAUNCH_CHECK(c, "k_scatter_sort");
     }
     c->cur = dst;
     c->state_in_bound = false;
@@ -521,9 +514,12 @@ int hpmc_bind(hpmc_ctx* c, float* d_pos4, float* d_quat4, void* d_workspace, siz
     }
     c->key_rank = (int2*)(c->d_ws + L.key_rank);
     c->cell_start = (int*)(c->d_ws + L.cell_start);
-    c->tile_sums = (int*)(c->d_ws + L.tile_sums);
+    c->counts = (int*)(c->d_ws + L.counts);
+    c->arrived = (int*)(c->d_ws + L.arrived);
+    c->tile_state = (unsigned long long*)(c->d_ws + L.tile_state);
     c->ctrl = (Control*)(c->d_ws + L.ctrl);
-    if (first) {  // a new workspace: (re)create the control block, keeping the host-side sweep counter
+    if (first) {  // a new workspace: zero the builder's scratch, (re)create the control block, keeping the host-side sweep counter
+        if (!cuda_ok(c, cudaMemsetAsync(c->d_ws + L.counts, 0, L.ctrl - L.counts, c->stream), "bind/memset")) return HPMC_E_CUDA;
         Control& init = c->h_ctrl;
         std::memset(&init, 0, sizeof init);
         init.t = c->t_host;
