@@ -35,27 +35,34 @@ FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # SMs x FP32 lanes x 2 (F
 HBM_FALLBACK_GBS = 6650.0                               # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 
 # Algorithmic work per trial (tariff of SURVEY.md 8(d) x the oracle's O7 work counters on
-# the melted state of each workload).  flops per trial, and state bytes per particle.
-ALGO = {
-    # kind: (flops per trial, state bytes S per particle)
-    wl.KIND_DISK: (10 + 8 + 8 * 4.08, 16),
-    wl.KIND_POLYGON: (20 + 4 + 8 * 6.94 + 1.83 * 180.0, 32),
-    wl.KIND_POLYHEDRON: (35 + 6 + 11 * 68.0 + 8.12 * 1500.0, 32),
+# the melted state of each workload): flops per trial.
+ALGO_FLOPS = {
+    wl.KIND_DISK: 10 + 8 + 8 * 4.08,
+    wl.KIND_POLYGON: 20 + 4 + 8 * 6.94 + 1.83 * 180.0,
+    wl.KIND_POLYHEDRON: 35 + 6 + 11 * 68.0 + 8.12 * 1500.0,
 }
+# ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (profiles/r1_v4.md)
+NCU_TRAFFIC = {"k2_pentagons_1M": 21.1e6}
+
+
+def state_bytes(w):
+    """Bytes per particle in the cell-sorted arrays: one pose float4 in 2-D, pos + quat float4 in 3-D."""
+    return 16 if w.dim == 2 else 32
 
 
 def algorithmic_bytes_per_sweep(w, C, accepted_per_sweep):
-    """B_sweep of SURVEY.md 8(d): N(32 + 2S + ncol S) + 16 C + S T_acc."""
-    S = ALGO[w.kind][1]
+    """B_sweep: build (read state + tag, keys written and read, counts + offsets, scatter) plus one
+    read of all state and all cell offsets per colour pass plus the accepted write-backs."""
+    S = state_bytes(w)
     ncol = 1 << w.dim
-    return w.N * (32 + 2 * S + ncol * S) + 16 * C + S * accepted_per_sweep
+    return w.N * (2 * (S + 4) + 16 + ncol * S) + C * (12 + 4 * ncol) + S * accepted_per_sweep
 
 
 def colour_pass_bytes(w, C, accepted_per_sweep):
-    """Bytes one colour-pass launch must move: all state once + CSR offsets + accepted write-backs."""
-    S = ALGO[w.kind][1]
+    """Bytes one colour-pass launch must move: all state once + all cell offsets once + accepted write-backs."""
+    S = state_bytes(w)
     ncol = 1 << w.dim
-    return w.N * S + 8 * C / ncol + S * accepted_per_sweep / ncol
+    return w.N * S + 4 * C + S * accepted_per_sweep / ncol
 
 
 def hbm_peak():
@@ -285,7 +292,7 @@ def main():
     acc_per_sweep = acc / args.steps
     hbm, hbm_src = hbm_peak()
     bytes_launch = colour_pass_bytes(w, g.C, acc_per_sweep)
-    flops_launch = ALGO[w.kind][0] * trials_per_launch
+    flops_launch = ALGO_FLOPS[w.kind] * trials_per_launch
     t_hbm = bytes_launch / (hbm * 1e9)
     t_alu = flops_launch / (FP32_PEAK_TFLOPS * 1e12)
     if t_hbm >= t_alu:
@@ -293,12 +300,13 @@ def main():
     else:
         roof = {"bound": "alu", "achieved": flops_launch / (colour_ms * 1e-3) / 1e12, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s"}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof.update({"traffic": None, "kernel": "k_sweep_colour", "avg_launch_ms": colour_ms, "launches_timed": prof["colour_n"],
+    roof.update({"traffic": NCU_TRAFFIC.get(w.name), "kernel": "k_sweep_tile2d" if w.dim == 2 else "k_sweep_warp3d", "avg_launch_ms": colour_ms, "launches_timed": prof["colour_n"],
                  "peak_source": f"{hbm_src} hbm_gbs (MEASURED_PEAKS.json)" if roof["bound"] == "hbm" else "148 SM x 128 lanes x 2 x 1.965 GHz",
                  "algorithmic_bytes_per_launch": bytes_launch, "algorithmic_flops_per_launch": flops_launch,
                  "kernel_share_of_step": prof["colour_ms"] / r["ms"], "build_share_of_step": prof["build_ms"] / r["ms"],
                  "sweep_frac": max(algorithmic_bytes_per_sweep(w, g.C, acc_per_sweep) / (hbm * 1e9),
-                                   ALGO[w.kind][0] * trials / args.steps / (FP32_PEAK_TFLOPS * 1e12)) / (r["ms"] * 1e-3 / args.steps)})
+                                   ALGO_FLOPS[w.kind] * trials / args.steps / (FP32_PEAK_TFLOPS * 1e12)) / (r["ms"] * 1e-3 / args.steps),
+                 "hbm_time_us": 1e6 * t_hbm, "fp32_time_us": 1e6 * t_alu})
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,

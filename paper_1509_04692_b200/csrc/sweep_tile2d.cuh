@@ -81,6 +81,34 @@ __device__ __noinline__ bool pair_overlap_2d_cold(const GridParams& g, const Sha
     return pair_overlap_2d<KIND, NV>(g, S, A, B, eps, true);
 }
 
+// a8, common path: kRowSlots fixed candidate slots per row run of the 3x3 block (bit kRowSlots*dy + j), no data-dependent
+// loop.  A slot past the end of its run holds a pose of a cell farther along (or the sentinel padding behind the last staged
+// pose): any pose within d_max of a trial that stayed in its cell lies in the 3x3 block (w >= d_max (1 + 2^-10), R11), so such
+// a slot can only repeat a genuine neighbour (tiny periodic grids) and needs no length predicate; the particle itself is
+// excluded explicitly.
+template <int KIND, bool SEAM>
+__device__ __forceinline__ void broad_slots(const GridParams& g, const ShapeF& S, const float2* sm_xy, const int (&rs)[3], int p,
+                                            const float4& T, unsigned& mask, bool& sure)
+{
+#pragma unroll
+    for (int dy = 0; dy < 3; ++dy) {
+#pragma unroll
+        for (int j = 0; j < kRowSlots; ++j) {
+            const int q = rs[dy] + j;
+            const float2 B = sm_xy[q];
+            float rx = B.x - T.x, ry = B.y - T.y;
+            if (SEAM) {
+                rx = min_image(B.x, T.x, g.hi[0], g.Ld[0]);
+                ry = min_image(B.y, T.y, g.hi[1], g.Ld[1]);
+            }
+            const float d2 = rx * rx + ry * ry;
+            const bool hit = (q != p) && (d2 < S.dmax2);                           // R16
+            if (hit) mask |= 1u << (kRowSlots * dy + j);
+            if (hit && (KIND == kKindDisk || d2 < S.din2)) sure = true;           // inside the inscribed-disk bound
+        }
+    }
+}
+
 template <int KIND, int NV, int WARPS, int R, int MINB>
 __global__ void __launch_bounds__(32 * WARPS, MINB)
 k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ MoveParams mv, const __grid_constant__ ShapeF S,
@@ -90,7 +118,12 @@ k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
 {
     using TL = Tile2D<WARPS, R>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    float4* sm_pose = reinterpret_cast<float4*>(smem_raw + TL::off_pose);       // staged (x, y, qw, qz)
+    // staged poses, positions and orientations apart: the broad phase reads only (x, y), and 8-byte elements halve the
+    // shared-memory bank conflicts of its per-lane gathers (lane stride ~2 poses) against one 16-byte array
+    float2* sm_xy = reinterpret_cast<float2*>(smem_raw + TL::off_pose);                          // (x, y)
+    float2* sm_qq = reinterpret_cast<float2*>(smem_raw + TL::off_pose) + (TL::CAP + 8);          // (qw, qz)
+    auto ld_pose = [&](int q) { const float2 a = sm_xy[q], b = sm_qq[q]; return make_float4(a.x, a.y, b.x, b.y); };
+    auto st_pose = [&](int q, const float4& v) { sm_xy[q] = make_float2(v.x, v.y); sm_qq[q] = make_float2(v.z, v.w); };
     float4* sm_trial = reinterpret_cast<float4*>(smem_raw + TL::off_trial);     // trial pose of every slot
     unsigned* sm_queue = reinterpret_cast<unsigned*>(smem_raw + TL::off_queue);
     int* sm_seg_g = reinterpret_cast<int*>(smem_raw + TL::off_seg_g);           // global start of each segment
@@ -188,10 +221,11 @@ k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
             const int cx = second ? rx - split : xs + rx;
             sm_lstart[ry * RW + rx] = (unsigned short)(row_start[cx] - (second ? g1 : g0) + (second ? l1 : l0));
         }
-        for (int e = lane; e < l1 - l0; e += 32) sm_pose[l0 + e] = pose[g0 + e];
-        for (int e = lane; e < l2 - l1; e += 32) sm_pose[l1 + e] = pose[g1 + e];
+        for (int e = lane; e < l1 - l0; e += 32) st_pose(l0 + e, pose[g0 + e]);
+        for (int e = lane; e < l2 - l1; e += 32) st_pose(l1 + e, pose[g1 + e]);
     }
     if (tid == 0) sm_lstart[ncells] = (unsigned short)ntot;
+    if (tid < 8) st_pose(ntot + tid, make_float4(3.0e18f, 3.0e18f, 1.0f, 0.0f));   // sentinels behind the last staged pose
     __syncthreads();
 
     // ---- this warp's non-empty active cells, compacted: sm_act[slot] = j*32 + lane of the cell ---------------------
@@ -241,7 +275,7 @@ k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
                     const int own_s = sm_lstart[lc], nmem = (int)sm_lstart[lc + 1] - own_s;
                     const U4 b0 = philox4x32_10((uint32_t)cell, t_lo, (uint32_t)k, c3, k0, k1);
                     const int p = own_s + (int)mulhi32(b0.x, (uint32_t)nmem);                 // R8
-                    const float4 P = sm_pose[p];
+                    const float4 P = ld_pose(p);
                     TrialState A;
                     bool rotate;
                     const bool inside = make_trial<KIND>(g, mv, shift, cell, 2, b0, 0u, make_float4(P.x, P.y, 0.f, 0.f),
@@ -261,31 +295,18 @@ k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
 #pragma unroll
                         for (int dy = 0; dy < 3; ++dy) {
                             const int row = (ryl + dy - 1) * RW + rxl;
-                            const int qs = sm_lstart[row - 1], n = (int)sm_lstart[row + 2] - qs;
-                            rs[dy] = qs;
-                            extra |= n > kRowSlots;
-#pragma unroll
-                            for (int j = 0; j < kRowSlots; ++j) {
-                                const int q = qs + j;
-                                const float4 B = sm_pose[q];        // the pose buffer is padded: q < ntot + kRowSlots
-                                float rx = B.x - T.x, ry = B.y - T.y;
-                                if (seam) {
-                                    rx = min_image(B.x, T.x, g.hi[0], g.Ld[0]);
-                                    ry = min_image(B.y, T.y, g.hi[1], g.Ld[1]);
-                                }
-                                const float d2 = rx * rx + ry * ry;
-                                const bool hit = (j < n) && (q != p) && (d2 < S.dmax2);       // R16
-                                if (hit) mask |= 1u << (kRowSlots * dy + j);
-                                if (hit && (KIND == kKindDisk || d2 < S.din2)) sure = true;  // inside the inscribed-disk bound
-                            }
+                            rs[dy] = sm_lstart[row - 1];
+                            extra |= (int)sm_lstart[row + 2] - rs[dy] > kRowSlots;
                         }
+                        if (seam) broad_slots<KIND, true>(g, S, sm_xy, rs, p, T, mask, sure);
+                        else broad_slots<KIND, false>(g, S, sm_xy, rs, p, T, mask, sure);
                         if (extra) {   // a row run with more than kRowSlots poses: the rest one by one
 #pragma unroll 1
                             for (int dy = 0; dy < 3; ++dy) {
                                 const int row = (ryl + dy - 1) * RW + rxl;
                                 for (int q = rs[dy] + kRowSlots; q < (int)sm_lstart[row + 2] && !sure; ++q) {
                                     if (q == p) continue;
-                                    const float4 B = sm_pose[q];
+                                    const float4 B = ld_pose(q);
                                     const float rx = min_image(B.x, T.x, g.hi[0], g.Ld[0]), ry = min_image(B.y, T.y, g.hi[1], g.Ld[1]);
                                     const float d2 = rx * rx + ry * ry;
                                     if (d2 >= S.dmax2) continue;
@@ -301,7 +322,7 @@ k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
                                 const int dy = (b >= 2 * kRowSlots) ? 2 : (b >= kRowSlots) ? 1 : 0;
                                 const int q = ((dy == 0) ? rs[0] : (dy == 1) ? rs[1] - kRowSlots : rs[2] - 2 * kRowSlots) + b;
                                 if (at < TL::QCAP) my_queue[at] = ((unsigned)slot << 16) | (unsigned)q;
-                                else if (!sure) sure = pair_overlap_2d_cold<KIND, NV>(g, S, T, sm_pose[q], mv.eps_g);   // queue full
+                                else if (!sure) sure = pair_overlap_2d_cold<KIND, NV>(g, S, T, ld_pose(q), mv.eps_g);   // queue full
                                 ++at;
                             }
                         }
@@ -317,7 +338,7 @@ k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
             for (int e = lane; e < nq; e += 32) {
                 const unsigned ent = my_queue[e];
                 const int o = (int)(ent >> 16), q = (int)(ent & 0xffffu);
-                if (pair_overlap_2d<KIND, NV>(g, S, my_trial[o], sm_pose[q], mv.eps_g, seam)) my_flag[o] = 1;
+                if (pair_overlap_2d<KIND, NV>(g, S, my_trial[o], ld_pose(q), mv.eps_g, seam)) my_flag[o] = 1;
             }
             __syncwarp();
         }
@@ -336,24 +357,21 @@ k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
                 const int ryl = 2 * ay + 1, rxl = 2 * al + 1;
                 const int seg = 2 * ryl + (rxl >= split ? 1 : 0);
                 const int gi = sm_seg_g[seg] + (p - sm_seg_l[seg]);
-                if (outcome == 1u) {
+                const bool acc = outcome == 1u;
+                if (acc) {
                     float4 T = my_trial[slot];
-                    if (!rotate) {
-                        float x = T.x, y = T.y;
-                        if (x >= g.hi[0]) x = __fsub_rn(x, g.L[0]); else if (x < g.lo[0]) x = __fadd_rn(x, g.L[0]);
-                        if (y >= g.hi[1]) y = __fsub_rn(y, g.L[1]); else if (y < g.lo[1]) y = __fadd_rn(y, g.L[1]);
-                        T.x = x; T.y = y;
-                        ++cc.tacc;
-                    } else {
-                        ++cc.racc;
+                    if (!rotate) {   // R-wrap: at most one add per axis
+                        T.x = (T.x >= g.hi[0]) ? __fsub_rn(T.x, g.L[0]) : (T.x < g.lo[0]) ? __fadd_rn(T.x, g.L[0]) : T.x;
+                        T.y = (T.y >= g.hi[1]) ? __fsub_rn(T.y, g.L[1]) : (T.y < g.lo[1]) ? __fadd_rn(T.y, g.L[1]) : T.y;
                     }
                     pose[gi] = T;
-                    sm_pose[p] = T;
-                } else if (outcome == 2u) {
-                    ++cc.trcell;
-                } else {
-                    if (rotate) ++cc.rrov; else ++cc.trov;
+                    st_pose(p, T);
                 }
+                cc.tacc += (acc && !rotate) ? 1u : 0u;
+                cc.racc += (acc && rotate) ? 1u : 0u;
+                cc.trcell += (outcome == 2u) ? 1u : 0u;
+                cc.trov += (outcome == 3u && !rotate) ? 1u : 0u;
+                cc.rrov += (outcome == 3u && rotate) ? 1u : 0u;
                 if (trace) {
                     const long long slot0 = (long long)((cx0 + 2 * al) + n0 * (cy0 + 2 * ay)) * mv.n_select;
                     trace[slot0 + k] = make_uint2((uint32_t)tag[gi], (rotate ? 1u : 0u) | (outcome << 8));
