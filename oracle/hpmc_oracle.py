@@ -137,7 +137,7 @@ class Shape:
             raise ValueError("oracle rejected the shape (non-convex, not CCW, too many vertices, bad dim)")
 
     def __del__(self):
-        if getattr(self, "_h", None):
+        if getattr(self, "_h", None) and lib is not None:
             lib().orc_shape_destroy(self._h)
             self._h = None
 
@@ -195,7 +195,7 @@ class Oracle:
         self.n_select = 4
 
     def __del__(self):
-        if getattr(self, "_h", None):
+        if getattr(self, "_h", None) and lib is not None:      # `lib` is gone during interpreter shutdown
             lib().orc_destroy(self._h)
             self._h = None
 
