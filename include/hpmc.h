@@ -133,7 +133,8 @@ int hpmc_sweep_host(hpmc_ctx* ctx, const float* h_pos4, const float* h_quat4, in
                     float* h_pos4_out, float* h_quat4_out, hpmc_counters* h_counters);
 
 /* Tuning and test knobs; results never depend on them (only speed does).
- *   "path"     0 = automatic, 1 = per-thread global-memory colour pass, 2 = shared-memory tile colour pass (2-D)
+ *   "path"     0 = automatic, 1 = per-thread global-memory colour pass, 2 = shared-memory tile colour pass (2-D; in 3-D
+ *              the warp-per-cell pass), 3 = warp-per-cell colour pass (automatic in 3-D and for small 2-D systems)
  *   "tile_cap" upper limit on the particles a tile may stage; tiles above it take the per-thread path
  *              (tests set 0 to force that fallback everywhere).
  *   "tile_shape" 2-D tile kernel shape: 0 = chosen by grid size, 1..7 = fixed (warps per CTA x rows of 32 active cells per

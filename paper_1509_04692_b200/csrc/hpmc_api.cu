@@ -13,7 +13,7 @@
 #include "overlap.cuh"
 #include "sweep.cuh"
 #include "sweep_tile2d.cuh"
-#include "sweep_warp3d.cuh"
+#include "sweep_warpcell.cuh"
 
 using namespace hpmc;
 
@@ -333,12 +333,27 @@ int pick_tile_shape(const hpmc_ctx* c)
     return 4;                                            // 2 warps x 1 row
 }
 
+template <int KIND, int NV, int DIM>
+bool launch_warpcell(hpmc_ctx* c, int ci, int nactive)
+{
+    k_sweep_warpcell<KIND, NV, DIM><<<(nactive + kW3Warps - 1) / kW3Warps, 32 * kW3Warps, 0, c->stream>>>(
+        c->g, c->mv, c->sf, c->sd, c->ctrl, ci, c->opt_tile_cap, c->pos[c->cur], c->quat[c->cur], c->tag[c->cur], c->cell_start, c->k0,
+        c->k1, c->trace);
+    return true;
+}
+
+// 2-D systems with fewer active cells per colour than this run one warp per cell instead of one lane per cell: the tile
+// kernel would leave most SMs idle (config 1: 961 active cells = 31 warps) and each warp round would be a long serial chain
+constexpr int kWarpCellMax2d = 148 * 48;
+
 template <int KIND, int NV>
 bool launch_colour(hpmc_ctx* c, int ci)
 {
     const GridParams& g = c->g;
+    const int nactive = (g.n[0] / 2) * (g.n[1] / 2) * (g.dim == 3 ? g.n[2] / 2 : 1);
     if constexpr (KIND != kKindPolyhedron) {
         if (g.dim == 2 && c->opt_path != 1) {
+            if (c->opt_path == 3 || (c->opt_path == 0 && c->opt_tile_shape == 0 && nactive <= kWarpCellMax2d)) return launch_warpcell<KIND, NV, 2>(c, ci, nactive);
             switch (pick_tile_shape(c)) {
                 case 1: return launch_tile2d<KIND, NV, 8, 2, 2>(c, ci);
                 case 2: return launch_tile2d<KIND, NV, 4, 2, 4>(c, ci);
@@ -350,14 +365,8 @@ bool launch_colour(hpmc_ctx* c, int ci)
             }
         }
     }
-    const int nactive = (g.n[0] / 2) * (g.n[1] / 2) * (g.dim == 3 ? g.n[2] / 2 : 1);
     if constexpr (KIND != kKindPolygon) {
-        if (g.dim == 3 && c->opt_path != 1) {   // one warp per active cell, neighbourhood staged in shared memory
-            k_sweep_warp3d<KIND><<<(nactive + kW3Warps - 1) / kW3Warps, 32 * kW3Warps, 0, c->stream>>>(
-                g, c->mv, c->sf, c->sd, c->ctrl, ci, c->opt_tile_cap, c->pos[c->cur], c->quat[c->cur], c->tag[c->cur], c->cell_start,
-                c->k0, c->k1, c->trace);
-            return true;
-        }
+        if (g.dim == 3 && c->opt_path != 1) return launch_warpcell<KIND, 0, 3>(c, ci, nactive);   // one warp per active cell
     }
     const int TB = 128;
     k_sweep_colour<KIND, NV><<<(nactive + TB - 1) / TB, TB, 0, c->stream>>>(g, c->mv, c->sf, c->sd, c->ctrl, ci, c->pos[c->cur], c->quat[c->cur],
@@ -737,7 +746,7 @@ int hpmc_set_option(hpmc_ctx* c, const char* name, int64_t value)
     if (n == "graph") {
         c->opt_graph = value != 0;
     } else if (n == "path") {
-        if (value < 0 || value > 2) return fail(c, HPMC_E_ARG, "path must be 0 (auto), 1 (per-thread) or 2 (tile)");
+        if (value < 0 || value > 3) return fail(c, HPMC_E_ARG, "path must be 0 (auto), 1 (per-thread), 2 (tile) or 3 (warp per cell)");
         c->opt_path = (int)value;
     } else if (n == "tile_cap") {
         if (value < 0) return fail(c, HPMC_E_ARG, "tile_cap must be >= 0");

@@ -59,21 +59,6 @@ struct Tile2D {
     static constexpr size_t bytes = off_act + SLOTS * WARPS;
 };
 
-// narrow phase of trial pose A against staged pose B, both (x, y, qw, qz); true = overlap (R15 guard band)
-template <int KIND, int NV>
-__device__ __forceinline__ bool pair_overlap_2d(const GridParams& g, const ShapeF& S, const float4& A, const float4& B, float eps, bool seam)
-{
-    float rx = B.x - A.x, ry = B.y - A.y;
-    if (seam) {
-        rx = min_image(B.x, A.x, g.hi[0], g.Ld[0]);
-        ry = min_image(B.y, A.y, g.hi[1], g.Ld[1]);
-    }
-    if (KIND == kKindDisk) return rx * rx + ry * ry < S.dmax2;
-    const float cA = A.z * A.z - A.w * A.w, sA = 2.0f * A.z * A.w;   // cos t = w^2 - z^2, sin t = 2wz (R30)
-    const float cB = B.z * B.z - B.w * B.w, sB = 2.0f * B.z * B.w;
-    return !(polygon_max_sep<float, NV>(S, rx, ry, cA, sA, cB, sB) >= eps);
-}
-
 // out-of-line copy for the rare direct evaluations (queue overflow, > 32 candidates): keeps the hot loop's code small
 template <int KIND, int NV>
 __device__ __noinline__ bool pair_overlap_2d_cold(const GridParams& g, const ShapeF& S, float4 A, float4 B, float eps)

@@ -1,15 +1,17 @@
-// 3-D colour pass, warp-per-cell version (S:8(a) rows a4-a11) -- the paper's block-level work queue
-// at warp scope, for spheres and convex polyhedra.
+// Colour pass, warp-per-cell version (S:8(a) rows a4-a11) -- the paper's block-level work queue at warp
+// scope.  Used for every 3-D system (spheres, convex polyhedra) and for 2-D systems too small to fill the GPU with one
+// lane per cell (config 1: 961 active cells per colour are 31 warps of the tile kernel but 961 warps here, and the serial
+// chain of a trial shrinks from a 32-cell warp round to one cell's work).
 //
-// One warp = one active cell of the current colour.  The warp first stages the particles of the 27 cells around
+// One warp = one active cell of the current colour.  The warp first stages the particles of the 3^d cells around
 // its cell (a7, "neighbour gather staged in shared memory") and then makes the cell's n_select trials one after
 // the other (R9):
 //
 //   A  every lane evaluates the same Philox block and builds the same trial pose (uniform, no divergence), then
 //      the lanes stride over the staged candidates for the circumsphere broad phase (a8: "100 particles in
 //      the cells around ... only five pass") and append the survivors to a per-warp queue with ballot/popc;
-//   B  the queue is drained one entry per lane: fp32 GJK on the Minkowski difference (a9, Eq. (1)-(2)); lanes whose
-//      fp32 verdict is "unsure" (near contact) re-run their pair in fp64 (mixed precision); one vote
+//   B  the queue is drained one entry per lane: polygon separating axes, or fp32 GJK on the Minkowski difference (a9,
+//      Eq. (1)-(2)) where lanes whose fp32 verdict is "unsure" (near contact) re-run their pair in fp64; one vote
 //      (__any_sync) gives the trial's fate -- the early exit of P:45 at warp granularity;
 //   C  lane 0 writes an accepted pose to the staged copy (so trial k+1 sees it) and to global memory (a11).
 //
@@ -35,9 +37,9 @@ struct Warp3dSmem {
     int start[28];
 };
 
-template <int KIND>
+template <int KIND, int NV, int DIM>
 __global__ void __launch_bounds__(32 * kW3Warps)
-k_sweep_warp3d(const __grid_constant__ GridParams g, const __grid_constant__ MoveParams mv, const __grid_constant__ ShapeF S,
+k_sweep_warpcell(const __grid_constant__ GridParams g, const __grid_constant__ MoveParams mv, const __grid_constant__ ShapeF S,
                const __grid_constant__ ShapeD SD, Control* __restrict__ ctrl, int colour_index, int cap_limit,
                float4* __restrict__ pos, float4* __restrict__ quat, const int* __restrict__ tag,
                const int* __restrict__ cell_start, uint32_t k0, uint32_t k1, uint2* __restrict__ trace)
@@ -49,26 +51,27 @@ k_sweep_warp3d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
     const SweepHeader& H = ctrl->hdr;
     const int gamma = H.perm[colour_index];
     const uint32_t t_lo = H.t_lo, t_hi16 = H.t_hi16;
-    const float shift[3] = {H.shift[0], H.shift[1], H.shift[2]};
-    const int nax = g.n[0] >> 1, nay = g.n[1] >> 1, naz = g.n[2] >> 1;
+    const float shift[3] = {H.shift[0], H.shift[1], DIM == 3 ? H.shift[2] : 0.0f};
+    constexpr int NNB = (DIM == 3) ? 27 : 9, OWN = (DIM == 3) ? 13 : 4;   // cells of the 3^d block; index of the own cell
+    const int nax = g.n[0] >> 1, nay = g.n[1] >> 1, naz = (DIM == 3) ? (g.n[2] >> 1) : 1;
     const int idx = blockIdx.x * kW3Warps + warp;
     if (idx >= nax * nay * naz) return;   // whole warp; nothing below synchronises across warps
     const int ix = idx % nax, iy = (idx / nax) % nay, iz = idx / (nax * nay);
-    const int cx = 2 * ix + (gamma & 1), cy = 2 * iy + ((gamma >> 1) & 1), cz = 2 * iz + ((gamma >> 2) & 1);
+    const int cx = 2 * ix + (gamma & 1), cy = 2 * iy + ((gamma >> 1) & 1), cz = (DIM == 3) ? 2 * iz + ((gamma >> 2) & 1) : 0;
     const int cell = cx + g.n[0] * (cy + g.n[1] * cz);
     const long long slot0 = (long long)cell * mv.n_select;
     // With the grid shifted by s in [0,w), the box edge lies inside cell n-1, so cell n-1 holds coordinates near both
     // +L/2 and -L/2.  Only cells 0, n-2 and n-1 can therefore see a neighbour across the periodic seam; only there is
     // the precise min_image needed (R21); elsewhere |x_j - x_t| < 2w <= L/2 and the plain fp32 difference is the same value.
-    const bool seam = cx == 0 || cy == 0 || cz == 0 || cx >= g.n[0] - 2 || cy >= g.n[1] - 2 || cz >= g.n[2] - 2;
+    const bool seam = cx == 0 || cy == 0 || cx >= g.n[0] - 2 || cy >= g.n[1] - 2 || (DIM == 3 && (cz == 0 || cz >= g.n[2] - 2));
 
-    // ---- staging: lane j < 27 owns neighbour cell j = (dz+1)*9 + (dy+1)*3 + (dx+1) ---------------------------------
+    // ---- staging: lane j < 3^d owns neighbour cell j = (dz+1)*9 + (dy+1)*3 + (dx+1) --------------------------------
     int my_start = 0, my_cnt = 0;
-    if (lane < 27) {
-        int nx = cx + (lane % 3) - 1, ny = cy + ((lane / 3) % 3) - 1, nz = cz + (lane / 9) - 1;
+    if (lane < NNB) {
+        int nx = cx + (lane % 3) - 1, ny = cy + ((lane / 3) % 3) - 1, nz = (DIM == 3) ? cz + (lane / 9) - 1 : 0;
         nx += (nx < 0) ? g.n[0] : 0; nx -= (nx >= g.n[0]) ? g.n[0] : 0;
         ny += (ny < 0) ? g.n[1] : 0; ny -= (ny >= g.n[1]) ? g.n[1] : 0;
-        nz += (nz < 0) ? g.n[2] : 0; nz -= (nz >= g.n[2]) ? g.n[2] : 0;
+        if (DIM == 3) { nz += (nz < 0) ? g.n[2] : 0; nz -= (nz >= g.n[2]) ? g.n[2] : 0; }
         const int c = nx + g.n[0] * (ny + g.n[1] * nz);
         my_start = cell_start[c];
         my_cnt = cell_start[c + 1] - my_start;
@@ -80,8 +83,8 @@ k_sweep_warp3d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
         if (lane >= o) incl += n;
     }
     const int total = __shfl_sync(0xffffffffu, incl, 31);
-    const int own_s = __shfl_sync(0xffffffffu, incl - my_cnt, 13);
-    const int nmem = __shfl_sync(0xffffffffu, my_cnt, 13);
+    const int own_s = __shfl_sync(0xffffffffu, incl - my_cnt, OWN);
+    const int nmem = __shfl_sync(0xffffffffu, my_cnt, OWN);
     CellCounters cc;
     if (nmem == 0) {
         if (trace && lane == 0)
@@ -90,20 +93,22 @@ k_sweep_warp3d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
     }
     if (total > min(cap_limit, kW3Cap)) {   // warp-uniform: neighbourhood does not fit the staging buffers
         if (lane == 0)
-            sweep_cell_global<KIND, 0>(g, mv, S, SD, gamma, t_lo, t_hi16, shift, cx, cy, cz, pos, quat, tag, cell_start, k0, k1, trace, cc);
+            sweep_cell_global<KIND, NV>(g, mv, S, SD, gamma, t_lo, t_hi16, shift, cx, cy, cz, pos, quat, tag, cell_start, k0, k1, trace, cc);
         flush_counters(ctrl, cc);
         return;
     }
-    if (lane < 28) { sm.off[lane] = incl - my_cnt; sm.start[lane] = my_start; }   // lane 27: off = total
+    if (lane <= NNB) { sm.off[lane] = incl - my_cnt; sm.start[lane] = my_start; }   // lane 3^d: off = total
     __syncwarp();
     for (int e = lane; e < total; e += 32) {
-        int j = 0;   // largest j with off[j] <= e (off is non-decreasing, off[27] = total > e)
+        int j = 0;   // largest j with off[j] <= e (off is non-decreasing, off[3^d] = total > e)
 #pragma unroll
         for (int s = 16; s >= 1; s >>= 1)
-            if (j + s < 27 && sm.off[j + s] <= e) j += s;
+            if (j + s < NNB && sm.off[j + s] <= e) j += s;
         const int gi = sm.start[j] + (e - sm.off[j]);
-        sm.pos[e] = pos[gi];
-        sm.quat[e] = (KIND != kKindDisk) ? quat[gi] : make_float4(1.f, 0.f, 0.f, 0.f);
+        float4 x4, q4;
+        load_state(DIM, pos, quat, gi, x4, q4);
+        sm.pos[e] = x4;
+        sm.quat[e] = q4;
         sm.gidx[e] = gi;
     }
     __syncwarp();
@@ -112,12 +117,13 @@ k_sweep_warp3d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
     for (int k = 0; k < mv.n_select; ++k) {
         // ---- phase A: trial generation (a0, a5, a6), identical on every lane -----------------------------------------
         const U4 b0 = philox4x32_10((uint32_t)cell, t_lo, (uint32_t)k, c3, k0, k1);
-        const uint32_t uc = philox4x32_10((uint32_t)cell, t_lo, (uint32_t)k | (1u << 16), c3, k0, k1).x;
+        uint32_t uc = 0u;
+        if (DIM == 3) uc = philox4x32_10((uint32_t)cell, t_lo, (uint32_t)k | (1u << 16), c3, k0, k1).x;
         const int p = own_s + (int)mulhi32(b0.x, (uint32_t)nmem);   // R8
         const float4 xp = sm.pos[p], qp = sm.quat[p];
         TrialState A;
         bool rotate;
-        int outcome = make_trial<KIND>(g, mv, shift, cell, 3, b0, uc, xp, qp, A, rotate) ? 1 : 2;
+        int outcome = make_trial<KIND>(g, mv, shift, cell, DIM, b0, uc, xp, qp, A, rotate) ? 1 : 2;
         if (lane == 0) ++cc.trials;
         if (outcome == 1) {
             float MA[9];
@@ -132,7 +138,7 @@ k_sweep_warp3d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
                     const float4 xq = sm.pos[q];
                     const float rx = seam ? min_image(xq.x, A.x, g.hi[0], g.Ld[0]) : xq.x - A.x;
                     const float ry = seam ? min_image(xq.y, A.y, g.hi[1], g.Ld[1]) : xq.y - A.y;
-                    const float rz = seam ? min_image(xq.z, A.z, g.hi[2], g.Ld[2]) : xq.z - A.z;
+                    const float rz = (DIM == 3) ? (seam ? min_image(xq.z, A.z, g.hi[2], g.Ld[2]) : xq.z - A.z) : 0.0f;
                     const float d2 = rx * rx + ry * ry + rz * rz;
                     hit = d2 < S.dmax2;                                  // R16
                     if (hit && (KIND == kKindDisk || d2 < S.din2)) sure = true;
@@ -144,6 +150,19 @@ k_sweep_warp3d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
             bool overlap = __any_sync(0xffffffffu, sure);
             __syncwarp();
             // ---- phase B: narrow phase (a9), one queue entry per lane ----------------------------------------------
+            if (KIND == kKindPolygon) {
+                const float4 T = make_float4(A.x, A.y, A.qw, A.qz);
+                for (int base = 0; base < nq && !overlap; base += 32) {
+                    const int e = base + lane;
+                    bool ov = false;
+                    if (e < nq) {
+                        const int q = sm.queue[e];
+                        const float4 xq = sm.pos[q], qq = sm.quat[q];
+                        ov = pair_overlap_2d<KIND, NV>(g, S, T, make_float4(xq.x, xq.y, qq.x, qq.w), mv.eps_g, seam);
+                    }
+                    overlap = __any_sync(0xffffffffu, ov);
+                }
+            }
             if (KIND == kKindPolyhedron) {
                 for (int base = 0; base < nq && !overlap; base += 32) {
                     const int e = base + lane;
@@ -172,21 +191,19 @@ k_sweep_warp3d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
         if (lane == 0) {
             if (outcome == 1) {
                 const int gi = sm.gidx[p];
-                if (!rotate) {
-                    float x = A.x, y = A.y, z = A.z;
+                float x = A.x, y = A.y, z = A.z;
+                if (!rotate) {   // R-wrap
                     if (x >= g.hi[0]) x = __fsub_rn(x, g.L[0]); else if (x < g.lo[0]) x = __fadd_rn(x, g.L[0]);
                     if (y >= g.hi[1]) y = __fsub_rn(y, g.L[1]); else if (y < g.lo[1]) y = __fadd_rn(y, g.L[1]);
-                    if (z >= g.hi[2]) z = __fsub_rn(z, g.L[2]); else if (z < g.lo[2]) z = __fadd_rn(z, g.L[2]);
-                    const float4 nx4 = make_float4(x, y, z, xp.w);
-                    pos[gi] = nx4;
-                    sm.pos[p] = nx4;
+                    if (DIM == 3) { if (z >= g.hi[2]) z = __fsub_rn(z, g.L[2]); else if (z < g.lo[2]) z = __fadd_rn(z, g.L[2]); }
                     ++cc.tacc;
                 } else {
-                    const float4 nq4 = make_float4(A.qw, A.qx, A.qy, A.qz);
-                    quat[gi] = nq4;
-                    sm.quat[p] = nq4;
                     ++cc.racc;
                 }
+                const float4 nx4 = make_float4(x, y, z, xp.w), nq4 = make_float4(A.qw, A.qx, A.qy, A.qz);
+                store_state(DIM, pos, quat, gi, nx4, nq4, rotate);
+                sm.pos[p] = nx4;
+                sm.quat[p] = nq4;
             } else if (outcome == 2) {
                 ++cc.trcell;
             } else {

@@ -178,6 +178,54 @@ def cubes(n_lat: int = 32, seed: int = 1, max_tilt: float = 0.15, name: str = "k
                     extra={"seed": seed, "phi": N / L ** 3})
 
 
+def dodecahedron_vertices(circumradius: float = 0.5) -> np.ndarray:
+    """The 20 vertices of a regular dodecahedron: (+-1,+-1,+-1) and the cyclic permutations of (0, +-1/phi, +-phi)."""
+    gr = 0.5 * (1.0 + np.sqrt(5.0))
+    v = [[sx, sy, sz] for sx in (-1, 1) for sy in (-1, 1) for sz in (-1, 1)]
+    for a in (-1, 1):
+        for b in (-1, 1):
+            v += [[0, a / gr, b * gr], [a / gr, b * gr, 0], [a * gr, 0, b / gr]]
+    v = np.array(v, dtype=np.float64)
+    return v * (circumradius / np.sqrt(3.0))
+
+
+def truncated_octahedron_vertices(circumradius: float = 0.5) -> np.ndarray:
+    """The 24 vertices of a truncated octahedron: all permutations of (0, +-1, +-2)."""
+    import itertools
+    v = set()
+    for perm in itertools.permutations((0, 1, 2)):
+        for s1 in (-1, 1):
+            for s2 in (-1, 1):
+                c = [0.0, 0.0, 0.0]
+                c[perm[1]] = s1 * 1.0
+                c[perm[2]] = s2 * 2.0
+                v.add(tuple(c))
+    v = np.array(sorted(v), dtype=np.float64)
+    return v * (circumradius / np.sqrt(5.0))
+
+
+def polyhedra(verts: np.ndarray, n_lat: int = 6, spacing: float = 1.05, seed: int = 1, max_tilt: float = 0.2,
+              name: str = "polyhedra") -> Workload:
+    """Generic convex polyhedra (the paper's other benchmark shapes) on a simple-cubic lattice: spacing above the
+    circumsphere diameter, so any orientation is overlap-free; small random tilts.  Parity cases for the GJK kernel with more
+    vertices than a cube; not one of the BASELINE.json configs."""
+    N = n_lat ** 3
+    dmax = 2.0 * float(np.max(np.linalg.norm(verts, axis=1)))
+    assert spacing > dmax
+    pos4 = _lattice(3, n_lat, spacing)
+    rng = _rng(seed, 404)
+    z = 2.0 * rng.random(N) - 1.0
+    phi = 2.0 * np.pi * rng.random(N)
+    rho = np.sqrt(1.0 - z * z)
+    axis = np.stack([rho * np.cos(phi), rho * np.sin(phi), z], axis=1)
+    ang = max_tilt * rng.random(N)
+    q = np.concatenate([np.cos(0.5 * ang)[:, None], np.sin(0.5 * ang)[:, None] * axis], axis=1)
+    L = n_lat * spacing
+    return Workload(name=name, dim=3, N=N, L=(L, L, L), kind=KIND_POLYHEDRON, diameter=0.0, verts=verts, d=0.1, a=0.2,
+                    n_select=4, sweeps=100, pos4=pos4, quat4=q.astype(np.float32), warmup_sweeps=50,
+                    extra={"seed": seed})
+
+
 def config(k: int, seed: int = 1) -> Workload:
     """BASELINE.json configs[k], k = 0..4."""
     if k == 0:

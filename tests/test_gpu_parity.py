@@ -33,6 +33,8 @@ CASES = {
     "k1_pentagons": lambda: wl.config(1),
     "cubes_12": lambda: wl.cubes(12),
     "spheres_8": lambda: spheres(8),
+    "dodecahedra_6": lambda: wl.polyhedra(wl.dodecahedron_vertices(0.5), 6, 1.04, name="dodecahedra_6"),
+    "trunc_octahedra_6": lambda: wl.polyhedra(wl.truncated_octahedron_vertices(0.5), 6, 1.04, name="trunc_octahedra_6"),
 }
 
 
@@ -105,7 +107,8 @@ def lockstep(w, n_sweeps, seed=1):
 
 
 @pytest.mark.parametrize("name,n", [("disks_24", 10), ("pentagons_24", 10), ("cubes_7", 10), ("spheres_8", 10),
-                                    ("k0_disks", 10), ("k1_pentagons", 10), ("cubes_12", 4)])
+                                    ("k0_disks", 10), ("k1_pentagons", 10), ("cubes_12", 4),
+                                    ("dodecahedra_6", 6), ("trunc_octahedra_6", 6)])
 def test_first_sweeps_lockstep_with_oracle(name, n):
     w = CASES[name]()
     stats, g, o = lockstep(w, n)
@@ -137,7 +140,8 @@ def test_colour_pass_variants_agree_bit_for_bit(name):
     ref = None
     some = 40 if w.dim == 2 else (84 if w.kind == wl.KIND_POLYHEDRON else 50)   # a capacity only some tiles/cells exceed
     shapes = [{"tile_shape": k} for k in (1, 2, 3, 4)] if w.dim == 2 else []   # every 2-D tile shape
-    for opts in [{"path": 2}, {"path": 2, "tile_cap": 0}, {"path": 1}, {"path": 2, "tile_cap": some}] + shapes:
+    warp = [{"path": 3}, {"path": 3, "tile_cap": 6}] if w.dim == 2 else []        # 2-D warp-per-cell pass and its fallback
+    for opts in [{"path": 2}, {"path": 2, "tile_cap": 0}, {"path": 1}, {"path": 2, "tile_cap": some}] + shapes + warp:
         g = gpu(w)
         for k, v in opts.items():
             g.set_option(k, v)
