@@ -48,7 +48,7 @@ def test_create_validation_and_grid(lib):
     gi = hb.GridInfo(); assert lib.hpmc_get_grid(h, C.byref(gi)) == 0
     assert list(gi.n)[:2] == [70, 70] and gi.num_cells == 4900 and gi.N == 4096
     assert np.float32(gi.L_f[0]) == np.float32(70.4)
-    assert lib.hpmc_workspace_bytes(h) > 4096 * (2 * 36 + 8)
+    assert lib.hpmc_workspace_bytes(h) > 4096 * (2 * 20 + 8)     # 2-D: two pose+tag buffers and the (cell, rank) keys
     # unbound context: sweeping is an error, not a crash
     assert lib.hpmc_sweep(h, 1) == -4
     assert b"not bound" in lib.hpmc_last_error(h)
