@@ -7,14 +7,14 @@
 
 namespace hpmc {
 
-constexpr int kScanThreads = 512;
+constexpr int kScanThreads = 1024;
 constexpr int kScanItems = 16;
 constexpr int kScanTile = kScanThreads * kScanItems;
 
-// Three launches build the cell list of a sweep:
+// Three to five launches build the cell list of a sweep:
 //   k_hist          header (a0, a1) + cell id and arrival rank of every particle (a2, first half of a3)
-//   k_scan          single-pass exclusive scan of the per-cell counts (decoupled look-back), zeroes the counts for the
-//                   next build, advances the sweep counter
+//   k_scan_*        exclusive scan of the per-cell counts (one launch when the grid fits one tile of 16 384 counts, else
+//                   reduce / spine / final), zeroes the counts for the next build, advances the sweep counter
 //   k_scatter_sort  scatter into the cell-sorted SoA; the last particle to arrive in a cell puts the cell's members in
 //                   ascending tag order (R8)
 // mode 0: header of the device sweep counter t; k_scan then does t++ and sweeps++   (a real sweep)
@@ -75,34 +75,67 @@ __device__ __forceinline__ int block_exclusive_scan(int v, int& total)
     return offset + inc - v;
 }
 
-// tile state of the single-pass scan: value (low 32 bits) | epoch << 34 | status << 32; status 1 = tile aggregate,
-// 2 = inclusive prefix.  The epoch makes words of earlier launches invalid without clearing the array.
-__device__ __forceinline__ unsigned long long scan_pack(unsigned int value, unsigned int status, unsigned long long epoch)
+// second quarter of a3: cell_start[i] = sum of counts[0..i) for i = 0..n (n = C: the grand total).  Warp w of a tile owns
+// 32*kScanItems consecutive counts; item k of lane l is element k*32 + l of that chunk, so every load and store is one
+// coalesced 128-byte line per warp.  A grid that fits one tile (configs 0, 1, 3) runs k_scan_final alone; larger ones run
+// reduce -> spine -> final.  (A single-pass decoupled look-back scan was measured slower here: its inclusive-prefix
+// wavefront advances 32 tiles per L2 round trip, 0.77 TB/s on 16.7 M counts.)
+__global__ void __launch_bounds__(kScanThreads) k_scan_reduce(const int* __restrict__ counts, int n, int* __restrict__ tile_sums)
 {
-    return (unsigned long long)value | ((unsigned long long)status << 32) | (epoch << 34);
+    __shared__ int s_wsum[kScanThreads / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int wbase = blockIdx.x * kScanTile + warp * (32 * kScanItems) + lane;
+    int s = 0;
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        const int idx = wbase + 32 * k;
+        if (idx <= n) s += counts[idx];
+    }
+    s = __reduce_add_sync(0xffffffffu, s);
+    if (lane == 0) s_wsum[warp] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int t = 0;
+#pragma unroll
+        for (int w = 0; w < kScanThreads / 32; ++w) t += s_wsum[w];
+        tile_sums[blockIdx.x] = t;
+    }
 }
 
-// second quarter of a3: cell_start[i] = sum of counts[0..i) for i = 0..n (n = C: the grand total), one pass.
-// Tiles take tickets so that every predecessor of a tile is already resident (no deadlock in the look-back).
-__global__ void __launch_bounds__(kScanThreads)
-k_scan(int* __restrict__ counts, int n, int* __restrict__ cell_start, unsigned long long* __restrict__ tile_state,
-       Control* __restrict__ ctrl, int ntiles, int mode)
+// exclusive scan of the tile totals by ONE block; also advances the sweep counter of a real sweep (mode 0)
+__global__ void __launch_bounds__(kScanThreads) k_scan_spine(int* __restrict__ tile_sums, int ntiles, Control* __restrict__ ctrl, int mode)
 {
-    __shared__ int s_tile;
-    __shared__ int s_prefix;
-    __shared__ unsigned long long s_epoch;
+    __shared__ int carry_s;
     if (threadIdx.x == 0) {
-        s_epoch = ctrl->scan_epoch;                       // read BEFORE taking the ticket (see the last tile below)
-        s_tile = (int)atomicAdd(&ctrl->scan_ticket, 1u);
+        carry_s = 0;
+        if (mode == 0) {
+            ctrl->t += 1ull;
+            ctrl->sweeps += 1ull;
+        }
     }
     __syncthreads();
-    const int tile = s_tile;
-    const unsigned long long epoch = s_epoch & 0x3fffffffull;
-    // warp w owns 32*kScanItems consecutive counts; item k of lane l is element k*32 + l of that chunk: every load and
-    // store is one coalesced 128-byte line per warp
+    for (int base = 0; base < ntiles; base += kScanThreads) {
+        const int i = base + threadIdx.x;
+        const int v = (i < ntiles) ? tile_sums[i] : 0;
+        int total;
+        const int ex = block_exclusive_scan(v, total);
+        const int carry = carry_s;
+        if (i < ntiles) tile_sums[i] = carry + ex;
+        __syncthreads();
+        if (threadIdx.x == 0) carry_s = carry + total;
+        __syncthreads();
+    }
+}
+
+// exclusive scan inside each tile plus the tile's offset; re-zeroes the counts for the next build.  single != 0: the whole
+// grid is one tile (no reduce/spine pass ran), so this kernel also advances the sweep counter.
+__global__ void __launch_bounds__(kScanThreads)
+k_scan_final(int* __restrict__ counts, int n, int* __restrict__ cell_start, const int* __restrict__ tile_sums, int single,
+             Control* __restrict__ ctrl, int mode)
+{
     __shared__ int s_wsum[kScanThreads / 32];
-    const int lane_ = threadIdx.x & 31, warp_ = threadIdx.x >> 5;
-    const int wbase = tile * kScanTile + warp_ * (32 * kScanItems) + lane_;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int wbase = blockIdx.x * kScanTile + warp * (32 * kScanItems) + lane;
     int v[kScanItems], ex[kScanItems];
 #pragma unroll
     for (int k = 0; k < kScanItems; ++k) {
@@ -118,49 +151,20 @@ k_scan(int* __restrict__ counts, int n, int* __restrict__ cell_start, unsigned l
         ex[k] = carry + inc - v[k];
         carry += __shfl_sync(0xffffffffu, inc, 31);
     }
-    if (lane_ == 0) s_wsum[warp_] = carry;
+    if (lane == 0) s_wsum[warp] = carry;
     __syncthreads();
-    int woff = 0, total = 0;
+    int off = single ? 0 : tile_sums[blockIdx.x];
 #pragma unroll
-    for (int w = 0; w < kScanThreads / 32; ++w) {
-        const int t = s_wsum[w];
-        if (w < warp_) woff += t;
-        total += t;
-    }
-    if (threadIdx.x < 32) {                               // warp 0: publish, look back 32 tiles at a time
-        volatile unsigned long long* st = tile_state;
-        const int lane = threadIdx.x;
-        int prefix = 0;
-        if (lane == 0) st[tile] = scan_pack((unsigned)total, tile == 0 ? 2u : 1u, epoch);
-        for (int j = tile - 1; j >= 0; j -= 32) {
-            const int idx = j - lane;
-            unsigned long long w = scan_pack(0u, 2u, epoch);          // before tile 0: an inclusive prefix of zero
-            if (idx >= 0)
-                do { w = st[idx]; } while ((w >> 34) != epoch || ((w >> 32) & 3ull) == 0ull);
-            const unsigned incl = __ballot_sync(0xffffffffu, ((w >> 32) & 3ull) == 2ull);
-            const int first = incl ? __ffs(incl) - 1 : 31;            // nearest tile that already knows its inclusive prefix
-            prefix += __reduce_add_sync(0xffffffffu, lane <= first ? (int)(unsigned int)w : 0);
-            if (incl) break;
-        }
-        if (lane == 0) {
-            if (tile != 0) st[tile] = scan_pack((unsigned)(prefix + total), 2u, epoch);
-            s_prefix = prefix;
-            if (tile == ntiles - 1) {                     // every other tile has already read the epoch and its ticket
-                ctrl->scan_ticket = 0u;
-                ctrl->scan_epoch = (epoch + 1ull) & 0x3fffffffull;
-                if (mode == 0) {
-                    ctrl->t += 1ull;
-                    ctrl->sweeps += 1ull;
-                }
-            }
-        }
-    }
-    __syncthreads();
-    const int off = s_prefix + woff;
+    for (int w = 0; w < kScanThreads / 32; ++w)
+        if (w < warp) off += s_wsum[w];
 #pragma unroll
     for (int k = 0; k < kScanItems; ++k) {
         const int idx = wbase + 32 * k;
         if (idx <= n) cell_start[idx] = off + ex[k];
+    }
+    if (single && mode == 0 && threadIdx.x == 0) {
+        ctrl->t += 1ull;
+        ctrl->sweeps += 1ull;
     }
 }
 

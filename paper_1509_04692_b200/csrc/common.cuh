@@ -51,8 +51,6 @@ struct Control {
     // pentagons).  Readers sum the replicas.
     unsigned long long counters[kCounterSets][8];
     unsigned long long overlaps;     // validator result
-    unsigned long long scan_epoch;   // k_scan: launch stamp of the tile-state words
-    unsigned int scan_ticket, pad0;  // k_scan: next tile to hand out
     SweepHeader hdr;
 };
 

@@ -50,7 +50,7 @@ struct hpmc_ctx {
     int* cell_start = nullptr;  // C+1 (+ padding)
     int* counts = nullptr;      // per-cell histogram, all zero between builds
     int* arrived = nullptr;     // per-cell arrival counter of k_scatter_sort, all zero between builds
-    unsigned long long* tile_state = nullptr;   // look-back words of k_scan
+    int* tile_sums = nullptr;   // per-tile totals of the scan
     Control* ctrl = nullptr;
 
     uint2* trace = nullptr;
@@ -110,7 +110,7 @@ struct Carve {
 int scan_tiles(const hpmc_ctx* c) { return (c->g.C + 1 + kScanTile - 1) / kScanTile; }
 
 struct Layout {
-    size_t pos[2], quat[2], tag[2], key_rank, cell_start, counts, arrived, tile_state, ctrl, total;
+    size_t pos[2], quat[2], tag[2], key_rank, cell_start, counts, arrived, tile_sums, ctrl, total;
 };
 
 Layout layout_of(const hpmc_ctx* c)
@@ -127,7 +127,7 @@ Layout layout_of(const hpmc_ctx* c)
     L.cell_start = cv.take(((size_t)c->g.C + 2) * sizeof(int));
     L.counts = cv.take(((size_t)c->g.C + 2) * sizeof(int));
     L.arrived = cv.take(((size_t)c->g.C + 2) * sizeof(int));
-    L.tile_state = cv.take((size_t)(scan_tiles(c) + 1) * sizeof(unsigned long long));
+    L.tile_sums = cv.take((size_t)(scan_tiles(c) + 1) * sizeof(int));
     L.ctrl = cv.take(sizeof(Control));
     L.total = cv.off;
     return L;
@@ -292,8 +292,14 @@ int build_cell_list(hpmc_ctx* c, int mode, unsigned long long t_override)
     k_hist<<<nblk_part > 0 ? nblk_part : 1, TB, 0, c->stream>>>(g, c->ctrl, src_pos, c->counts, c->key_rank, c->k0, c->k1, mode, t_override);
     LAUNCH_CHECK(c, "k_hist");
     const int tiles = scan_tiles(c);
-    k_scan<<<tiles, kScanThreads, 0, c->stream>>>(c->counts, g.C, c->cell_start, c->tile_state, c->ctrl, tiles, mode);
-    LAUNCH_CHECK(c, "k_scan");
+    if (tiles > 1) {
+        k_scan_reduce<<<tiles, kScanThreads, 0, c->stream>>>(c->counts, g.C, c->tile_sums);
+        LAUNCH_CHECK(c, "k_scan_reduce");
+        k_scan_spine<<<1, kScanThreads, 0, c->stream>>>(c->tile_sums, tiles, c->ctrl, mode);
+        LAUNCH_CHECK(c, "k_scan_spine");
+    }
+    k_scan_final<<<tiles, kScanThreads, 0, c->stream>>>(c->counts, g.C, c->cell_start, c->tile_sums, tiles == 1, c->ctrl, mode);
+    LAUNCH_CHECK(c, "k_scan_final");
     if (g.N > 0) {
         k_scatter_sort<<<nblk_part, TB, 0, c->stream>>>(g.N, g.dim, src_pos, src_quat, src_tag, c->key_rank, c->cell_start, c->arrived,
                                                        c->pos[dst], c->quat[dst], c->tag[dst]);
@@ -525,7 +531,7 @@ int hpmc_bind(hpmc_ctx* c, float* d_pos4, float* d_quat4, void* d_workspace, siz
     c->cell_start = (int*)(c->d_ws + L.cell_start);
     c->counts = (int*)(c->d_ws + L.counts);
     c->arrived = (int*)(c->d_ws + L.arrived);
-    c->tile_state = (unsigned long long*)(c->d_ws + L.tile_state);
+    c->tile_sums = (int*)(c->d_ws + L.tile_sums);
     c->ctrl = (Control*)(c->d_ws + L.ctrl);
     if (first) {  // a new workspace: zero the builder's scratch, (re)create the control block, keeping the host-side sweep counter
         if (!cuda_ok(c, cudaMemsetAsync(c->d_ws + L.counts, 0, L.ctrl - L.counts, c->stream), "bind/memset")) return HPMC_E_CUDA;
