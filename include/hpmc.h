@@ -139,6 +139,8 @@ int hpmc_sweep_host(hpmc_ctx* ctx, const float* h_pos4, const float* h_quat4, in
  *              (tests set 0 to force that fallback everywhere).
  *   "tile_shape" 2-D tile kernel shape: 0 = chosen by grid size, 1..7 = fixed (warps per CTA x rows of 32 active cells per
  *              warp x minimum CTAs per SM; see pick_tile_shape in hpmc_api.cu).
+ *   "flow"     2-D tile pass: -1 (default) or 1 = the four colours of a sweep go out as ONE persistent launch in which a tile
+ *              of colour c+1 starts as soon as the nine tiles of colour c around it are done; 0 = one launch per colour.
  *   "graph"    1 (default): hpmc_sweep(n >= 3) replays a captured CUDA graph of two sweeps; 0: plain launches.
  *              Needs a real stream: contexts created on the legacy default stream (NULL) always use plain launches.  */
 int hpmc_set_option(hpmc_ctx* ctx, const char* name, int64_t value);

@@ -51,6 +51,7 @@ struct Control {
     // pentagons).  Readers sum the replicas.
     unsigned long long counters[kCounterSets][8];
     unsigned long long overlaps;     // validator result
+    unsigned int flow_ticket, flow_exited;   // k_sweep_tile2d_flow: next (colour, tile) ticket; CTAs that have left
     SweepHeader hdr;
 };
 
@@ -59,13 +60,13 @@ struct Control {
 __device__ __forceinline__ void load_state(int dim, const float4* __restrict__ pos, const float4* __restrict__ quat, int i,
                                            float4& x, float4& q)
 {
-    const float4 P = pos[i];
+    const float4 P = __ldcg(&pos[i]);   // L2-coherent: the dataflow pass reads poses other CTAs of the same launch wrote
     if (dim == 2) {
         x = make_float4(P.x, P.y, 0.0f, 0.0f);
         q = make_float4(P.z, 0.0f, 0.0f, P.w);
     } else {
         x = P;
-        q = quat[i];
+        q = __ldcg(&quat[i]);
     }
 }
 

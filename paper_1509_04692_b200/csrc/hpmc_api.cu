@@ -51,6 +51,9 @@ struct hpmc_ctx {
     int* counts = nullptr;      // per-cell histogram, all zero between builds
     int* arrived = nullptr;     // per-cell arrival counter of k_scatter_sort, all zero between builds
     int* tile_sums = nullptr;   // per-tile totals of the scan
+    unsigned int* flow_done = nullptr;   // per (colour, tile) stamps of the dataflow pass
+    int num_sms = 0;
+    bool flow_now = false;               // this sweep's colour passes go out as one dataflow launch
     Control* ctrl = nullptr;
 
     uint2* trace = nullptr;
@@ -60,6 +63,7 @@ struct hpmc_ctx {
     int opt_path = 0;                 // 0 auto, 1 per-thread global path, 2 tile path (2-D only)
     int opt_tile_cap = 1 << 30;       // staging capacity limit of the tile kernel (tests force the overflow path)
     int opt_tile_shape = 0;           // 0 = by grid size, 1..7 = fixed (see pick_tile_shape)
+    int opt_flow = -1;                // 2-D tile pass as one dataflow launch per sweep: -1 = when it pays (auto), 0 = never, 1 = always
     int opt_graph = 1;                // 1: hpmc_sweep(n >= 3) replays a captured two-sweep CUDA graph
 
     // CUDA graph of two consecutive sweeps (the ping-pong buffers return to where they started), one per parity of `cur`
@@ -109,8 +113,16 @@ struct Carve {
 
 int scan_tiles(const hpmc_ctx* c) { return (c->g.C + 1 + kScanTile - 1) / kScanTile; }
 
+// `done` stamps of the 2-D dataflow pass: 4 colours x tiles of the smallest tile shape (2 rows of 32 active cells)
+size_t flow_words(const hpmc_ctx* c)
+{
+    if (c->g.dim != 2) return 1;
+    const size_t nax = c->g.n[0] / 2, nay = c->g.n[1] / 2;
+    return 4 * ((nax + kTileW - 1) / kTileW) * ((nay + 1) / 2) + 4;
+}
+
 struct Layout {
-    size_t pos[2], quat[2], tag[2], key_rank, cell_start, counts, arrived, tile_sums, ctrl, total;
+    size_t pos[2], quat[2], tag[2], key_rank, cell_start, counts, arrived, tile_sums, flow_done, ctrl, total;
 };
 
 Layout layout_of(const hpmc_ctx* c)
@@ -128,6 +140,7 @@ Layout layout_of(const hpmc_ctx* c)
     L.counts = cv.take(((size_t)c->g.C + 2) * sizeof(int));
     L.arrived = cv.take(((size_t)c->g.C + 2) * sizeof(int));
     L.tile_sums = cv.take((size_t)(scan_tiles(c) + 1) * sizeof(int));
+    L.flow_done = cv.take(flow_words(c) * sizeof(unsigned int));
     L.ctrl = cv.take(sizeof(Control));
     L.total = cv.off;
     return L;
@@ -241,8 +254,8 @@ bool profile_fold(hpmc_ctx* c)
     for (size_t i = 0; i < c->ev_class.size(); ++i) {
         float ms = 0.f;
         if (!cuda_ok(c, cudaEventElapsedTime(&ms, c->ev_pool[2 * i], c->ev_pool[2 * i + 1]), "profile/elapsed")) return false;
-        c->prof_ms[c->ev_class[i]] += (double)ms;
-        c->prof_n[c->ev_class[i]] += 1;
+        c->prof_ms[c->ev_class[i] & 15] += (double)ms;
+        c->prof_n[c->ev_class[i] & 15] += c->ev_class[i] >> 4;   // a bracket may cover several colour passes (dataflow launch)
     }
     c->ev_class.clear();
     c->ev_used = 0;
@@ -252,7 +265,7 @@ bool profile_fold(hpmc_ctx* c)
 struct ProfileScope {
     hpmc_ctx* c;
     bool on;
-    ProfileScope(hpmc_ctx* ctx, int cls) : c(ctx), on(ctx->profile && !ctx->cuda_failed)
+    ProfileScope(hpmc_ctx* ctx, int cls, int weight = 1) : c(ctx), on(ctx->profile && !ctx->cuda_failed)
     {
         if (!on) return;
         if (c->ev_class.size() >= 4096) profile_fold(c);
@@ -261,7 +274,7 @@ struct ProfileScope {
             if (cudaEventCreate(&e) != cudaSuccess) { on = false; return; }
             c->ev_pool.push_back(e);
         }
-        c->ev_class.push_back(cls);
+        c->ev_class.push_back(cls | (weight << 4));
         cudaEventRecord(c->ev_pool[c->ev_used], c->stream);
     }
     ~ProfileScope()
@@ -316,14 +329,27 @@ bool launch_tile2d(hpmc_ctx* c, int ci)
 {
     using TL = Tile2D<WARPS, R>;
     const GridParams& g = c->g;
+    const int nax = g.n[0] / 2, nay = g.n[1] / 2;
+    const int tiles = ((nax + kTileW - 1) / kTileW) * ((nay + TL::TH - 1) / TL::TH);
+    if (c->flow_now) {   // all four colours in one persistent dataflow launch (issued for colour index 0 only)
+        auto kern = k_sweep_tile2d_flow<KIND, NV, WARPS, R, MINB>;
+        static bool attr_set = false;   // per template instance
+        if (!attr_set) {
+            if (!cuda_ok(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TL::bytes), "flow/attr")) return false;
+            attr_set = true;
+        }
+        const int slots = c->num_sms * MINB;
+        kern<<<4 * tiles < slots ? 4 * tiles : slots, TL::NT, TL::bytes, c->stream>>>(g, c->mv, c->sf, c->sd, c->ctrl, c->opt_tile_cap,
+                                                                                        c->pos[c->cur], c->tag[c->cur], c->cell_start, c->k0,
+                                                                                        c->k1, c->trace, c->flow_done);
+        return true;
+    }
     auto kern = k_sweep_tile2d<KIND, NV, WARPS, R, MINB>;
     static bool attr_set = false;   // per template instance
     if (!attr_set) {
         if (!cuda_ok(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TL::bytes), "tile/attr")) return false;
         attr_set = true;
     }
-    const int nax = g.n[0] / 2, nay = g.n[1] / 2;
-    const int tiles = ((nax + kTileW - 1) / kTileW) * ((nay + TL::TH - 1) / TL::TH);
     kern<<<tiles, TL::NT, TL::bytes, c->stream>>>(g, c->mv, c->sf, c->sd, c->ctrl, ci, c->opt_tile_cap, c->pos[c->cur], c->tag[c->cur],
                                                   c->cell_start, c->k0, c->k1, c->trace);
     return true;
@@ -380,9 +406,26 @@ bool launch_colour(hpmc_ctx* c, int ci)
     return true;
 }
 
+// does the 2-D tile pass apply (not the warp-per-cell pass, not the per-thread path), and as a dataflow launch?
+bool use_flow(const hpmc_ctx* c)
+{
+    const GridParams& g = c->g;
+    if (g.dim != 2 || c->sf.kind == kKindPolyhedron || c->opt_path == 1 || c->opt_path == 3 || c->opt_flow == 0) return false;
+    const int nactive = (g.n[0] / 2) * (g.n[1] / 2);
+    if (c->opt_path == 0 && c->opt_tile_shape == 0 && nactive <= kWarpCellMax2d) return false;
+    if (c->opt_flow == 1) return true;
+    // auto: the dataflow launch pays when a colour is one to a few waves of tiles (measured on B200: +9 % at 1M pentagons,
+    // 1.7 waves; slower below one wave, where the stamps only add latency; no difference from 4M up)
+    const long long slots = (long long)c->num_sms * 8;
+    const long long tiles = (long long)((g.n[0] / 2 + kTileW - 1) / kTileW) * ((g.n[1] / 2 + 3) / 4);
+    return c->opt_tile_shape == 0 && tiles > slots && tiles <= 4 * slots;
+}
+
 int launch_colour_dispatch(hpmc_ctx* c, int ci)
 {
-    ProfileScope prof(c, 1);
+    c->flow_now = use_flow(c);
+    if (c->flow_now && ci > 0) return HPMC_OK;   // colour 0's dataflow launch covers all four colours
+    ProfileScope prof(c, 1, c->flow_now ? 4 : 1);
     bool ok = true;
     switch (c->sf.kind) {
         case kKindDisk: ok = launch_colour<kKindDisk, 0>(c, ci); break;
@@ -476,6 +519,11 @@ int hpmc_create(const hpmc_box* box, const hpmc_shape* shape, int64_t N, uint64_
     c->k0 = (uint32_t)seed;
     c->k1 = (uint32_t)(seed >> 32);
     c->stream = (cudaStream_t)cuda_stream;
+    {
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess) c->num_sms = sms;
+        if (c->num_sms <= 0) c->num_sms = 148;   // no device visible (CPU-side ABI checks): B200
+    }
     c->mv.d = 0.1f; c->mv.a = 0.1f; c->mv.n_select = 4; c->mv.eps_g = 2e-6f;  // R15
     refresh_sweep_range(c);
     *out = c;
@@ -532,6 +580,7 @@ int hpmc_bind(hpmc_ctx* c, float* d_pos4, float* d_quat4, void* d_workspace, siz
     c->counts = (int*)(c->d_ws + L.counts);
     c->arrived = (int*)(c->d_ws + L.arrived);
     c->tile_sums = (int*)(c->d_ws + L.tile_sums);
+    c->flow_done = (unsigned int*)(c->d_ws + L.flow_done);
     c->ctrl = (Control*)(c->d_ws + L.ctrl);
     if (first) {  // a new workspace: zero the builder's scratch, (re)create the control block, keeping the host-side sweep counter
         if (!cuda_ok(c, cudaMemsetAsync(c->d_ws + L.counts, 0, L.ctrl - L.counts, c->stream), "bind/memset")) return HPMC_E_CUDA;
@@ -668,6 +717,8 @@ int hpmc_set_sweep_counter(hpmc_ctx* c, uint64_t t)
     if (c->cuda_failed) return HPMC_E_CUDA;
     c->t_host = t;
     if (c->ctrl) {
+        // the dataflow pass stamps tiles with the sweep counter: a counter set back must not meet its old stamps
+        if (!cuda_ok(c, cudaMemsetAsync(c->flow_done, 0, flow_words(c) * sizeof(unsigned int), c->stream), "set_t/memset")) return HPMC_E_CUDA;
         const unsigned long long v = t;
         if (!cuda_ok(c, cudaMemcpyAsync(&c->ctrl->t, &v, sizeof v, cudaMemcpyHostToDevice, c->stream), "set_t/memcpy")) return HPMC_E_CUDA;
         if (!cuda_ok(c, cudaStreamSynchronize(c->stream), "set_t/sync")) return HPMC_E_CUDA;
@@ -757,6 +808,9 @@ int hpmc_set_option(hpmc_ctx* c, const char* name, int64_t value)
     } else if (n == "tile_cap") {
         if (value < 0) return fail(c, HPMC_E_ARG, "tile_cap must be >= 0");
         c->opt_tile_cap = value > (1 << 30) ? (1 << 30) : (int)value;
+    } else if (n == "flow") {
+        if (value < -1 || value > 1) return fail(c, HPMC_E_ARG, "flow must be -1 (auto), 0 or 1");
+        c->opt_flow = (int)value;
     } else if (n == "tile_shape") {
         if (value < 0 || value > 7) return fail(c, HPMC_E_ARG, "tile_shape must be 0 (auto) or 1..7");
         c->opt_tile_shape = (int)value;

@@ -218,13 +218,13 @@ __device__ void sweep_cell_global(const GridParams& g, const MoveParams& mv, con
                                 const int qs = cell_start[row + nx], qe = cell_start[row + nx + 1];
                                 for (int q = qs; q < qe; ++q) {
                                     if (q == p) continue;
-                                    const float4 xq = pos[q];   // 2-D: the pose (x, y, qw, qz)
+                                    const float4 xq = __ldcg(&pos[q]);   // 2-D: the pose (x, y, qw, qz)
                                     const float rx = min_image(xq.x, A.x, g.hi[0], g.Ld[0]);
                                     const float ry = min_image(xq.y, A.y, g.hi[1], g.Ld[1]);
                                     const float rz = (g.dim == 3) ? min_image(xq.z, A.z, g.hi[2], g.Ld[2]) : 0.0f;
                                     if (rx * rx + ry * ry + rz * rz >= S.dmax2) continue;   // a8 circumsphere (R16)
                                     float4 qq = make_float4(1.f, 0.f, 0.f, 0.f);
-                                    if (KIND != kKindDisk) qq = (g.dim == 2) ? make_float4(xq.z, 0.f, 0.f, xq.w) : quat[q];
+                                    if (KIND != kKindDisk) qq = (g.dim == 2) ? make_float4(xq.z, 0.f, 0.f, xq.w) : __ldcg(&quat[q]);
                                     double rd[3] = {0.0, 0.0, 0.0};
                                     if (KIND == kKindPolyhedron) {
                                         rd[0] = min_image_d(xq.x, A.x, g.Ld[0]);

@@ -94,15 +94,15 @@ __device__ __forceinline__ void broad_slots(const GridParams& g, const ShapeF& S
     }
 }
 
-template <int KIND, int NV, int WARPS, int R, int MINB>
-__global__ void __launch_bounds__(32 * WARPS, MINB)
-k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ MoveParams mv, const __grid_constant__ ShapeF S,
-               const __grid_constant__ ShapeD SD, Control* __restrict__ ctrl, int colour_index, int cap_limit,
-               float4* __restrict__ pose, const int* __restrict__ tag, const int* __restrict__ cell_start, uint32_t k0,
-               uint32_t k1, uint2* __restrict__ trace)
+// The work of one tile of colour gamma (see the header of this file).  FLOW: the caller is the persistent dataflow kernel,
+// where other CTAs of the same launch wrote some of the poses read here: stage them with L2-coherent loads.
+template <int KIND, int NV, int WARPS, int R, bool FLOW>
+__device__ __forceinline__ void tile2d_body(const GridParams& g, const MoveParams& mv, const ShapeF& S, const ShapeD& SD,
+                                            Control* __restrict__ ctrl, int gamma, int tile, int cap_limit, float4* __restrict__ pose,
+                                            const int* __restrict__ tag, const int* __restrict__ cell_start, uint32_t k0, uint32_t k1,
+                                            uint2* __restrict__ trace, unsigned char* smem_raw)
 {
     using TL = Tile2D<WARPS, R>;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
     // staged poses, positions and orientations apart: the broad phase reads only (x, y), and 8-byte elements halve the
     // shared-memory bank conflicts of its per-lane gathers (lane stride ~2 poses) against one 16-byte array
     float2* sm_xy = reinterpret_cast<float2*>(smem_raw + TL::off_pose);                          // (x, y)
@@ -119,14 +119,13 @@ k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
     unsigned char* sm_act = smem_raw + TL::off_act;
 
     const SweepHeader& H = ctrl->hdr;
-    const int gamma = H.perm[colour_index];
     const uint32_t t_lo = H.t_lo, t_hi16 = H.t_hi16;
     const float shift[3] = {H.shift[0], H.shift[1], 0.0f};
     const int gx = gamma & 1, gy = (gamma >> 1) & 1;
     const int n0 = g.n[0], n1 = g.n[1];
     const int nax = n0 >> 1, nay = n1 >> 1;
     const int tiles_x = (nax + kTileW - 1) / kTileW;
-    const int tx = blockIdx.x % tiles_x, ty = blockIdx.x / tiles_x;
+    const int tx = tile % tiles_x, ty = tile / tiles_x;
     const int ix0 = tx * kTileW, iy0 = ty * TL::TH;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // region = cells [cx0-1, cx0-1+RW) x [cy0-1, cy0-1+RHv) (unwrapped), clipped to what the valid active cells need
@@ -206,8 +205,8 @@ k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
             const int cx = second ? rx - split : xs + rx;
             sm_lstart[ry * RW + rx] = (unsigned short)(row_start[cx] - (second ? g1 : g0) + (second ? l1 : l0));
         }
-        for (int e = lane; e < l1 - l0; e += 32) st_pose(l0 + e, pose[g0 + e]);
-        for (int e = lane; e < l2 - l1; e += 32) st_pose(l1 + e, pose[g1 + e]);
+        for (int e = lane; e < l1 - l0; e += 32) st_pose(l0 + e, FLOW ? __ldcg(&pose[g0 + e]) : pose[g0 + e]);
+        for (int e = lane; e < l2 - l1; e += 32) st_pose(l1 + e, FLOW ? __ldcg(&pose[g1 + e]) : pose[g1 + e]);
     }
     if (tid == 0) sm_lstart[ncells] = (unsigned short)ntot;
     if (tid < 8) st_pose(ntot + tid, make_float4(3.0e18f, 3.0e18f, 1.0f, 0.0f));   // sentinels behind the last staged pose
@@ -366,6 +365,71 @@ k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ Mov
         __syncwarp();
     }
     flush_counters(ctrl, cc);
+}
+
+// One launch = one colour: one tile per CTA.
+template <int KIND, int NV, int WARPS, int R, int MINB>
+__global__ void __launch_bounds__(32 * WARPS, MINB)
+k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ MoveParams mv, const __grid_constant__ ShapeF S,
+               const __grid_constant__ ShapeD SD, Control* __restrict__ ctrl, int colour_index, int cap_limit,
+               float4* __restrict__ pose, const int* __restrict__ tag, const int* __restrict__ cell_start, uint32_t k0,
+               uint32_t k1, uint2* __restrict__ trace)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    tile2d_body<KIND, NV, WARPS, R, false>(g, mv, S, SD, ctrl, ctrl->hdr.perm[colour_index], (int)blockIdx.x, cap_limit, pose, tag,
+                                           cell_start, k0, k1, trace, smem_raw);
+}
+
+// One launch = all four colours of a sweep, as a dataflow over (colour, tile) tickets.  A colour pass ends with a tail in
+// which the last tiles run on a nearly empty GPU (a tile is four sequential trial rounds, ~20 us), and the next launch cannot
+// start before it drains: ~16 of the 70 us of a pass on 1M pentagons.  But a tile of colour c+1 only needs the tiles of
+// colour c that overlap its staged region -- the 3x3 tiles around it (they wrote poses it reads, and they read poses it will
+// write) -- so persistent CTAs take tickets in (colour, tile) order and a tile waits just for those nine `done` stamps.  Every
+// ticket a tile waits for is lower than its own, hence already held by a running or finished CTA: no deadlock.  Stamps are
+// the sweep counter + 1, so the array is never cleared between sweeps.
+template <int KIND, int NV, int WARPS, int R, int MINB>
+__global__ void __launch_bounds__(32 * WARPS, MINB)
+k_sweep_tile2d_flow(const __grid_constant__ GridParams g, const __grid_constant__ MoveParams mv, const __grid_constant__ ShapeF S,
+                    const __grid_constant__ ShapeD SD, Control* __restrict__ ctrl, int cap_limit, float4* __restrict__ pose,
+                    const int* __restrict__ tag, const int* __restrict__ cell_start, uint32_t k0, uint32_t k1,
+                    uint2* __restrict__ trace, unsigned int* __restrict__ done)
+{
+    using TL = Tile2D<WARPS, R>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ int s_ticket;
+    const int nax = g.n[0] >> 1, nay = g.n[1] >> 1;
+    const int tiles_x = (nax + kTileW - 1) / kTileW, tiles_y = (nay + TL::TH - 1) / TL::TH;
+    const int ntiles = tiles_x * tiles_y;
+    const unsigned stamp = ctrl->hdr.t_lo + 1u;
+    volatile unsigned int* vdone = done;
+    for (;;) {
+        __syncthreads();                                   // the previous tile's shared memory is no longer in use
+        if (threadIdx.x == 0) s_ticket = (int)atomicAdd(&ctrl->flow_ticket, 1u);
+        __syncthreads();
+        const int ticket = s_ticket;
+        if (ticket >= 4 * ntiles) break;
+        const int ci = ticket / ntiles, tile = ticket - ci * ntiles;
+        if (ci > 0 && threadIdx.x < 9) {                   // the nine tiles of the previous colour around this one
+            const int tx = tile % tiles_x, ty = tile / tiles_x;
+            int nx = tx + (int)(threadIdx.x % 3) - 1, ny = ty + (int)(threadIdx.x / 3) - 1;
+            nx += (nx < 0) ? tiles_x : 0; nx -= (nx >= tiles_x) ? tiles_x : 0;
+            ny += (ny < 0) ? tiles_y : 0; ny -= (ny >= tiles_y) ? tiles_y : 0;
+            const int dep = (ci - 1) * ntiles + ny * tiles_x + nx;
+            while (vdone[dep] != stamp) __nanosleep(100);
+            __threadfence();
+        }
+        __syncthreads();
+        tile2d_body<KIND, NV, WARPS, R, true>(g, mv, S, SD, ctrl, ctrl->hdr.perm[ci], tile, cap_limit, pose, tag, cell_start, k0, k1,
+                                              trace, smem_raw);
+        __threadfence();                                   // this thread's pose write-backs are visible device-wide ...
+        __syncthreads();
+        if (threadIdx.x == 0) vdone[ci * ntiles + tile] = stamp;   // ... before the tile is announced
+    }
+    // the last CTA to leave re-arms the ticket counter for the next launch
+    if (threadIdx.x == 0 && atomicAdd(&ctrl->flow_exited, 1u) == gridDim.x - 1) {
+        ctrl->flow_exited = 0u;
+        ctrl->flow_ticket = 0u;
+    }
 }
 
 }  // namespace hpmc

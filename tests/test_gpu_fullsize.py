@@ -54,6 +54,13 @@ def _lockstep_full(k, n_lock, n_more):
     g2.sweep(n_lock)
     p2, q2 = g2.get_state()
     assert np.array_equal(p2, gp) and np.array_equal(q2, gq) and g2.counters() == gc
+    # one launch per colour instead of the dataflow launch (or the reverse): the same trajectory
+    g3 = hb.from_workload(w, seed=1)
+    g3.set_option("flow", 0 if k == 2 else 1)
+    g3.sweep(n_lock)
+    p3, q3 = g3.get_state()
+    assert np.array_equal(p3, gp) and np.array_equal(q3, gq) and g3.counters() == gc
+    del g3, p3, q3
     del g, o, gp, gq, op, oq
     # properties at any size, after more sweeps in the timed configuration
     g2.reset_counters()
