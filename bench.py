@@ -300,7 +300,8 @@ def main():
     else:
         roof = {"bound": "alu", "achieved": flops_launch / (colour_ms * 1e-3) / 1e12, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s"}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof.update({"traffic": NCU_TRAFFIC.get(w.name), "kernel": "k_sweep_tile2d" if w.dim == 2 else "k_sweep_warp3d", "avg_launch_ms": colour_ms, "launches_timed": prof["colour_n"],
+    roof.update({"traffic": NCU_TRAFFIC.get(w.name), "kernel": g.describe_pass(), "avg_launch_ms": colour_ms,
+                 "avg_launch_ms_note": "per colour pass; a dataflow launch covers 4 passes and is counted as 4", "launches_timed": prof["colour_n"],
                  "peak_source": f"{hbm_src} hbm_gbs (MEASURED_PEAKS.json)" if roof["bound"] == "hbm" else "148 SM x 128 lanes x 2 x 1.965 GHz",
                  "algorithmic_bytes_per_launch": bytes_launch, "algorithmic_flops_per_launch": flops_launch,
                  "kernel_share_of_step": prof["colour_ms"] / r["ms"], "build_share_of_step": prof["build_ms"] / r["ms"],

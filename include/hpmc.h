@@ -152,6 +152,10 @@ int hpmc_set_option(hpmc_ctx* ctx, const char* name, int64_t value);
 int hpmc_set_profile(hpmc_ctx* ctx, int on);
 int hpmc_get_profile(hpmc_ctx* ctx, double* h_ms_build, int64_t* h_n_build, double* h_ms_colour, int64_t* h_n_colour);
 
+/* Which colour-pass kernel the current options select for this system, as text (for reports), e.g.
+ * "k_sweep_tile2d_flow<4 warps x 1 row, 8 CTAs/SM>: 4 colour passes per launch".  Returns the length written.   */
+int hpmc_describe_pass(const hpmc_ctx* ctx, char* h_buf, size_t buf_bytes);
+
 /* Launch bookkeeping for bench.py: kernels launched by this context so far.                        */
 int64_t hpmc_launch_count(const hpmc_ctx* ctx);
 

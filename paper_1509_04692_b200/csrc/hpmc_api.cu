@@ -1,5 +1,6 @@
 // C-ABI of libhpmc.so (include/hpmc.h): host-side context, validation, workspace carving and the launch
 // sequence of one sweep.  Every step of the hot path runs in the kernels of cell_list.cuh / sweep.cuh.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -840,6 +841,26 @@ int hpmc_get_profile(hpmc_ctx* c, double* h_ms_build, int64_t* h_n_build, double
     if (h_ms_colour) *h_ms_colour = c->prof_ms[1];
     if (h_n_colour) *h_n_colour = c->prof_n[1];
     return HPMC_OK;
+}
+
+int hpmc_describe_pass(const hpmc_ctx* c, char* h_buf, size_t n)
+{
+    if (!c || !h_buf || n == 0) return HPMC_E_ARG;
+    const GridParams& g = c->g;
+    const int nactive = (g.n[0] / 2) * (g.n[1] / 2) * (g.dim == 3 ? g.n[2] / 2 : 1);
+    std::string d;
+    if (c->opt_path == 1) d = "k_sweep_colour: one thread per active cell";
+    else if (g.dim == 3 || c->opt_path == 3 || (c->opt_path == 0 && c->opt_tile_shape == 0 && nactive <= kWarpCellMax2d))
+        d = "k_sweep_warpcell: one warp per active cell, 1 colour pass per launch";
+    else {
+        static const char* shapes[8] = {"", "8 warps x 2 rows, 2 CTAs/SM", "4 x 2, 4 CTAs/SM", "4 x 1, 5 CTAs/SM", "2 x 1, 8 CTAs/SM",
+                                        "4 warps x 1 row, 8 CTAs/SM", "8 x 1, 3 CTAs/SM", "4 x 1, 6 CTAs/SM"};
+        const bool flow = use_flow(c);
+        d = std::string(flow ? "k_sweep_tile2d_flow<" : "k_sweep_tile2d<") + shapes[pick_tile_shape(c)] + ">: " +
+            (flow ? "4 colour passes per launch (dataflow)" : "1 colour pass per launch");
+    }
+    std::snprintf(h_buf, n, "%s", d.c_str());
+    return (int)std::min(d.size(), n - 1);
 }
 
 int64_t hpmc_launch_count(const hpmc_ctx* c) { return c ? c->launches : 0; }

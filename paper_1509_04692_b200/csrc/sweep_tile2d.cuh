@@ -75,6 +75,7 @@ template <int KIND, bool SEAM>
 __device__ __forceinline__ void broad_slots(const GridParams& g, const ShapeF& S, const float2* sm_xy, const int (&rs)[3], int p,
                                             const float4& T, unsigned& mask, bool& sure)
 {
+    float closest = 3.0e38f;   // smallest squared centre distance: one compare after the loop instead of a branch per slot
 #pragma unroll
     for (int dy = 0; dy < 3; ++dy) {
 #pragma unroll
@@ -87,11 +88,12 @@ __device__ __forceinline__ void broad_slots(const GridParams& g, const ShapeF& S
                 ry = min_image(B.y, T.y, g.hi[1], g.Ld[1]);
             }
             const float d2 = rx * rx + ry * ry;
-            const bool hit = (q != p) && (d2 < S.dmax2);                           // R16
-            if (hit) mask |= 1u << (kRowSlots * dy + j);
-            if (hit && (KIND == kKindDisk || d2 < S.din2)) sure = true;           // inside the inscribed-disk bound
+            const bool hit = (q != p) & (d2 < S.dmax2);                            // R16
+            mask |= hit ? (1u << (kRowSlots * dy + j)) : 0u;
+            closest = fminf(closest, (q != p) ? d2 : 3.0e38f);
         }
     }
+    sure = closest < ((KIND == kKindDisk) ? S.dmax2 : S.din2);                    // inside the inscribed-disk bound (disks: any hit)
 }
 
 // The work of one tile of colour gamma (see the header of this file).  FLOW: the caller is the persistent dataflow kernel,
