@@ -340,7 +340,7 @@ bool launch_tile2d(hpmc_ctx* c, int ci)
             attr_set = true;
         }
         const int slots = c->num_sms * MINB;
-        kern<<<4 * tiles < slots ? 4 * tiles : slots, TL::NT, TL::bytes, c->stream>>>(g, c->mv, c->sf, c->sd, c->ctrl, c->opt_tile_cap,
+        kern<<<tiles < slots ? tiles : slots, TL::NT, TL::bytes, c->stream>>>(g, c->mv, c->sf, c->sd, c->ctrl, c->opt_tile_cap,
                                                                                         c->pos[c->cur], c->tag[c->cur], c->cell_start, c->k0,
                                                                                         c->k1, c->trace, c->flow_done);
         return true;

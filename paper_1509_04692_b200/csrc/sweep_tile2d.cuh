@@ -417,7 +417,11 @@ k_sweep_tile2d_flow(const __grid_constant__ GridParams g, const __grid_constant_
             nx += (nx < 0) ? tiles_x : 0; nx -= (nx >= tiles_x) ? tiles_x : 0;
             ny += (ny < 0) ? tiles_y : 0; ny -= (ny >= tiles_y) ? tiles_y : 0;
             const int dep = (ci - 1) * ntiles + ny * tiles_x + nx;
-            while (vdone[dep] != stamp) __nanosleep(100);
+            unsigned ns = 128u;
+            while (vdone[dep] != stamp) {   // exponential back-off: every poll is an L2 access competing with working CTAs
+                __nanosleep(ns);
+                ns = ns < 2048u ? 2u * ns : ns;
+            }
             __threadfence();
         }
         __syncthreads();
