@@ -88,3 +88,26 @@ def test_binding_fails_loudly_without_gpu():
     w = wl.disks(8)
     with pytest.raises(hb.HpmcError):
         hb.from_workload(w)
+
+
+def test_options_and_pass_description_need_no_gpu(lib):
+    """hpmc_set_option validates names and ranges; hpmc_describe_pass names the kernel the options select."""
+    def describe(h):
+        buf = C.create_string_buffer(256)
+        assert lib.hpmc_describe_pass(h, buf, 256) > 0
+        return buf.value.decode()
+    rc, h = _create(lib, 2, (1024.0, 1024.0), hb.KIND_POLYGON, 1 << 20, verts=wl.regular_polygon(5, 0.5))
+    assert rc == 0
+    assert describe(h).startswith("k_sweep_tile2d_flow<4 warps x 1 row")          # 1.7 waves of tiles: dataflow launch
+    assert lib.hpmc_set_option(h, b"flow", 0) == 0 and describe(h).startswith("k_sweep_tile2d<")
+    assert lib.hpmc_set_option(h, b"path", 1) == 0 and describe(h).startswith("k_sweep_colour")
+    assert lib.hpmc_set_option(h, b"path", 7) == -1 and lib.hpmc_set_option(h, b"flow", 2) == -1
+    assert lib.hpmc_set_option(h, b"tile_shape", 9) == -1 and lib.hpmc_set_option(h, b"no_such_option", 1) == -1
+    assert lib.hpmc_destroy(h) == 0
+    rc, h = _create(lib, 2, (64.0, 64.0), hb.KIND_POLYGON, 4096, verts=wl.regular_polygon(5, 0.5))
+    assert rc == 0 and describe(h).startswith("k_sweep_warpcell")                  # 961 active cells per colour
+    assert lib.hpmc_set_option(h, b"path", 2) == 0 and describe(h).startswith("k_sweep_tile2d<")   # below one wave: per colour
+    assert lib.hpmc_destroy(h) == 0
+    rc, h = _create(lib, 3, (40.0, 40.0, 40.0), hb.KIND_POLYHEDRON, 32768, verts=wl.cube_vertices(1.0))
+    assert rc == 0 and describe(h).startswith("k_sweep_warpcell")
+    assert lib.hpmc_destroy(h) == 0
