@@ -239,3 +239,63 @@ def test_sweep_host_round_trip():
     c = b.sweep_host(hp, hq, 5, op, oq)
     assert np.array_equal(op.numpy(), pa) and np.array_equal(oq.numpy(), qa)
     assert c["trials"] == a.counters()["trials"]
+
+
+def _lattice_workload(dim, n, spacing, kind, verts=None, diameter=0.0, d=0.1, a=0.2, n_select=4, seed=3):
+    """Particles on an n[0] x n[1] (x n[2]) lattice in a box with DIFFERENT edges per axis, random orientations."""
+    idx = np.stack(np.meshgrid(*[np.arange(k) for k in n], indexing="ij"), axis=-1).reshape(-1, dim)
+    L = np.array([n[k] * spacing[k] for k in range(dim)])
+    pos = np.zeros((idx.shape[0], 4), np.float32)
+    pos[:, :dim] = ((idx + 0.5) * np.array(spacing) - 0.5 * L).astype(np.float32)
+    rng = np.random.default_rng(seed)
+    quat = np.zeros((idx.shape[0], 4), np.float32)
+    if dim == 2:
+        th = rng.uniform(0, 2 * np.pi, idx.shape[0])
+        quat[:, 0], quat[:, 3] = np.cos(th / 2), np.sin(th / 2)
+    else:
+        q = rng.normal(size=(idx.shape[0], 4))
+        quat[:] = (q / np.linalg.norm(q, axis=1, keepdims=True)).astype(np.float32)
+    return wl.Workload(name="lattice", dim=dim, N=idx.shape[0], L=tuple(L), kind=kind, diameter=diameter, verts=verts, d=d, a=a,
+                       n_select=n_select, sweeps=1, pos4=pos, quat4=quat)
+
+
+@pytest.mark.parametrize("case", ["rect_pentagons_tile", "rect_pentagons_warp", "rect_disks_ns1", "slab_cubes", "slab_spheres_ns9",
+                                  "big_step"])
+def test_lockstep_on_rectangular_boxes_and_other_move_settings(case):
+    """Grids with different cell counts per axis (partial tiles, seams of different lengths), n_select 1 and 9, and a step
+    size above half a cell (legal, most trials leave the cell)."""
+    pent = wl.regular_polygon(5, 0.5)
+    opts = {}
+    if case == "rect_pentagons_tile":
+        w = _lattice_workload(2, (70, 37), (1.07, 1.12), wl.KIND_POLYGON, verts=pent); opts = {"path": 2}
+    elif case == "rect_pentagons_warp":
+        w = _lattice_workload(2, (23, 41), (1.1, 1.05), wl.KIND_POLYGON, verts=pent); opts = {"path": 3}
+    elif case == "rect_disks_ns1":
+        w = _lattice_workload(2, (45, 90), (1.2, 1.08), wl.KIND_DISK, diameter=1.0, d=0.2, n_select=1); opts = {"path": 2, "flow": 1}
+    elif case == "slab_cubes":
+        w = _lattice_workload(3, (5, 8, 6), (1.8, 1.75, 1.9), wl.KIND_POLYHEDRON, verts=wl.cube_vertices(1.0))
+    elif case == "slab_spheres_ns9":
+        w = _lattice_workload(3, (9, 6, 12), (1.15, 1.2, 1.1), wl.KIND_DISK, diameter=1.0, d=0.15, n_select=9)
+    else:
+        w = _lattice_workload(2, (40, 40), (1.15, 1.15), wl.KIND_POLYGON, verts=pent, d=0.8, a=1.5)
+    from paper_1509_04692_b200 import binding as hb
+    g, o = hb.from_workload(w, seed=5), orc(w, seed=5)
+    for k, v in opts.items():
+        g.set_option(k, v)
+    assert g.n[0] != g.n[1] or case == "big_step"
+    g.enable_trace(True)
+    marginal = 0
+    for s in range(6):
+        g.sweep(1)
+        f = o.sweep(follow=g.read_trace(), follow_tol=MARGIN_TOL)["follow"]
+        assert f["hard_mismatch"] == 0, (case, s, f)
+        marginal += f["marginal"]
+        gp, gq = g.get_state()
+        op, oq = o.get_state()
+        assert np.array_equal(gp, op) and np.max(np.abs(gq.astype(np.float64) - oq)) < 1e-5
+        o.set_state(op, gq)
+    gc, oc = g.counters(), o.counters()
+    assert all(gc[k] == oc[k] for k in oc)
+    assert g.count_overlaps() == 0 and o.count_overlaps_cells() == 0 and marginal <= 3
+    if case == "big_step":
+        assert gc["trans_rej_cell"] > 0.4 * (gc["trans_acc"] + gc["trans_rej_overlap"] + gc["trans_rej_cell"])
