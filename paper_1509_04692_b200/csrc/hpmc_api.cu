@@ -399,7 +399,7 @@ bool launch_colour(hpmc_ctx* c, int ci)
         }
     }
     if constexpr (KIND != kKindPolygon) {
-        if (g.dim == 3 && c->opt_path != 1) return launch_warpcell<KIND, 0, 3>(c, ci, nactive);   // one warp per active cell
+        if (g.dim == 3 && c->opt_path != 1) return launch_warpcell<KIND, NV, 3>(c, ci, nactive);   // one warp per active cell
     }
     const int TB = 128;
     k_sweep_colour<KIND, NV><<<(nactive + TB - 1) / TB, TB, 0, c->stream>>>(g, c->mv, c->sf, c->sd, c->ctrl, ci, c->pos[c->cur], c->quat[c->cur],
@@ -442,7 +442,9 @@ int launch_colour_dispatch(hpmc_ctx* c, int ci)
                 default: ok = launch_colour<kKindPolygon, 0>(c, ci); break;
             }
             break;
-        default: ok = launch_colour<kKindPolyhedron, 0>(c, ci); break;
+        default:   // polyhedra: the 8-vertex case (cubes, config 3) has an unrolled support function
+            ok = (c->sf.nverts == 8) ? launch_colour<kKindPolyhedron, 8>(c, ci) : launch_colour<kKindPolyhedron, 0>(c, ci);
+            break;
     }
     if (!ok) return HPMC_E_CUDA;
     LAUNCH_CHECK(c, "colour pass");
@@ -801,6 +803,9 @@ int hpmc_set_option(hpmc_ctx* c, const char* name, int64_t value)
     if (!c || !name) return HPMC_E_ARG;
     const std::string n(name);
     graph_reset(c);
+    // another tile shape indexes the dataflow stamps differently: start from the cleared state
+    if (c->flow_done && !c->cuda_failed &&
+        !cuda_ok(c, cudaMemsetAsync(c->flow_done, 0, flow_words(c) * sizeof(unsigned int), c->stream), "option/memset")) return HPMC_E_CUDA;
     if (n == "graph") {
         c->opt_graph = value != 0;
     } else if (n == "path") {

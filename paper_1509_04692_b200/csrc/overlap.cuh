@@ -157,7 +157,8 @@ __device__ __forceinline__ T polygon_max_sep(const ShapeT<T>& S, T rx, T ry, T c
 // convex polyhedra: GJK.  Rm = rotation taking B's body frame into A's body frame (row major),
 // r = r_AB expressed in A's frame.
 // ---------------------------------------------------------------------------------------------
-template <typename T>
+// NVP > 0: compile-time vertex count (the loop unrolls and the vertices become constant-bank operands); 0: runtime count.
+template <typename T, int NVP = 0>
 __device__ __forceinline__ V3<T> support_minkowski(const ShapeT<T>& S, const T* Rm, const V3<T>& r, const V3<T>& dir)
 {
     // R^-1 dir = R^T dir
@@ -165,7 +166,9 @@ __device__ __forceinline__ V3<T> support_minkowski(const ShapeT<T>& S, const T* 
                    Rm[2] * dir.x + Rm[5] * dir.y + Rm[8] * dir.z};
     T bestA = -(T)3.0e38, bestB = -(T)3.0e38;
     int ia = 0, ib = 0;
-    for (int i = 0; i < S.nverts; ++i) {
+    const int nv = (NVP > 0) ? NVP : S.nverts;
+#pragma unroll
+    for (int i = 0; i < nv; ++i) {
         const T da = -(dir.x * S.vx[i] + dir.y * S.vy[i] + dir.z * S.vz[i]);   // S_A(-dir)
         const T dbv = db.x * S.vx[i] + db.y * S.vy[i] + db.z * S.vz[i];        // S_B(R^-1 dir)
         if (da > bestA) { bestA = da; ia = i; }
@@ -207,7 +210,7 @@ __device__ __forceinline__ V3<T> closest_on_triangle(const V3<T>& a, const V3<T>
 // unreliable for gaps below ~1e-3: the fp32 caller re-runs kGjkUnsure pairs in fp64 (mixed precision);
 // the fp64 caller treats kGjkUnsure as overlap (conservative, R-poly).
 constexpr int kGjkSeparated = 1, kGjkOverlap = 0, kGjkUnsure = -1;
-template <typename T>
+template <typename T, int NVP = 0>
 __device__ int gjk_classify(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T eps, T deep)
 {
     const T tiny = (sizeof(T) == 4) ? (T)1e-14 : (T)1e-28;
@@ -218,7 +221,7 @@ __device__ int gjk_classify(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T e
     V3<T> W[4];
     int nW = 0;
     for (int iter = 0; iter < 40; ++iter) {
-        const V3<T> w = support_minkowski(S, Rm, r, V3<T>{-v.x, -v.y, -v.z});
+        const V3<T> w = support_minkowski<T, NVP>(S, Rm, r, V3<T>{-v.x, -v.y, -v.z});
         const T vw = dot(v, w);
         if (vw >= 0 && vw * vw >= eps * eps * vv) return kGjkSeparated;   // certificate: v^.w >= eps
         if (iter > 0 && vv - vw <= reltol * vv) return kGjkUnsure;           // converged: distance |v| < eps
@@ -302,7 +305,7 @@ __device__ __forceinline__ void quat_to_matrix(T w, T x, T y, T z, T* M)
 }
 
 // polyhedron pair in A's frame: MA, MB = world rotation matrices of A and B, rw = r_AB (world).  GJK verdict.
-template <typename T>
+template <typename T, int NVP = 0>
 __device__ __forceinline__ int polyhedron_classify(const ShapeT<T>& S, const T* MA, const T* MB, const V3<T>& rw, T eps, T deep)
 {
     T Rm[9];  // R = MA^T MB takes B's frame into A's frame (q = q_A* q_B)
@@ -312,7 +315,7 @@ __device__ __forceinline__ int polyhedron_classify(const ShapeT<T>& S, const T* 
         for (int j = 0; j < 3; ++j) Rm[3 * i + j] = MA[i] * MB[j] + MA[3 + i] * MB[3 + j] + MA[6 + i] * MB[6 + j];
     const V3<T> r{MA[0] * rw.x + MA[3] * rw.y + MA[6] * rw.z, MA[1] * rw.x + MA[4] * rw.y + MA[7] * rw.z,
                   MA[2] * rw.x + MA[5] * rw.y + MA[8] * rw.z};
-    return gjk_classify(S, Rm, r, eps, deep);
+    return gjk_classify<T, NVP>(S, Rm, r, eps, deep);
 }
 
 // fp64 narrow phase from the raw fp32 state: normalised quaternions, exact separation rd (already minimum image)

@@ -402,7 +402,9 @@ k_sweep_tile2d_flow(const __grid_constant__ GridParams g, const __grid_constant_
     const int nax = g.n[0] >> 1, nay = g.n[1] >> 1;
     const int tiles_x = (nax + kTileW - 1) / kTileW, tiles_y = (nay + TL::TH - 1) / TL::TH;
     const int ntiles = tiles_x * tiles_y;
-    const unsigned stamp = ctrl->hdr.t_lo + 1u;
+    // stamp of this sweep: 1 + (t mod (2^32 - 1)).  Never 0 (the cleared state), and different from the stamp of the sweep
+    // before, which is what every entry holds when the sweep starts -- also across the 2^32 wrap of the counter
+    const unsigned stamp = (unsigned)((((unsigned long long)ctrl->hdr.t_hi16 << 32) | ctrl->hdr.t_lo) % 0xFFFFFFFFull) + 1u;
     volatile unsigned int* vdone = done;
     for (;;) {
         __syncthreads();                                   // the previous tile's shared memory is no longer in use

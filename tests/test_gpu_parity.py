@@ -299,3 +299,19 @@ def test_lockstep_on_rectangular_boxes_and_other_move_settings(case):
     assert g.count_overlaps() == 0 and o.count_overlaps_cells() == 0 and marginal <= 3
     if case == "big_step":
         assert gc["trans_rej_cell"] > 0.4 * (gc["trans_acc"] + gc["trans_rej_overlap"] + gc["trans_rej_cell"])
+
+
+def test_dataflow_pass_across_the_32_bit_wrap_of_the_sweep_counter():
+    """The dataflow launch stamps finished tiles with a value derived from the sweep counter; the stamps must stay distinct
+    from sweep to sweep (and from the cleared state) when the low word of the counter wraps."""
+    w = wl.pentagons(48)
+    out = []
+    for flow in (0, 1):
+        g = gpu(w)
+        g.set_option("path", 2); g.set_option("flow", flow)
+        g.sweep(2)
+        g.set_sweep_counter(2 ** 32 - 3)
+        g.sweep(1); g.sweep(7)                       # plain launches and graph replays: t = 2^32 - 3 .. 2^32 + 4
+        assert g.counters()["sweep_counter"] == 2 ** 32 + 5 and g.count_overlaps() == 0
+        out.append((g.get_state(), g.counters()))
+    assert np.array_equal(out[0][0][0], out[1][0][0]) and np.array_equal(out[0][0][1], out[1][0][1]) and out[0][1] == out[1][1]
