@@ -137,8 +137,8 @@ int hpmc_sweep_host(hpmc_ctx* ctx, const float* h_pos4, const float* h_quat4, in
  *              the warp-per-cell pass), 3 = warp-per-cell colour pass (automatic in 3-D and for small 2-D systems)
  *   "tile_cap" upper limit on the particles a tile may stage; tiles above it take the per-thread path
  *              (tests set 0 to force that fallback everywhere).
- *   "tile_shape" 2-D tile kernel shape: 0 = chosen by grid size, 1..7 = fixed (warps per CTA x rows of 32 active cells per
- *              warp x minimum CTAs per SM; see pick_tile_shape in hpmc_api.cu).
+ *   "tile_shape" 2-D tile kernel shape: 0 = chosen by grid size, 1 = 8 warps per CTA x 2 rows of 32 active cells per warp,
+ *              2 = 4 warps x 1 row at 64 registers (8 CTAs per SM; large grids), 3 = 2 warps x 1 row (small grids).
  *   "flow"     2-D tile pass: -1 (default) or 1 = the four colours of a sweep go out as ONE persistent launch in which a tile
  *              of colour c+1 starts as soon as the nine tiles of colour c around it are done; 0 = one launch per colour.
  *   "graph"    1 (default): hpmc_sweep(n >= 3) replays a captured CUDA graph of two sweeps; 0: plain launches.

@@ -1,13 +1,19 @@
-"""Build libhpmc.so in-tree with nvcc for sm_100a (no JIT cache: the .so travels with the repo snapshot)."""
+"""Build libhpmc.so in-tree with nvcc for sm_100a (no JIT cache: the .so travels with the repo snapshot).
+
+The library is several translation units (the C-ABI + cell-list kernels, and one per family of colour-pass kernels) that
+are compiled in parallel and linked; no relocatable device code is needed, every kernel is self-contained.
+"""
 import os
 import subprocess
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "_obj")
 LIB = os.path.join(HERE, "libhpmc.so")
-SOURCES = [os.path.join(CSRC, "hpmc_api.cu")]
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--shared",
-              "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+UNITS = ["hpmc_api", "pass_colour", "pass_tile2d_disk", "pass_tile2d_pentagon", "pass_tile2d_polygon", "pass_warpcell_2d",
+         "pass_warpcell_3d"]
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
 
 def _newest_source() -> float:
@@ -22,16 +28,32 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_source():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    fast = ["-DHPMC_FAST_BUILD"] if os.environ.get("HPMC_FAST_BUILD") == "1" else []   # development: fewer unrolled polygon sizes
-    cmd = [nvcc] + NVCC_FLAGS + fast + ["-o", LIB] + SOURCES
-    res = subprocess.run(cmd, capture_output=True, text=True)
+    os.makedirs(OBJ, exist_ok=True)
+
+    def compile_unit(u):
+        cmd = [nvcc] + NVCC_FLAGS + ["-c", os.path.join(CSRC, u + ".cu"), "-o", os.path.join(OBJ, u + ".o")]
+        return u, cmd, subprocess.run(cmd, capture_output=True, text=True)
+
+    with ThreadPoolExecutor(max_workers=min(len(UNITS), os.cpu_count() or 1)) as ex:
+        results = list(ex.map(compile_unit, UNITS))
+    log = []
+    for u, cmd, res in results:
+        log.append(" ".join(cmd) + "\n" + res.stderr)
+        if verbose or res.returncode != 0:
+            print(res.stdout)
+            print(res.stderr)
+        if res.returncode != 0:
+            raise RuntimeError(f"nvcc failed compiling {u}.cu")
+    link = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "--shared", "-Xcompiler", "-fPIC", "-o", LIB] + \
+           [os.path.join(OBJ, u + ".o") for u in UNITS]
+    res = subprocess.run(link, capture_output=True, text=True)
     if verbose or res.returncode != 0:
         print(res.stdout)
         print(res.stderr)
     if res.returncode != 0:
-        raise RuntimeError("nvcc failed building libhpmc.so")
+        raise RuntimeError("nvcc failed linking libhpmc.so")
     with open(os.path.join(HERE, "build_ptxas.log"), "w") as f:
-        f.write(" ".join(cmd) + "\n" + res.stderr)
+        f.write("\n".join(log))
     return LIB
 
 

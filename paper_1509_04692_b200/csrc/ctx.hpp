@@ -1,0 +1,92 @@
+// Host-side context of libhpmc.so and the launchers of the colour-pass kernels, shared by the translation units of the
+// library: hpmc_api.cu and pass_*.cu are compiled in parallel and linked (no relocatable device code is needed, every
+// kernel is self-contained).
+#pragma once
+#include <string>
+#include <vector>
+
+#include "../../include/hpmc.h"
+#include "common.cuh"
+#include "overlap.cuh"
+
+using namespace hpmc;
+
+struct hpmc_ctx {
+    GridParams g{};
+    MoveParams mv{};
+    ShapeF sf{};
+    ShapeD sd{};
+    double d_max = 0.0;
+    double w[3] = {1, 1, 1};
+    uint64_t seed = 0;
+    uint32_t k0 = 0, k1 = 0;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    bool cuda_failed = false;
+    int64_t launches = 0;
+    uint64_t t_host = 0;  // mirror of the device sweep counter
+    Control h_ctrl{};     // host landing buffer for the control block
+
+    // caller-owned
+    float4* d_pos_bound = nullptr;
+    float4* d_quat_bound = nullptr;
+    char* d_ws = nullptr;
+    size_t ws_bytes = 0;
+    bool state_in_bound = false;  // true: next build reads the bound arrays (tag order)
+    bool have_sorted = false;
+
+    // carved from the workspace
+    float4* pos[2] = {nullptr, nullptr};
+    float4* quat[2] = {nullptr, nullptr};
+    int* tag[2] = {nullptr, nullptr};
+    int cur = 0;
+    int2* key_rank = nullptr;
+    int* cell_start = nullptr;  // C+1 (+ padding)
+    int* counts = nullptr;      // per-cell histogram, all zero between builds
+    int* arrived = nullptr;     // per-cell arrival counter of k_scatter_sort, all zero between builds
+    int* tile_sums = nullptr;   // per-tile totals of the scan
+    unsigned int* flow_done = nullptr;   // per (colour, tile) stamps of the dataflow pass
+    int num_sms = 0;
+    bool flow_now = false;               // this sweep's colour passes go out as one dataflow launch
+    Control* ctrl = nullptr;
+
+    uint2* trace = nullptr;
+    int64_t trace_words = 0;
+
+    // tuning / test knobs (hpmc_set_option)
+    int opt_path = 0;                 // 0 auto, 1 per-thread global path, 2 tile path (2-D only)
+    int opt_tile_cap = 1 << 30;       // staging capacity limit of the tile kernel (tests force the overflow path)
+    int opt_tile_shape = 0;           // 0 = by grid size, 1..3 = fixed (see pick_tile_shape)
+    int opt_flow = -1;                // 2-D tile pass as one dataflow launch per sweep: -1 = when it pays (auto), 0 = never, 1 = always
+    int opt_graph = 1;                // 1: hpmc_sweep(n >= 3) replays a captured two-sweep CUDA graph
+
+    // CUDA graph of two consecutive sweeps (the ping-pong buffers return to where they started), one per parity of `cur`
+    cudaGraphExec_t graph_exec[2] = {nullptr, nullptr};
+    int64_t graph_launches = 0;       // kernels inside one replay
+
+    // optional per-kernel device timing (hpmc_set_profile): event pairs around the cell-list build (class 0)
+    // and around every colour-pass launch (class 1)
+    bool profile = false;
+    std::vector<cudaEvent_t> ev_pool;
+    std::vector<int> ev_class;     // one per recorded pair
+    size_t ev_used = 0;            // events handed out (2 per pair)
+    double prof_ms[2] = {0.0, 0.0};
+    int64_t prof_n[2] = {0, 0};
+};
+
+inline bool cuda_ok(hpmc_ctx* c, cudaError_t e, const char* what)
+{
+    if (e == cudaSuccess) return true;
+    c->cuda_failed = true;
+    c->err = std::string("CUDA error in ") + what + ": " + cudaGetErrorString(e);
+    return false;
+}
+
+
+constexpr int kTileWHost = 32;   // active cells per tile row (= kTileW of sweep_tile2d.cuh)
+
+// Colour-pass launchers; each returns false after recording a CUDA error in the context.
+//   kind: kKindDisk / kKindPolygon / kKindPolyhedron; nv: unrolled vertex count (5 pentagons, 8 cubes) or 0 = runtime count
+bool hpmc_launch_tile2d(hpmc_ctx* c, int ci, int kind, int nv, int shape);       // pass_tile2d_*.cu (2-D, not polyhedra)
+bool hpmc_launch_warpcell(hpmc_ctx* c, int ci, int kind, int nv, int nactive);   // pass_warpcell_*.cu
+bool hpmc_launch_colour(hpmc_ctx* c, int ci, int kind, int nv, int nactive);     // pass_colour.cu

@@ -13,73 +13,9 @@
 #include "common.cuh"
 #include "overlap.cuh"
 #include "sweep.cuh"
-#include "sweep_tile2d.cuh"
-#include "sweep_warpcell.cuh"
+#include "ctx.hpp"
 
 using namespace hpmc;
-
-struct hpmc_ctx {
-    GridParams g{};
-    MoveParams mv{};
-    ShapeF sf{};
-    ShapeD sd{};
-    double d_max = 0.0;
-    double w[3] = {1, 1, 1};
-    uint64_t seed = 0;
-    uint32_t k0 = 0, k1 = 0;
-    cudaStream_t stream = nullptr;
-    std::string err;
-    bool cuda_failed = false;
-    int64_t launches = 0;
-    uint64_t t_host = 0;  // mirror of the device sweep counter
-    Control h_ctrl{};     // host landing buffer for the control block
-
-    // caller-owned
-    float4* d_pos_bound = nullptr;
-    float4* d_quat_bound = nullptr;
-    char* d_ws = nullptr;
-    size_t ws_bytes = 0;
-    bool state_in_bound = false;  // true: next build reads the bound arrays (tag order)
-    bool have_sorted = false;
-
-    // carved from the workspace
-    float4* pos[2] = {nullptr, nullptr};
-    float4* quat[2] = {nullptr, nullptr};
-    int* tag[2] = {nullptr, nullptr};
-    int cur = 0;
-    int2* key_rank = nullptr;
-    int* cell_start = nullptr;  // C+1 (+ padding)
-    int* counts = nullptr;      // per-cell histogram, all zero between builds
-    int* arrived = nullptr;     // per-cell arrival counter of k_scatter_sort, all zero between builds
-    int* tile_sums = nullptr;   // per-tile totals of the scan
-    unsigned int* flow_done = nullptr;   // per (colour, tile) stamps of the dataflow pass
-    int num_sms = 0;
-    bool flow_now = false;               // this sweep's colour passes go out as one dataflow launch
-    Control* ctrl = nullptr;
-
-    uint2* trace = nullptr;
-    int64_t trace_words = 0;
-
-    // tuning / test knobs (hpmc_set_option)
-    int opt_path = 0;                 // 0 auto, 1 per-thread global path, 2 tile path (2-D only)
-    int opt_tile_cap = 1 << 30;       // staging capacity limit of the tile kernel (tests force the overflow path)
-    int opt_tile_shape = 0;           // 0 = by grid size, 1..7 = fixed (see pick_tile_shape)
-    int opt_flow = -1;                // 2-D tile pass as one dataflow launch per sweep: -1 = when it pays (auto), 0 = never, 1 = always
-    int opt_graph = 1;                // 1: hpmc_sweep(n >= 3) replays a captured two-sweep CUDA graph
-
-    // CUDA graph of two consecutive sweeps (the ping-pong buffers return to where they started), one per parity of `cur`
-    cudaGraphExec_t graph_exec[2] = {nullptr, nullptr};
-    int64_t graph_launches = 0;       // kernels inside one replay
-
-    // optional per-kernel device timing (hpmc_set_profile): event pairs around the cell-list build (class 0)
-    // and around every colour-pass launch (class 1)
-    bool profile = false;
-    std::vector<cudaEvent_t> ev_pool;
-    std::vector<int> ev_class;     // one per recorded pair
-    size_t ev_used = 0;            // events handed out (2 per pair)
-    double prof_ms[2] = {0.0, 0.0};
-    int64_t prof_n[2] = {0, 0};
-};
 
 namespace {
 
@@ -90,14 +26,6 @@ int fail(hpmc_ctx* c, int code, const std::string& msg)
     if (c) c->err = msg;
     else g_err_noctx = msg;
     return code;
-}
-
-bool cuda_ok(hpmc_ctx* c, cudaError_t e, const char* what)
-{
-    if (e == cudaSuccess) return true;
-    c->cuda_failed = true;
-    c->err = std::string("CUDA error in ") + what + ": " + cudaGetErrorString(e);
-    return false;
 }
 
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -119,7 +47,7 @@ size_t flow_words(const hpmc_ctx* c)
 {
     if (c->g.dim != 2) return 1;
     const size_t nax = c->g.n[0] / 2, nay = c->g.n[1] / 2;
-    return 4 * ((nax + kTileW - 1) / kTileW) * ((nay + 1) / 2) + 4;
+    return 4 * ((nax + kTileWHost - 1) / kTileWHost) * ((nay + 1) / 2) + 4;
 }
 
 struct Layout {
@@ -325,87 +253,19 @@ int build_cell_list(hpmc_ctx* c, int mode, unsigned long long t_override)
     return HPMC_OK;
 }
 
-template <int KIND, int NV, int WARPS, int R, int MINB>
-bool launch_tile2d(hpmc_ctx* c, int ci)
-{
-    using TL = Tile2D<WARPS, R>;
-    const GridParams& g = c->g;
-    const int nax = g.n[0] / 2, nay = g.n[1] / 2;
-    const int tiles = ((nax + kTileW - 1) / kTileW) * ((nay + TL::TH - 1) / TL::TH);
-    if (c->flow_now) {   // all four colours in one persistent dataflow launch (issued for colour index 0 only)
-        auto kern = k_sweep_tile2d_flow<KIND, NV, WARPS, R, MINB>;
-        static bool attr_set = false;   // per template instance
-        if (!attr_set) {
-            if (!cuda_ok(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TL::bytes), "flow/attr")) return false;
-            attr_set = true;
-        }
-        const int slots = c->num_sms * MINB;
-        kern<<<tiles < slots ? tiles : slots, TL::NT, TL::bytes, c->stream>>>(g, c->mv, c->sf, c->sd, c->ctrl, c->opt_tile_cap,
-                                                                                        c->pos[c->cur], c->tag[c->cur], c->cell_start, c->k0,
-                                                                                        c->k1, c->trace, c->flow_done);
-        return true;
-    }
-    auto kern = k_sweep_tile2d<KIND, NV, WARPS, R, MINB>;
-    static bool attr_set = false;   // per template instance
-    if (!attr_set) {
-        if (!cuda_ok(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TL::bytes), "tile/attr")) return false;
-        attr_set = true;
-    }
-    kern<<<tiles, TL::NT, TL::bytes, c->stream>>>(g, c->mv, c->sf, c->sd, c->ctrl, ci, c->opt_tile_cap, c->pos[c->cur], c->tag[c->cur],
-                                                  c->cell_start, c->k0, c->k1, c->trace);
-    return true;
-}
-
 // tile shapes (warps per CTA, rows of 32 active cells per warp); "tile_shape" option, 0 = by grid size
 int pick_tile_shape(const hpmc_ctx* c)
 {
     if (c->opt_tile_shape) return c->opt_tile_shape;
     const int nax = c->g.n[0] / 2, nay = c->g.n[1] / 2;
-    const long long cols = (nax + kTileW - 1) / kTileW;
-    if (cols * ((nay + 3) / 4) >= 2 * 148) return 5;     // 4 warps x 1 row, 64 registers: 8 CTAs per SM
-    return 4;                                            // 2 warps x 1 row
-}
-
-template <int KIND, int NV, int DIM>
-bool launch_warpcell(hpmc_ctx* c, int ci, int nactive)
-{
-    k_sweep_warpcell<KIND, NV, DIM><<<(nactive + kW3Warps - 1) / kW3Warps, 32 * kW3Warps, 0, c->stream>>>(
-        c->g, c->mv, c->sf, c->sd, c->ctrl, ci, c->opt_tile_cap, c->pos[c->cur], c->quat[c->cur], c->tag[c->cur], c->cell_start, c->k0,
-        c->k1, c->trace);
-    return true;
+    const long long cols = (nax + kTileWHost - 1) / kTileWHost;
+    if (cols * ((nay + 3) / 4) >= 2 * 148) return 2;     // 4 warps x 1 row, 64 registers: 8 CTAs per SM
+    return 3;                                            // 2 warps x 1 row
 }
 
 // 2-D systems with fewer active cells per colour than this run one warp per cell instead of one lane per cell: the tile
 // kernel would leave most SMs idle (config 1: 961 active cells = 31 warps) and each warp round would be a long serial chain
 constexpr int kWarpCellMax2d = 148 * 48;
-
-template <int KIND, int NV>
-bool launch_colour(hpmc_ctx* c, int ci)
-{
-    const GridParams& g = c->g;
-    const int nactive = (g.n[0] / 2) * (g.n[1] / 2) * (g.dim == 3 ? g.n[2] / 2 : 1);
-    if constexpr (KIND != kKindPolyhedron) {
-        if (g.dim == 2 && c->opt_path != 1) {
-            if (c->opt_path == 3 || (c->opt_path == 0 && c->opt_tile_shape == 0 && nactive <= kWarpCellMax2d)) return launch_warpcell<KIND, NV, 2>(c, ci, nactive);
-            switch (pick_tile_shape(c)) {
-                case 1: return launch_tile2d<KIND, NV, 8, 2, 2>(c, ci);
-                case 2: return launch_tile2d<KIND, NV, 4, 2, 4>(c, ci);
-                case 3: return launch_tile2d<KIND, NV, 4, 1, 5>(c, ci);
-                case 5: return launch_tile2d<KIND, NV, 4, 1, 8>(c, ci);
-                case 6: return launch_tile2d<KIND, NV, 8, 1, 3>(c, ci);
-                case 7: return launch_tile2d<KIND, NV, 4, 1, 6>(c, ci);
-                default: return launch_tile2d<KIND, NV, 2, 1, 8>(c, ci);
-            }
-        }
-    }
-    if constexpr (KIND != kKindPolygon) {
-        if (g.dim == 3 && c->opt_path != 1) return launch_warpcell<KIND, NV, 3>(c, ci, nactive);   // one warp per active cell
-    }
-    const int TB = 128;
-    k_sweep_colour<KIND, NV><<<(nactive + TB - 1) / TB, TB, 0, c->stream>>>(g, c->mv, c->sf, c->sd, c->ctrl, ci, c->pos[c->cur], c->quat[c->cur],
-                                                                           c->tag[c->cur], c->cell_start, c->k0, c->k1, c->trace);
-    return true;
-}
 
 // does the 2-D tile pass apply (not the warp-per-cell pass, not the per-thread path), and as a dataflow launch?
 bool use_flow(const hpmc_ctx* c)
@@ -418,7 +278,7 @@ bool use_flow(const hpmc_ctx* c)
     // auto: the dataflow launch pays when a colour is one to a few waves of tiles (measured on B200: +9 % at 1M pentagons,
     // 1.7 waves; slower below one wave, where the stamps only add latency; no difference from 4M up)
     const long long slots = (long long)c->num_sms * 8;
-    const long long tiles = (long long)((g.n[0] / 2 + kTileW - 1) / kTileW) * ((g.n[1] / 2 + 3) / 4);
+    const long long tiles = (long long)((g.n[0] / 2 + kTileWHost - 1) / kTileWHost) * ((g.n[1] / 2 + 3) / 4);
     return c->opt_tile_shape == 0 && tiles > slots && tiles <= 4 * slots;
 }
 
@@ -427,25 +287,16 @@ int launch_colour_dispatch(hpmc_ctx* c, int ci)
     c->flow_now = use_flow(c);
     if (c->flow_now && ci > 0) return HPMC_OK;   // colour 0's dataflow launch covers all four colours
     ProfileScope prof(c, 1, c->flow_now ? 4 : 1);
+    // the (kind, unrolled vertex count) variants of each pass are compiled in separate translation units (pass_*.cu)
+    const int kind = c->sf.kind;
+    const int nv = (kind == kKindPolygon && c->sf.nverts == 5) ? 5 : (kind == kKindPolyhedron && c->sf.nverts == 8) ? 8 : 0;
+    const GridParams& g = c->g;
+    const int nactive = (g.n[0] / 2) * (g.n[1] / 2) * (g.dim == 3 ? g.n[2] / 2 : 1);
     bool ok = true;
-    switch (c->sf.kind) {
-        case kKindDisk: ok = launch_colour<kKindDisk, 0>(c, ci); break;
-        case kKindPolygon:
-            switch (c->sf.nverts) {
-#ifndef HPMC_FAST_BUILD
-                case 3: ok = launch_colour<kKindPolygon, 3>(c, ci); break;
-                case 4: ok = launch_colour<kKindPolygon, 4>(c, ci); break;
-                case 6: ok = launch_colour<kKindPolygon, 6>(c, ci); break;
-                case 8: ok = launch_colour<kKindPolygon, 8>(c, ci); break;
-#endif
-                case 5: ok = launch_colour<kKindPolygon, 5>(c, ci); break;
-                default: ok = launch_colour<kKindPolygon, 0>(c, ci); break;
-            }
-            break;
-        default:   // polyhedra: the 8-vertex case (cubes, config 3) has an unrolled support function
-            ok = (c->sf.nverts == 8) ? launch_colour<kKindPolyhedron, 8>(c, ci) : launch_colour<kKindPolyhedron, 0>(c, ci);
-            break;
-    }
+    if (c->opt_path == 1 || (g.dim == 2 && kind == kKindPolyhedron)) ok = hpmc_launch_colour(c, ci, kind, nv, nactive);
+    else if (g.dim == 3 || c->opt_path == 3 || (c->opt_path == 0 && c->opt_tile_shape == 0 && nactive <= kWarpCellMax2d))
+        ok = hpmc_launch_warpcell(c, ci, kind, nv, nactive);
+    else ok = hpmc_launch_tile2d(c, ci, kind, nv, pick_tile_shape(c));
     if (!ok) return HPMC_E_CUDA;
     LAUNCH_CHECK(c, "colour pass");
     return HPMC_OK;
@@ -818,7 +669,7 @@ int hpmc_set_option(hpmc_ctx* c, const char* name, int64_t value)
         if (value < -1 || value > 1) return fail(c, HPMC_E_ARG, "flow must be -1 (auto), 0 or 1");
         c->opt_flow = (int)value;
     } else if (n == "tile_shape") {
-        if (value < 0 || value > 7) return fail(c, HPMC_E_ARG, "tile_shape must be 0 (auto) or 1..7");
+        if (value < 0 || value > 3) return fail(c, HPMC_E_ARG, "tile_shape must be 0 (auto) or 1..3");
         c->opt_tile_shape = (int)value;
     } else
         return fail(c, HPMC_E_ARG, "unknown option");
@@ -858,8 +709,7 @@ int hpmc_describe_pass(const hpmc_ctx* c, char* h_buf, size_t n)
     else if (g.dim == 3 || c->opt_path == 3 || (c->opt_path == 0 && c->opt_tile_shape == 0 && nactive <= kWarpCellMax2d))
         d = "k_sweep_warpcell: one warp per active cell, 1 colour pass per launch";
     else {
-        static const char* shapes[8] = {"", "8 warps x 2 rows, 2 CTAs/SM", "4 x 2, 4 CTAs/SM", "4 x 1, 5 CTAs/SM", "2 x 1, 8 CTAs/SM",
-                                        "4 warps x 1 row, 8 CTAs/SM", "8 x 1, 3 CTAs/SM", "4 x 1, 6 CTAs/SM"};
+        static const char* shapes[4] = {"", "8 warps x 2 rows, 2 CTAs/SM", "4 warps x 1 row, 8 CTAs/SM", "2 warps x 1 row, 8 CTAs/SM"};
         const bool flow = use_flow(c);
         d = std::string(flow ? "k_sweep_tile2d_flow<" : "k_sweep_tile2d<") + shapes[pick_tile_shape(c)] + ">: " +
             (flow ? "4 colour passes per launch (dataflow)" : "1 colour pass per launch");

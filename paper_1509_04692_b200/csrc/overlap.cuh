@@ -319,7 +319,7 @@ __device__ __forceinline__ int polyhedron_classify(const ShapeT<T>& S, const T* 
 }
 
 // fp64 narrow phase from the raw fp32 state: normalised quaternions, exact separation rd (already minimum image)
-__device__ __noinline__ bool polyhedron_overlap_f64(const ShapeD& S, float4 qA, float4 qB, double rx, double ry, double rz, double eps)
+static __device__ __noinline__ bool polyhedron_overlap_f64(const ShapeD& S, float4 qA, float4 qB, double rx, double ry, double rz, double eps)
 {
     double MA[9], MB[9];
     const double na = 1.0 / sqrt((double)qA.x * qA.x + (double)qA.y * qA.y + (double)qA.z * qA.z + (double)qA.w * qA.w);

@@ -102,7 +102,7 @@ def test_options_and_pass_description_need_no_gpu(lib):
     assert lib.hpmc_set_option(h, b"flow", 0) == 0 and describe(h).startswith("k_sweep_tile2d<")
     assert lib.hpmc_set_option(h, b"path", 1) == 0 and describe(h).startswith("k_sweep_colour")
     assert lib.hpmc_set_option(h, b"path", 7) == -1 and lib.hpmc_set_option(h, b"flow", 2) == -1
-    assert lib.hpmc_set_option(h, b"tile_shape", 9) == -1 and lib.hpmc_set_option(h, b"no_such_option", 1) == -1
+    assert lib.hpmc_set_option(h, b"tile_shape", 4) == -1 and lib.hpmc_set_option(h, b"no_such_option", 1) == -1
     assert lib.hpmc_destroy(h) == 0
     rc, h = _create(lib, 2, (64.0, 64.0), hb.KIND_POLYGON, 4096, verts=wl.regular_polygon(5, 0.5))
     assert rc == 0 and describe(h).startswith("k_sweep_warpcell")                  # 961 active cells per colour

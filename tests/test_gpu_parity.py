@@ -139,8 +139,9 @@ def test_colour_pass_variants_agree_bit_for_bit(name):
     w = CASES[name]()
     ref = None
     some = 40 if w.dim == 2 else (84 if w.kind == wl.KIND_POLYHEDRON else 50)   # a capacity only some tiles/cells exceed
-    shapes = [{"tile_shape": k} for k in (1, 2, 3, 4)] if w.dim == 2 else []   # every 2-D tile shape
-    shapes += [{"path": 2, "flow": 1}, {"tile_shape": 3, "flow": 1}, {"path": 2, "flow": 1, "tile_cap": some}] if w.dim == 2 else []
+    shapes = [{"tile_shape": k} for k in (1, 2, 3)] if w.dim == 2 else []   # every 2-D tile shape
+    shapes += [{"path": 2, "flow": 1}, {"tile_shape": 1, "flow": 1}, {"tile_shape": 2, "flow": 1},
+               {"path": 2, "flow": 1, "tile_cap": some}] if w.dim == 2 else []
     warp = [{"path": 3}, {"path": 3, "tile_cap": 6}] if w.dim == 2 else []        # 2-D warp-per-cell pass and its fallback
     for opts in [{"path": 2}, {"path": 2, "tile_cap": 0}, {"path": 1}, {"path": 2, "tile_cap": some}] + shapes + warp:
         g = gpu(w)
