@@ -141,6 +141,8 @@ int hpmc_sweep_host(hpmc_ctx* ctx, const float* h_pos4, const float* h_quat4, in
  *              2 = 4 warps x 1 row at 64 registers (8 CTAs per SM; large grids), 3 = 2 warps x 1 row (small grids).
  *   "flow"     2-D tile pass: -1 (default) or 1 = the four colours of a sweep go out as ONE persistent launch in which a tile
  *              of colour c+1 starts as soon as the nine tiles of colour c around it are done; 0 = one launch per colour.
+ *   "small_build" 1 (default): a system with at most 11 500 cells and 8192 particles builds its cell list in one CTA
+ *              (one launch instead of three); 0: always the multi-launch build.
  *   "graph"    1 (default): hpmc_sweep(n >= 3) replays a captured CUDA graph of two sweeps; 0: plain launches.
  *              Needs a real stream: contexts created on the legacy default stream (NULL) always use plain launches.  */
 int hpmc_set_option(hpmc_ctx* ctx, const char* name, int64_t value);

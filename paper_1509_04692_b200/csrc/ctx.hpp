@@ -58,6 +58,7 @@ struct hpmc_ctx {
     int opt_tile_cap = 1 << 30;       // staging capacity limit of the tile kernel (tests force the overflow path)
     int opt_tile_shape = 0;           // 0 = by grid size, 1..3 = fixed (see pick_tile_shape)
     int opt_flow = -1;                // 2-D tile pass as one dataflow launch per sweep: -1 = when it pays (auto), 0 = never, 1 = always
+    int opt_small_build = 1;          // 1: systems with few cells build their cell list in one CTA (k_build_small)
     int opt_graph = 1;                // 1: hpmc_sweep(n >= 3) replays a captured two-sweep CUDA graph
 
     // CUDA graph of two consecutive sweeps (the ping-pong buffers return to where they started), one per parity of `cur`

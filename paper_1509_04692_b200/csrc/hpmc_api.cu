@@ -230,6 +230,16 @@ int build_cell_list(hpmc_ctx* c, int mode, unsigned long long t_override)
     const float4* src_quat = c->state_in_bound ? c->d_quat_bound : c->quat[c->cur];
     const int* src_tag = c->state_in_bound ? nullptr : c->tag[c->cur];
     const int dst = c->state_in_bound ? 0 : 1 - c->cur;
+    if (c->opt_small_build && g.C <= kSmallBuildMaxCells && g.N <= kSmallBuildMaxN) {   // one CTA does the whole build
+        k_build_small<<<1, kSmallBuildThreads, ((size_t)g.C + 2) * sizeof(int), c->stream>>>(
+            g, c->ctrl, c->k0, c->k1, mode, t_override, src_pos, src_quat, src_tag, c->key_rank, c->cell_start, c->pos[dst], c->quat[dst],
+            c->tag[dst]);
+        LAUNCH_CHECK(c, "k_build_small");
+        c->cur = dst;
+        c->state_in_bound = false;
+        c->have_sorted = true;
+        return HPMC_OK;
+    }
     const int nblk_part = (g.N + TB - 1) / TB;
     k_hist<<<nblk_part > 0 ? nblk_part : 1, TB, 0, c->stream>>>(g, c->ctrl, src_pos, c->counts, c->key_rank, c->k0, c->k1, mode, t_override);
     LAUNCH_CHECK(c, "k_hist");
@@ -665,6 +675,8 @@ int hpmc_set_option(hpmc_ctx* c, const char* name, int64_t value)
     } else if (n == "tile_cap") {
         if (value < 0) return fail(c, HPMC_E_ARG, "tile_cap must be >= 0");
         c->opt_tile_cap = value > (1 << 30) ? (1 << 30) : (int)value;
+    } else if (n == "small_build") {
+        c->opt_small_build = value != 0;
     } else if (n == "flow") {
         if (value < -1 || value > 1) return fail(c, HPMC_E_ARG, "flow must be -1 (auto), 0 or 1");
         c->opt_flow = (int)value;
