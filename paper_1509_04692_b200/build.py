@@ -38,7 +38,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         results = list(ex.map(compile_unit, UNITS))
     log = []
     for u, cmd, res in results:
-        log.append(" ".join(cmd) + "\n" + res.stderr)
+        # the register / spill report, without the timing lines that change from build to build
+        log.append(" ".join(cmd) + "\n" + "\n".join(l for l in res.stderr.splitlines() if "Compile time" not in l) + "\n")
         if verbose or res.returncode != 0:
             print(res.stdout)
             print(res.stderr)
