@@ -17,7 +17,7 @@ def build(force: bool = False) -> str:
         newest = max(os.path.getmtime(SRC), os.path.getmtime(HDR))
         if os.path.getmtime(LIB) >= newest:
             return LIB
-    cmd = ["gcc", "-O2", "-std=c99", "-Wall", "-ffp-contract=off", "-fPIC", "-shared", "-o", LIB, SRC, "-lm"]
+    cmd = ["gcc", "-O2", "-std=c99", "-Wall", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared", "-o", LIB, SRC, "-lm"]
     subprocess.check_call(cmd)
     return LIB
 

@@ -5,8 +5,12 @@
  * arXiv:1509.04692.  P:<n> = /root/reference/PAPER.md line n; R<k>/O<k> = the
  * readings and oracle items listed in DESIGN.md.
  *
- * Build: gcc -O2 -std=c99 -ffp-contract=off -fPIC -shared  (no fast-math:
+ * Build: gcc -O2 -std=c99 -ffp-contract=off -fopenmp -fPIC -shared  (no fast-math:
  * the fp32 pins need IEEE single operations with no FMA contraction).
+ *
+ * Threads: serial by default (the definition).  orc_set_threads(n > 1) runs the cells of ONE colour as an
+ * OpenMP parallel-for -- the "any order" of O3.4, legal because same-colour cells are independent (P:21,
+ * P:59; pinned by the P4 tests); every result is identical to the serial run.  Nothing else is parallel.
  */
 #define _DEFAULT_SOURCE 1 /* M_PI under -std=c99 */
 #include "hpmc_oracle.h"
@@ -446,7 +450,8 @@ static int gjk_tetrahedron(double P[4][3], int* np, double d[3])
     return gjk_triangle(P, np, d, 3);
 }
 
-int orc_shape_gjk(const orc_shape* s, const double r_ab[3], const double qa[4], const double qb[4])
+/* support_calls (may be NULL): number of support-function evaluations (Eq. (1)), O7 */
+static int gjk_run(const orc_shape* s, const double r_ab[3], const double qa[4], const double qb[4], uint64_t* support_calls)
 {
     if (s->kind == ORC_KIND_DISK) return (norm3(r_ab) - s->diameter) < 0.0 ? 1 : 0;
     double wa[ORC_MAX_VERTS][3], wb[ORC_MAX_VERTS][3];
@@ -462,6 +467,7 @@ int orc_shape_gjk(const orc_shape* s, const double r_ab[3], const double qa[4], 
     for (int iter = 0; iter < 256; ++iter) {
         double a[3];
         gjk_support(&g, d, a);
+        if (support_calls) ++*support_calls;
         if (dot3(a, d) <= 0.0) return 0; /* a support plane separates the origin: disjoint (touching counts as disjoint) */
         memcpy(P[np++], a, sizeof a);
         int hit;
@@ -472,6 +478,33 @@ int orc_shape_gjk(const orc_shape* s, const double r_ab[3], const double qa[4], 
         if (hit) return 1;
     }
     return -1;
+}
+
+int orc_shape_gjk(const orc_shape* s, const double r_ab[3], const double qa[4], const double qb[4])
+{
+    return gjk_run(s, r_ab, qa, qb, NULL);
+}
+
+/* O7: separating axes of a convex polygon pair evaluated in serial order -- the outward edge normals of A
+ * (k = 0..n-1), then the negated edge normals of B -- until the first axis whose separation is >= eps
+ * ("separating planes method"); all 2n when none separates (the pair overlaps). */
+static int polygon_axes_until_separation(const orc_shape* s, const double r_ab[3], const double qa[4], const double qb[4], double eps)
+{
+    double wa[ORC_MAX_VERTS][3], wb[ORC_MAX_VERTS][3];
+    int nv = s->nverts, count = 0;
+    for (int i = 0; i < nv; ++i) {
+        quat_rotate(qa, s->verts[i], wa[i]);
+        quat_rotate(qb, s->verts[i], wb[i]);
+    }
+    for (int side = 0; side < 2; ++side)
+        for (int f = 0; f < s->nfaces; ++f) {
+            double n[3];
+            quat_rotate(side == 0 ? qa : qb, s->face_n[f], n);
+            if (side == 1) for (int c = 0; c < 3; ++c) n[c] = -n[c];
+            ++count;
+            if (axis_separation(n, r_ab, wa, wb, nv) >= eps) return count;
+        }
+    return count;
 }
 
 /* ------------------------------------------------------------------------ */
@@ -497,6 +530,8 @@ struct orc_sys {
     orc_counters cnt;
     orc_work work;
     int mut_no_shift, mut_fixed_order, mut_no_leave;
+    int work_detail; /* O7: also count separating axes / GJK support calls (costs extra narrow-phase work) */
+    int nthreads;    /* 1 = serial (the definition); > 1 = same-colour cells as an OpenMP parallel-for */
     int32_t *cell_id, *cell_start, *members;
 };
 
@@ -536,6 +571,7 @@ orc_sys* orc_create(int dim, const double L[3], int kind, double diameter, int n
     s->members = (int32_t*)malloc(sizeof(int32_t) * (size_t)(N > 0 ? N : 1));
     s->cell_start = (int32_t*)malloc(sizeof(int32_t) * (size_t)(s->C + 1));
     s->d = 0.1; s->a = 0.1; s->d_f = 0.1f; s->a_f = 0.1f; s->n_select = 4;
+    s->nthreads = 1;
     return s;
 }
 
@@ -577,6 +613,9 @@ void orc_get_grid(const orc_sys* s, int32_t n[3], double w[3], float w_f[3], flo
 }
 int64_t orc_num_cells(const orc_sys* s) { return s->C; }
 void orc_set_mutations(orc_sys* s, int a, int b, int c) { s->mut_no_shift = a; s->mut_fixed_order = b; s->mut_no_leave = c; }
+void orc_set_work_detail(orc_sys* s, int on) { s->work_detail = on; }
+void orc_set_threads(orc_sys* s, int n) { s->nthreads = n > 1 ? n : 1; }
+int orc_get_threads(const orc_sys* s) { return s->nthreads; }
 
 /* ------------------------------------------------------------------------ */
 /* O3.1, O3.2: sweep header                                                 */
@@ -656,8 +695,8 @@ static void min_image(const orc_sys* s, const float* xj, const float* xt, double
 
 static void quat_to_double(const float* q, double out[4]) { for (int c = 0; c < 4; ++c) out[c] = (double)q[c]; }
 
-/* scan the candidates of one trial; returns m_min (INFINITY if no candidate in range) */
-static double scan_candidates(orc_sys* s, int neighbour_mode, int64_t i, const float xt[3], const float qt[4],
+/* scan the candidates of one trial; returns m_min (INFINITY if no candidate in range).  wk: O7 work tallies */
+static double scan_candidates(const orc_sys* s, orc_work* wk, int neighbour_mode, int64_t i, const float xt[3], const float qt[4],
                               const int32_t cc[3])
 {
     const orc_shape* sh = s->shape;
@@ -691,14 +730,20 @@ static double scan_candidates(orc_sys* s, int neighbour_mode, int64_t i, const f
                     int64_t j = s->members[p];
                     if (j == i) continue;
                     double r[3], qb[4];
-                    s->work.cand_scanned_full++;
-                    if (!found) s->work.cand_scanned_early++;
+                    wk->cand_scanned_full++;
+                    if (!found) wk->cand_scanned_early++;
                     min_image(s, &s->pos[4 * j], xt, r);
                     if (dot3(r, r) >= dmax2) continue; /* R16 circumsphere */
-                    s->work.sphere_pass_full++;
-                    if (!found) s->work.narrow_tests_early++;
+                    wk->sphere_pass_full++;
+                    if (!found) wk->narrow_tests_early++;
                     quat_to_double(&s->quat[4 * j], qb);
                     double m = orc_shape_margin(sh, r, qa, qb);
+                    if (!found && s->work_detail) { /* O7: what an early-exit narrow phase would have evaluated */
+                        if (sh->kind == ORC_KIND_POLYGON)
+                            wk->polygon_axes_early += (uint64_t)polygon_axes_until_separation(sh, r, qa, qb, s->eps_g);
+                        else if (sh->kind == ORC_KIND_POLYHEDRON)
+                            gjk_run(sh, r, qa, qb, &wk->gjk_support_calls_early);
+                    }
                     if (m < m_min) m_min = m;
                     if (m < s->eps_g) found = 1;
                 }
@@ -750,18 +795,117 @@ static void wrap_store(orc_sys* s, int64_t i, const float xt[3], const float qt[
 /* ------------------------------------------------------------------------ */
 /* O3: one checkerboard sweep                                               */
 /* ------------------------------------------------------------------------ */
+typedef struct { /* everything one cell's trials need to know about the sweep */
+    uint32_t key[2], t_lo, t_hi16;
+    float shift[3];
+    int gamma, neighbour_mode;
+    const uint32_t* follow;
+    double follow_tol;
+    uint32_t* trace_out;
+    double* mmin_out;
+} sweep_ctx;
+
+static void note_bad(orc_follow_stats* fs, int64_t slot, const uint32_t mine[2], const uint32_t* th, double m_min)
+{
+    fs->hard_mismatch++;
+    if (fs->first_bad_slot < 0) { fs->first_bad_slot = slot; memcpy(fs->first_bad_mine, mine, 8); memcpy(fs->first_bad_theirs, th, 8); fs->first_bad_mmin = m_min; }
+}
+
+/* O3.4: the n_select sequential trials of one cell (R9).  Tallies go to the caller's cnt / wk / fs. */
+static void sweep_cell(orc_sys* s, const sweep_ctx* x, int64_t cell, const int32_t cc[3], orc_counters* cnt, orc_work* wk,
+                       orc_follow_stats* fs)
+{
+    const int32_t nmem = s->cell_start[cell + 1] - s->cell_start[cell];
+    for (int k = 0; k < s->n_select; ++k) {
+        const int64_t slot = cell * s->n_select + k;
+        uint32_t mine[2] = {0u, 0u};
+        double m_min = NAN;
+        if (nmem > 0) { /* R9: empty cells make no trials */
+            uint32_t ctr[4] = {(uint32_t)cell, x->t_lo, (uint32_t)k, (TAG_TRIAL << 24) | ((uint32_t)x->gamma << 16) | x->t_hi16};
+            uint32_t b0[4], b1[4] = {0, 0, 0, 0};
+            orc_philox4x32_10(ctr, x->key, b0);
+            if (s->dim == 3) { ctr[2] = (uint32_t)k | (1u << 16); orc_philox4x32_10(ctr, x->key, b1); }
+            const int64_t i = s->members[s->cell_start[cell] + (int32_t)(((uint64_t)b0[0] * (uint64_t)nmem) >> 32)]; /* R8 */
+            const int rotate = (s->shape->kind != ORC_KIND_DISK) && (b0[1] >> 31); /* R7 */
+            float xt[3], qt[4];
+            int outcome;
+            cnt->trials++;
+            if (!rotate) {
+                uint32_t u[3] = {b0[2], b0[3], b1[0]};
+                gen_translate(s, &s->pos[4 * i], u, xt);
+                memcpy(qt, &s->quat[4 * i], sizeof qt);
+            } else {
+                memcpy(xt, &s->pos[4 * i], sizeof xt);
+                gen_rotate(s, &s->quat[4 * i], b0[2], b0[3], b1[0], qt);
+            }
+            if (!rotate && !s->mut_no_leave && orc_cell_of(s, xt, x->shift) != (int32_t)cell) {
+                outcome = 2; /* O3.4e: leaves its cell -> reject */
+            } else {
+                m_min = scan_candidates(s, wk, x->neighbour_mode, i, xt, qt, cc);
+                outcome = (m_min < s->eps_g) ? 3 : 1; /* R15 guard band */
+            }
+            mine[0] = (uint32_t)i;
+            mine[1] = (uint32_t)rotate | ((uint32_t)outcome << 8);
+            if (x->follow) { /* O8 lock-step */
+                const uint32_t* th = &x->follow[2 * slot];
+                int their_outcome = (int)(th[1] >> 8);
+                if (th[0] != mine[0] || (th[1] & 0xFFu) != (mine[1] & 0xFFu)) {
+                    note_bad(fs, slot, mine, th, m_min);
+                } else if (their_outcome != outcome) {
+                    int both_overlap_kind = (outcome == 1 || outcome == 3) && (their_outcome == 1 || their_outcome == 3);
+                    if (both_overlap_kind && fabs(m_min - s->eps_g) < x->follow_tol) {
+                        fs->marginal++;
+                        outcome = their_outcome; /* adopt the GPU's decision and continue */
+                    } else
+                        note_bad(fs, slot, mine, th, m_min);
+                }
+                fs->compared++;
+            }
+            if (outcome == 1) {
+                wrap_store(s, i, xt, qt);
+                if (rotate) cnt->rot_acc++; else cnt->trans_acc++;
+            } else if (outcome == 2) {
+                cnt->trans_rej_cell++;
+            } else {
+                if (rotate) cnt->rot_rej_overlap++; else cnt->trans_rej_overlap++;
+            }
+        } else if (x->follow) {
+            const uint32_t* th = &x->follow[2 * slot];
+            if (th[0] != 0u || th[1] != 0u) note_bad(fs, slot, mine, th, NAN);
+            fs->compared++;
+        }
+        if (x->trace_out) { x->trace_out[2 * slot] = mine[0]; x->trace_out[2 * slot + 1] = mine[1]; }
+        if (x->mmin_out) x->mmin_out[slot] = m_min;
+    }
+}
+
+static void add_tallies(orc_sys* s, orc_follow_stats* fs, const orc_counters* c, const orc_work* w, const orc_follow_stats* f)
+{
+    s->cnt.trans_acc += c->trans_acc; s->cnt.trans_rej_overlap += c->trans_rej_overlap; s->cnt.trans_rej_cell += c->trans_rej_cell;
+    s->cnt.rot_acc += c->rot_acc; s->cnt.rot_rej_overlap += c->rot_rej_overlap; s->cnt.trials += c->trials;
+    s->work.cand_scanned_full += w->cand_scanned_full; s->work.sphere_pass_full += w->sphere_pass_full;
+    s->work.cand_scanned_early += w->cand_scanned_early; s->work.narrow_tests_early += w->narrow_tests_early;
+    s->work.polygon_axes_early += w->polygon_axes_early; s->work.gjk_support_calls_early += w->gjk_support_calls_early;
+    fs->compared += f->compared; fs->marginal += f->marginal; fs->hard_mismatch += f->hard_mismatch;
+    if (f->first_bad_slot >= 0 && (fs->first_bad_slot < 0 || f->first_bad_slot < fs->first_bad_slot)) {
+        fs->first_bad_slot = f->first_bad_slot; fs->first_bad_mmin = f->first_bad_mmin;
+        memcpy(fs->first_bad_mine, f->first_bad_mine, 8); memcpy(fs->first_bad_theirs, f->first_bad_theirs, 8);
+    }
+}
+
 int orc_sweep(orc_sys* s, int neighbour_mode, int reverse_cells, const uint32_t* follow, double follow_tol,
               uint32_t* trace_out, double* mmin_out, orc_follow_stats* fs)
 {
     const uint64_t t = s->t;
-    const uint32_t key[2] = {(uint32_t)s->seed, (uint32_t)(s->seed >> 32)};
-    const uint32_t t_lo = (uint32_t)t, t_hi16 = (uint32_t)((t >> 32) & 0xFFFFu);
-    float shift[3];
+    sweep_ctx x;
+    x.key[0] = (uint32_t)s->seed; x.key[1] = (uint32_t)(s->seed >> 32);
+    x.t_lo = (uint32_t)t; x.t_hi16 = (uint32_t)((t >> 32) & 0xFFFFu);
+    x.neighbour_mode = neighbour_mode; x.follow = follow; x.follow_tol = follow_tol; x.trace_out = trace_out; x.mmin_out = mmin_out;
     int32_t perm[8];
-    orc_sweep_header(s, t, shift, perm);
-    if (s->mut_no_shift) shift[0] = shift[1] = shift[2] = 0.0f;
+    orc_sweep_header(s, t, x.shift, perm);
+    if (s->mut_no_shift) x.shift[0] = x.shift[1] = x.shift[2] = 0.0f;
     if (s->mut_fixed_order) for (int c = 0; c < 8; ++c) perm[c] = c;
-    orc_cell_list(s, shift, s->cell_id, s->cell_start, s->members);
+    orc_cell_list(s, x.shift, s->cell_id, s->cell_start, s->members);
     const int ncol = 1 << s->dim;
     const int64_t nslots = s->C * s->n_select;
     if (trace_out) memset(trace_out, 0, sizeof(uint32_t) * 2 * (size_t)nslots);
@@ -772,83 +916,26 @@ int orc_sweep(orc_sys* s, int neighbour_mode, int reverse_cells, const uint32_t*
     fs->first_bad_slot = -1;
 
     for (int ci = 0; ci < ncol; ++ci) {
-        const int gamma = perm[ci];
-        for (int64_t cq = 0; cq < s->C; ++cq) {
-            const int64_t cell = reverse_cells ? (s->C - 1 - cq) : cq;
-            int32_t cc[3];
-            cc[0] = (int32_t)(cell % s->n[0]);
-            cc[1] = (int32_t)((cell / s->n[0]) % s->n[1]);
-            cc[2] = (int32_t)(cell / ((int64_t)s->n[0] * s->n[1]));
-            int colour = (cc[0] & 1) | ((cc[1] & 1) << 1) | ((cc[2] & 1) << 2);
-            if (colour != gamma) continue;
-            const int32_t nmem = s->cell_start[cell + 1] - s->cell_start[cell];
-            for (int k = 0; k < s->n_select; ++k) {
-                const int64_t slot = cell * s->n_select + k;
-                uint32_t mine[2] = {0u, 0u};
-                double m_min = NAN;
-                if (nmem > 0) { /* R9: empty cells make no trials */
-                    uint32_t ctr[4] = {(uint32_t)cell, t_lo, (uint32_t)k, (TAG_TRIAL << 24) | ((uint32_t)gamma << 16) | t_hi16};
-                    uint32_t b0[4], b1[4] = {0, 0, 0, 0};
-                    orc_philox4x32_10(ctr, key, b0);
-                    if (s->dim == 3) { ctr[2] = (uint32_t)k | (1u << 16); orc_philox4x32_10(ctr, key, b1); }
-                    const int64_t i = s->members[s->cell_start[cell] + (int32_t)(((uint64_t)b0[0] * (uint64_t)nmem) >> 32)]; /* R8 */
-                    const int rotate = (s->shape->kind != ORC_KIND_DISK) && (b0[1] >> 31); /* R7 */
-                    float xt[3], qt[4];
-                    int outcome;
-                    s->cnt.trials++;
-                    if (!rotate) {
-                        uint32_t u[3] = {b0[2], b0[3], b1[0]};
-                        gen_translate(s, &s->pos[4 * i], u, xt);
-                        memcpy(qt, &s->quat[4 * i], sizeof qt);
-                    } else {
-                        memcpy(xt, &s->pos[4 * i], sizeof xt);
-                        gen_rotate(s, &s->quat[4 * i], b0[2], b0[3], b1[0], qt);
-                    }
-                    if (!rotate && !s->mut_no_leave && orc_cell_of(s, xt, shift) != (int32_t)cell) {
-                        outcome = 2; /* O3.4e: leaves its cell -> reject */
-                    } else {
-                        m_min = scan_candidates(s, neighbour_mode, i, xt, qt, cc);
-                        outcome = (m_min < s->eps_g) ? 3 : 1; /* R15 guard band */
-                    }
-                    mine[0] = (uint32_t)i;
-                    mine[1] = (uint32_t)rotate | ((uint32_t)outcome << 8);
-                    if (follow) { /* O8 lock-step */
-                        const uint32_t* th = &follow[2 * slot];
-                        int their_outcome = (int)(th[1] >> 8);
-                        if (th[0] != mine[0] || (th[1] & 0xFFu) != (mine[1] & 0xFFu)) {
-                            fs->hard_mismatch++;
-                            if (fs->first_bad_slot < 0) { fs->first_bad_slot = slot; memcpy(fs->first_bad_mine, mine, 8); memcpy(fs->first_bad_theirs, th, 8); fs->first_bad_mmin = m_min; }
-                        } else if (their_outcome != outcome) {
-                            int both_overlap_kind = (outcome == 1 || outcome == 3) && (their_outcome == 1 || their_outcome == 3);
-                            if (both_overlap_kind && fabs(m_min - s->eps_g) < follow_tol) {
-                                fs->marginal++;
-                                outcome = their_outcome; /* adopt the GPU's decision and continue */
-                            } else {
-                                fs->hard_mismatch++;
-                                if (fs->first_bad_slot < 0) { fs->first_bad_slot = slot; memcpy(fs->first_bad_mine, mine, 8); memcpy(fs->first_bad_theirs, th, 8); fs->first_bad_mmin = m_min; }
-                            }
-                        }
-                        fs->compared++;
-                    }
-                    if (outcome == 1) {
-                        wrap_store(s, i, xt, qt);
-                        if (rotate) s->cnt.rot_acc++; else s->cnt.trans_acc++;
-                    } else if (outcome == 2) {
-                        s->cnt.trans_rej_cell++;
-                    } else {
-                        if (rotate) s->cnt.rot_rej_overlap++; else s->cnt.trans_rej_overlap++;
-                    }
-                } else if (follow) {
-                    const uint32_t* th = &follow[2 * slot];
-                    if (th[0] != 0u || th[1] != 0u) {
-                        fs->hard_mismatch++;
-                        if (fs->first_bad_slot < 0) { fs->first_bad_slot = slot; memcpy(fs->first_bad_mine, mine, 8); memcpy(fs->first_bad_theirs, th, 8); fs->first_bad_mmin = NAN; }
-                    }
-                    fs->compared++;
-                }
-                if (trace_out) { trace_out[2 * slot] = mine[0]; trace_out[2 * slot + 1] = mine[1]; }
-                if (mmin_out) mmin_out[slot] = m_min;
+        x.gamma = perm[ci];
+        /* every cell of colour gamma, in ascending (or descending) id when serial; "any order" is legal (P4) */
+#pragma omp parallel num_threads(s->nthreads) if (s->nthreads > 1)
+        {
+            orc_counters lc; orc_work lw; orc_follow_stats lf;
+            memset(&lc, 0, sizeof lc); memset(&lw, 0, sizeof lw); memset(&lf, 0, sizeof lf);
+            lf.first_bad_slot = -1;
+#pragma omp for schedule(static)
+            for (int64_t cq = 0; cq < s->C; ++cq) {
+                const int64_t cell = reverse_cells ? (s->C - 1 - cq) : cq;
+                int32_t cc[3];
+                cc[0] = (int32_t)(cell % s->n[0]);
+                cc[1] = (int32_t)((cell / s->n[0]) % s->n[1]);
+                cc[2] = (int32_t)(cell / ((int64_t)s->n[0] * s->n[1]));
+                int colour = (cc[0] & 1) | ((cc[1] & 1) << 1) | ((cc[2] & 1) << 2);
+                if (colour != x.gamma) continue;
+                sweep_cell(s, &x, cell, cc, &lc, &lw, &lf);
             }
+#pragma omp critical
+            add_tallies(s, fs, &lc, &lw, &lf);
         }
     }
     s->t = t + 1;
@@ -892,7 +979,7 @@ int orc_textbook_trials(orc_sys* s, int64_t n_trials)
             memcpy(xt, &s->pos[4 * i], sizeof xt);
             gen_rotate(s, &s->quat[4 * i], b0[2], b0[3], b1[0], qt);
         }
-        double m_min = scan_candidates(s, 1, i, xt, qt, cc);            /* 3. check all other particles   */
+        double m_min = scan_candidates(s, &s->work, 1, i, xt, qt, cc);            /* 3. check all other particles   */
         if (m_min < s->eps_g) {                                         /* 4. reject on overlap           */
             if (rotate) s->cnt.rot_rej_overlap++; else s->cnt.trans_rej_overlap++;
         } else {

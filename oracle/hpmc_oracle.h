@@ -57,6 +57,10 @@ typedef struct {
     uint64_t sphere_pass_full;   /* of those, inside the circumsphere range          */
     uint64_t cand_scanned_early; /* scanned until the first overlapping neighbour    */
     uint64_t narrow_tests_early; /* narrow-phase tests until the first overlap       */
+    /* filled only with orc_set_work_detail(1): per narrow test counted in narrow_tests_early, */
+    uint64_t polygon_axes_early;      /* polygons: separating axes evaluated up to and including the first
+                                         one that separates (A's normals, then B's; all 2n if none) */
+    uint64_t gjk_support_calls_early; /* polyhedra: support-function calls (Eq. (1)) of the fp64 GJK */
 } orc_work;
 
 typedef struct {
@@ -123,6 +127,12 @@ int orc_sweeps(orc_sys*, int64_t n);
 
 /* mutation switches for O11-style checks (default all 0 = the real scheme) */
 void orc_set_mutations(orc_sys*, int no_shift, int fixed_colour_order, int no_leave_cell_reject);
+
+/* O7: count separating axes / GJK support calls too (extra narrow-phase work; default off) */
+void orc_set_work_detail(orc_sys*, int on);
+/* n > 1: the cells of one colour as an OpenMP parallel-for (same results, P4); default 1 = serial */
+void orc_set_threads(orc_sys*, int n);
+int orc_get_threads(const orc_sys*);
 
 /* O11: textbook Metropolis, n_trials single-particle trials, own RNG tag */
 int orc_textbook_trials(orc_sys*, int64_t n_trials);

@@ -24,7 +24,8 @@ class Counters(C.Structure):
 
 class Work(C.Structure):
     _fields_ = [(n, C.c_uint64) for n in
-                ("cand_scanned_full", "sphere_pass_full", "cand_scanned_early", "narrow_tests_early")]
+                ("cand_scanned_full", "sphere_pass_full", "cand_scanned_early", "narrow_tests_early",
+                 "polygon_axes_early", "gjk_support_calls_early")]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}
@@ -84,6 +85,9 @@ def lib():
     L.orc_sweep.restype = C.c_int
     L.orc_sweeps.argtypes = [vp, C.c_int64]; L.orc_sweeps.restype = C.c_int
     L.orc_set_mutations.argtypes = [vp, C.c_int, C.c_int, C.c_int]
+    L.orc_set_work_detail.argtypes = [vp, C.c_int]
+    L.orc_set_threads.argtypes = [vp, C.c_int]
+    L.orc_get_threads.argtypes = [vp]; L.orc_get_threads.restype = C.c_int
     L.orc_textbook_trials.argtypes = [vp, C.c_int64]; L.orc_textbook_trials.restype = C.c_int
     L.orc_count_overlaps_bruteforce.argtypes = [vp]; L.orc_count_overlaps_bruteforce.restype = C.c_int64
     L.orc_count_overlaps_cells.argtypes = [vp]; L.orc_count_overlaps_cells.restype = C.c_int64
@@ -272,6 +276,14 @@ class Oracle:
 
     def set_mutations(self, no_shift=0, fixed_colour_order=0, no_leave_cell_reject=0):
         lib().orc_set_mutations(self._h, no_shift, fixed_colour_order, no_leave_cell_reject)
+
+    def set_work_detail(self, on=True):
+        """O7: also count separating axes (polygons) / GJK support calls (polyhedra) per early-exit narrow test."""
+        lib().orc_set_work_detail(self._h, int(bool(on)))
+
+    def set_threads(self, n):
+        """n > 1: same-colour cells as an OpenMP parallel-for (identical results, P4); 1 = serial (default)."""
+        lib().orc_set_threads(self._h, int(n))
 
     def textbook_trials(self, n):
         assert lib().orc_textbook_trials(self._h, int(n)) == 0
