@@ -102,6 +102,15 @@ int build_shape(hpmc_ctx* c, const hpmc_shape* s, int dim)
         c->d_max = 2.0 * rmax;  // circumsphere centred on the particle position
         double r_in = 1e300;    // inscribed radius about the body origin = smallest face/edge offset
         if (poly2) {
+            // regular n-gon centred on the origin: equal radii and equal angular steps (see polygon_separated)
+            bool regular = true;
+            for (int k = 0; k < nv; ++k) {
+                const int k1 = (k + 1) % nv;
+                const double rk = std::hypot(D.vx[k], D.vy[k]);
+                const double cs = (D.vx[k] * D.vx[k1] + D.vy[k] * D.vy[k1]) / (rmax * rmax);
+                if (std::fabs(rk - rmax) > 1e-12 * rmax || std::fabs(cs - std::cos(2.0 * 3.14159265358979323846 / nv)) > 1e-12) regular = false;
+            }
+            D.regular = regular ? 1 : 0;
             for (int k = 0; k < nv; ++k) {
                 const int k1 = (k + 1) % nv, k2 = (k + 2) % nv;
                 const double ex = D.vx[k1] - D.vx[k], ey = D.vy[k1] - D.vy[k];
@@ -152,6 +161,7 @@ int build_shape(hpmc_ctx* c, const hpmc_shape* s, int dim)
         }
         const double din = std::fmax(0.0, 2.0 * r_in - 1e-5);
         D.din2 = din * din;
+        D.rin = r_in;
     } else
         return fail(c, HPMC_E_SHAPE, "unknown shape kind");
     D.dmax2 = c->d_max * c->d_max;  // the validator is strict: no guard band
@@ -161,6 +171,8 @@ int build_shape(hpmc_ctx* c, const hpmc_shape* s, int dim)
     F.nverts = D.nverts;
     F.diameter = (float)D.diameter;
     F.din2 = (float)D.din2;
+    F.rin = (float)(D.rin * (1.0 - 1e-6));   // rounded DOWN: the candidate-axis test of polygon_separated must never exclude an axis that separates
+    F.regular = D.regular;
     for (int i = 0; i < kMaxVerts; ++i) {
         F.vx[i] = (float)D.vx[i]; F.vy[i] = (float)D.vy[i]; F.vz[i] = (float)D.vz[i];
         F.nx[i] = (float)D.nx[i]; F.ny[i] = (float)D.ny[i]; F.fc[i] = (float)D.fc[i];
@@ -299,7 +311,7 @@ int launch_colour_dispatch(hpmc_ctx* c, int ci)
     ProfileScope prof(c, 1, c->flow_now ? 4 : 1);
     // the (kind, unrolled vertex count) variants of each pass are compiled in separate translation units (pass_*.cu)
     const int kind = c->sf.kind;
-    const int nv = (kind == kKindPolygon && c->sf.nverts == 5) ? 5 : (kind == kKindPolyhedron && c->sf.nverts == 8) ? 8 : 0;
+    const int nv = (kind == kKindPolygon && c->sf.nverts == 5 && c->sf.regular) ? 5 : (kind == kKindPolyhedron && c->sf.nverts == 8) ? 8 : 0;
     const GridParams& g = c->g;
     const int nactive = (g.n[0] / 2) * (g.n[1] / 2) * (g.dim == 3 ? g.n[2] / 2 : 1);
     bool ok = true;

@@ -17,6 +17,8 @@ struct ShapeT {
     T dmax2;              // d_max^2, broad phase R16
     T din2;               // (2 r_in - 1e-5)^2: centres closer than this certainly overlap (r_in = inscribed radius about
                           // the body origin); 0 for disks (the broad phase is the whole test)
+    T rin;                // inscribed radius about the body origin (polygons: min_k fc[k]); every support height h(u) >= rin
+    int regular;          // polygon: regular n-gon centred on the body origin (all |v| equal, equal angles): see polygon_separated
     T vx[kMaxVerts], vy[kMaxVerts], vz[kMaxVerts];
     T nx[kMaxVerts], ny[kMaxVerts], fc[kMaxVerts];  // polygon: outward unit edge normals and offsets n.v
 };
@@ -58,7 +60,8 @@ __device__ __forceinline__ V3<T> operator*(T s, const V3<T>& a)
 // be rotated ("a local coordinate system centered on particle A").
 // (rx, ry) = r_AB in the world frame; (cA,sA), (cB,sB) = cos/sin of the orientation angles.
 // NV > 0: compile-time vertex count (fully unrolled, registers); NV == 0: runtime count.
-// Returns true iff NO axis separates the pair by at least eps.
+// Returns true iff NO axis separates the pair by at least eps.  Used by the fp64 validator (a12) with eps = 0; the
+// sweep kernels use polygon_separated below.
 // ---------------------------------------------------------------------------------------------
 template <typename T, int NV>
 __device__ __forceinline__ bool polygon_overlap(const ShapeT<T>& S, T rx, T ry, T cA, T sA, T cB, T sB, T eps)
@@ -105,52 +108,70 @@ __device__ __forceinline__ bool polygon_overlap(const ShapeT<T>& S, T rx, T ry, 
     return true;
 }
 
-// Branch-free variant for the dense narrow-phase pass of the tile kernel: the largest separation over the
-// same 2*nv axes with the same formulas as polygon_overlap: overlap <=> !(polygon_max_sep(...) >= eps).
-// No early exit: all lanes of a warp run the
-// same instruction stream (a warp finishes with its slowest lane anyway).
-template <typename T, int NV>
-__device__ __forceinline__ T polygon_max_sep(const ShapeT<T>& S, T rx, T ry, T cA, T sA, T cB, T sB)
+// The sweep's polygon test (fp32): is the pair separated by at least eps along one of the 2 nv edge normals?  Same axis set
+// and the same definition of the separation as polygon_overlap, organised by support functions so that only axes that CAN
+// separate are evaluated:
+//
+//   axis k of A (unit normal n_k, offset c_k, A's frame):  sep_k = n_k . l_A - c_k - h_B(-R^T n_k)
+//   axis k of B (as a direction from A toward B: -n_k):    sep_k = -n_k . l_B - c_k - h_A(-R n_k)
+//
+// with l_A = R_A^T r, l_B = R_B^T r (r = r_AB, world), R = R_A^T R_B and h_X(u) = max_j u . v_j over the BODY-frame
+// vertices -- the axis is rotated into the other particle's frame instead of rotating that particle's vertices.
+// Every support height is >= r_in, so axis k can only separate if g_k = n_k . l - c_k >= r_in + eps: a cheap test (one dot
+// product with constants) that rules out most axes before their nv-vertex support maximum is taken.
+//
+// Regular n-gon (S.regular; NV > 0 = compile-time n, unrolled): all c_k = r_in and the normals are 2 pi / n apart, so for
+// |r| < d_max + eps_g (the broad phase, R16') only the normal closest to l can pass the test -- the next one has
+// n . l <= |l| cos(pi/n) < 2 r_in + eps.  One support maximum per side instead of n: 2 x (n dots + select + n dots).
+// Branch-free, no early exit (dense narrow phase: a warp finishes with its slowest lane anyway).
+// General convex polygon: every axis that passes the test is evaluated (data-dependent loop).
+// All fp32 colour-pass variants call this one function, so their decisions agree bit for bit.
+template <int NV>
+__device__ __forceinline__ bool polygon_separated(const ShapeT<float>& S, float rx, float ry, float cA, float sA, float cB, float sB, float eps)
 {
     const int nv = (NV > 0) ? NV : S.nverts;
-    const T lx = cA * rx + sA * ry;
-    const T ly = -sA * rx + cA * ry;
-    const T c = cA * cB + sA * sB;
-    const T s = cA * sB - sA * cB;
-    T best = -(T)3.0e38;
-    {
-        T px[(NV > 0) ? NV : kMaxVerts], py[(NV > 0) ? NV : kMaxVerts];
-#pragma unroll
-        for (int j = 0; j < nv; ++j) {
-            px[j] = c * S.vx[j] - s * S.vy[j] + lx;
-            py[j] = s * S.vx[j] + c * S.vy[j] + ly;
-        }
+    const float lAx = cA * rx + sA * ry, lAy = cA * ry - sA * rx;      // R_A^T r
+    const float lBx = cB * rx + sB * ry, lBy = cB * ry - sB * rx;      // R_B^T r
+    const float c = cA * cB + sA * sB, s = cA * sB - sA * cB;          // R = R_A^T R_B: (x, y) -> (c x - s y, s x + c y)
+    if (NV > 0 || S.regular) {
+        // the normal of A closest to l_A and the normal of B closest to -l_B
+        float gA = -3.0e38f, nAx = 0.f, nAy = 0.f, gB = -3.0e38f, nBx = 0.f, nBy = 0.f;
 #pragma unroll
         for (int k = 0; k < nv; ++k) {
-            T m = S.nx[k] * px[0] + S.ny[k] * py[0];
+            const float a = fmaf(S.nx[k], lAx, fmaf(S.ny[k], lAy, -S.fc[k]));
+            const float b = -fmaf(S.nx[k], lBx, fmaf(S.ny[k], lBy, S.fc[k]));
+            const bool pa = a > gA, pb = b > gB;
+            gA = pa ? a : gA; nAx = pa ? S.nx[k] : nAx; nAy = pa ? S.ny[k] : nAy;
+            gB = pb ? b : gB; nBx = pb ? S.nx[k] : nBx; nBy = pb ? S.ny[k] : nBy;
+        }
+        const float uAx = -(c * nAx + s * nAy), uAy = s * nAx - c * nAy;     // -R^T n_A, in B's frame
+        const float uBx = s * nBy - c * nBx, uBy = -(s * nBx + c * nBy);     // -R n_B, in A's frame
+        float hB = uAx * S.vx[0] + uAy * S.vy[0], hA = uBx * S.vx[0] + uBy * S.vy[0];
 #pragma unroll
-            for (int j = 1; j < nv; ++j) m = min(m, S.nx[k] * px[j] + S.ny[k] * py[j]);
-            best = max(best, m - S.fc[k]);
+        for (int j = 1; j < nv; ++j) {
+            hB = fmaxf(hB, uAx * S.vx[j] + uAy * S.vy[j]);
+            hA = fmaxf(hA, uBx * S.vx[j] + uBy * S.vy[j]);
+        }
+        return fmaxf(gA - hB, gB - hA) >= eps;
+    }
+    const float need = S.rin + eps;
+    for (int k = 0; k < nv; ++k) {
+        const float a = fmaf(S.nx[k], lAx, fmaf(S.ny[k], lAy, -S.fc[k]));
+        if (a >= need) {
+            const float ux = -(c * S.nx[k] + s * S.ny[k]), uy = s * S.nx[k] - c * S.ny[k];
+            float h = ux * S.vx[0] + uy * S.vy[0];
+            for (int j = 1; j < nv; ++j) h = fmaxf(h, ux * S.vx[j] + uy * S.vy[j]);
+            if (a - h >= eps) return true;
+        }
+        const float b = -fmaf(S.nx[k], lBx, fmaf(S.ny[k], lBy, S.fc[k]));
+        if (b >= need) {
+            const float ux = s * S.ny[k] - c * S.nx[k], uy = -(s * S.nx[k] + c * S.ny[k]);
+            float h = ux * S.vx[0] + uy * S.vy[0];
+            for (int j = 1; j < nv; ++j) h = fmaxf(h, ux * S.vx[j] + uy * S.vy[j]);
+            if (b - h >= eps) return true;
         }
     }
-    {
-        T qx[(NV > 0) ? NV : kMaxVerts], qy[(NV > 0) ? NV : kMaxVerts];
-#pragma unroll
-        for (int j = 0; j < nv; ++j) {
-            qx[j] = S.vx[j] - lx;
-            qy[j] = S.vy[j] - ly;
-        }
-#pragma unroll
-        for (int k = 0; k < nv; ++k) {
-            const T nxk = c * S.nx[k] - s * S.ny[k];
-            const T nyk = s * S.nx[k] + c * S.ny[k];
-            T m = nxk * qx[0] + nyk * qy[0];
-#pragma unroll
-            for (int j = 1; j < nv; ++j) m = min(m, nxk * qx[j] + nyk * qy[j]);
-            best = max(best, m - S.fc[k]);
-        }
-    }
-    return best;
+    return false;
 }
 
 // ---------------------------------------------------------------------------------------------

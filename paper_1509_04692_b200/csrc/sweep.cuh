@@ -46,7 +46,7 @@ __device__ __forceinline__ bool pair_overlap_2d(const GridParams& g, const Shape
     if (KIND == kKindDisk) return rx * rx + ry * ry < S.dmax2;
     const float cA = A.z * A.z - A.w * A.w, sA = 2.0f * A.z * A.w;   // cos t = w^2 - z^2, sin t = 2wz (R30)
     const float cB = B.z * B.z - B.w * B.w, sB = 2.0f * B.z * B.w;
-    return !(polygon_max_sep<float, NV>(S, rx, ry, cA, sA, cB, sB) >= eps);
+    return !polygon_separated<NV>(S, rx, ry, cA, sA, cB, sB, eps);
 }
 
 struct TrialState {
@@ -123,7 +123,7 @@ __device__ __forceinline__ bool narrow_overlap(const ShapeF& S, const ShapeD& SD
     } else if (KIND == kKindPolygon) {
         // 2-D orientation angle from q = (cos t/2, 0, 0, sin t/2): cos t = w^2 - z^2, sin t = 2wz
         const float cB = qB.x * qB.x - qB.w * qB.w, sB = 2.0f * qB.x * qB.w;
-        return polygon_overlap<float, NV>(S, rx, ry, MA[0], MA[1], cB, sB, eps);
+        return !polygon_separated<NV>(S, rx, ry, MA[0], MA[1], cB, sB, eps);
     } else {
         float MB[9];
         quat_to_matrix<float>(qB.x, qB.y, qB.z, qB.w, MB);
@@ -138,6 +138,7 @@ __device__ __forceinline__ bool narrow_overlap(const ShapeF& S, const ShapeD& SD
 // memory.  Used for 3-D systems and as the overflow fallback of the 2-D tile kernel.
 struct CellCounters {
     unsigned int tacc = 0, trov = 0, trcell = 0, racc = 0, rrov = 0, trials = 0;
+    unsigned int nrot = 0;   // rotation trials (tile pass only: it derives trov / rrov from the totals when it flushes)
 };
 
 __device__ __forceinline__ void flush_counters(Control* ctrl, CellCounters c)

@@ -42,7 +42,7 @@ struct Tile2D {
     static constexpr int NCELLS = RW * RH;
     static constexpr int CAP = (NCELLS * 5 / 4 + 63) / 64 * 64;   // staged poses (pentagon fluid: ~1.0 per cell)
     static constexpr int NSEG = 2 * RH;                  // contiguous runs: two per region row (periodic wrap in x)
-    static constexpr int QCAP = 96 * R;                  // narrow-phase queue entries per warp and trial round
+    static constexpr int QCAP = 32 * R * 3 * kRowSlots;  // narrow-phase queue entries per warp and trial round: every slot of every lane fits
     static constexpr int SLOTS = 32 * R;                 // trial slots per warp and round
     static_assert(NSEG + 1 <= NT, "one thread per segment");
     static_assert(CAP < 65536, "16-bit local offsets");
@@ -59,6 +59,25 @@ struct Tile2D {
     static constexpr size_t bytes = off_act + SLOTS * WARPS;
 };
 
+// a10: one predicated shared-memory store per candidate slot B .. 3 kRowSlots - 1 of the hit mask `pm`; `qaddr` (shared-memory
+// byte address of the lane's next queue entry) advances by one entry per hit.  Four instructions per slot, no branch.
+template <int B>
+__device__ __forceinline__ void push_bits(unsigned& qaddr, unsigned pm, const unsigned (&base)[3])
+{
+    if constexpr (B < 3 * kRowSlots) {
+        asm volatile("{\n\t.reg .pred q;\n\t.reg .b32 t;\n\tand.b32 t, %1, %2;\n\tsetp.ne.u32 q, t, 0;\n\t"
+                     "@q st.shared.u32 [%0], %3;\n\t@q add.u32 %0, %0, 4;\n\t}"
+                     : "+r"(qaddr) : "r"(pm), "n"(1u << B), "r"(base[B / kRowSlots] + (unsigned)(B % kRowSlots)) : "memory");
+        push_bits<B + 1>(qaddr, pm, base);
+    }
+}
+
+// out of line so that the colour pass without a trace pays one uniform branch, not a dozen predicated instructions
+static __device__ __noinline__ void trace_store(uint2* __restrict__ trace, const int* __restrict__ tag, int gi, long long at, bool rotate, unsigned outcome)
+{
+    trace[at] = make_uint2((uint32_t)tag[gi], (rotate ? 1u : 0u) | (outcome << 8));
+}
+
 // out-of-line copy for the rare direct evaluations (queue overflow, > 32 candidates): keeps the hot loop's code small
 template <int KIND, int NV>
 __device__ __noinline__ bool pair_overlap_2d_cold(const GridParams& g, const ShapeF& S, float4 A, float4 B, float eps)
@@ -69,31 +88,35 @@ __device__ __noinline__ bool pair_overlap_2d_cold(const GridParams& g, const Sha
 // a8, common path: kRowSlots fixed candidate slots per row run of the 3x3 block (bit kRowSlots*dy + j), no data-dependent
 // loop.  A slot past the end of its run holds a pose of a cell farther along (or the sentinel padding behind the last staged
 // pose): any pose within d_max of a trial that stayed in its cell lies in the 3x3 block (w >= d_max (1 + 2^-10), R11), so such
-// a slot can only repeat a genuine neighbour (tiny periodic grids) and needs no length predicate; the particle itself is
-// excluded explicitly.
+// a slot can only repeat a genuine neighbour (tiny periodic grids) or the particle itself and needs no length predicate; the
+// particle's own slots are cleared from both masks after the loop.
+//   mask : centres inside the circumsphere range (R16')          sure : some centre inside the inscribed-disk bound
 template <int KIND, bool SEAM>
 __device__ __forceinline__ void broad_slots(const GridParams& g, const ShapeF& S, const float2* sm_xy, const int (&rs)[3], int p,
                                             const float4& T, unsigned& mask, bool& sure)
 {
-    float closest = 3.0e38f;   // smallest squared centre distance: one compare after the loop instead of a branch per slot
+    unsigned smask = 0u;
 #pragma unroll
     for (int dy = 0; dy < 3; ++dy) {
 #pragma unroll
         for (int j = 0; j < kRowSlots; ++j) {
-            const int q = rs[dy] + j;
-            const float2 B = sm_xy[q];
+            const float2 B = sm_xy[rs[dy] + j];
             float rx = B.x - T.x, ry = B.y - T.y;
             if (SEAM) {
                 rx = min_image(B.x, T.x, g.hi[0], g.Ld[0]);
                 ry = min_image(B.y, T.y, g.hi[1], g.Ld[1]);
             }
             const float d2 = rx * rx + ry * ry;
-            const bool hit = (q != p) & (d2 < S.dmax2);                            // R16
-            mask |= hit ? (1u << (kRowSlots * dy + j)) : 0u;
-            closest = fminf(closest, (q != p) ? d2 : 3.0e38f);
+            if (d2 < S.dmax2) mask |= 1u << (kRowSlots * dy + j);                        // R16
+            if (KIND != kKindDisk && d2 < S.din2) smask |= 1u << (kRowSlots * dy + j);
         }
     }
-    sure = closest < ((KIND == kKindDisk) ? S.dmax2 : S.din2);                    // inside the inscribed-disk bound (disks: any hit)
+    // the particle itself: slot p - rs[1] of the middle run, and -- when the cells between are empty, so that the slots of
+    // the first run reach into the next staged row -- slot p - rs[0] of the first run (the last run starts behind p)
+    const unsigned j0 = (unsigned)(p - rs[0]), j1 = (unsigned)(p - rs[1]);
+    const unsigned keep = ~(((j1 < (unsigned)kRowSlots) ? (1u << (kRowSlots + j1)) : 0u) | ((j0 < (unsigned)kRowSlots) ? (1u << j0) : 0u));
+    mask &= keep;
+    sure = ((KIND == kKindDisk) ? mask : (smask & keep)) != 0u;                          // disks: any hit is an overlap
 }
 
 // The work of one tile of colour gamma (see the header of this file).  FLOW: the caller is the persistent dataflow kernel,
@@ -115,7 +138,6 @@ __device__ __forceinline__ void tile2d_body(const GridParams& g, const MoveParam
     unsigned* sm_queue = reinterpret_cast<unsigned*>(smem_raw + TL::off_queue);
     int* sm_seg_g = reinterpret_cast<int*>(smem_raw + TL::off_seg_g);           // global start of each segment
     int* sm_seg_l = reinterpret_cast<int*>(smem_raw + TL::off_seg_l);           // local start of each segment (+ total)
-    int* sm_qcount = reinterpret_cast<int*>(smem_raw + TL::off_qcount);
     unsigned short* sm_lstart = reinterpret_cast<unsigned short*>(smem_raw + TL::off_lstart);   // local CSR over region cells
     unsigned char* sm_flag = smem_raw + TL::off_flag;
     unsigned char* sm_act = smem_raw + TL::off_act;
@@ -242,16 +264,19 @@ __device__ __forceinline__ void tile2d_body(const GridParams& g, const MoveParam
     const uint32_t c3 = (kTagTrial << 24) | ((uint32_t)gamma << 16) | t_hi16;
 
     for (int k = 0; k < mv.n_select; ++k) {
-        if (lane == 0) sm_qcount[warp] = 0;
-        __syncwarp();
+        int qn = 0;   // entries in this warp's queue (warp-uniform)
         // per-slot state kept in registers between phases A and C: member index | rotate<<16 | outcome<<17 | sure<<19
         unsigned st[R];
         // ---- phase A: trial generation (a0, a5, a6) + broad phase (a8) + queue fill (a10) ------------------------
 #pragma unroll
         for (int s = 0; s < R; ++s) {
             st[s] = 0u;
-            if (s < nrounds) {
+            if (s < nrounds) {   // warp-uniform
                 const int slot = s * 32 + lane;
+                unsigned mask = 0u, outcome = 0u;
+                int rs[3] = {0, 0, 0}, p = 0;
+                bool sure = false, rotate = false;
+                float4 T = make_float4(0.f, 0.f, 1.f, 0.f);
                 if (slot < n_act) {
                     const int id = my_act[slot];
                     const int ay = warp * R + (id >> 5), al = id & 31;
@@ -260,23 +285,18 @@ __device__ __forceinline__ void tile2d_body(const GridParams& g, const MoveParam
                     const int lc = ryl * RW + rxl;
                     const int own_s = sm_lstart[lc], nmem = (int)sm_lstart[lc + 1] - own_s;
                     const U4 b0 = philox4x32_10((uint32_t)cell, t_lo, (uint32_t)k, c3, k0, k1);
-                    const int p = own_s + (int)mulhi32(b0.x, (uint32_t)nmem);                 // R8
+                    p = own_s + (int)mulhi32(b0.x, (uint32_t)nmem);                 // R8
                     const float4 P = ld_pose(p);
                     TrialState A;
-                    bool rotate;
                     const bool inside = make_trial<KIND>(g, mv, shift, cell, 2, b0, 0u, make_float4(P.x, P.y, 0.f, 0.f),
                                                          make_float4(P.z, 0.f, 0.f, P.w), A, rotate);
-                    const float4 T = make_float4(A.x, A.y, A.qw, A.qz);
+                    T = make_float4(A.x, A.y, A.qw, A.qz);
                     my_trial[slot] = T;
                     my_flag[slot] = 0;
-                    unsigned outcome = inside ? 1u : 2u;
-                    ++cc.trials;
-                    bool sure = false;
+                    outcome = inside ? 1u : 2u;
                     if (inside) {
                         // a8: the three row runs of the 3x3 block hold <= kRowSlots poses each in all but rare cases: fixed,
                         // predicated candidate slots (bit kRowSlots*dy + j), no data-dependent loop in the common path
-                        unsigned mask = 0u;
-                        int rs[3];
                         bool extra = false;
 #pragma unroll
                         for (int dy = 0; dy < 3; ++dy) {
@@ -300,27 +320,34 @@ __device__ __forceinline__ void tile2d_body(const GridParams& g, const MoveParam
                                 }
                             }
                         }
-                        if (KIND != kKindDisk && !sure && mask) {                     // early exit otherwise
-                            int at = atomicAdd(&sm_qcount[warp], __popc(mask));
-                            while (mask) {
-                                const int b = __ffs(mask) - 1;
-                                mask &= mask - 1u;
-                                const int dy = (b >= 2 * kRowSlots) ? 2 : (b >= kRowSlots) ? 1 : 0;
-                                const int q = ((dy == 0) ? rs[0] : (dy == 1) ? rs[1] - kRowSlots : rs[2] - 2 * kRowSlots) + b;
-                                if (at < TL::QCAP) my_queue[at] = ((unsigned)slot << 16) | (unsigned)q;
-                                else if (!sure) sure = pair_overlap_2d_cold<KIND, NV>(g, S, T, ld_pose(q), mv.eps_g);   // queue full
-                                ++at;
-                            }
-                        }
                     }
-                    st[s] = (unsigned)p | (rotate ? 1u << 16 : 0u) | (outcome << 17) | (sure ? 1u << 19 : 0u);
                 }
+                if (KIND != kKindDisk) {
+                    // a10: the lanes append their surviving candidates to the warp's queue -- positions from a warp prefix sum
+                    // of the hit counts, then one predicated store per candidate slot (all lanes in step, no per-lane loop).
+                    // A trial that is already decided ("sure", or left its cell) queues nothing: the early exit of P:45.
+                    const unsigned pm = (outcome == 1u && !sure) ? mask : 0u;
+                    const int cnt = __popc(pm);
+                    int inc = cnt;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const int n = __shfl_up_sync(0xffffffffu, inc, o);
+                        inc += (lane >= o) ? n : 0;
+                    }
+                    // shared-memory address of this lane's first entry; the queue holds every slot of every lane (QCAP), no overflow
+                    unsigned qaddr = (unsigned)__cvta_generic_to_shared(my_queue) + 4u * (unsigned)(qn + inc - cnt);
+                    qn += __shfl_sync(0xffffffffu, inc, 31);
+                    const unsigned base[3] = {((unsigned)slot << 16) + (unsigned)rs[0], ((unsigned)slot << 16) + (unsigned)rs[1],
+                                              ((unsigned)slot << 16) + (unsigned)rs[2]};
+                    push_bits<0>(qaddr, pm, base);   // entry = owner slot << 16 | staged index of the neighbour
+                }
+                st[s] = (unsigned)p | (rotate ? 1u << 16 : 0u) | (outcome << 17) | (sure ? 1u << 19 : 0u);
             }
         }
         __syncwarp();
         // ---- phase B: dense narrow phase (a9) --------------------------------------------------------------------------
         if (KIND != kKindDisk) {
-            const int nq = min(sm_qcount[warp], TL::QCAP);
+            const int nq = qn;
             for (int e = lane; e < nq; e += 32) {
                 const unsigned ent = my_queue[e];
                 const int o = (int)(ent >> 16), q = (int)(ent & 0xffffu);
@@ -338,34 +365,35 @@ __device__ __forceinline__ void tile2d_body(const GridParams& g, const MoveParam
                 const bool rotate = (st[s] >> 16) & 1u;
                 unsigned outcome = outcome0;
                 if (outcome == 1u && (((st[s] >> 19) & 1u) || my_flag[slot])) outcome = 3u;
-                const int id = my_act[slot];
-                const int ay = warp * R + (id >> 5), al = id & 31;
-                const int ryl = 2 * ay + 1, rxl = 2 * al + 1;
-                const int seg = 2 * ryl + (rxl >= split ? 1 : 0);
-                const int gi = sm_seg_g[seg] + (p - sm_seg_l[seg]);
                 const bool acc = outcome == 1u;
-                if (acc) {
-                    float4 T = my_trial[slot];
-                    if (!rotate) {   // R-wrap: at most one add per axis
-                        T.x = (T.x >= g.hi[0]) ? __fsub_rn(T.x, g.L[0]) : (T.x < g.lo[0]) ? __fadd_rn(T.x, g.L[0]) : T.x;
-                        T.y = (T.y >= g.hi[1]) ? __fsub_rn(T.y, g.L[1]) : (T.y < g.lo[1]) ? __fadd_rn(T.y, g.L[1]) : T.y;
+                if (acc || trace) {   // global index of the particle: only a write-back or the trace needs it
+                    const int id = my_act[slot];
+                    const int ay = warp * R + (id >> 5), al = id & 31;
+                    const int seg = 2 * (2 * ay + 1) + ((2 * al + 1) >= split ? 1 : 0);
+                    const int gi = sm_seg_g[seg] + (p - sm_seg_l[seg]);
+                    if (acc) {
+                        float4 T = my_trial[slot];
+                        if (!rotate) {   // R-wrap: at most one add per axis (x + (-L) is the same fp32 operation as x - L)
+                            T.x = __fadd_rn(T.x, (T.x >= g.hi[0]) ? -g.L[0] : (T.x < g.lo[0]) ? g.L[0] : 0.0f);
+                            T.y = __fadd_rn(T.y, (T.y >= g.hi[1]) ? -g.L[1] : (T.y < g.lo[1]) ? g.L[1] : 0.0f);
+                        }
+                        pose[gi] = T;
+                        st_pose(p, T);
                     }
-                    pose[gi] = T;
-                    st_pose(p, T);
+                    if (trace) trace_store(trace, tag, gi, (long long)((cx0 + 2 * al) + n0 * (cy0 + 2 * ay)) * mv.n_select + k, rotate, outcome);
                 }
                 cc.tacc += (acc && !rotate) ? 1u : 0u;
                 cc.racc += (acc && rotate) ? 1u : 0u;
                 cc.trcell += (outcome == 2u) ? 1u : 0u;
-                cc.trov += (outcome == 3u && !rotate) ? 1u : 0u;
-                cc.rrov += (outcome == 3u && rotate) ? 1u : 0u;
-                if (trace) {
-                    const long long slot0 = (long long)((cx0 + 2 * al) + n0 * (cy0 + 2 * ay)) * mv.n_select;
-                    trace[slot0 + k] = make_uint2((uint32_t)tag[gi], (rotate ? 1u : 0u) | (outcome << 8));
-                }
+                cc.nrot += rotate ? 1u : 0u;
             }
         }
         __syncwarp();
     }
+    // per-lane tallies, summed over the warp by flush_counters (modulo 2^32, so a lane's negative share is harmless)
+    cc.trials = (lane == 0) ? (unsigned)(n_act * mv.n_select) : 0u;   // every non-empty cell makes exactly n_select trials (R9)
+    cc.trov = cc.trials - cc.nrot - cc.tacc - cc.trcell;              // neither accepted nor out of its cell: overlapped
+    cc.rrov = cc.nrot - cc.racc;
     flush_counters(ctrl, cc);
 }
 
