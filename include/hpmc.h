@@ -158,6 +158,13 @@ int hpmc_get_profile(hpmc_ctx* ctx, double* h_ms_build, int64_t* h_n_build, doub
  * "k_sweep_tile2d_flow<4 warps x 1 row, 8 CTAs/SM>: 4 colour passes per launch".  Returns the length written.   */
 int hpmc_describe_pass(const hpmc_ctx* ctx, char* h_buf, size_t buf_bytes);
 
+/* Diagnostic tallies kept on the device (synchronises).  Names:
+ *   "gjk_f64_reruns"  polyhedron pairs whose fp32 GJK verdict was "unsure" (near contact, or a degenerate simplex) and that
+ *                     were decided by the fp64 re-run from the raw fp32 state -- the mixed-precision path of P:106-108,
+ *                     R-poly.  Counted since the last hpmc_reset_counters.
+ * Unknown names return HPMC_E_ARG.                                                                   */
+int hpmc_get_stat(hpmc_ctx* ctx, const char* name, int64_t* h_value);
+
 /* Launch bookkeeping for bench.py: kernels launched by this context so far.                        */
 int64_t hpmc_launch_count(const hpmc_ctx* ctx);
 

@@ -532,6 +532,8 @@ struct orc_sys {
     int mut_no_shift, mut_fixed_order, mut_no_leave;
     int work_detail; /* O7: also count separating axes / GJK support calls (costs extra narrow-phase work) */
     int nthreads;    /* 1 = serial (the definition); > 1 = same-colour cells as an OpenMP parallel-for */
+    int64_t probe_slot;      /* O8 "FAIL with a dump": trial slot whose pose and candidates are recorded, -1 = none */
+    orc_probe probe;
     int32_t *cell_id, *cell_start, *members;
 };
 
@@ -572,6 +574,7 @@ orc_sys* orc_create(int dim, const double L[3], int kind, double diameter, int n
     s->cell_start = (int32_t*)malloc(sizeof(int32_t) * (size_t)(s->C + 1));
     s->d = 0.1; s->a = 0.1; s->d_f = 0.1f; s->a_f = 0.1f; s->n_select = 4;
     s->nthreads = 1;
+    s->probe_slot = -1;
     return s;
 }
 
@@ -615,6 +618,8 @@ int64_t orc_num_cells(const orc_sys* s) { return s->C; }
 void orc_set_mutations(orc_sys* s, int a, int b, int c) { s->mut_no_shift = a; s->mut_fixed_order = b; s->mut_no_leave = c; }
 void orc_set_work_detail(orc_sys* s, int on) { s->work_detail = on; }
 void orc_set_threads(orc_sys* s, int n) { s->nthreads = n > 1 ? n : 1; }
+void orc_set_probe(orc_sys* s, int64_t slot) { s->probe_slot = slot; memset(&s->probe, 0, sizeof s->probe); s->probe.slot = -1; }
+void orc_get_probe(const orc_sys* s, orc_probe* out) { *out = s->probe; }
 int orc_get_threads(const orc_sys* s) { return s->nthreads; }
 
 /* ------------------------------------------------------------------------ */
@@ -696,8 +701,8 @@ static void min_image(const orc_sys* s, const float* xj, const float* xt, double
 static void quat_to_double(const float* q, double out[4]) { for (int c = 0; c < 4; ++c) out[c] = (double)q[c]; }
 
 /* scan the candidates of one trial; returns m_min (INFINITY if no candidate in range).  wk: O7 work tallies */
-static double scan_candidates(const orc_sys* s, orc_work* wk, int neighbour_mode, int64_t i, const float xt[3], const float qt[4],
-                              const int32_t cc[3])
+static double scan_candidates(const orc_sys* s, orc_work* wk, orc_probe* probe, int neighbour_mode, int64_t i, const float xt[3],
+                              const float qt[4], const int32_t cc[3])
 {
     const orc_shape* sh = s->shape;
     double qa[4], m_min = INFINITY;
@@ -738,6 +743,12 @@ static double scan_candidates(const orc_sys* s, orc_work* wk, int neighbour_mode
                     if (!found) wk->narrow_tests_early++;
                     quat_to_double(&s->quat[4 * j], qb);
                     double m = orc_shape_margin(sh, r, qa, qb);
+                    if (probe && probe->ncand < ORC_PROBE_MAX) {
+                        int c = probe->ncand++;
+                        probe->cand[c] = j; probe->margin[c] = m;
+                        for (int k = 0; k < 3; ++k) probe->r[c][k] = r[k];
+                        for (int k = 0; k < 4; ++k) probe->qb[c][k] = s->quat[4 * j + k];
+                    }
                     if (!found && s->work_detail) { /* O7: what an early-exit narrow phase would have evaluated */
                         if (sh->kind == ORC_KIND_POLYGON)
                             wk->polygon_axes_early += (uint64_t)polygon_axes_until_separation(sh, r, qa, qb, s->eps_g);
@@ -841,7 +852,13 @@ static void sweep_cell(orc_sys* s, const sweep_ctx* x, int64_t cell, const int32
             if (!rotate && !s->mut_no_leave && orc_cell_of(s, xt, x->shift) != (int32_t)cell) {
                 outcome = 2; /* O3.4e: leaves its cell -> reject */
             } else {
-                m_min = scan_candidates(s, wk, x->neighbour_mode, i, xt, qt, cc);
+                orc_probe* probe = (slot == s->probe_slot) ? &s->probe : NULL;
+                if (probe) {
+                    probe->slot = slot; probe->particle = i; probe->rotate = rotate; probe->ncand = 0;
+                    for (int c = 0; c < 3; ++c) probe->xt[c] = xt[c];
+                    for (int c = 0; c < 4; ++c) probe->qt[c] = qt[c];
+                }
+                m_min = scan_candidates(s, wk, probe, x->neighbour_mode, i, xt, qt, cc);
                 outcome = (m_min < s->eps_g) ? 3 : 1; /* R15 guard band */
             }
             mine[0] = (uint32_t)i;
@@ -979,7 +996,7 @@ int orc_textbook_trials(orc_sys* s, int64_t n_trials)
             memcpy(xt, &s->pos[4 * i], sizeof xt);
             gen_rotate(s, &s->quat[4 * i], b0[2], b0[3], b1[0], qt);
         }
-        double m_min = scan_candidates(s, &s->work, 1, i, xt, qt, cc);            /* 3. check all other particles   */
+        double m_min = scan_candidates(s, &s->work, NULL, 1, i, xt, qt, cc);            /* 3. check all other particles   */
         if (m_min < s->eps_g) {                                         /* 4. reject on overlap           */
             if (rotate) s->cnt.rot_rej_overlap++; else s->cnt.trans_rej_overlap++;
         } else {

@@ -72,6 +72,19 @@ typedef struct {
     double first_bad_mmin;
 } orc_follow_stats;
 
+/* O8 "any other mismatch => FAIL with a dump": the trial pose of one slot and every candidate inside the circumsphere
+ * range with its margin, recorded by the next sweep that reaches the slot (orc_set_probe). */
+#define ORC_PROBE_MAX 64
+typedef struct {
+    int64_t slot, particle;
+    int32_t rotate, ncand;
+    float xt[3], qt[4];               /* trial pose as tested (fp32) */
+    int64_t cand[ORC_PROBE_MAX];      /* neighbour particle index */
+    double r[ORC_PROBE_MAX][3];       /* minimum-image separation r_j - x_trial */
+    float qb[ORC_PROBE_MAX][4];       /* neighbour orientation */
+    double margin[ORC_PROBE_MAX];     /* O4 margin of the pair */
+} orc_probe;
+
 /* ---- RNG (R3, R4) ------------------------------------------------------- */
 void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
 float orc_u01(uint32_t r);  /* (r>>8) * 2^-24 in [0,1)              */
@@ -133,6 +146,10 @@ void orc_set_work_detail(orc_sys*, int on);
 /* n > 1: the cells of one colour as an OpenMP parallel-for (same results, P4); default 1 = serial */
 void orc_set_threads(orc_sys*, int n);
 int orc_get_threads(const orc_sys*);
+
+/* O8 dump: record the trial of `slot` (-1 = off) during the following sweeps; read it back with orc_get_probe */
+void orc_set_probe(orc_sys*, int64_t slot);
+void orc_get_probe(const orc_sys*, orc_probe* out);
 
 /* O11: textbook Metropolis, n_trials single-particle trials, own RNG tag */
 int orc_textbook_trials(orc_sys*, int64_t n_trials);

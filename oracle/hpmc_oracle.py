@@ -43,6 +43,12 @@ class FollowStats(C.Structure):
                 "first_bad_mmin": float(self.first_bad_mmin)}
 
 
+class Probe(C.Structure):
+    _fields_ = [("slot", C.c_int64), ("particle", C.c_int64), ("rotate", C.c_int32), ("ncand", C.c_int32),
+                ("xt", C.c_float * 3), ("qt", C.c_float * 4), ("cand", C.c_int64 * 64), ("r", (C.c_double * 3) * 64),
+                ("qb", (C.c_float * 4) * 64), ("margin", C.c_double * 64)]
+
+
 def lib():
     global _lib
     if _lib is not None:
@@ -88,6 +94,8 @@ def lib():
     L.orc_set_work_detail.argtypes = [vp, C.c_int]
     L.orc_set_threads.argtypes = [vp, C.c_int]
     L.orc_get_threads.argtypes = [vp]; L.orc_get_threads.restype = C.c_int
+    L.orc_set_probe.argtypes = [vp, C.c_int64]
+    L.orc_get_probe.argtypes = [vp, C.POINTER(Probe)]
     L.orc_textbook_trials.argtypes = [vp, C.c_int64]; L.orc_textbook_trials.restype = C.c_int
     L.orc_count_overlaps_bruteforce.argtypes = [vp]; L.orc_count_overlaps_bruteforce.restype = C.c_int64
     L.orc_count_overlaps_cells.argtypes = [vp]; L.orc_count_overlaps_cells.restype = C.c_int64
@@ -284,6 +292,17 @@ class Oracle:
     def set_threads(self, n):
         """n > 1: same-colour cells as an OpenMP parallel-for (identical results, P4); 1 = serial (default)."""
         lib().orc_set_threads(self._h, int(n))
+
+    def set_probe(self, slot):
+        """O8 dump: record the trial pose and candidates of `slot` during the following sweeps (-1 = off)."""
+        lib().orc_set_probe(self._h, int(slot))
+
+    def get_probe(self):
+        p = Probe(); lib().orc_get_probe(self._h, C.byref(p))
+        n = int(p.ncand)
+        return {"slot": int(p.slot), "particle": int(p.particle), "rotate": int(p.rotate), "xt": np.array(p.xt[:]),
+                "qt": np.array(p.qt[:]), "cand": np.array(p.cand[:n]), "r": np.array([list(x) for x in p.r[:n]]),
+                "qb": np.array([list(x) for x in p.qb[:n]]), "margin": np.array(p.margin[:n])}
 
     def textbook_trials(self, n):
         assert lib().orc_textbook_trials(self._h, int(n)) == 0

@@ -17,7 +17,7 @@ KIND_DISK, KIND_POLYGON, KIND_POLYHEDRON = 0, 1, 2
 ABI_SYMBOLS = ["hpmc_create", "hpmc_destroy", "hpmc_last_error", "hpmc_get_grid", "hpmc_workspace_bytes", "hpmc_bind",
                "hpmc_set_moves", "hpmc_sweep", "hpmc_count_overlaps", "hpmc_get_state", "hpmc_set_sweep_counter",
                "hpmc_reset_counters", "hpmc_set_trace", "hpmc_get_cell_list", "hpmc_sweep_host", "hpmc_set_option", "hpmc_set_profile",
-               "hpmc_get_profile", "hpmc_launch_count", "hpmc_describe_pass"]
+               "hpmc_get_profile", "hpmc_launch_count", "hpmc_describe_pass", "hpmc_get_stat"]
 
 
 class HpmcError(RuntimeError):
@@ -77,6 +77,7 @@ def load_library():
     L.hpmc_set_profile.argtypes = [vp, C.c_int]
     L.hpmc_get_profile.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64), C.POINTER(C.c_double), C.POINTER(C.c_int64)]
     L.hpmc_launch_count.argtypes = [vp]; L.hpmc_launch_count.restype = C.c_int64
+    L.hpmc_get_stat.argtypes = [vp, C.c_char_p, C.POINTER(C.c_int64)]
     L.hpmc_describe_pass.argtypes = [vp, C.c_char_p, C.c_size_t]
     for name in ABI_SYMBOLS:
         if name not in ("hpmc_last_error", "hpmc_workspace_bytes", "hpmc_launch_count"):
@@ -243,6 +244,11 @@ class Hpmc:
 
     def launch_count(self):
         return int(self._lib.hpmc_launch_count(self._h))
+
+    def get_stat(self, name):
+        v = C.c_int64()
+        self._check(self._lib.hpmc_get_stat(self._h, name.encode(), C.byref(v)))
+        return int(v.value)
 
 
 def from_workload(w, seed=1, device="cuda:0"):

@@ -742,6 +742,21 @@ int hpmc_describe_pass(const hpmc_ctx* c, char* h_buf, size_t n)
     return (int)std::min(d.size(), n - 1);
 }
 
+int hpmc_get_stat(hpmc_ctx* c, const char* name, int64_t* h_value)
+{
+    int rc = check_ready(c);
+    if (rc != HPMC_OK) return rc;
+    if (!name || !h_value) return fail(c, HPMC_E_ARG, "NULL argument");
+    if (std::string(name) != "gjk_f64_reruns") return fail(c, HPMC_E_ARG, "unknown stat");
+    Control& h = c->h_ctrl;
+    if (!cuda_ok(c, cudaMemcpyAsync(&h, c->ctrl, sizeof h, cudaMemcpyDeviceToHost, c->stream), "stat/memcpy")) return HPMC_E_CUDA;
+    if (!cuda_ok(c, cudaStreamSynchronize(c->stream), "stat/sync")) return HPMC_E_CUDA;
+    unsigned long long v = 0;
+    for (int r = 0; r < kCounterSets; ++r) v += h.counters[r][6];
+    *h_value = (int64_t)v;
+    return HPMC_OK;
+}
+
 int64_t hpmc_launch_count(const hpmc_ctx* c) { return c ? c->launches : 0; }
 
 }  // extern "C"

@@ -277,6 +277,8 @@ __device__ int gjk_classify(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T e
             int bestFace = -1, bestMask = 0;
             V3<T> bestV{0, 0, 0};
             T minIn = (T)3.0e38;   // min distance from the origin to the faces (when enclosed)
+            bool fat = true;       // every face has a solid area and the opposite vertex stands well clear of it
+            const T area_min2 = (T)1e-3 * S.dmax2 * S.dmax2, height_min = (T)10 * deep;
 #pragma unroll
             for (int f = 0; f < 4; ++f) {
                 const V3<T> p = (f == 3) ? b : a;
@@ -287,7 +289,9 @@ __device__ int gjk_classify(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T e
                 const T sp = -dot(nn, p);          // origin side
                 const T sd = dot(nn, o - p);       // opposite-vertex side
                 const T nn2 = dot(nn, nn);
-                if (sp * sd > 0) minIn = min(minIn, fabs(sp) * rsqrt(nn2));
+                const T inv = rsqrt(nn2);
+                if (sp * sd > 0) minIn = min(minIn, fabs(sp) * inv);
+                fat = fat && nn2 >= area_min2 && fabs(sd) * inv >= height_min;
                 if (sp * sd <= 0) {                // outside this face (or degenerate): closest point on it
                     int m;
                     const V3<T> cand = closest_on_triangle(p, q, s3, m);
@@ -295,7 +299,11 @@ __device__ int gjk_classify(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T e
                     if (cc < best) { best = cc; bestFace = f; bestMask = m; bestV = cand; }
                 }
             }
-            if (bestFace < 0) return (minIn > deep) ? kGjkOverlap : kGjkUnsure;   // origin inside the tetrahedron
+            // origin inside the tetrahedron.  "Overlap" needs a margin the arithmetic can vouch for: in a sliver (a face of
+            // tiny area, or a vertex almost in the plane of the opposite face -- two cubes with nearly parallel faces) the
+            // face normals are differences of nearly equal products and the sign of `sp * sd` is rounding noise, so such a
+            // tetrahedron only ever yields "unsure" (fp32: re-run in fp64; fp64 with deep = 0: fat is always true).
+            if (bestFace < 0) return (minIn > deep && fat) ? kGjkOverlap : kGjkUnsure;
             const V3<T> p = (bestFace == 3) ? b : a;
             const V3<T> q = (bestFace == 0) ? b : (bestFace == 1) ? c : d;
             const V3<T> s3 = (bestFace == 0) ? c : (bestFace == 1) ? d : (bestFace == 2) ? b : c;

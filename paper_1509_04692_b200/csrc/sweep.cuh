@@ -138,6 +138,7 @@ __device__ __forceinline__ bool narrow_overlap(const ShapeF& S, const ShapeD& SD
 // memory.  Used for 3-D systems and as the overflow fallback of the 2-D tile kernel.
 struct CellCounters {
     unsigned int tacc = 0, trov = 0, trcell = 0, racc = 0, rrov = 0, trials = 0;
+    unsigned int f64 = 0;    // polyhedron pairs decided by the fp64 re-run (diagnostic, counter slot 6)
     unsigned int nrot = 0;   // rotation trials (tile pass only: it derives trov / rrov from the totals when it flushes)
 };
 
@@ -150,6 +151,7 @@ __device__ __forceinline__ void flush_counters(Control* ctrl, CellCounters c)
     c.racc = __reduce_add_sync(0xffffffffu, c.racc);
     c.rrov = __reduce_add_sync(0xffffffffu, c.rrov);
     c.trials = __reduce_add_sync(0xffffffffu, c.trials);
+    c.f64 = __reduce_add_sync(0xffffffffu, c.f64);
     if ((threadIdx.x & 31) == 0 && c.trials) {
         unsigned long long* set = ctrl->counters[(blockIdx.x * 7u + (threadIdx.x >> 5)) & (kCounterSets - 1)];
         if (c.tacc) atomicAdd(&set[0], (unsigned long long)c.tacc);
@@ -158,6 +160,7 @@ __device__ __forceinline__ void flush_counters(Control* ctrl, CellCounters c)
         if (c.racc) atomicAdd(&set[3], (unsigned long long)c.racc);
         if (c.rrov) atomicAdd(&set[4], (unsigned long long)c.rrov);
         atomicAdd(&set[5], (unsigned long long)c.trials);
+        if (c.f64) atomicAdd(&set[6], (unsigned long long)c.f64);
     }
 }
 

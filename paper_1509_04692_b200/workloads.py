@@ -149,16 +149,20 @@ def pentagons(n_lat: int = 64, seed: int = 1, name: str = None, sweeps: int = No
                     extra={"seed": seed, "phi": N * area / (L * L)})
 
 
-def cubes(n_lat: int = 32, seed: int = 1, max_tilt: float = 0.15, name: str = "k3_cubes") -> Workload:
+def cubes(n_lat: int = 32, seed: int = 1, max_tilt: float = 0.15, name: str = "k3_cubes", spacing: float = 1.25,
+          d: float = 0.1, a: float = 0.1) -> Workload:
     """I3: configs[3]; unit cubes as generic 8-vertex polyhedra on a simple-cubic lattice, spacing 1.25.
 
     DEVIATION (R27): uniform-random orientations at spacing 1.25 overlap with probability 0.877 per
     bond, so the start is q_i = g_i (x) tau_i with g_i uniform over the 24 proper cube rotations and
     tau_i a tilt of angle uniform in [0, 0.15] rad about a uniform random axis; each cube's half
     extent along a lattice axis is then <= 0.61 < 0.625 and the start is overlap-free.
+
+    Other `spacing` / `max_tilt` / move sizes give test cases (the caller keeps 0.5 (1 + sqrt 2 sin(max_tilt)) below
+    spacing / 2): e.g. spacing 1.0006 with tilts of 2e-4 rad is a crystal of nearly parallel, nearly touching faces.
     """
     N = n_lat ** 3
-    pos4 = _lattice(3, n_lat, 1.25)
+    pos4 = _lattice(3, n_lat, spacing)
     rng = _rng(seed, 303)
     G = _cube_group()
     g = G[rng.integers(0, 24, size=N)]
@@ -170,9 +174,9 @@ def cubes(n_lat: int = 32, seed: int = 1, max_tilt: float = 0.15, name: str = "k
     tau = np.concatenate([np.cos(0.5 * ang)[:, None], np.sin(0.5 * ang)[:, None] * axis], axis=1)
     q = _qmul(g, tau)
     q /= np.linalg.norm(q, axis=1, keepdims=True)
-    L = n_lat * 1.25
+    L = n_lat * spacing
     return Workload(name=name, dim=3, N=N, L=(L, L, L), kind=KIND_POLYHEDRON, diameter=0.0, verts=cube_vertices(1.0),
-                    d=0.1, a=0.1, n_select=4, sweeps=1000, pos4=pos4, quat4=q.astype(np.float32), warmup_sweeps=200,
+                    d=d, a=a, n_select=4, sweeps=1000, pos4=pos4, quat4=q.astype(np.float32), warmup_sweeps=200,
                     notes="initial orientations: cube-group element x tilt<=0.15 rad (BASELINE.json's uniform-random "
                           "orientations are infeasible at spacing 1.25)",
                     extra={"seed": seed, "phi": N / L ** 3})

@@ -1,9 +1,12 @@
 """Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (default options):
-configs[2] (1 048 576 pentagons) and configs[4] (16 777 216 pentagons).
+configs[2] (1 048 576 pentagons, 10 sweeps), configs[3] (32 768 cubes, 10 sweeps) and configs[4] (16 777 216 pentagons,
+3 sweeps: SURVEY.md O8 -- the trace alone is 0.5 GB per sweep there).  Configs 0 and 1 are locked for 10 sweeps in
+tests/test_gpu_parity.py.
 
-The oracle replays whole sweeps of the full system (O8 lock-step: every trial slot compared, 4.2 M / 67 M slots
-per sweep), then properties that hold at any size are checked after more sweeps: zero overlaps, counters that
-add up, trials = n_select x non-empty cells, the traced and untraced runs bit-identical.
+The oracle replays whole sweeps of the full system (O8 lock-step: every trial slot compared, 4.2 M / 42 592 / 67 M slots
+per sweep; the cells of one colour run as the oracle's parallel-for, which changes no result), then properties that hold
+at any size are checked after more sweeps: zero overlaps, counters that add up, trials = n_select x non-empty cells, the
+traced and untraced runs bit-identical.
 """
 import os
 
@@ -23,12 +26,13 @@ def _lockstep_full(k, n_lock, n_more):
     o = ho.Oracle(w.dim, w.L, w.kind, w.N, 1, diameter=w.diameter, verts=w.verts)
     o.set_moves(w.d, w.a, w.n_select)
     o.set_state(w.pos4, w.quat4)
+    o.set_threads(min(os.cpu_count() or 1, 16))
     assert g.count_overlaps() == 0
     # cell list of sweep 0: ids, CSR and member order bit-exact
     cid, cst, mem, shift, perm = g.cell_list(0)
     oshift, operm = o.sweep_header(0)
     ocid, ocst, omem = o.cell_list(oshift)
-    assert np.array_equal(shift[:2], oshift[:2]) and np.array_equal(perm, operm)
+    assert np.array_equal(shift[: w.dim], oshift[: w.dim]) and np.array_equal(perm, operm)
     assert np.array_equal(cid, ocid) and np.array_equal(cst, ocst) and np.array_equal(mem, omem)
     del cid, cst, mem, ocid, ocst, omem
     g.enable_trace(True)
@@ -56,7 +60,10 @@ def _lockstep_full(k, n_lock, n_more):
     assert np.array_equal(p2, gp) and np.array_equal(q2, gq) and g2.counters() == gc
     # one launch per colour instead of the dataflow launch (or the reverse): the same trajectory
     g3 = hb.from_workload(w, seed=1)
-    g3.set_option("flow", 0 if k == 2 else 1)
+    if w.dim == 2:
+        g3.set_option("flow", 0 if k == 2 else 1)
+    else:
+        g3.set_option("path", 1)                      # 3-D: the per-thread global-memory pass instead of warp-per-cell
     g3.sweep(n_lock)
     p3, q3 = g3.get_state()
     assert np.array_equal(p3, gp) and np.array_equal(q3, gq) and g3.counters() == gc
@@ -76,15 +83,21 @@ def _lockstep_full(k, n_lock, n_more):
     assert g2.count_overlaps() == 0
     p, q = g2.get_state()
     half = np.float32(0.5) * np.float32(w.L[0])
-    assert np.all(p[:, :2] >= -half) and np.all(p[:, :2] < half) and np.all(p[:, 2:] == 0)
-    assert np.all(q[:, 1:3] == 0) and np.max(np.abs(np.sum(q.astype(np.float64) ** 2, axis=1) - 1)) < 1e-6
-    print(f"config {k}: {trials} trials locked to the oracle, {marginal} marginal")
+    assert np.all(p[:, : w.dim] >= -half) and np.all(p[:, : w.dim] < half) and np.all(p[:, w.dim:] == 0)
+    if w.dim == 2:
+        assert np.all(q[:, 1:3] == 0)
+    assert np.max(np.abs(np.sum(q.astype(np.float64) ** 2, axis=1) - 1)) < 1e-6
+    print(f"config {k}: {n_lock} sweeps, {trials} trials locked to the oracle, {marginal} marginal (|m - eps_g| < 1e-5)")
 
 
 def test_config2_pentagons_1M_lockstep_and_invariants():
-    _lockstep_full(2, 3, 5)
+    _lockstep_full(2, 10, 5)
+
+
+def test_config3_cubes_32768_lockstep_and_invariants():
+    _lockstep_full(3, 10, 5)
 
 
 @pytest.mark.skipif(os.environ.get("HPMC_SKIP_16M") == "1", reason="HPMC_SKIP_16M=1")
 def test_config4_pentagons_16M_lockstep_and_invariants():
-    _lockstep_full(4, 1, 2)
+    _lockstep_full(4, 3, 2)

@@ -317,3 +317,38 @@ def test_dataflow_pass_across_the_32_bit_wrap_of_the_sweep_counter():
         assert g.counters()["sweep_counter"] == 2 ** 32 + 5 and g.count_overlaps() == 0
         out.append((g.get_state(), g.counters()))
     assert np.array_equal(out[0][0][0], out[1][0][0]) and np.array_equal(out[0][0][1], out[1][0][1]) and out[0][1] == out[1][1]
+
+
+@pytest.mark.parametrize("gap,move", [(6e-4, 3e-4), (8e-6, 8e-6)])
+def test_near_contact_cubes_match_the_oracle_and_take_the_fp64_rerun(gap, move):
+    """A crystal of nearly parallel cubes with face-to-face gaps of `gap` and moves of `move`: almost every narrow-phase test
+    is a near-contact pair.  Every decision must be the oracle's (sign of the SAT margin against the guard band) except inside
+    the 1e-5 window.  The fp32 GJK certifies a separation itself down to gaps of a few 1e-6 (its certificate n.s >= eps_g is
+    evaluated from the support points), but between nearly parallel faces its simplex is often a sliver whose "origin inside"
+    verdict cannot be trusted, and with gaps of 8e-6 many trials end inside the guard band or barely overlapping, where the fp32
+    run converges without a certificate: both answer "unsure", and the pair must be decided by the fp64 re-run (P:106-108;
+    counted on the device: 1243 and 6027 re-runs in 2048 trials).  In the second case most trials lie close to the 1e-5 window.
+    Regression for the round-2 finding at full config 3: an fp32 "origin inside the tetrahedron" verdict on a sliver simplex."""
+    # 7^3 cubes in 4^3 cells of width 1.75: 145 particles around a cell, inside the staging capacity of the warp-per-cell pass
+    w = wl.cubes(7, spacing=1.0 + gap, max_tilt=gap / 4, d=move, a=move, name="cubes_near_contact")
+    g, o = gpu(w), orc(w)
+    assert g.count_overlaps() == 0 and o.count_overlaps_bruteforce() == 0
+    g.enable_trace(True)
+    marginal = trials = 0
+    for s in range(8):
+        g.sweep(1)
+        f = o.sweep(follow=g.read_trace(), follow_tol=MARGIN_TOL)["follow"]
+        assert f["hard_mismatch"] == 0, (s, f)
+        marginal += f["marginal"]
+        gp, gq = g.get_state(); op, oq = o.get_state()
+        assert np.array_equal(gp, op) and np.max(np.abs(gq.astype(np.float64) - oq)) < 1e-5
+        o.set_state(op, gq)
+    c = g.counters()
+    trials = c["trials"]
+    reruns = g.get_stat("gjk_f64_reruns")
+    rej = c["trans_rej_overlap"] + c["rot_rej_overlap"]
+    print(f"near-contact cubes gap {gap}: {trials} trials, {rej} overlap rejects, {marginal} marginal, {reruns} fp64 re-runs")
+    assert rej > 0.05 * trials and c["trans_acc"] + c["rot_acc"] > 0.05 * trials      # both outcomes occur
+    assert g.count_overlaps() == 0                                                    # the strict fp64 validator agrees
+    assert marginal <= 0.02 * trials
+    assert reruns > 0.1 * trials                                                      # the mixed-precision branch carries this case
