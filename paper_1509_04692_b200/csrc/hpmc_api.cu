@@ -304,6 +304,52 @@ bool use_flow(const hpmc_ctx* c)
     return c->opt_tile_shape == 0 && tiles > slots && tiles <= 4 * slots;
 }
 
+// Whole-sweep cluster pass (sweep_cluster2d.cuh): 2-D disks / polygons small enough for one cluster of 16 x 1024 threads
+// (one thread per particle in its build) and for a cell_start copy in every CTA's shared memory.
+constexpr int kClusterMaxCtas = 16, kClusterThreads = 1024, kClusterMaxCells = 11500;
+bool cluster_eligible(const hpmc_ctx* c)
+{
+    const GridParams& g = c->g;
+    if (g.dim != 2 || c->sf.kind == kKindPolyhedron || c->cluster_ctas == 0) return false;
+    if (g.N < 1 || g.N > kClusterMaxCtas * kClusterThreads || g.C + 2 > kClusterMaxCells) return false;
+    // measured on B200 (profiles/r2_cluster.md): 58 us per sweep of 4096 pentagons against 39 us for the graph of five launches --
+    // a trial is a ~2 us dependent chain either way and seven cluster barriers do not beat four launch gaps -- so the pass is
+    // chosen only on request
+    return c->opt_path == 4;
+}
+
+// n sweeps through the cluster pass; returns the sweeps done (0: not available here, the caller uses the other passes)
+int64_t sweep_cluster(hpmc_ctx* c, int64_t n)
+{
+    const int kind = c->sf.kind;
+    const int nv = (kind == kKindPolygon && c->sf.nverts == 5 && c->sf.regular) ? 5 : 0;
+    int64_t done = 0;
+    while (done < n) {
+        const int64_t want = std::min<int64_t>(n - done, 1 << 20);   // sweeps per launch
+        int got = 0;
+        {
+            ProfileScope prof(c, 1, (int)(4 * want));   // timed as 4 colour passes per sweep (the build is inside the launch)
+            if (c->cluster_ctas < 0) {   // first use: the largest cluster this device schedules that covers the particles
+                for (int ncta = kClusterMaxCtas; ncta >= 1 && c->cluster_ctas < 0; ncta >>= 1) {
+                    if (ncta * kClusterThreads < c->g.N) break;
+                    got = hpmc_launch_cluster2d(c, want, ncta, kind, nv);
+                    if (got < 0) return -1;
+                    if (got > 0) c->cluster_ctas = ncta;
+                }
+                if (c->cluster_ctas < 0) { c->cluster_ctas = 0; prof.on = false; return done; }
+            } else {
+                got = hpmc_launch_cluster2d(c, want, c->cluster_ctas, kind, nv);
+                if (got <= 0) return -1;
+            }
+        }
+        ++c->launches;
+        c->cur ^= (got & 1);
+        c->t_host += (uint64_t)got;
+        done += got;
+    }
+    return done;
+}
+
 int launch_colour_dispatch(hpmc_ctx* c, int ci)
 {
     c->flow_now = use_flow(c);
@@ -490,6 +536,20 @@ int hpmc_sweep(hpmc_ctx* c, int64_t n)
     if (n < 0) return fail(c, HPMC_E_ARG, "n must be >= 0");
     if (c->trace && c->trace_words < 2 * (int64_t)c->g.C * c->mv.n_select) return fail(c, HPMC_E_TRACE, "trace buffer too small");
     int64_t s = 0;
+    // Small 2-D systems: whole sweeps inside one thread-block cluster, any number per launch (sweep_cluster2d.cuh)
+    if (cluster_eligible(c)) {
+        if (c->state_in_bound) {   // the first build reads the caller's tag-order arrays: one plain sweep
+            rc = sweep_once(c);
+            if (rc != HPMC_OK) return rc;
+            ++s;
+        }
+        if (s < n) {
+            const int64_t got = sweep_cluster(c, n - s);
+            if (got < 0) return HPMC_E_CUDA;
+            s += got;
+        }
+        if (s == n) return HPMC_OK;
+    }
     // Launch-bound systems (config 1: 11 launches of a few microseconds per sweep): replay a captured graph of two
     // sweeps.  The sweep counter, header and counters live on the device, so the replay needs no new arguments.
     if (c->opt_graph && c->stream != nullptr && !c->trace && !c->profile && n >= 3) {   // the legacy default stream cannot be captured
@@ -682,7 +742,7 @@ int hpmc_set_option(hpmc_ctx* c, const char* name, int64_t value)
     if (n == "graph") {
         c->opt_graph = value != 0;
     } else if (n == "path") {
-        if (value < 0 || value > 3) return fail(c, HPMC_E_ARG, "path must be 0 (auto), 1 (per-thread), 2 (tile) or 3 (warp per cell)");
+        if (value < 0 || value > 4) return fail(c, HPMC_E_ARG, "path must be 0 (auto), 1 (per-thread), 2 (tile), 3 (warp per cell) or 4 (cluster)");
         c->opt_path = (int)value;
     } else if (n == "tile_cap") {
         if (value < 0) return fail(c, HPMC_E_ARG, "tile_cap must be >= 0");
@@ -729,7 +789,10 @@ int hpmc_describe_pass(const hpmc_ctx* c, char* h_buf, size_t n)
     const GridParams& g = c->g;
     const int nactive = (g.n[0] / 2) * (g.n[1] / 2) * (g.dim == 3 ? g.n[2] / 2 : 1);
     std::string d;
-    if (c->opt_path == 1) d = "k_sweep_colour: one thread per active cell";
+    if (cluster_eligible(c) && c->cluster_ctas != 0)
+        d = "k_sweep_cluster2d: whole sweeps (build + 4 colour passes) in one launch of one thread-block cluster of " +
+            std::to_string(c->cluster_ctas > 0 ? c->cluster_ctas : kClusterMaxCtas) + " CTAs";
+    else if (c->opt_path == 1) d = "k_sweep_colour: one thread per active cell";
     else if (g.dim == 3 || c->opt_path == 3 || (c->opt_path == 0 && c->opt_tile_shape == 0 && nactive <= kWarpCellMax2d))
         d = "k_sweep_warpcell: one warp per active cell, 1 colour pass per launch";
     else {

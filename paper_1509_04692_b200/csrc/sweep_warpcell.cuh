@@ -114,11 +114,19 @@ k_sweep_warpcell(const __grid_constant__ GridParams g, const __grid_constant__ M
     __syncwarp();
 
     const uint32_t c3 = (kTagTrial << 24) | ((uint32_t)gamma << 16) | t_hi16;
+    U4 blk{0u, 0u, 0u, 0u};
+    uint32_t blk_uc = 0u;
     for (int k = 0; k < mv.n_select; ++k) {
-        // ---- phase A: trial generation (a0, a5, a6), identical on every lane -----------------------------------------
-        const U4 b0 = philox4x32_10((uint32_t)cell, t_lo, (uint32_t)k, c3, k0, k1);
-        uint32_t uc = 0u;
-        if (DIM == 3) uc = philox4x32_10((uint32_t)cell, t_lo, (uint32_t)k | (1u << 16), c3, k0, k1).x;
+        // ---- a0: the Philox blocks of the next 32 trials, one trial per lane, off the critical path of the sequential trials
+        // (a trial is a chain of dependent instructions; ten Philox rounds are a quarter of it); trial k broadcasts its block
+        if ((k & 31) == 0) {
+            blk = philox4x32_10((uint32_t)cell, t_lo, (uint32_t)(k + lane), c3, k0, k1);
+            if (DIM == 3) blk_uc = philox4x32_10((uint32_t)cell, t_lo, (uint32_t)(k + lane) | (1u << 16), c3, k0, k1).x;
+        }
+        const U4 b0{__shfl_sync(0xffffffffu, blk.x, k & 31), __shfl_sync(0xffffffffu, blk.y, k & 31), __shfl_sync(0xffffffffu, blk.z, k & 31),
+                    __shfl_sync(0xffffffffu, blk.w, k & 31)};
+        const uint32_t uc = (DIM == 3) ? __shfl_sync(0xffffffffu, blk_uc, k & 31) : 0u;
+        // ---- phase A: trial pose (a5, a6), identical on every lane ------------------------------------------------------
         const int p = own_s + (int)mulhi32(b0.x, (uint32_t)nmem);   // R8
         const float4 xp = sm.pos[p], qp = sm.quat[p];
         TrialState A;

@@ -143,6 +143,7 @@ def test_colour_pass_variants_agree_bit_for_bit(name):
     shapes += [{"path": 2, "flow": 1}, {"tile_shape": 1, "flow": 1}, {"tile_shape": 2, "flow": 1},
                {"path": 2, "flow": 1, "tile_cap": some}] if w.dim == 2 else []
     warp = [{"path": 3}, {"path": 3, "tile_cap": 6}] if w.dim == 2 else []        # 2-D warp-per-cell pass and its fallback
+    warp += [{"path": 4}] if w.dim == 2 else []                                   # whole sweeps in one thread-block cluster
     builds = [{"small_build": 0}, {"small_build": 0, "path": 2}]                   # the multi-launch cell-list build
     for opts in [{"path": 2}, {"path": 2, "tile_cap": 0}, {"path": 1}, {"path": 2, "tile_cap": some}] + shapes + warp + builds:
         g = gpu(w)
