@@ -1,8 +1,15 @@
 """BASELINE.json's five configs at their full stated run lengths on the GPU path (north_star target: "zero overlaps ... on all
 five configs"): 1000 / 10^4 / 1000 / 1000 / 100 sweeps through `hpmc_sweep`, in the default launch configuration (CUDA-graph
 replay, dataflow or warp-per-cell pass as chosen by size).  Checked: the fp64 validator finds no overlapping pair before and
-after, every trial is accounted for, the sweep counter advanced by the run length, and the acceptance ratio sits where the
-oracle puts it for this state point (8-seed means of tests/test_gpu_statistics.py, +- 0.02)."""
+after, every trial is accounted for, the sweep counter advanced by the run length, and the acceptance ratios accumulated from
+the lattice start sit where the ORACLE puts them: tests/golden/oracle_expectations.json, written by
+tests/golden/make_oracle_expectations.py from the oracle alone (8 seeds, the same run lengths; configs 0, 1 and 3 at full size).
+Configs 2 and 4 are compared with config 1's state point after the same number of sweeps; their cell grid differs
+(w / d_max = 1.002 / 1.001 against 1.032), so the translate acceptance is compared after dividing by the closed-form
+probability (1 - d / 2w)^2 of staying in the cell, to 1 % (see tests/test_gpu_statistics.py)."""
+import json
+import os
+
 import numpy as np
 import pytest
 
@@ -10,8 +17,13 @@ from paper_1509_04692_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
 
-# (config, translate acceptance, rotate acceptance) from the oracle's 8-seed statistics at these state points
-EXPECT = {0: (0.330, None), 1: (0.485, 0.903), 2: (0.485, 0.903), 3: (0.30, 0.73), 4: (0.485, 0.903)}
+EXPECT = json.load(open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "oracle_expectations.json")))["full_runs"]
+# config -> (state point in the file, checkpoint = run length in sweeps)
+WHERE = {0: ("k0", "1000"), 1: ("k1", "10000"), 2: ("k1", "1000"), 3: ("k3", "1000"), 4: ("k1", "100")}
+
+
+def stay_probability(w, cells):
+    return (1.0 - w.d / (2.0 * w.L[0] / cells)) ** w.dim
 
 
 @pytest.mark.parametrize("k", [0, 1, 2, 3, 4])
@@ -27,11 +39,20 @@ def test_full_length_run_ends_without_overlaps(k):
     nt = c["trans_acc"] + c["trans_rej_overlap"] + c["trans_rej_cell"]
     nr = c["rot_acc"] + c["rot_rej_overlap"]
     assert nt + nr == c["trials"] and c["trials"] > 0.8 * w.n_select * min(g.C, w.N) * w.sweeps
-    ta, ra = EXPECT[k]
-    tol = 0.02 if k != 3 else 0.06          # config 3 keeps relaxing from its tilted-lattice orientations over the 1000 sweeps
-    assert abs(c["trans_acc"] / nt - ta) < tol, c
-    if ra is not None:
-        assert abs(c["rot_acc"] / nr - ra) < tol and abs(nr / c["trials"] - 0.5) < 0.01, c
+    state, cp = WHERE[k]
+    e = EXPECT[state][cp]
+    ta, ra = e["translate_acceptance"]["mean"], e["rotate_acceptance"]["mean"]
+    # one GPU seed against the oracle's 8-seed mean: 5 single-seed standard deviations, at least 0.002
+    tol_t = max(5.0 * e["translate_acceptance"]["se"] * np.sqrt(8.0), 0.002)
+    tol_r = max(5.0 * e["rotate_acceptance"]["se"] * np.sqrt(8.0), 0.002)
+    got_t = c["trans_acc"] / nt
+    if k in (2, 4):   # another cell grid than config 1's: compare per trial that stays in its cell, to 1 %
+        w1 = wl.config(1)
+        got_t *= stay_probability(w1, 62) / stay_probability(w, int(g.n[0]))
+        tol_t, tol_r = 0.01 * ta, 0.005 * ra
+    assert abs(got_t - ta) < tol_t, (k, got_t, ta, tol_t, c)
+    if ra > 0:
+        assert abs(c["rot_acc"] / nr - ra) < tol_r and abs(nr / c["trials"] - 0.5) < 0.01, (k, c["rot_acc"] / nr, ra, tol_r)
     else:
         assert nr == 0
     p, q = g.get_state()
