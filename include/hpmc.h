@@ -17,6 +17,10 @@
  *     TAG order (particle i at row i).  2-D systems keep z = 0 and quat = (cos t/2, 0, 0, sin t/2) (R30).
  *   - box: orthorhombic, periodic, centred on the origin, coordinates in [-L/2, L/2) (R14).  The box
  *     edge is L rounded to fp32 (R-box).
+ *   - precondition on the state handed to hpmc_bind / hpmc_sweep_host: finite coordinates inside the box.  A violation never
+ *     corrupts memory (the cell index is clamped) but is counted on the device, and the next hpmc_count_overlaps or
+ *     hpmc_get_state(counters) returns HPMC_E_ARG.  A new hpmc_bind clears the count.
+ *   - every entry point makes the device of the context (the one current at hpmc_create) current for its duration.
  *   - there is no CPU implementation behind this interface.
  */
 #ifndef HPMC_H
@@ -39,7 +43,8 @@ extern "C" {
 #define HPMC_OK 0
 #define HPMC_E_ARG (-1)       /* bad argument (dim, N, d, a, n_select, NULL pointer, ...)          */
 #define HPMC_E_SHAPE (-2)     /* non-convex / not CCW / too many vertices / vertex not on the hull */
-#define HPMC_E_GRID (-3)      /* fewer than 4 cells per side (R11) or more than 2^31-2 cells       */
+#define HPMC_E_GRID (-3)      /* fewer than 4 cells per side (R11), more than 2^31-2 cells, or a box so large that the
+                                 fp32 rounding of cell_of (3 ulp(L)) exceeds the slack w - d_max of the cell width      */
 #define HPMC_E_UNBOUND (-4)   /* state/workspace not bound, or workspace too small                 */
 #define HPMC_E_CUDA (-5)      /* a CUDA call failed (sticky)                                       */
 #define HPMC_E_TRACE (-6)     /* trace buffer too small for C * n_select slots                     */
@@ -166,6 +171,11 @@ int hpmc_describe_pass(const hpmc_ctx* ctx, char* h_buf, size_t buf_bytes);
  *                     R-poly.  Counted since the last hpmc_reset_counters.
  * Unknown names return HPMC_E_ARG.                                                                   */
 int hpmc_get_stat(hpmc_ctx* ctx, const char* name, int64_t* h_value);
+
+/* Measured FP32 roofline denominator (S:8(d)): runs a pure-FMA microkernel (16 independent fused multiply-add chains per
+ * thread, 8 CTAs of 256 threads per SM, no memory traffic) on the context's stream and returns the best of three timed
+ * launches in TFLOP/s (FMA = 2 flops).  Synchronises.  Nominal on B200: 148 SMs x 128 lanes x 2 x 1.965 GHz = 74.4.   */
+int hpmc_measure_fp32_peak(hpmc_ctx* ctx, double* h_tflops);
 
 /* Launch bookkeeping for bench.py: kernels launched by this context so far.                        */
 int64_t hpmc_launch_count(const hpmc_ctx* ctx);

@@ -17,7 +17,7 @@ KIND_DISK, KIND_POLYGON, KIND_POLYHEDRON = 0, 1, 2
 ABI_SYMBOLS = ["hpmc_create", "hpmc_destroy", "hpmc_last_error", "hpmc_get_grid", "hpmc_workspace_bytes", "hpmc_bind",
                "hpmc_set_moves", "hpmc_sweep", "hpmc_count_overlaps", "hpmc_get_state", "hpmc_set_sweep_counter",
                "hpmc_reset_counters", "hpmc_set_trace", "hpmc_get_cell_list", "hpmc_sweep_host", "hpmc_set_option", "hpmc_set_profile",
-               "hpmc_get_profile", "hpmc_launch_count", "hpmc_describe_pass", "hpmc_get_stat"]
+               "hpmc_get_profile", "hpmc_launch_count", "hpmc_describe_pass", "hpmc_get_stat", "hpmc_measure_fp32_peak"]
 
 
 class HpmcError(RuntimeError):
@@ -78,6 +78,7 @@ def load_library():
     L.hpmc_get_profile.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64), C.POINTER(C.c_double), C.POINTER(C.c_int64)]
     L.hpmc_launch_count.argtypes = [vp]; L.hpmc_launch_count.restype = C.c_int64
     L.hpmc_get_stat.argtypes = [vp, C.c_char_p, C.POINTER(C.c_int64)]
+    L.hpmc_measure_fp32_peak.argtypes = [vp, C.POINTER(C.c_double)]
     L.hpmc_describe_pass.argtypes = [vp, C.c_char_p, C.c_size_t]
     for name in ABI_SYMBOLS:
         if name not in ("hpmc_last_error", "hpmc_workspace_bytes", "hpmc_launch_count"):
@@ -244,6 +245,12 @@ class Hpmc:
 
     def launch_count(self):
         return int(self._lib.hpmc_launch_count(self._h))
+
+    def measure_fp32_peak(self):
+        """TFLOP/s of the library's pure-FMA microkernel on this device (the measured FP32 roofline denominator)."""
+        v = C.c_double()
+        self._check(self._lib.hpmc_measure_fp32_peak(self._h, C.byref(v)))
+        return float(v.value)
 
     def get_stat(self, name):
         v = C.c_int64()

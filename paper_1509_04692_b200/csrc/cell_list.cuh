@@ -39,8 +39,9 @@ __global__ void k_hist(const __grid_constant__ GridParams g, Control* __restrict
     if (p >= g.N) return;
     const float shift[3] = {sh.shift[0], sh.shift[1], sh.shift[2]};
     const float4 x = pos[p];
-    int cx, cy, cz;
-    const int c = cell_of(g, shift, x.x, x.y, x.z, cx, cy, cz);
+    bool bad;
+    const int c = cell_of_checked(g, shift, x.x, x.y, (g.dim == 3) ? x.z : 0.0f, bad);
+    if (bad) atomicAdd(&ctrl->bad_coords, 1u);
     const int rank = atomicAdd(&counts[c], 1);
     key_rank[p] = make_int2(c, rank);
 }
@@ -253,8 +254,9 @@ k_build_small(const __grid_constant__ GridParams g, Control* __restrict__ ctrl, 
     const float shift[3] = {sh.shift[0], sh.shift[1], sh.shift[2]};
     for (int p = tid; p < g.N; p += kSmallBuildThreads) {
         const float4 x = src_pos[p];
-        int cx, cy, cz;
-        const int c = cell_of(g, shift, x.x, x.y, x.z, cx, cy, cz);
+        bool bad;
+        const int c = cell_of_checked(g, shift, x.x, x.y, (g.dim == 3) ? x.z : 0.0f, bad);
+        if (bad) atomicAdd(&ctrl->bad_coords, 1u);
         key_rank[p] = make_int2(c, atomicAdd(&s_off[c], 1));
     }
     __syncthreads();

@@ -52,6 +52,7 @@ struct Control {
     unsigned long long counters[kCounterSets][8];
     unsigned long long overlaps;     // validator result
     unsigned int flow_ticket, flow_exited;   // k_sweep_tile2d_flow: next (colour, tile) ticket; CTAs that have left
+    unsigned int bad_coords, pad_bc;         // particles whose coordinates were not finite or not in [-L/2, L/2) when a cell list was built
     SweepHeader hdr;
 };
 
@@ -88,6 +89,23 @@ __device__ __forceinline__ int cell_axis(float x, float lo, float s, float L, fl
     int c = (int)floorf(__fmul_rn(f, inv_w));
     if (c >= n) c -= n;
     return c;
+}
+
+// The cell-list builders use the same function but may meet caller data that breaks the precondition (coordinates in
+// [-L/2, L/2), finite): such a particle is counted in Control::bad_coords and its cell index clamped into the grid, so that no
+// histogram or scatter ever indexes out of bounds; hpmc_count_overlaps / hpmc_get_state then report HPMC_E_ARG.
+__device__ __forceinline__ int cell_of_checked(const GridParams& g, const float shift[3], float x, float y, float z, bool& bad)
+{
+    bad = !(x >= g.lo[0] && x < g.hi[0] && y >= g.lo[1] && y < g.hi[1]) || (g.dim == 3 && !(z >= g.lo[2] && z < g.hi[2]));
+    int cx = cell_axis(x, g.lo[0], shift[0], g.L[0], g.inv_w[0], g.n[0]);
+    int cy = cell_axis(y, g.lo[1], shift[1], g.L[1], g.inv_w[1], g.n[1]);
+    int cz = (g.dim == 3) ? cell_axis(z, g.lo[2], shift[2], g.L[2], g.inv_w[2], g.n[2]) : 0;
+    if (bad) {
+        cx = min(max(cx, 0), g.n[0] - 1);
+        cy = min(max(cy, 0), g.n[1] - 1);
+        cz = min(max(cz, 0), g.n[2] - 1);
+    }
+    return cx + g.n[0] * (cy + g.n[1] * cz);
 }
 
 __device__ __forceinline__ int cell_of(const GridParams& g, const float shift[3], float x, float y, float z, int& cx,

@@ -47,6 +47,8 @@ struct hpmc_ctx {
     int* tile_sums = nullptr;   // per-tile totals of the scan
     unsigned int* flow_done = nullptr;   // per (colour, tile) stamps of the dataflow pass
     int num_sms = 0;
+    int device = 0;                      // CUDA device of the context (the one current at hpmc_create); every entry point switches to it
+    uint32_t attr_done = 0;              // cudaFuncSetAttribute(MaxDynamicSharedMemorySize) done for this context: bit per tile shape / flow
     bool flow_now = false;               // this sweep's colour passes go out as one dataflow launch
     Control* ctrl = nullptr;
 
@@ -74,6 +76,17 @@ struct hpmc_ctx {
     size_t ev_used = 0;            // events handed out (2 per pair)
     double prof_ms[2] = {0.0, 0.0};
     int64_t prof_n[2] = {0, 0};
+};
+
+// Makes the context's device current for the duration of an entry point (the caller's current device may be another one).
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(const hpmc_ctx* c)
+    {
+        if (c && cudaGetDevice(&prev) == cudaSuccess && prev != c->device) cudaSetDevice(c->device);
+        else prev = -1;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 
 inline bool cuda_ok(hpmc_ctx* c, cudaError_t e, const char* what)

@@ -17,6 +17,25 @@
 
 using namespace hpmc;
 
+// Pure-FMA microkernel for the measured FP32 roofline denominator (S:8(d): "time a pure-FMA microkernel in the same run"):
+// kFmaChains independent dependent-FMA chains per thread, no memory traffic but one store that keeps the result alive.
+constexpr int kFmaChains = 16;
+__global__ void __launch_bounds__(256) k_fma_peak(float* sink, int iters, float a)
+{
+    float x[kFmaChains];
+#pragma unroll
+    for (int j = 0; j < kFmaChains; ++j) x[j] = 1.0f + 1e-3f * (float)(threadIdx.x + j);
+    const float b = 1e-6f;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int j = 0; j < kFmaChains; ++j) x[j] = fmaf(x[j], a, b);
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int j = 0; j < kFmaChains; ++j) s += x[j];
+    if (s == 123.456f) *sink = s;   // never true: keeps the chains alive without a store per thread
+}
+
 namespace {
 
 thread_local std::string g_err_noctx;
@@ -426,6 +445,13 @@ int hpmc_create(const hpmc_box* box, const hpmc_shape* shape, int64_t N, uint64_
             g.n[k] = 2 * (int)std::floor(g.Ld[k] / (2.0 * c->d_max * (1.0 + 1.0 / 1024.0)));  // R11
             if (g.n[k] < 4) { delete c; return fail(nullptr, HPMC_E_GRID, "fewer than 4 cells per side (R11)"); }
             c->w[k] = g.Ld[k] / g.n[k];
+            {   // R11/R22: fl(fl(x - lo) - s) * inv_w misplaces a cell boundary by up to ~1.5 ulp of a coordinate difference just
+                // below L; two boundaries lie between particles of cells c and c + 2, which must stay >= d_max apart
+                int e = 0;
+                std::frexp(g.Ld[k], &e);                         // L = m 2^e, m in [0.5, 1)
+                const double ulp = std::ldexp(1.0, e - 24);      // fp32 ulp of values in [L/2, L)
+                if (3.0 * ulp > c->w[k] - c->d_max) { delete c; return fail(nullptr, HPMC_E_GRID, "box too large for fp32 coordinates at this particle size: cell slack below 3 ulp(L) (R11, R22)"); }
+            }
             g.w_f[k] = (float)c->w[k];
             g.inv_w[k] = (float)((double)g.n[k] / g.Ld[k]);
         } else {
@@ -444,6 +470,7 @@ int hpmc_create(const hpmc_box* box, const hpmc_shape* shape, int64_t N, uint64_
     {
         int dev = 0, sms = 0;
         if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess) c->num_sms = sms;
+        c->device = dev;
         if (c->num_sms <= 0) c->num_sms = 148;   // no device visible (CPU-side ABI checks): B200
     }
     c->mv.d = 0.1f; c->mv.a = 0.1f; c->mv.n_select = 4; c->mv.eps_g = 2e-6f;  // R15
@@ -479,6 +506,7 @@ size_t hpmc_workspace_bytes(const hpmc_ctx* c) { return c ? layout_of(c).total :
 
 int hpmc_bind(hpmc_ctx* c, float* d_pos4, float* d_quat4, void* d_workspace, size_t bytes)
 {
+    DeviceGuard dev_guard(c);
     if (!c) return HPMC_E_ARG;
     if (c->cuda_failed) return HPMC_E_CUDA;
     if (((!d_pos4 || !d_quat4) && c->g.N > 0) || !d_workspace) return fail(c, HPMC_E_ARG, "NULL device pointer");
@@ -511,6 +539,8 @@ int hpmc_bind(hpmc_ctx* c, float* d_pos4, float* d_quat4, void* d_workspace, siz
         init.t = c->t_host;
         if (!cuda_ok(c, cudaMemcpyAsync(c->ctrl, &init, sizeof init, cudaMemcpyHostToDevice, c->stream), "bind/memcpy")) return HPMC_E_CUDA;
         if (!cuda_ok(c, cudaStreamSynchronize(c->stream), "bind/sync")) return HPMC_E_CUDA;  // `init` is a stack object
+    } else if (!cuda_ok(c, cudaMemsetAsync(&c->ctrl->bad_coords, 0, sizeof(unsigned int), c->stream), "bind/memset")) {
+        return HPMC_E_CUDA;   // a new state: its coordinates are checked afresh
     }
     c->state_in_bound = true;
     c->have_sorted = false;
@@ -531,6 +561,7 @@ int hpmc_set_moves(hpmc_ctx* c, double d, double a, int n_select)
 
 int hpmc_sweep(hpmc_ctx* c, int64_t n)
 {
+    DeviceGuard dev_guard(c);
     int rc = check_ready(c);
     if (rc != HPMC_OK) return rc;
     if (n < 0) return fail(c, HPMC_E_ARG, "n must be >= 0");
@@ -590,6 +621,7 @@ int hpmc_sweep(hpmc_ctx* c, int64_t n)
 
 int hpmc_count_overlaps(hpmc_ctx* c, int64_t* h_count)
 {
+    DeviceGuard dev_guard(c);
     int rc = check_ready(c);
     if (rc != HPMC_OK) return rc;
     if (!h_count) return fail(c, HPMC_E_ARG, "h_count is NULL");
@@ -606,14 +638,18 @@ int hpmc_count_overlaps(hpmc_ctx* c, int64_t* h_count)
         LAUNCH_CHECK(c, "k_count_overlaps");
     }
     unsigned long long v = 0;
+    unsigned int bad = 0;
     if (!cuda_ok(c, cudaMemcpyAsync(&v, &c->ctrl->overlaps, sizeof v, cudaMemcpyDeviceToHost, c->stream), "count/memcpy")) return HPMC_E_CUDA;
+    if (!cuda_ok(c, cudaMemcpyAsync(&bad, &c->ctrl->bad_coords, sizeof bad, cudaMemcpyDeviceToHost, c->stream), "count/memcpy")) return HPMC_E_CUDA;
     if (!cuda_ok(c, cudaStreamSynchronize(c->stream), "count/sync")) return HPMC_E_CUDA;
     *h_count = (int64_t)v;
+    if (bad) return fail(c, HPMC_E_ARG, "the bound state holds coordinates that are not finite or not in [-L/2, L/2)");
     return HPMC_OK;
 }
 
 int hpmc_get_state(hpmc_ctx* c, float* d_pos4_out, float* d_quat4_out, hpmc_counters* h_counters, int64_t* h_sweep_counter)
 {
+    DeviceGuard dev_guard(c);
     int rc = check_ready(c);
     if (rc != HPMC_OK) return rc;
     if ((d_pos4_out || d_quat4_out) && c->g.N > 0) {
@@ -643,12 +679,14 @@ int hpmc_get_state(hpmc_ctx* c, float* d_pos4_out, float* d_quat4_out, hpmc_coun
             h_counters->rot_rej_overlap = sum[4]; h_counters->trials = sum[5]; h_counters->sweeps = h.sweeps;
         }
         if (h_sweep_counter) *h_sweep_counter = (int64_t)h.t;
+        if (h.bad_coords) return fail(c, HPMC_E_ARG, "the bound state holds coordinates that are not finite or not in [-L/2, L/2)");
     }
     return HPMC_OK;
 }
 
 int hpmc_set_sweep_counter(hpmc_ctx* c, uint64_t t)
 {
+    DeviceGuard dev_guard(c);
     if (!c) return HPMC_E_ARG;
     if (c->cuda_failed) return HPMC_E_CUDA;
     c->t_host = t;
@@ -664,6 +702,7 @@ int hpmc_set_sweep_counter(hpmc_ctx* c, uint64_t t)
 
 int hpmc_reset_counters(hpmc_ctx* c)
 {
+    DeviceGuard dev_guard(c);
     if (!c) return HPMC_E_ARG;
     if (c->cuda_failed) return HPMC_E_CUDA;
     if (!c->ctrl) return fail(c, HPMC_E_UNBOUND, "workspace not bound");
@@ -684,6 +723,7 @@ int hpmc_set_trace(hpmc_ctx* c, uint32_t* d_trace, int64_t capacity_words)
 int hpmc_get_cell_list(hpmc_ctx* c, uint64_t t, int32_t* d_cell_start, int32_t* d_member_tags, int32_t* d_cell_of_tag,
                        float* h_shift3, int32_t* h_colour_perm8)
 {
+    DeviceGuard dev_guard(c);
     int rc = check_ready(c);
     if (rc != HPMC_OK) return rc;
     const bool from_bound = c->state_in_bound;
@@ -711,11 +751,13 @@ int hpmc_get_cell_list(hpmc_ctx* c, uint64_t t, int32_t* d_cell_start, int32_t* 
 int hpmc_sweep_host(hpmc_ctx* c, const float* h_pos4, const float* h_quat4, int64_t n, float* h_pos4_out, float* h_quat4_out,
                     hpmc_counters* h_counters)
 {
+    DeviceGuard dev_guard(c);
     if (!c) return HPMC_E_ARG;
     if (c->cuda_failed) return HPMC_E_CUDA;
     if (!c->d_ws || !c->d_pos_bound) return fail(c, HPMC_E_UNBOUND, "state/workspace not bound");
     if (!h_pos4 || !h_quat4) return fail(c, HPMC_E_ARG, "NULL host pointer");
     const size_t bytes = (size_t)c->g.N * sizeof(float4);
+    if (!cuda_ok(c, cudaMemsetAsync(&c->ctrl->bad_coords, 0, sizeof(unsigned int), c->stream), "sweep_host/memset")) return HPMC_E_CUDA;
     if (!cuda_ok(c, cudaMemcpyAsync(c->d_pos_bound, h_pos4, bytes, cudaMemcpyHostToDevice, c->stream), "sweep_host/h2d")) return HPMC_E_CUDA;
     if (!cuda_ok(c, cudaMemcpyAsync(c->d_quat_bound, h_quat4, bytes, cudaMemcpyHostToDevice, c->stream), "sweep_host/h2d")) return HPMC_E_CUDA;
     c->state_in_bound = true;
@@ -733,6 +775,7 @@ int hpmc_sweep_host(hpmc_ctx* c, const float* h_pos4, const float* h_quat4, int6
 
 int hpmc_set_option(hpmc_ctx* c, const char* name, int64_t value)
 {
+    DeviceGuard dev_guard(c);
     if (!c || !name) return HPMC_E_ARG;
     const std::string n(name);
     graph_reset(c);
@@ -762,6 +805,7 @@ int hpmc_set_option(hpmc_ctx* c, const char* name, int64_t value)
 
 int hpmc_set_profile(hpmc_ctx* c, int on)
 {
+    DeviceGuard dev_guard(c);
     if (!c) return HPMC_E_ARG;
     if (c->cuda_failed) return HPMC_E_CUDA;
     if (!profile_fold(c)) return HPMC_E_CUDA;
@@ -773,6 +817,7 @@ int hpmc_set_profile(hpmc_ctx* c, int on)
 
 int hpmc_get_profile(hpmc_ctx* c, double* h_ms_build, int64_t* h_n_build, double* h_ms_colour, int64_t* h_n_colour)
 {
+    DeviceGuard dev_guard(c);
     if (!c) return HPMC_E_ARG;
     if (c->cuda_failed) return HPMC_E_CUDA;
     if (!profile_fold(c)) return HPMC_E_CUDA;
@@ -807,6 +852,7 @@ int hpmc_describe_pass(const hpmc_ctx* c, char* h_buf, size_t n)
 
 int hpmc_get_stat(hpmc_ctx* c, const char* name, int64_t* h_value)
 {
+    DeviceGuard dev_guard(c);
     int rc = check_ready(c);
     if (rc != HPMC_OK) return rc;
     if (!name || !h_value) return fail(c, HPMC_E_ARG, "NULL argument");
@@ -817,6 +863,36 @@ int hpmc_get_stat(hpmc_ctx* c, const char* name, int64_t* h_value)
     unsigned long long v = 0;
     for (int r = 0; r < kCounterSets; ++r) v += h.counters[r][6];
     *h_value = (int64_t)v;
+    return HPMC_OK;
+}
+
+int hpmc_measure_fp32_peak(hpmc_ctx* c, double* h_tflops)
+{
+    DeviceGuard dev_guard(c);
+    if (!c || !h_tflops) return HPMC_E_ARG;
+    if (c->cuda_failed) return HPMC_E_CUDA;
+    float* d_sink = nullptr;
+    cudaEvent_t e0, e1;
+    if (!cuda_ok(c, cudaMalloc(&d_sink, sizeof(float)), "peak/malloc")) return HPMC_E_CUDA;   // 4 bytes: the only allocation the library ever makes
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    const int threads = 256, blocks = c->num_sms * 8, iters = 8192;
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(e0, c->stream);
+        k_fma_peak<<<blocks, threads, 0, c->stream>>>(d_sink, iters, 1.0f + 1e-7f * (float)rep);
+        cudaEventRecord(e1, c->stream);
+        if (!cuda_ok(c, cudaEventSynchronize(e1), "peak/sync")) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double flops = 2.0 * kFmaChains * (double)iters * threads * blocks;
+        if (rep > 0 && ms > 0.f) best = std::max(best, flops / (ms * 1e-3) / 1e12);   // the first launch loads the kernel
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d_sink);
+    if (c->cuda_failed) return HPMC_E_CUDA;
+    *h_tflops = best;
     return HPMC_OK;
 }
 

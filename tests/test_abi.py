@@ -22,7 +22,7 @@ def lib():
 
 def test_header_symbols_all_exported(lib):
     hdr = open(os.path.join(ROOT, "include", "hpmc.h")).read()
-    declared = sorted(set(re.findall(r"\b(hpmc_[a-z_]+)\s*\(", hdr)))
+    declared = sorted(set(re.findall(r"\b(hpmc_[a-z0-9_]+)\s*\(", hdr)))
     assert declared == sorted(hb.ABI_SYMBOLS)
     for name in declared:
         assert getattr(lib, name) is not None
@@ -79,6 +79,11 @@ def test_create_rejects_bad_input(lib):
     assert _create(lib, 3, (10,) * 3, hb.KIND_POLYHEDRON, 4, verts=inner)[0] == -2                           # not a hull vertex
     assert _create(lib, 2, (10, 10), hb.KIND_POLYHEDRON, 4, verts=wl.cube_vertices(1.0))[0] == -2            # wrong dim
     assert b"" != lib.hpmc_last_error(None)
+    # R11/R22: from L ~ 6000 the fp32 rounding of cell_of (3 ulp(L)) exceeds the slack of the cell width for unit particles
+    assert _create(lib, 2, (4096.0, 4096.0), hb.KIND_POLYGON, 4, verts=wl.regular_polygon(5, 0.5))[0] == 0
+    assert _create(lib, 2, (8192.0, 8192.0), hb.KIND_POLYGON, 4, verts=wl.regular_polygon(5, 0.5))[0] == -3
+    assert b"fp32" in lib.hpmc_last_error(None)
+    assert _create(lib, 2, (8192.0, 8192.0), hb.KIND_DISK, 4, diameter=4.0)[0] == 0       # larger particles: larger slack
 
 
 def test_binding_fails_loudly_without_gpu():

@@ -353,3 +353,45 @@ def test_near_contact_cubes_match_the_oracle_and_take_the_fp64_rerun(gap, move):
     assert g.count_overlaps() == 0                                                    # the strict fp64 validator agrees
     assert marginal <= 0.02 * trials
     assert reruns > 0.1 * trials                                                      # the mixed-precision branch carries this case
+
+
+def test_out_of_box_and_non_finite_coordinates_are_reported_not_fatal():
+    """a coordinate outside [-L/2, L/2) or an inf used to index the histogram out of bounds.  Now the cell index is
+    clamped, the particle counted, and the next synchronising call reports HPMC_E_ARG; a fresh bind of a valid state works."""
+    from paper_1509_04692_b200 import binding as hb
+    for w in (wl.pentagons(24), wl.config(2) if False else wl.pentagons(200), wl.cubes(6)):   # single-CTA and multi-launch builds, 3-D
+        for bad_value in (0.75 * w.L[0], -3.0 * w.L[0], np.inf, np.nan):
+            g = gpu(w)
+            pos = w.pos4.copy()
+            pos[5, 0] = bad_value
+            g.bind(pos, w.quat4)
+            g.sweep(2)                                   # must not fault
+            with pytest.raises(hb.HpmcError):
+                g.count_overlaps()
+            g.bind(w.pos4, w.quat4)                      # a valid state clears the condition
+            g.sweep(2)
+            assert g.count_overlaps() == 0
+
+
+def test_dataflow_pass_with_many_tiles_and_partial_edges_matches_per_colour_launches():
+    """every other forced-dataflow case has 1-4 tiles per colour.  256 x 160 pentagons with the 2-warp tile shape:
+    64 x 79 active cells per colour = 2 x 40 tiles with a partial last tile in x and in y, more (colour, tile) tickets than the
+    GPU holds CTAs at once is not reached at this size, but tiles do wait on the stamps of their nine neighbours; 20 sweeps,
+    including CUDA-graph replay, bit for bit against one launch per colour."""
+    base = wl.pentagons(256)
+    ny = 160
+    keep = np.arange(256 * ny)
+    L = (256.0, float(ny))
+    pos = base.pos4[keep].copy()
+    pos[:, 1] += 0.5 * (256.0 - ny)                      # rows 0..159 recentred in the shorter box
+    w = wl.Workload(name="pentagons_256x160", dim=2, N=256 * ny, L=L, kind=base.kind, diameter=0.0, verts=base.verts, d=base.d,
+                    a=base.a, n_select=4, sweeps=1, pos4=pos, quat4=base.quat4[keep].copy())
+    out = []
+    for flow in (1, 0):
+        g = gpu(w)
+        assert g.count_overlaps() == 0
+        g.set_option("tile_shape", 3); g.set_option("flow", flow)
+        g.sweep(1); g.sweep(19)
+        out.append((g.get_state(), g.counters()))
+        assert g.count_overlaps() == 0
+    assert np.array_equal(out[0][0][0], out[1][0][0]) and np.array_equal(out[0][0][1], out[1][0][1]) and out[0][1] == out[1][1]
