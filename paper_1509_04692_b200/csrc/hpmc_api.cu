@@ -448,7 +448,7 @@ int hpmc_create(const hpmc_box* box, const hpmc_shape* shape, int64_t N, uint64_
             {   // R11/R22: fl(fl(x - lo) - s) * inv_w misplaces a cell boundary by up to ~1.5 ulp of a coordinate difference just
                 // below L; two boundaries lie between particles of cells c and c + 2, which must stay >= d_max apart
                 int e = 0;
-                std::frexp(g.Ld[k], &e);                         // L = m 2^e, m in [0.5, 1)
+                std::frexp(std::nextafter(g.Ld[k], 0.0), &e);     // the largest coordinate difference below L = m 2^e, m in [0.5, 1)
                 const double ulp = std::ldexp(1.0, e - 24);      // fp32 ulp of values in [L/2, L)
                 if (3.0 * ulp > c->w[k] - c->d_max) { delete c; return fail(nullptr, HPMC_E_GRID, "box too large for fp32 coordinates at this particle size: cell slack below 3 ulp(L) (R11, R22)"); }
             }
