@@ -7,15 +7,17 @@
 
 namespace hpmc {
 
-constexpr int kScanThreads = 1024;
+constexpr int kScanThreads = 256;
 constexpr int kScanItems = 16;
 constexpr int kScanTile = kScanThreads * kScanItems;
+constexpr int kHistItems = 4;     // particles per thread of k_hist
+constexpr int kFusedSpineMax = 1024;   // up to this many scan tiles k_scan_final adds up the preceding tile totals itself (no spine launch)
 
 // Three to five launches build the cell list of a sweep:
 //   k_hist          header (a0, a1) + cell id and arrival rank of every particle (a2, first half of a3)
 //   k_scan_*        exclusive scan of the per-cell counts (one launch when the grid fits one tile of 16 384 counts, else
 //                   reduce / spine / final), zeroes the counts for the next build, advances the sweep counter
-//   k_scatter_sort  scatter into the cell-sorted SoA; the last particle to arrive in a cell puts the cell's members in
+//   k_scatter       scatter into the cell-sorted SoA; k_sort_cells then puts the members of every cell in
 //                   ascending tag order (R8)
 // mode 0: header of the device sweep counter t; k_scan then does t++ and sweeps++   (a real sweep)
 // mode 1: header of t_override, nothing advanced                                     (debug cell list)
@@ -35,15 +37,31 @@ __global__ void k_hist(const __grid_constant__ GridParams g, Control* __restrict
         if (blockIdx.x == 0) ctrl->hdr = sh;
     }
     __syncthreads();
-    const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= g.N) return;
     const float shift[3] = {sh.shift[0], sh.shift[1], sh.shift[2]};
-    const float4 x = pos[p];
-    bool bad;
-    const int c = cell_of_checked(g, shift, x.x, x.y, (g.dim == 3) ? x.z : 0.0f, bad);
-    if (bad) atomicAdd(&ctrl->bad_coords, 1u);
-    const int rank = atomicAdd(&counts[c], 1);
-    key_rank[p] = make_int2(c, rank);
+    // kHistItems particles per thread, a block-wide stride apart (coalesced): their loads and their atomics are in flight together
+    const int base = blockIdx.x * (blockDim.x * kHistItems) + threadIdx.x;
+    float4 x[kHistItems];
+    int c[kHistItems], rank[kHistItems];
+#pragma unroll
+    for (int j = 0; j < kHistItems; ++j) {
+        const int p = base + j * blockDim.x;
+        if (p < g.N) x[j] = pos[p];
+    }
+#pragma unroll
+    for (int j = 0; j < kHistItems; ++j) {
+        const int p = base + j * blockDim.x;
+        if (p < g.N) {
+            bool bad;
+            c[j] = cell_of_checked(g, shift, x[j].x, x[j].y, (g.dim == 3) ? x[j].z : 0.0f, bad);
+            if (bad) atomicAdd(&ctrl->bad_coords, 1u);
+            rank[j] = atomicAdd(&counts[c[j]], 1);
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < kHistItems; ++j) {
+        const int p = base + j * blockDim.x;
+        if (p < g.N) key_rank[p] = make_int2(c[j], rank[j]);
+    }
 }
 
 __device__ __forceinline__ int warp_inclusive_scan(int v)
@@ -128,8 +146,9 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_spine(int* __restrict__ t
     }
 }
 
-// exclusive scan inside each tile plus the tile's offset; re-zeroes the counts for the next build.  single != 0: the whole
-// grid is one tile (no reduce/spine pass ran), so this kernel also advances the sweep counter.
+// exclusive scan inside each tile plus the tile's offset; re-zeroes the counts for the next build.  single = 1: the whole grid
+// is one tile (no reduce pass ran); single = 2: the reduce pass ran but no spine -- the block sums the preceding tile totals
+// itself; in both cases this kernel also advances the sweep counter.  single = 0: tile_sums holds the spine's prefix.
 __global__ void __launch_bounds__(kScanThreads)
 k_scan_final(int* __restrict__ counts, int n, int* __restrict__ cell_start, const int* __restrict__ tile_sums, int single,
              Control* __restrict__ ctrl, int mode)
@@ -153,8 +172,25 @@ k_scan_final(int* __restrict__ counts, int n, int* __restrict__ cell_start, cons
         carry += __shfl_sync(0xffffffffu, inc, 31);
     }
     if (lane == 0) s_wsum[warp] = carry;
+    // offset of this tile: nothing (one tile), the spine's exclusive prefix, or -- fused -- the sum of the preceding tile totals,
+    // added up here by the block itself (a few hundred L2-resident values: cheaper than a launch of its own)
+    __shared__ int s_tile_off;
+    if (single == 2) {
+        int part = 0;
+        for (int i = threadIdx.x; i < (int)blockIdx.x; i += kScanThreads) part += tile_sums[i];
+        part = __reduce_add_sync(0xffffffffu, part);
+        __shared__ int s_psum[kScanThreads / 32];
+        if (lane == 0) s_psum[warp] = part;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int t = 0;
+#pragma unroll
+            for (int w = 0; w < kScanThreads / 32; ++w) t += s_psum[w];
+            s_tile_off = t;
+        }
+    }
     __syncthreads();
-    int off = single ? 0 : tile_sums[blockIdx.x];
+    int off = (single == 1) ? 0 : (single == 2) ? s_tile_off : tile_sums[blockIdx.x];
 #pragma unroll
     for (int w = 0; w < kScanThreads / 32; ++w)
         if (w < warp) off += s_wsum[w];
@@ -163,25 +199,22 @@ k_scan_final(int* __restrict__ counts, int n, int* __restrict__ cell_start, cons
         const int idx = wbase + 32 * k;
         if (idx <= n) cell_start[idx] = off + ex[k];
     }
-    if (single && mode == 0 && threadIdx.x == 0) {
+    if (single && mode == 0 && threadIdx.x == 0 && blockIdx.x == 0) {
         ctrl->t += 1ull;
         ctrl->sweeps += 1ull;
     }
 }
 
 // second half of a3: scatter into the cell-sorted SoA.  src_tag == nullptr: source is the caller's tag-order pos4/quat4;
-// otherwise the source is the other sorted buffer (2-D: poses only).  In a cell with several members the LAST particle to
-// arrive (counted in `arrived`, which it resets) sorts the members by tag (R8), whatever order the atomics produced.
-__global__ void k_scatter_sort(int N, int dim, const float4* __restrict__ src_pos, const float4* __restrict__ src_quat,
-                               const int* __restrict__ src_tag, const int2* __restrict__ key_rank,
-                               const int* __restrict__ cell_start, int* __restrict__ arrived, float4* dst_pos, float4* dst_quat,
-                               int* dst_tag)
+// otherwise the source is the other sorted buffer (2-D: poses only).  Members of a cell land in arrival order (k_sort_cells).
+__global__ void k_scatter(int N, int dim, const float4* __restrict__ src_pos, const float4* __restrict__ src_quat,
+                          const int* __restrict__ src_tag, const int2* __restrict__ key_rank, const int* __restrict__ cell_start,
+                          float4* __restrict__ dst_pos, float4* __restrict__ dst_quat, int* __restrict__ dst_tag)
 {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= N) return;
     const int2 kr = key_rank[p];
-    const int s = cell_start[kr.x], cnt = cell_start[kr.x + 1] - s;
-    const int dst = s + kr.y;
+    const int dst = cell_start[kr.x] + kr.y;
     const float4 P = src_pos[p];
     if (dim == 2) {
         if (src_tag) dst_pos[dst] = P;
@@ -194,34 +227,39 @@ __global__ void k_scatter_sort(int N, int dim, const float4* __restrict__ src_po
         dst_quat[dst] = src_quat[p];
     }
     dst_tag[dst] = src_tag ? src_tag[p] : p;
-    if (cnt < 2) return;
-    __threadfence();
-    if (atomicAdd(&arrived[kr.x], 1) != cnt - 1) return;
-    __threadfence();
-    arrived[kr.x] = 0;
-    // insertion sort of the cell by tag; loads bypass L1 (other SMs wrote these lines during this kernel)
-    for (int i = s + 1; i < s + cnt; ++i) {
-        const int ti = __ldcg(&dst_tag[i]);
+}
+
+// last quarter of a3 (R8): one thread per cell puts the members of a multiply-occupied cell in ascending tag, whatever order
+// the atomics of k_hist produced.  A launch of its own: the scatter's stores are then visible without fences, the cells of
+// neighbouring threads are neighbours in memory, and no thread spins through dependent L2 loads while its warp waits
+// (measured on 1 M pentagons: scatter + sort 9.8 + ~5 us against 25 us for the scatter whose last arrival sorted the cell).
+__global__ void k_sort_cells(int C, int dim, const int* __restrict__ cell_start, float4* pos, float4* quat, int* tag)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= C) return;
+    const int s = cell_start[c], e = cell_start[c + 1];
+    for (int i = s + 1; i < e; ++i) {
+        const int ti = tag[i];
         int j = i - 1;
-        if (__ldcg(&dst_tag[j]) <= ti) continue;
-        const float4 pi = __ldcg(&dst_pos[i]);
+        if (tag[j] <= ti) continue;
+        const float4 pi = pos[i];
         float4 qi = pi;
-        if (dim == 3) qi = __ldcg(&dst_quat[i]);
-        while (j >= s && __ldcg(&dst_tag[j]) > ti) {
-            dst_tag[j + 1] = __ldcg(&dst_tag[j]);
-            dst_pos[j + 1] = __ldcg(&dst_pos[j]);
-            if (dim == 3) dst_quat[j + 1] = __ldcg(&dst_quat[j]);
+        if (dim == 3) qi = quat[i];
+        while (j >= s && tag[j] > ti) {
+            tag[j + 1] = tag[j];
+            pos[j + 1] = pos[j];
+            if (dim == 3) quat[j + 1] = quat[j];
             --j;
         }
-        dst_tag[j + 1] = ti;
-        dst_pos[j + 1] = pi;
-        if (dim == 3) dst_quat[j + 1] = qi;
+        tag[j + 1] = ti;
+        pos[j + 1] = pi;
+        if (dim == 3) quat[j + 1] = qi;
     }
 }
 
 // Small systems (configs 0, 1): the whole cell-list build in ONE CTA -- header, histogram in shared memory, scan, scatter,
 // in-cell tag sort -- instead of three launches whose latencies and gaps are a third of such a sweep.  Same results as the
-// k_hist / k_scan_final / k_scatter_sort sequence (the arrival ranks differ, the sorted result does not).  Dynamic shared
+// k_hist / k_scan_final / k_scatter / k_sort_cells sequence (the arrival ranks differ, the sorted result does not).  Dynamic shared
 // memory: (C + 2) ints.  `counts` and `arrived` are not touched (they stay all-zero).
 constexpr int kSmallBuildThreads = 1024;
 constexpr int kSmallBuildMaxCells = 11500;    // (C + 2) * 4 bytes of shared memory <= 46 KB

@@ -272,21 +272,27 @@ int build_cell_list(hpmc_ctx* c, int mode, unsigned long long t_override)
         return HPMC_OK;
     }
     const int nblk_part = (g.N + TB - 1) / TB;
-    k_hist<<<nblk_part > 0 ? nblk_part : 1, TB, 0, c->stream>>>(g, c->ctrl, src_pos, c->counts, c->key_rank, c->k0, c->k1, mode, t_override);
+    const int nblk_hist = (g.N + TB * kHistItems - 1) / (TB * kHistItems);
+    k_hist<<<nblk_hist > 0 ? nblk_hist : 1, TB, 0, c->stream>>>(g, c->ctrl, src_pos, c->counts, c->key_rank, c->k0, c->k1, mode, t_override);
     LAUNCH_CHECK(c, "k_hist");
     const int tiles = scan_tiles(c);
+    const bool fused = tiles > 1 && tiles <= kFusedSpineMax;
     if (tiles > 1) {
         k_scan_reduce<<<tiles, kScanThreads, 0, c->stream>>>(c->counts, g.C, c->tile_sums);
         LAUNCH_CHECK(c, "k_scan_reduce");
-        k_scan_spine<<<1, kScanThreads, 0, c->stream>>>(c->tile_sums, tiles, c->ctrl, mode);
-        LAUNCH_CHECK(c, "k_scan_spine");
+        if (!fused) {
+            k_scan_spine<<<1, kScanThreads, 0, c->stream>>>(c->tile_sums, tiles, c->ctrl, mode);
+            LAUNCH_CHECK(c, "k_scan_spine");
+        }
     }
-    k_scan_final<<<tiles, kScanThreads, 0, c->stream>>>(c->counts, g.C, c->cell_start, c->tile_sums, tiles == 1, c->ctrl, mode);
+    k_scan_final<<<tiles, kScanThreads, 0, c->stream>>>(c->counts, g.C, c->cell_start, c->tile_sums, tiles == 1 ? 1 : fused ? 2 : 0, c->ctrl, mode);
     LAUNCH_CHECK(c, "k_scan_final");
     if (g.N > 0) {
-        k_scatter_sort<<<nblk_part, TB, 0, c->stream>>>(g.N, g.dim, src_pos, src_quat, src_tag, c->key_rank, c->cell_start, c->arrived,
-                                                       c->pos[dst], c->quat[dst], c->tag[dst]);
-        LAUNCH_CHECK(c, "k_scatter_sort");
+        k_scatter<<<nblk_part, TB, 0, c->stream>>>(g.N, g.dim, src_pos, src_quat, src_tag, c->key_rank, c->cell_start, c->pos[dst], c->quat[dst],
+                                                  c->tag[dst]);
+        LAUNCH_CHECK(c, "k_scatter");
+        k_sort_cells<<<(g.C + TB - 1) / TB, TB, 0, c->stream>>>(g.C, g.dim, c->cell_start, c->pos[dst], c->quat[dst], c->tag[dst]);
+        LAUNCH_CHECK(c, "k_sort_cells");
     }
     c->cur = dst;
     c->state_in_bound = false;
