@@ -34,15 +34,39 @@ UNIT = "trial moves/s"
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # SMs x FP32 lanes x 2 (FMA) x max SM clock
 HBM_FALLBACK_GBS = 6650.0                               # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 
-# Algorithmic work per trial (tariff of SURVEY.md 8(d) x the oracle's O7 work counters on
-# the melted state of each workload): flops per trial.
-ALGO_FLOPS = {
-    wl.KIND_DISK: 10 + 8 + 8 * 4.08,
-    wl.KIND_POLYGON: 20 + 4 + 8 * 6.94 + 1.83 * 180.0,
-    wl.KIND_POLYHEDRON: 35 + 6 + 11 * 68.0 + 8.12 * 1500.0,
-}
-# ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (profiles/r1_v4.md)
-NCU_TRAFFIC = {"k2_pentagons_1M": 21.1e6}
+# Algorithmic work per trial: the flop tariff of SURVEY.md 8(d)-F applied to the oracle's O7 work counters
+# on the melted state of each state point -- candidates scanned, narrow-phase tests, separating axes per polygon test, GJK
+# support calls per polyhedron test, all in early-exit serial order -- read from tests/golden/oracle_expectations.json (a data
+# file written by tests/golden/make_oracle_expectations.py from the oracle alone; nothing of the oracle is executed here).
+WORK_KEY = {0: "k0_disks", 1: "k1_pentagons", 2: "k1_pentagons", 3: "k3_cubes", 4: "k1_pentagons"}
+
+
+def algo_flops_per_trial(k, w):
+    """FMA = 2, compare/min/max = 1, RNG and integer work not counted."""
+    wk = json.load(open(os.path.join(ROOT, "tests", "golden", "oracle_expectations.json")))["work"][WORK_KEY[k]]
+    rot = wk["rotate_fraction"]
+    gen = (1.0 - rot) * 10.0 + rot * (30.0 if w.dim == 2 else 60.0)            # trial generation
+    leave = (1.0 - rot) * 4.0 * w.dim                                          # leave-cell test (translations)
+    broad = (3.0 * w.dim + 2.0) * wk["candidates_scanned_per_trial"]           # subtract, dot, compare per candidate
+    if w.kind == wl.KIND_DISK:
+        narrow, per_test = 0.0, 0.0                                            # the broad phase is the whole test (P:89)
+    elif w.kind == wl.KIND_POLYGON:
+        nv = w.verts.shape[0]
+        axes = wk["polygon_axes_per_narrow_test"]                              # A's normals first, then B's, to the first that separates
+        per_test = 14.0 * nv + (4.0 * nv + 1.0) * min(axes, nv) + (4.0 * nv + 3.0) * max(axes - nv, 0.0)
+        narrow = wk["narrow_tests_per_trial"] * per_test
+    else:
+        nv = w.verts.shape[0]
+        support = 10.0 * nv + 48.0 + 6.0 + 2.0 * nv                            # Eq. (2): two vertex scans, two rotations, argmax compares
+        per_test = wk["gjk_support_calls_per_narrow_test"] * (support + 60.0)  # + simplex update per iteration
+        narrow = wk["narrow_tests_per_trial"] * per_test
+    return {"flops_per_trial": gen + leave + broad + narrow, "trial_generation": gen, "leave_cell": leave, "broad_phase": broad,
+            "narrow_phase": narrow, "flops_per_narrow_test": per_test, "oracle_work": wk}
+
+
+# ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per colour pass of the dominant kernel, round-2 kernels
+# (profiles/r2_final.md lists the captures; a dataflow / whole-sweep launch is divided by the passes it covers)
+NCU_TRAFFIC = {}
 
 
 def state_bytes(w):
@@ -121,12 +145,51 @@ class ClockSampler:
         return out
 
 
+def roofline_of(k, w, g, prof, counters, steps, total_ms, fp32_measured):
+    """The roofline object of the dominant kernel (the colour pass) for one timed window: DESIGN.md section 7."""
+    acc = counters["trans_acc"] + counters["rot_acc"]
+    trials = counters["trials"]
+    colour_ms = prof["colour_ms"] / max(prof["colour_n"], 1)
+    trials_per_launch = trials / max(prof["colour_n"], 1)
+    acc_per_sweep = acc / steps
+    hbm, hbm_src = hbm_peak()
+    work = algo_flops_per_trial(k, w)
+    fp32_peak = fp32_measured if fp32_measured and fp32_measured > 0 else FP32_PEAK_TFLOPS
+    bytes_launch = colour_pass_bytes(w, g.C, acc_per_sweep)
+    flops_launch = work["flops_per_trial"] * trials_per_launch
+    t_hbm = bytes_launch / (hbm * 1e9)
+    t_alu = flops_launch / (fp32_peak * 1e12)
+    if t_hbm >= t_alu:
+        roof = {"bound": "hbm", "achieved": bytes_launch / (colour_ms * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
+                "peak_source": f"{hbm_src} hbm_gbs (MEASURED_PEAKS.json)"}
+    else:
+        roof = {"bound": "alu", "achieved": flops_launch / (colour_ms * 1e-3) / 1e12, "peak": fp32_peak, "unit": "TFLOP/s",
+                "peak_source": "pure-FMA microkernel timed in this run (hpmc_measure_fp32_peak)" if fp32_measured else
+                               "nominal 148 SM x 128 lanes x 2 x 1.965 GHz"}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    whole = prof["colour_ms"] + prof["build_ms"]
+    roof.update({"traffic": NCU_TRAFFIC.get(w.name), "kernel": g.describe_pass(), "avg_launch_ms": colour_ms,
+                 "avg_launch_ms_note": "per colour pass; a launch that covers several passes is counted as that many",
+                 "launches_timed": prof["colour_n"], "fp32_peak_measured": fp32_measured, "fp32_peak_nominal": FP32_PEAK_TFLOPS,
+                 "algorithmic_bytes_per_launch": bytes_launch, "algorithmic_flops_per_launch": flops_launch,
+                 "algorithmic_flops_per_trial": work["flops_per_trial"],
+                 "flops_breakdown": {q: work[q] for q in ("trial_generation", "leave_cell", "broad_phase", "narrow_phase", "flops_per_narrow_test")},
+                 "oracle_work_counters": {q: work["oracle_work"][q] for q in ("sample", "candidates_scanned_per_trial", "narrow_tests_per_trial",
+                                                                              "polygon_axes_per_narrow_test", "gjk_support_calls_per_narrow_test")},
+                 "kernel_share_of_step": prof["colour_ms"] / total_ms, "build_share_of_step": prof["build_ms"] / total_ms,
+                 "sweep_frac": max(algorithmic_bytes_per_sweep(w, g.C, acc_per_sweep) / (hbm * 1e9),
+                                   work["flops_per_trial"] * trials / steps / (fp32_peak * 1e12)) / (total_ms * 1e-3 / steps),
+                 "hbm_time_us": 1e6 * t_hbm, "fp32_time_us": 1e6 * t_alu, "profiled_ms_per_step": whole / steps})
+    return roof
+
+
 def time_gpu(w, seed, device, steps, warmup, flush, dist_ctx):
     """W untimed + K timed hpmc_sweep(1) steps on one replica; returns a dict of raw measurements."""
     import torch
     from paper_1509_04692_b200 import binding as hb
     g = hb.from_workload(w, seed=seed, device=device)
     assert g.count_overlaps() == 0, "initial state has overlaps"
+    fp32_peak = g.measure_fp32_peak()              # the FP32 roofline denominator, measured on this GPU in this run
     g.sweep(w.warmup_sweeps)                       # melt the lattice (setup, DESIGN.md section 6), untimed
     stream = g.stream
     fbuf = torch.empty(256 << 20, dtype=torch.uint8, device=device) if flush else None
@@ -161,7 +224,7 @@ def time_gpu(w, seed, device, steps, warmup, flush, dist_ctx):
     c = g.counters()
     launches = g.launch_count() - l0
     assert g.count_overlaps() == 0, "overlaps after the timed window"
-    return dict(g=g, ms=ms, wall_s=t_wall, counters=c, prof=prof, launches=launches, clocks=clocks)
+    return dict(g=g, ms=ms, wall_s=t_wall, counters=c, prof=prof, launches=launches, clocks=clocks, fp32_peak=fp32_peak)
 
 
 def time_e2e(g, w, steps, device):
@@ -186,17 +249,6 @@ def time_e2e(g, w, steps, device):
     return dict(seconds=t, trials=trials, h2d=nbytes, d2h=nbytes + 56)
 
 
-def oracle_rate(w_sample, sweeps, seed=1):
-    from oracle import hpmc_oracle as ho
-    o = ho.Oracle(w_sample.dim, w_sample.L, w_sample.kind, w_sample.N, seed, diameter=w_sample.diameter, verts=w_sample.verts)
-    o.set_moves(w_sample.d, w_sample.a, w_sample.n_select)
-    o.set_state(w_sample.pos4, w_sample.quat4)
-    t = time.perf_counter()
-    o.sweeps(sweeps)
-    t = time.perf_counter() - t
-    return o.counters()["trials"], t, o
-
-
 def sample_of(k, n_lat):
     """A smaller system at the same state point (same lattice recipe, density, shape, moves) as config k."""
     if k == 0:
@@ -206,45 +258,67 @@ def sample_of(k, n_lat):
     return wl.pentagons(n_lat, name=f"pentagons_{n_lat * n_lat}_sample")
 
 
+def make_oracle(ws, threads, seed=1):
+    from oracle import hpmc_oracle as ho
+    o = ho.Oracle(ws.dim, ws.L, ws.kind, ws.N, seed, diameter=ws.diameter, verts=ws.verts)
+    o.set_moves(ws.d, ws.a, ws.n_select)
+    o.set_state(ws.pos4, ws.quat4)
+    o.set_threads(threads)
+    return o
+
+
+def timed_oracle_sweeps(o, sweeps):
+    o.reset_counters()
+    t = time.perf_counter()
+    o.sweeps(sweeps)
+    t = time.perf_counter() - t
+    return o.counters()["trials"], t
+
+
+def cpu_baseline(k, w):
+    """The oracle as it stands (oracle/, fp64 C), timed on this box's host cores on a bounded sample of the workload: a smaller
+    system at the same state point, melted first (untimed) like the GPU's, then (i) one thread -- the oracle's definition -- and
+    (ii) all cores, the cells of one colour as a parallel-for (identical results)."""
+    cores = os.cpu_count() or 1
+    n_lat, melt, n1, nall = {0: (64, 200, 60, 300), 1: (64, 200, 60, 300), 2: (256, 50, 12, 60), 3: (12, 100, 12, 60),
+                             4: (256, 10, 12, 60)}[k]
+    ws = sample_of(k, n_lat)
+    o = make_oracle(ws, cores)
+    o.sweeps(melt)
+    o.set_threads(1)
+    tr1, t1 = timed_oracle_sweeps(o, n1)
+    o.set_threads(cores)
+    tra, ta = timed_oracle_sweeps(o, nall)
+    what = f"{ws.name}: N={ws.N} at the state point of {w.name}, melted by {melt} sweeps (as the GPU run)"
+    return {"value": tr1 / t1, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": t1, "sample": f"{what}; {n1} sweeps on one thread",
+            "all_cores": {"value": tra / ta, "unit": UNIT, "cores": cores, "seconds": ta,
+                          "sample": f"{what}; {nall} sweeps, same-colour cells as an OpenMP parallel-for over {cores} threads"},
+            "host_cores_available": cores}
+
+
 def run_reference(args):
-    """The oracle as it stands on the host cores: each step = one oracle sweep of a bounded sample of the workload."""
+    """The reference arm: the oracle as it stands on ALL host cores of the box (the cells of one colour as a parallel-for,
+    results identical to the serial run), one oracle sweep per step on the config's own system -- configs 0-3 in full, config 4
+    on a 1024 x 1024 sample at the same state point (a full sweep of 16.8 M particles is ~67 M fp64 trials: minutes per step)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     k = args.config
-    full = wl.config(k) if k in (0, 1, 3) else None
-    total_steps = args.steps + args.warmup
-    # size the sample so that the whole run stays within ~2 minutes at the oracle's ~0.5 M pentagon trials/s
-    budget_trials = {0: 3.0e6, 1: 0.6e6, 2: 0.6e6, 3: 0.04e6, 4: 0.6e6}[k] * 100.0
-    per_step = budget_trials / total_steps
-    if k in (1, 2, 4):
-        n_full = {1: 64, 2: 1024, 4: 4096}[k]
-        n_lat = int(min(n_full, max(32, np.sqrt(per_step / 4.0)))) // 2 * 2
-        ws = sample_of(k, n_lat)
-    elif k == 0:
-        n_lat = int(min(64, max(16, np.sqrt(per_step / 4.0)))) // 2 * 2
-        ws = sample_of(0, n_lat)
-    else:
-        n_lat = int(min(32, max(6, (per_step / 1.3) ** (1.0 / 3.0))))
-        ws = sample_of(3, n_lat)
-    from oracle import hpmc_oracle as ho
-    o = ho.Oracle(ws.dim, ws.L, ws.kind, ws.N, 1, diameter=ws.diameter, verts=ws.verts)
-    o.set_moves(ws.d, ws.a, ws.n_select)
-    o.set_state(ws.pos4, ws.quat4)
+    cores = os.cpu_count() or 1
+    full = wl.config(k)
+    ws = full if k != 4 else sample_of(4, 1024)
+    o = make_oracle(ws, cores)
     o.sweeps(args.warmup)
-    o.reset_counters()
-    t = time.perf_counter()
-    o.sweeps(args.steps)
-    t = time.perf_counter() - t
-    trials = o.counters()["trials"]
+    trials, t = timed_oracle_sweeps(o, args.steps)
     v = trials / t
-    wname = wl.config(k).name if full is not None else {2: "k2_pentagons_1M", 4: "k4_pentagons_16M"}[k]
-    sample = f"{ws.name}: N={ws.N} particles at the state point of {wname}; {args.steps} oracle sweeps after {args.warmup} warm-up sweeps"
+    sample = (f"{ws.name}: N={ws.N}" + ("" if k != 4 else f" at the state point of {full.name}") +
+              f"; {args.steps} oracle sweeps after {args.warmup} warm-up sweeps from the lattice start; same-colour cells as an OpenMP "
+              f"parallel-for over {cores} threads")
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": wname, "sample": sample},
-            "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "config": {"workload": full.name, "N": ws.N, "same_system_as_gpu_arm": k != 4, "sample": sample},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "particle_sweeps_per_sec": ws.N * args.steps / t}
     print(json.dumps(line), flush=True)
@@ -285,29 +359,7 @@ def main():
     acc = r["counters"]["trans_acc"] + r["counters"]["rot_acc"]
     trials = r["counters"]["trials"]
 
-    # roofline of the dominant kernel (the colour pass): DESIGN.md section 7
-    prof = r["prof"]
-    colour_ms = prof["colour_ms"] / max(prof["colour_n"], 1)
-    trials_per_launch = trials / max(prof["colour_n"], 1)
-    acc_per_sweep = acc / args.steps
-    hbm, hbm_src = hbm_peak()
-    bytes_launch = colour_pass_bytes(w, g.C, acc_per_sweep)
-    flops_launch = ALGO_FLOPS[w.kind] * trials_per_launch
-    t_hbm = bytes_launch / (hbm * 1e9)
-    t_alu = flops_launch / (FP32_PEAK_TFLOPS * 1e12)
-    if t_hbm >= t_alu:
-        roof = {"bound": "hbm", "achieved": bytes_launch / (colour_ms * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s"}
-    else:
-        roof = {"bound": "alu", "achieved": flops_launch / (colour_ms * 1e-3) / 1e12, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s"}
-    roof["frac"] = roof["achieved"] / roof["peak"]
-    roof.update({"traffic": NCU_TRAFFIC.get(w.name), "kernel": g.describe_pass(), "avg_launch_ms": colour_ms,
-                 "avg_launch_ms_note": "per colour pass; a dataflow launch covers 4 passes and is counted as 4", "launches_timed": prof["colour_n"],
-                 "peak_source": f"{hbm_src} hbm_gbs (MEASURED_PEAKS.json)" if roof["bound"] == "hbm" else "148 SM x 128 lanes x 2 x 1.965 GHz",
-                 "algorithmic_bytes_per_launch": bytes_launch, "algorithmic_flops_per_launch": flops_launch,
-                 "kernel_share_of_step": prof["colour_ms"] / r["ms"], "build_share_of_step": prof["build_ms"] / r["ms"],
-                 "sweep_frac": max(algorithmic_bytes_per_sweep(w, g.C, acc_per_sweep) / (hbm * 1e9),
-                                   ALGO_FLOPS[w.kind] * trials / args.steps / (FP32_PEAK_TFLOPS * 1e12)) / (r["ms"] * 1e-3 / args.steps),
-                 "hbm_time_us": 1e6 * t_hbm, "fp32_time_us": 1e6 * t_alu})
+    roof = roofline_of(k, w, g, r["prof"], r["counters"], args.steps, r["ms"], r["fp32_peak"])
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -328,17 +380,11 @@ def main():
         e_trials = D.reduce(e["trials"], "SUM")
         line["e2e"] = {"value": e_trials / e_t, "unit": UNIT, "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"],
                        "steps": min(args.steps, 20), "call": "hpmc_sweep_host(n=1), pinned host buffers"}
+    fp32_peak_run = r["fp32_peak"]
     del g, r
     if not args.no_extras and D.rank == 0:
         if args.gpus == 1:
-            # the oracle as it stands, one host thread, on a bounded sample of the same workload
-            n_lat = {0: 64, 1: 64, 2: 256, 3: 8, 4: 256}[k]
-            ws = sample_of(k, n_lat)
-            ns = {0: 100, 1: 100, 2: 40, 3: 20, 4: 40}[k]
-            tr, ts, _ = oracle_rate(ws, ns)
-            line["cpu_baseline"] = {"value": tr / ts, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": ts,
-                                    "host_cores_available": os.cpu_count(),
-                                    "sample": f"{ws.name}: N={ws.N} at the state point of {w.name}, {ns} sweeps from the lattice start"}
+            line["cpu_baseline"] = cpu_baseline(k, w)
         if k == 2:
             # north_star also quotes 4096 pentagons; 65 536 pentagons is the per-GPU size of the paper's own benchmark.
             # Both are latency-bound, L2-resident by size, and timed as one hpmc_sweep(1000) call (CUDA-graph replay).
@@ -357,8 +403,16 @@ def main():
                 msx = s.elapsed_time(e2)
                 cx = gx.counters()
                 assert gx.count_overlaps() == 0
+                # the colour-pass launches of the same system bracketed one by one (plain launches, no graph) for its roofline
+                gx.reset_counters(); gx.set_profile(True)
+                for _ in range(200):
+                    gx.sweep(1)
+                px = gx.get_profile(); gx.set_profile(False)
+                rx = roofline_of(1, wx, gx, px, gx.counters(), 200, px["colour_ms"] + px["build_ms"], fp32_peak_run)
+                rx["sweep_frac"] *= (px["colour_ms"] + px["build_ms"]) / 200 / (msx / 1000)     # against the graph-replay time per sweep
                 line["also"][label] = {"value": cx["trials"] / (msx * 1e-3), "unit": UNIT, "sweeps": 1000, "ms_per_sweep": msx / 1000,
-                                       "particle_sweeps_per_sec": wx.N * 1000 / (msx * 1e-3), "kernel": gx.describe_pass(), "l2": note}
+                                       "particle_sweeps_per_sec": wx.N * 1000 / (msx * 1e-3), "kernel": gx.describe_pass(), "l2": note,
+                                       "roofline": rx}
                 del gx
     if D.rank == 0:
         print(json.dumps(line), flush=True)
