@@ -324,6 +324,38 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def paper_states(device):
+    """S:8(f)-1/2: the paper's own benchmark states, prepared by the harness (paper_1509_04692_b200/statepoints.py) and timed as
+    one hpmc_sweep(n) call each; the paper's per-GPU figures (K20X, mixed precision) are quoted as context only."""
+    import torch
+    from paper_1509_04692_b200 import binding as hb
+    from paper_1509_04692_b200 import statepoints as sp
+    out = {}
+    for label, make, sweeps, paper in (("pentagons_65536_phi0.676", lambda: sp.pentagons_paper_state(256, device=device), 1000,
+                                        "3.89e7 trial moves/s per K20X at 65 536 per GPU (P:237)"),
+                                       ("dodecahedra_32768_phi0.5", lambda: sp.dodecahedra_paper_state(32, device=device), 200,
+                                        "8.16e6 trial moves/s per K20X (P:239)")):
+        t0 = time.perf_counter()
+        w, (acc_t, acc_r) = make()
+        prep = time.perf_counter() - t0
+        g = hb.from_workload(w, seed=1, device=device)
+        g.sweep(50)
+        g.reset_counters()
+        s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(device)
+        s.record(g.stream); g.sweep(sweeps); e.record(g.stream)
+        torch.cuda.synchronize(device)
+        ms = s.elapsed_time(e)
+        c = g.counters()
+        assert g.count_overlaps() == 0
+        out[label] = {"value": c["trials"] / (ms * 1e-3), "unit": UNIT, "N": w.N, "phi": sp.packing_fraction(w), "d": w.d, "a": w.a,
+                      "translate_acceptance": acc_t, "rotate_acceptance": acc_r, "sweeps": sweeps, "ms_per_sweep": ms / sweeps,
+                      "particle_sweeps_per_sec": w.N * sweeps / (ms * 1e-3), "kernel": g.describe_pass(), "prepared_in_s": prep,
+                      "state": w.notes, "paper_context_other_hardware": paper}
+        del g
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -333,6 +365,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-flush", action="store_true", help="do not evict L2 between steps (L2-resident number)")
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, cpu_baseline and the small-system line")
+    ap.add_argument("--paper-states", action="store_true",
+                    help="also prepare and time the paper's own benchmark states (65 536 pentagons at phi = 0.676 with tuned moves, "
+                         "32 768 dodecahedra at phi = 0.5; P:183, P:237): about two more minutes")
     args = ap.parse_args()
     if args.impl == "reference":
         args.steps = 20 if args.steps is None else args.steps
@@ -414,6 +449,8 @@ def main():
                                        "particle_sweeps_per_sec": wx.N * 1000 / (msx * 1e-3), "kernel": gx.describe_pass(), "l2": note,
                                        "roofline": rx}
                 del gx
+    if args.paper_states and D.rank == 0 and args.gpus == 1:
+        line["paper_states"] = paper_states(device)
     if D.rank == 0:
         print(json.dumps(line), flush=True)
     D.close()
