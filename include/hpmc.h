@@ -86,14 +86,18 @@ typedef struct {
  * initial state is overlap-free -- call hpmc_count_overlaps (mirrors P:247).                       */
 int hpmc_create(const hpmc_box* box, const hpmc_shape* shape, int64_t N, uint64_t seed,
                 void* cuda_stream, hpmc_ctx** out);
-int hpmc_destroy(hpmc_ctx* ctx);
+int hpmc_destroy(hpmc_ctx* ctx);                  /* frees the context only: state and workspace belong to the caller (BASELINE.json
+                                                     north_star: "PyTorch is used only for device memory and streams")              */
 const char* hpmc_last_error(const hpmc_ctx* ctx); /* valid until the next call on ctx; ctx may be NULL */
 int hpmc_get_grid(const hpmc_ctx* ctx, hpmc_grid_info* h_out);
 
-/* Bytes of scratch the CALLER must allocate (256-byte aligned) and pass to hpmc_bind.             */
+/* Bytes of scratch the CALLER must allocate (256-byte aligned) and pass to hpmc_bind: the two cell-sorted SoA buffers of the
+ * cell list of P:59 ("a bucket sort efficiently assigns particles to cells"), its keys, histogram and offsets, the dataflow
+ * stamps and the control block.                                                                   */
 size_t hpmc_workspace_bytes(const hpmc_ctx* ctx);
 
-/* Bind the state (tag order, see layout above) and the workspace.  d_pos4/d_quat4 are read by the
+/* Bind the state -- positions r_i and orientations q_i of the N particles, tag order, see layout above -- and the
+ * workspace.  d_pos4/d_quat4 are read by the
  * next hpmc_sweep / hpmc_count_overlaps (the library then works on its own cell-sorted copy inside
  * the workspace) and are used as device staging by hpmc_sweep_host.  Re-binding restarts from the
  * bound arrays; counters and the sweep counter are kept.                                           */

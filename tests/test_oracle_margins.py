@@ -28,7 +28,30 @@ def rand_quat(rng):
 
 
 def qmul(a, b):
-    return wl._qmul(np.asarray(a), np.asarray(b))
+    """Hamilton product (w, x, y, z): this file's own algebra, not the input generator's."""
+    aw, ax, ay, az = np.asarray(a, dtype=np.float64)
+    bw, bx, by, bz = np.asarray(b, dtype=np.float64)
+    return np.array([aw * bw - ax * bx - ay * by - az * bz, aw * bx + ax * bw + ay * bz - az * by,
+                     aw * by - ax * bz + ay * bw + az * bx, aw * bz + ax * by - ay * bx + az * bw])
+
+
+def cube_group():
+    """The 24 proper rotations of the cube as unit quaternions: identity, 90/180/270 about the 3 face axes (9), 120/240 about
+    the 4 body diagonals (8), 180 about the 6 edge axes (6) -- written out from the axis-angle form."""
+    out = [np.array([1.0, 0, 0, 0])]
+    for ax in np.eye(3):
+        for ang in (np.pi / 2, np.pi, 3 * np.pi / 2):
+            out.append(np.concatenate([[np.cos(ang / 2)], np.sin(ang / 2) * ax]))
+    for sx in (1, -1):
+        for sy in (1, -1):
+            d = np.array([1.0, sx, sy]) / np.sqrt(3.0)
+            for ang in (2 * np.pi / 3, 4 * np.pi / 3):
+                out.append(np.concatenate([[np.cos(ang / 2)], np.sin(ang / 2) * d]))
+    for e in ([1, 1, 0], [1, -1, 0], [1, 0, 1], [1, 0, -1], [0, 1, 1], [0, 1, -1]):
+        d = np.array(e, dtype=np.float64) / np.sqrt(2.0)
+        out.append(np.concatenate([[0.0], d]))
+    assert len(out) == 24
+    return np.array(out)
 
 
 def qrot(q, v):
@@ -181,7 +204,7 @@ def test_axis_aligned_cubes_reduce_to_aabb():
     s = ho.Shape(3, ho.KIND_POLYHEDRON, verts=CUBE)
     rng = np.random.default_rng(9)
     ident = np.array([1.0, 0, 0, 0])
-    G = wl._cube_group()
+    G = cube_group()
     for _ in range(300):
         r = rng.uniform(-1.7, 1.7, size=3)
         expect = np.max(np.abs(r)) - 1.0
