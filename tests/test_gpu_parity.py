@@ -395,3 +395,38 @@ def test_dataflow_pass_with_many_tiles_and_partial_edges_matches_per_colour_laun
         out.append((g.get_state(), g.counters()))
         assert g.count_overlaps() == 0
     assert np.array_equal(out[0][0][0], out[1][0][0]) and np.array_equal(out[0][0][1], out[1][0][1]) and out[0][1] == out[1][1]
+
+
+@pytest.mark.parametrize("shape", ["triangle", "square", "hexagon", "irregular_heptagon", "irregular_pentagon"])
+@pytest.mark.parametrize("path", [2, 3])
+def test_polygon_test_variants_lockstep_with_oracle(shape, path):
+    """polygon_separated has three routes: regular pentagons unrolled (every other pentagon test), regular n-gons with a
+    runtime n (only the normal closest to the separation is evaluated), and general convex polygons (every axis that passes the
+    inscribed-radius test).  The last two through the tile pass and the warp-per-cell pass, against the oracle's full SAT margin."""
+    rng = np.random.default_rng(4)
+    if shape == "irregular_heptagon":
+        ang = np.sort(rng.uniform(0, 2 * np.pi, 7)); ang[0] = 0.1
+        verts = 0.5 * np.stack([np.cos(ang), np.sin(ang)], axis=1)
+    elif shape == "irregular_pentagon":                      # five vertices, not regular: must NOT take the unrolled pentagon route
+        verts = np.array([[0.5, 0.0], [0.1, 0.42], [-0.4, 0.2], [-0.3, -0.3], [0.2, -0.35]])
+    else:
+        verts = wl.regular_polygon({"triangle": 3, "square": 4, "hexagon": 6}[shape], 0.5)
+    w = _lattice_workload(2, (34, 30), (1.06, 1.1), wl.KIND_POLYGON, verts=verts, d=0.15, a=0.4, seed=8)
+    from paper_1509_04692_b200 import binding as hb
+    g, o = hb.from_workload(w, seed=2), orc(w, seed=2)
+    g.set_option("path", path)
+    assert g.count_overlaps() == 0 and o.count_overlaps_cells() == 0
+    g.enable_trace(True)
+    marginal = 0
+    for s in range(8):
+        g.sweep(1)
+        f = o.sweep(follow=g.read_trace(), follow_tol=MARGIN_TOL)["follow"]
+        assert f["hard_mismatch"] == 0, (shape, path, s, f)
+        marginal += f["marginal"]
+        gp, gq = g.get_state(); op, oq = o.get_state()
+        assert np.array_equal(gp, op) and np.max(np.abs(gq.astype(np.float64) - oq)) < 1e-5
+        o.set_state(op, gq)
+    gc, oc = g.counters(), o.counters()
+    assert all(gc[k] == oc[k] for k in oc)
+    assert gc["trans_rej_overlap"] + gc["rot_rej_overlap"] > 0.05 * gc["trials"]          # the narrow phase decides many trials
+    assert g.count_overlaps() == 0 and o.count_overlaps_cells() == 0 and marginal <= 3
