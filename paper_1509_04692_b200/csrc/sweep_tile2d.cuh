@@ -163,10 +163,11 @@ __device__ __forceinline__ void tile2d_body(const GridParams& g, const MoveParam
     const bool seam = (cx0 - 1 < 0) || (cx0 - 1 + RW - 1 >= n0 - 1) || (cy0 - 1 < 0) || (cy0 - 1 + RHv - 1 >= n1 - 1);
 
     // ---- staging 1: the contiguous runs of the region rows -------------------------------------------------------
-    if (tid < TL::NSEG) {
-        const int ry = tid >> 1, second = tid & 1;
-        int gb = 0, len = 0;
-        if (ry < RHv) {
+    // global start and length of segment i (two per region row: before and after the periodic wrap in x)
+    auto segment = [&](int i, int& gb, int& len) {
+        const int ry = i >> 1, second = i & 1;
+        gb = 0; len = 0;
+        if (i < TL::NSEG && ry < RHv) {
             int cy = cy0 - 1 + ry;
             cy += (cy < 0) ? n1 : 0;
             cy -= (cy >= n1) ? n1 : 0;
@@ -176,30 +177,52 @@ __device__ __forceinline__ void tile2d_body(const GridParams& g, const MoveParam
                 len = cell_start[cy * n0 + first + ncol] - gb;
             }
         }
-        sm_seg_g[tid] = gb;
-        sm_seg_l[tid] = len;
-    }
-    __syncthreads();
-    if (warp == 0) {   // exclusive scan of the segment lengths
-        int carry = 0;
+    };
+    int ntot;
+    if constexpr (TL::NSEG <= 32) {
+        // every warp works out all segments for itself (lane i: segment i; exclusive scan by shuffles) and writes the same
+        // values to shared memory: no block barrier and no idle warps before the poses can be staged
+        int gb, len;
+        segment(lane, gb, len);
+        int inc = len;
 #pragma unroll
-        for (int b = 0; b < (TL::NSEG + 31) / 32; ++b) {
-            const int i = b * 32 + lane;
-            const int v = (i < TL::NSEG) ? sm_seg_l[i] : 0;
-            int inc = v;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int n = __shfl_up_sync(0xffffffffu, inc, o);
-                if (lane >= o) inc += n;
-            }
-            __syncwarp();
-            if (i < TL::NSEG) sm_seg_l[i] = carry + inc - v;
-            carry += __shfl_sync(0xffffffffu, inc, 31);
+        for (int o = 1; o < 32; o <<= 1) {
+            const int n = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += n;
         }
-        if (lane == 0) sm_seg_l[TL::NSEG] = carry;
+        ntot = __shfl_sync(0xffffffffu, inc, 31);
+        if (lane < TL::NSEG) { sm_seg_g[lane] = gb; sm_seg_l[lane] = inc - len; }
+        if (lane == 0) sm_seg_l[TL::NSEG] = ntot;
+        __syncwarp();
+    } else {
+        if (tid < TL::NSEG) {
+            int gb, len;
+            segment(tid, gb, len);
+            sm_seg_g[tid] = gb;
+            sm_seg_l[tid] = len;
+        }
+        __syncthreads();
+        if (warp == 0) {   // exclusive scan of the segment lengths
+            int carry = 0;
+#pragma unroll
+            for (int b = 0; b < (TL::NSEG + 31) / 32; ++b) {
+                const int i = b * 32 + lane;
+                const int v = (i < TL::NSEG) ? sm_seg_l[i] : 0;
+                int inc = v;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int n = __shfl_up_sync(0xffffffffu, inc, o);
+                    if (lane >= o) inc += n;
+                }
+                __syncwarp();
+                if (i < TL::NSEG) sm_seg_l[i] = carry + inc - v;
+                carry += __shfl_sync(0xffffffffu, inc, 31);
+            }
+            if (lane == 0) sm_seg_l[TL::NSEG] = carry;
+        }
+        __syncthreads();
+        ntot = sm_seg_l[TL::NSEG];
     }
-    __syncthreads();
-    const int ntot = sm_seg_l[TL::NSEG];
     const bool staged = ntot <= min(cap_limit, TL::CAP);   // block-uniform
     CellCounters cc;
 
@@ -434,11 +457,10 @@ k_sweep_tile2d_flow(const __grid_constant__ GridParams g, const __grid_constant_
     // before, which is what every entry holds when the sweep starts -- also across the 2^32 wrap of the counter
     const unsigned stamp = (unsigned)((((unsigned long long)ctrl->hdr.t_hi16 << 32) | ctrl->hdr.t_lo) % 0xFFFFFFFFull) + 1u;
     volatile unsigned int* vdone = done;
+    if (threadIdx.x == 0) s_ticket = (int)atomicAdd(&ctrl->flow_ticket, 1u);
+    __syncthreads();
     for (;;) {
-        __syncthreads();                                   // the previous tile's shared memory is no longer in use
-        if (threadIdx.x == 0) s_ticket = (int)atomicAdd(&ctrl->flow_ticket, 1u);
-        __syncthreads();
-        const int ticket = s_ticket;
+        const int ticket = s_ticket;                       // written before the barrier that ends the previous iteration
         if (ticket >= 4 * ntiles) break;
         const int ci = ticket / ntiles, tile = ticket - ci * ntiles;
         if (ci > 0 && threadIdx.x < 9) {                   // the nine tiles of the previous colour around this one
@@ -454,12 +476,16 @@ k_sweep_tile2d_flow(const __grid_constant__ GridParams g, const __grid_constant_
             }
             __threadfence();
         }
-        __syncthreads();
+        __syncthreads();                                   // dependencies met; every thread has read its ticket
         tile2d_body<KIND, NV, WARPS, R, true>(g, mv, S, SD, ctrl, ctrl->hdr.perm[ci], tile, cap_limit, pose, tag, cell_start, k0, k1,
                                               trace, smem_raw);
         __threadfence();                                   // this thread's pose write-backs are visible device-wide ...
+        __syncthreads();                                   // ... and the tile's shared memory is no longer in use
+        if (threadIdx.x == 0) {
+            vdone[ci * ntiles + tile] = stamp;             // ... before the tile is announced
+            s_ticket = (int)atomicAdd(&ctrl->flow_ticket, 1u);
+        }
         __syncthreads();
-        if (threadIdx.x == 0) vdone[ci * ntiles + tile] = stamp;   // ... before the tile is announced
     }
     // the last CTA to leave re-arms the ticket counter for the next launch
     if (threadIdx.x == 0 && atomicAdd(&ctrl->flow_exited, 1u) == gridDim.x - 1) {
