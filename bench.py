@@ -340,6 +340,67 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def run_partitioned(args, D):
+    """--partition: ONE system on all ranks (paper_1509_04692_b200/partition.py): replicated state, the colour-pass tiles of a
+    slab of cell rows per rank, boundary rows after every colour and the slabs after the last over NCCL.  Same step, metric
+    and timing rules as the default arm; "scaling": "strong"."""
+    import torch
+    from paper_1509_04692_b200 import binding as hb
+    from paper_1509_04692_b200.partition import DistributedRank, LocalRanks
+    device = f"cuda:{D.local}"
+    torch.cuda.set_device(D.local)
+    w = wl.config(args.config, seed=1)               # the SAME system and Philox seed on every rank
+    assert w.dim == 2, "--partition: 2-D configs (0, 1, 2, 4)"
+    g = hb.from_workload(w, seed=1, device=device)
+    g.set_option("path", 2); g.set_option("flow", 0)
+    assert g.count_overlaps() == 0
+    g.sweep(w.warmup_sweeps)                         # melt: every rank on its own (identical trajectories)
+    runner = DistributedRank(g, D.dist) if D.on else None
+    if runner is None:                               # one rank: the same phase calls, nothing to exchange
+        g.set_partition(0, 1)
+
+    def one_step():
+        if runner is not None:
+            runner.sweep(1)
+        else:
+            g.sweep_phase(-1)
+            for ci in range(4):
+                g.sweep_phase(ci)
+
+    fbuf = torch.empty(256 << 20, dtype=torch.uint8, device=device) if not args.no_flush else None
+    for _ in range(max(args.warmup, 3)):
+        one_step()
+    g.reset_counters()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    D.barrier(); torch.cuda.synchronize(device)
+    sampler = ClockSampler(torch.device(device).index or 0) if D.rank == 0 else None
+    for s, e in ev:
+        if fbuf is not None:
+            with torch.cuda.stream(g.stream):
+                fbuf.add_(1)
+        s.record(g.stream)
+        one_step()
+        e.record(g.stream)
+    torch.cuda.synchronize(device); D.barrier()
+    clocks = sampler.stop() if sampler else None
+    ms = float(sum(s.elapsed_time(e) for s, e in ev))
+    c = g.counters()
+    t_max = D.reduce(ms * 1e-3, "MAX")
+    trials_all = D.reduce(c["trials"], "SUM")        # every rank counts the trials of its own tiles
+    g.set_partition(0, 1)
+    assert g.count_overlaps() == 0
+    if D.rank == 0:
+        print(json.dumps({"metric": METRIC, "value": trials_all / t_max, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+                          "warmup": args.warmup, "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "strong",
+                          "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                          "config": {"workload": w.name, "N": w.N, "cells": g.C,
+                                     "parallelism": f"{args.gpus} ranks: partitioned colour passes over a replicated state, boundary rows "
+                                                    "exchanged after every colour, slabs after the last (NCCL)",
+                                     "l2": "flushed between steps" if fbuf is not None else "not flushed"},
+                          "particle_sweeps_per_sec": w.N * args.steps / t_max, "trials_per_step": trials_all / args.steps,
+                          "gpu_launches": int(D.reduce(g.launch_count(), "SUM")), "roofline": None, "clocks": clocks}), flush=True)
+
+
 def paper_states(device):
     """S:8(f)-1/2: the paper's own benchmark states, prepared by the harness (paper_1509_04692_b200/statepoints.py) and timed as
     one hpmc_sweep(n) call each; the paper's per-GPU figures (K20X, mixed precision) are quoted as context only."""
@@ -381,6 +442,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-flush", action="store_true", help="do not evict L2 between steps (L2-resident number)")
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, cpu_baseline and the small-system line")
+    ap.add_argument("--partition", action="store_true",
+                    help="--gpus N as ONE system: every rank holds the whole state and runs the colour-pass tiles of its own slab of "
+                         "cell rows, boundary rows exchanged after every colour (strong scaling; 2-D configs; default: N replicas)")
     ap.add_argument("--paper-states", action="store_true",
                     help="also prepare and time the paper's own benchmark states (65 536 pentagons at phi = 0.676 with tuned moves, "
                          "32 768 dodecahedra at phi = 0.5; P:183, P:237): about two more minutes")
@@ -398,6 +462,10 @@ def main():
     hbuild.build()                                   # no-op when the in-tree libhpmc.so is current
     from paper_1509_04692_b200.replicas import Replicas
     D = Replicas("nccl")
+    if args.partition:
+        run_partitioned(args, D)
+        D.close()
+        return
     device = f"cuda:{D.local}"
     torch.cuda.set_device(D.local)
     k = args.config

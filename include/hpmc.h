@@ -169,6 +169,29 @@ int hpmc_get_profile(hpmc_ctx* ctx, double* h_ms_build, int64_t* h_n_build, doub
  * "k_sweep_tile2d_flow<4 warps x 1 row, 8 CTAs/SM>: 4 colour passes per launch".  Returns the length written.   */
 int hpmc_describe_pass(const hpmc_ctx* ctx, char* h_buf, size_t buf_bytes);
 
+/* ---- One system on several GPUs: partitioned compute over a replicated state -------------------------
+ * The checkerboard makes the cells of one colour independent, so their tiles can be dealt to several contexts --
+ * one per GPU -- that all hold the WHOLE state (the paper instead distributes the state; on NVLink the state of
+ * these systems is a few MB to 1 GB and cheap to replicate).  Every context builds the same cell list (the build is
+ * deterministic: members of a cell in ascending tag), runs the colour-pass tiles of its own slab of cell rows, and the caller
+ * copies rows of the cell-sorted pose array between the contexts: after every colour pass the first and last cell row of a
+ * slab to the contexts that hold the slabs next to it, after the last colour every slab to everybody.  Rows of cells are
+ * contiguous in that array and sit at the same offsets in every context.  The trajectory is bit-identical to the
+ * single-context one (same Philox keys per cell).  2-D systems, tile pass, no trace.
+ *   hpmc_set_partition   this context owns share `rank` of `nranks` (tile rows dealt evenly); (0, 1) = the whole system
+ *   hpmc_sweep_phase     phase -1: grid shift + cell list of the next sweep (advances the sweep counter);
+ *                        phase 0 .. 2^d - 1: the colour pass of that index in the sweep's random order, own tiles only
+ *   hpmc_partition_rows  cell rows [begin, end) of the slab of share `rank` (host arithmetic; same answer in every context)
+ *   hpmc_row_offsets     index in the cell-sorted arrays of the first particle of each of n <= 64 cell rows (row n_y = N);
+ *                        reads the current cell list, synchronises
+ *   hpmc_sorted_pose     device pointer of the current cell-sorted pose array (N x float4 (x, y, qw, qz)); valid until
+ *                        the next phase -1                                                                              */
+int hpmc_set_partition(hpmc_ctx* ctx, int rank, int nranks);
+int hpmc_sweep_phase(hpmc_ctx* ctx, int phase);
+int hpmc_partition_rows(const hpmc_ctx* ctx, int rank, int nranks, int32_t* h_row_begin, int32_t* h_row_end);
+int hpmc_row_offsets(hpmc_ctx* ctx, const int32_t* h_rows, int n, int64_t* h_offsets);
+int hpmc_sorted_pose(hpmc_ctx* ctx, void** d_pose);
+
 /* Diagnostic tallies kept on the device (synchronises).  Names:
  *   "gjk_f64_reruns"  polyhedron pairs whose fp32 GJK verdict was "unsure" (near contact, or a degenerate simplex) and that
  *                     were decided by the fp64 re-run from the raw fp32 state -- the mixed-precision path of P:106-108,

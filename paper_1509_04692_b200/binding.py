@@ -17,7 +17,8 @@ KIND_DISK, KIND_POLYGON, KIND_POLYHEDRON = 0, 1, 2
 ABI_SYMBOLS = ["hpmc_create", "hpmc_destroy", "hpmc_last_error", "hpmc_get_grid", "hpmc_workspace_bytes", "hpmc_bind",
                "hpmc_set_moves", "hpmc_sweep", "hpmc_count_overlaps", "hpmc_get_state", "hpmc_set_sweep_counter",
                "hpmc_reset_counters", "hpmc_set_trace", "hpmc_get_cell_list", "hpmc_sweep_host", "hpmc_set_option", "hpmc_set_profile",
-               "hpmc_get_profile", "hpmc_launch_count", "hpmc_describe_pass", "hpmc_get_stat", "hpmc_measure_fp32_peak"]
+               "hpmc_get_profile", "hpmc_launch_count", "hpmc_describe_pass", "hpmc_get_stat", "hpmc_measure_fp32_peak", "hpmc_set_partition", "hpmc_sweep_phase",
+               "hpmc_partition_rows", "hpmc_row_offsets", "hpmc_sorted_pose"]
 
 
 class HpmcError(RuntimeError):
@@ -79,6 +80,11 @@ def load_library():
     L.hpmc_launch_count.argtypes = [vp]; L.hpmc_launch_count.restype = C.c_int64
     L.hpmc_get_stat.argtypes = [vp, C.c_char_p, C.POINTER(C.c_int64)]
     L.hpmc_measure_fp32_peak.argtypes = [vp, C.POINTER(C.c_double)]
+    L.hpmc_set_partition.argtypes = [vp, C.c_int, C.c_int]
+    L.hpmc_sweep_phase.argtypes = [vp, C.c_int]
+    L.hpmc_partition_rows.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+    L.hpmc_row_offsets.argtypes = [vp, C.POINTER(C.c_int32), C.c_int, C.POINTER(C.c_int64)]
+    L.hpmc_sorted_pose.argtypes = [vp, C.POINTER(vp)]
     L.hpmc_describe_pass.argtypes = [vp, C.c_char_p, C.c_size_t]
     for name in ABI_SYMBOLS:
         if name not in ("hpmc_last_error", "hpmc_workspace_bytes", "hpmc_launch_count"):
@@ -251,6 +257,32 @@ class Hpmc:
         v = C.c_double()
         self._check(self._lib.hpmc_measure_fp32_peak(self._h, C.byref(v)))
         return float(v.value)
+
+    # -- partitioned compute (one system on several GPUs / contexts), see paper_1509_04692_b200/partition.py -----------
+    def set_partition(self, rank, nranks):
+        self._check(self._lib.hpmc_set_partition(self._h, int(rank), int(nranks)))
+
+    def sweep_phase(self, phase):
+        self._check(self._lib.hpmc_sweep_phase(self._h, int(phase)))
+
+    def partition_rows(self, rank, nranks):
+        a, b = C.c_int32(), C.c_int32()
+        self._check(self._lib.hpmc_partition_rows(self._h, int(rank), int(nranks), C.byref(a), C.byref(b)))
+        return int(a.value), int(b.value)
+
+    def row_offsets(self, rows):
+        r = (C.c_int32 * len(rows))(*[int(x) for x in rows])
+        o = (C.c_int64 * len(rows))()
+        self._check(self._lib.hpmc_row_offsets(self._h, r, len(rows), o))
+        return [int(x) for x in o]
+
+    def sorted_pose(self):
+        """The current cell-sorted pose array as a torch view (N, 4) into the workspace (valid until the next build)."""
+        p = C.c_void_p()
+        self._check(self._lib.hpmc_sorted_pose(self._h, C.byref(p)))
+        off = int(p.value) - self.workspace.data_ptr()
+        assert 0 <= off and off + 16 * self.N <= self.workspace.numel()
+        return self.workspace[off:off + 16 * self.N].view(self._torch.float32).view(self.N, 4)
 
     def get_stat(self, name):
         v = C.c_int64()

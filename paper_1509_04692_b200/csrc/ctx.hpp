@@ -55,6 +55,9 @@ struct hpmc_ctx {
     uint2* trace = nullptr;
     int64_t trace_words = 0;
 
+    // compute partition (hpmc_set_partition): this context runs the colour-pass tiles of tile rows [ty0, ty1) only
+    int part_rank = 0, part_n = 1;
+
     // tuning / test knobs (hpmc_set_option)
     int opt_path = 0;                 // 0 auto, 1 per-thread global path, 2 tile path (2-D only), 3 warp per cell, 4 cluster (small 2-D)
     int cluster_ctas = -1;            // CTAs per cluster of the whole-sweep pass: -1 = not probed yet, 0 = unavailable on this device

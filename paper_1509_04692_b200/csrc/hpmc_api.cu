@@ -319,6 +319,7 @@ bool use_flow(const hpmc_ctx* c)
 {
     const GridParams& g = c->g;
     if (g.dim != 2 || c->sf.kind == kKindPolyhedron || c->opt_path == 1 || c->opt_path == 3 || c->opt_flow == 0) return false;
+    if (c->part_n > 1) return false;   // the ranks exchange boundary rows between the colours: one launch per colour
     const int nactive = (g.n[0] / 2) * (g.n[1] / 2);
     if (c->opt_path == 0 && c->opt_tile_shape == 0 && nactive <= kWarpCellMax2d) return false;
     if (c->opt_flow == 1) return true;
@@ -335,7 +336,7 @@ constexpr int kClusterMaxCtas = 16, kClusterThreads = 1024, kClusterMaxCells = 1
 bool cluster_eligible(const hpmc_ctx* c)
 {
     const GridParams& g = c->g;
-    if (g.dim != 2 || c->sf.kind == kKindPolyhedron || c->cluster_ctas == 0) return false;
+    if (g.dim != 2 || c->sf.kind == kKindPolyhedron || c->cluster_ctas == 0 || c->part_n > 1) return false;
     if (g.N < 1 || g.N > kClusterMaxCtas * kClusterThreads || g.C + 2 > kClusterMaxCells) return false;
     // measured on B200 (profiles/r2_cluster.md): 58 us per sweep of 4096 pentagons against 39 us for the graph of five launches --
     // a trial is a ~2 us dependent chain either way and seven cluster barriers do not beat four launch gaps -- so the pass is
@@ -386,7 +387,8 @@ int launch_colour_dispatch(hpmc_ctx* c, int ci)
     const GridParams& g = c->g;
     const int nactive = (g.n[0] / 2) * (g.n[1] / 2) * (g.dim == 3 ? g.n[2] / 2 : 1);
     bool ok = true;
-    if (c->opt_path == 1 || (g.dim == 2 && kind == kKindPolyhedron)) ok = hpmc_launch_colour(c, ci, kind, nv, nactive);
+    if (c->part_n > 1) ok = hpmc_launch_tile2d(c, ci, kind, nv, pick_tile_shape(c));
+    else if (c->opt_path == 1 || (g.dim == 2 && kind == kKindPolyhedron)) ok = hpmc_launch_colour(c, ci, kind, nv, nactive);
     else if (g.dim == 3 || c->opt_path == 3 || (c->opt_path == 0 && c->opt_tile_shape == 0 && nactive <= kWarpCellMax2d))
         ok = hpmc_launch_warpcell(c, ci, kind, nv, nactive);
     else ok = hpmc_launch_tile2d(c, ci, kind, nv, pick_tile_shape(c));
@@ -854,6 +856,83 @@ int hpmc_describe_pass(const hpmc_ctx* c, char* h_buf, size_t n)
     }
     std::snprintf(h_buf, n, "%s", d.c_str());
     return (int)std::min(d.size(), n - 1);
+}
+
+// ---- compute partition across contexts / GPUs --------------------------------------------------------
+namespace {
+int tile_rows_of_shape(int shape) { return shape == 1 ? 16 : shape == 2 ? 4 : 2; }   // active rows per tile (WARPS x R)
+void slab_rows(const hpmc_ctx* c, int rank, int nranks, int& r0, int& r1)
+{
+    const int TH = tile_rows_of_shape(pick_tile_shape(c));
+    const int nay = c->g.n[1] / 2, tiles_y = (nay + TH - 1) / TH;
+    const int ty0 = (int)((long long)tiles_y * rank / nranks), ty1 = (int)((long long)tiles_y * (rank + 1) / nranks);
+    r0 = std::min(2 * TH * ty0, c->g.n[1]);
+    r1 = std::min(2 * TH * ty1, c->g.n[1]);
+}
+}  // namespace
+
+int hpmc_set_partition(hpmc_ctx* c, int rank, int nranks)
+{
+    if (!c) return HPMC_E_ARG;
+    if (nranks < 1 || rank < 0 || rank >= nranks) return fail(c, HPMC_E_ARG, "need 0 <= rank < nranks");
+    if (nranks > 1 && (c->g.dim != 2 || c->sf.kind == kKindPolyhedron)) return fail(c, HPMC_E_ARG, "partitioned sweeps: 2-D tile pass only");
+    if (nranks > 1 && c->trace) return fail(c, HPMC_E_ARG, "partitioned sweeps keep no trace");
+    graph_reset(c);
+    c->part_rank = rank;
+    c->part_n = nranks;
+    return HPMC_OK;
+}
+
+int hpmc_sweep_phase(hpmc_ctx* c, int phase)
+{
+    DeviceGuard dev_guard(c);
+    int rc = check_ready(c);
+    if (rc != HPMC_OK) return rc;
+    if (phase == -1) {
+        rc = build_cell_list(c, 0, 0ull);
+        if (rc == HPMC_OK) ++c->t_host;
+        return rc;
+    }
+    if (phase < 0 || phase >= (1 << c->g.dim)) return fail(c, HPMC_E_ARG, "phase must be -1 (build) or a colour index");
+    if (!c->have_sorted) return fail(c, HPMC_E_UNBOUND, "no cell list: run phase -1 first");
+    return launch_colour_dispatch(c, phase);
+}
+
+int hpmc_partition_rows(const hpmc_ctx* c, int rank, int nranks, int32_t* h_row_begin, int32_t* h_row_end)
+{
+    if (!c || !h_row_begin || !h_row_end || nranks < 1 || rank < 0 || rank >= nranks) return HPMC_E_ARG;
+    int r0, r1;
+    slab_rows(c, rank, nranks, r0, r1);
+    *h_row_begin = r0;
+    *h_row_end = r1;
+    return HPMC_OK;
+}
+
+int hpmc_row_offsets(hpmc_ctx* c, const int32_t* h_rows, int n, int64_t* h_offsets)
+{
+    DeviceGuard dev_guard(c);
+    int rc = check_ready(c);
+    if (rc != HPMC_OK) return rc;
+    if (!h_rows || !h_offsets || n < 0 || n > 64) return fail(c, HPMC_E_ARG, "need 0 <= n <= 64 rows");
+    if (!c->have_sorted) return fail(c, HPMC_E_UNBOUND, "no cell list: run phase -1 first");
+    int vals[64];
+    for (int i = 0; i < n; ++i) {
+        if (h_rows[i] < 0 || h_rows[i] > c->g.n[1]) return fail(c, HPMC_E_ARG, "cell row out of range");
+        if (!cuda_ok(c, cudaMemcpyAsync(&vals[i], c->cell_start + (size_t)h_rows[i] * c->g.n[0], sizeof(int), cudaMemcpyDeviceToHost, c->stream), "rows/memcpy")) return HPMC_E_CUDA;
+    }
+    if (!cuda_ok(c, cudaStreamSynchronize(c->stream), "rows/sync")) return HPMC_E_CUDA;
+    for (int i = 0; i < n; ++i) h_offsets[i] = vals[i];
+    return HPMC_OK;
+}
+
+int hpmc_sorted_pose(hpmc_ctx* c, void** d_pose)
+{
+    int rc = check_ready(c);
+    if (rc != HPMC_OK) return rc;
+    if (!d_pose) return fail(c, HPMC_E_ARG, "d_pose is NULL");
+    if (!c->have_sorted) return fail(c, HPMC_E_UNBOUND, "no cell list: run phase -1 first");
+    *d_pose = c->pos[c->cur];
+    return HPMC_OK;
 }
 
 int hpmc_get_stat(hpmc_ctx* c, const char* name, int64_t* h_value)

@@ -426,10 +426,11 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
 k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ MoveParams mv, const __grid_constant__ ShapeF S,
                const __grid_constant__ ShapeD SD, Control* __restrict__ ctrl, int colour_index, int cap_limit,
                float4* __restrict__ pose, const int* __restrict__ tag, const int* __restrict__ cell_start, uint32_t k0,
-               uint32_t k1, uint2* __restrict__ trace)
+               uint32_t k1, uint2* __restrict__ trace, int tile0)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    tile2d_body<KIND, NV, WARPS, R, false>(g, mv, S, SD, ctrl, ctrl->hdr.perm[colour_index], (int)blockIdx.x, cap_limit, pose, tag,
+    // tile0: first tile of this launch (0 unless the context runs a partition of the tile rows, hpmc_set_partition)
+    tile2d_body<KIND, NV, WARPS, R, false>(g, mv, S, SD, ctrl, ctrl->hdr.perm[colour_index], tile0 + (int)blockIdx.x, cap_limit, pose, tag,
                                            cell_start, k0, k1, trace, smem_raw);
 }
 
