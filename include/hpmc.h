@@ -43,8 +43,7 @@ extern "C" {
 #define HPMC_OK 0
 #define HPMC_E_ARG (-1)       /* bad argument (dim, N, d, a, n_select, NULL pointer, ...)          */
 #define HPMC_E_SHAPE (-2)     /* non-convex / not CCW / too many vertices / vertex not on the hull */
-#define HPMC_E_GRID (-3)      /* fewer than 4 cells per side (R11), more than 2^31-2 cells, or a box so large that the
-                                 fp32 rounding of cell_of (3 ulp(L)) exceeds the slack w - d_max of the cell width      */
+#define HPMC_E_GRID (-3)      /* fewer than 4 cells per side (R11) or more than 2^31-2 cells                             */
 #define HPMC_E_UNBOUND (-4)   /* state/workspace not bound, or workspace too small                 */
 #define HPMC_E_CUDA (-5)      /* a CUDA call failed (sticky)                                       */
 #define HPMC_E_TRACE (-6)     /* trace buffer too small for C * n_select slots                     */
@@ -72,7 +71,8 @@ typedef struct {
 
 typedef struct {
     int dim;
-    int n[3];        /* cells per side: n_k = 2*floor(L_k / (2 d_max (1 + 2^-10))) (R11)            */
+    int n[3];        /* cells per side: n_k = 2*floor(L_k / (2 (d_max + slack))), slack = max(d_max 2^-10,
+                        3 ulp_fp32(L_k)) (R11)                                                       */
     double w[3];     /* cell width L_k / n_k                                                        */
     float L_f[3];    /* box edge as used by the fp32 state                                          */
     float inv_w[3];  /* (float)(n_k / L_k), the factor inside cell_of (R13)                         */

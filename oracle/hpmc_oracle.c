@@ -553,8 +553,16 @@ orc_sys* orc_create(int dim, const double L[3], int kind, double diameter, int n
         if (k < dim) {
             s->L_f[k] = (float)L[k];
             s->L[k] = (double)s->L_f[k];
-            /* O2 / R11: even count, relative slack 2^-10 on d_max, at least 4 */
-            s->n[k] = 2 * (int32_t)floor(s->L[k] / (2.0 * sh->dmax * (1.0 + 1.0 / 1024.0)));
+            /* O2 / R11: even count, cell width >= d_max + slack, at least 4 cells.  slack = d_max 2^-10, or 3 ulp_fp32(L) in
+             * boxes so large that the fp32 rounding of cell_of (R13) would eat the former (R11); the two coincide
+             * for every config of BASELINE.json. */
+            {
+                int e = 0;
+                frexp(nextafter(s->L[k], 0.0), &e);
+                double ulp = ldexp(1.0, e - 24);
+                double slack = fmax(sh->dmax / 1024.0, 3.0 * ulp);
+                s->n[k] = 2 * (int32_t)floor(s->L[k] / (2.0 * (sh->dmax + slack)));
+            }
             if (s->n[k] < 4) { orc_shape_destroy(sh); free(s); return NULL; }
             s->w[k] = s->L[k] / s->n[k];
             s->w_f[k] = (float)s->w[k];

@@ -450,16 +450,18 @@ int hpmc_create(const hpmc_box* box, const hpmc_shape* shape, int64_t N, uint64_
             if (!(box->L[k] > 0.0)) { delete c; return fail(nullptr, HPMC_E_ARG, "box edge must be > 0"); }
             g.L[k] = (float)box->L[k];            // R-box: the box edge is L rounded to fp32
             g.Ld[k] = (double)g.L[k];
-            g.n[k] = 2 * (int)std::floor(g.Ld[k] / (2.0 * c->d_max * (1.0 + 1.0 / 1024.0)));  // R11
-            if (g.n[k] < 4) { delete c; return fail(nullptr, HPMC_E_GRID, "fewer than 4 cells per side (R11)"); }
-            c->w[k] = g.Ld[k] / g.n[k];
-            {   // R11/R22: fl(fl(x - lo) - s) * inv_w misplaces a cell boundary by up to ~1.5 ulp of a coordinate difference just
-                // below L; two boundaries lie between particles of cells c and c + 2, which must stay >= d_max apart
+            {   // R11: even count, cell width >= d_max + slack.  The slack is d_max 2^-10, or -- in boxes so large that this is
+                // not enough -- 3 ulp_fp32(L): fl(fl(x - lo) - s) * inv_w misplaces a cell boundary by up to ~1.5 ulp of a
+                // coordinate difference just below L, and two boundaries lie between particles of cells c and c + 2, which
+                // must stay >= d_max apart (R22).  Identical to the plain 2^-10 rule up to L ~ 5000 d_max.
                 int e = 0;
                 std::frexp(std::nextafter(g.Ld[k], 0.0), &e);     // the largest coordinate difference below L = m 2^e, m in [0.5, 1)
                 const double ulp = std::ldexp(1.0, e - 24);      // fp32 ulp of values in [L/2, L)
-                if (3.0 * ulp > c->w[k] - c->d_max) { delete c; return fail(nullptr, HPMC_E_GRID, "box too large for fp32 coordinates at this particle size: cell slack below 3 ulp(L) (R11, R22)"); }
+                const double slack = std::fmax(c->d_max / 1024.0, 3.0 * ulp);
+                g.n[k] = 2 * (int)std::floor(g.Ld[k] / (2.0 * (c->d_max + slack)));
             }
+            if (g.n[k] < 4) { delete c; return fail(nullptr, HPMC_E_GRID, "fewer than 4 cells per side (R11)"); }
+            c->w[k] = g.Ld[k] / g.n[k];
             g.w_f[k] = (float)c->w[k];
             g.inv_w[k] = (float)((double)g.n[k] / g.Ld[k]);
         } else {

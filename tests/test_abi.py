@@ -79,12 +79,15 @@ def test_create_rejects_bad_input(lib):
     assert _create(lib, 3, (10,) * 3, hb.KIND_POLYHEDRON, 4, verts=inner)[0] == -2                           # not a hull vertex
     assert _create(lib, 2, (10, 10), hb.KIND_POLYHEDRON, 4, verts=wl.cube_vertices(1.0))[0] == -2            # wrong dim
     assert b"" != lib.hpmc_last_error(None)
-    # R11/R22: from L ~ 6000 the fp32 rounding of cell_of (3 ulp(L)) exceeds the slack of the cell width for unit particles
-    assert _create(lib, 2, (4096.0, 4096.0), hb.KIND_POLYGON, 4, verts=wl.regular_polygon(5, 0.5))[0] == 0
-    assert _create(lib, 2, (8192.0, 8192.0), hb.KIND_POLYGON, 4, verts=wl.regular_polygon(5, 0.5))[0] == -3
-    assert b"fp32" in lib.hpmc_last_error(None)
-    assert _create(lib, 2, (8192.0, 8192.0), hb.KIND_DISK, 4, diameter=4.0)[0] == 0       # larger particles: larger slack
-
+    # R11/R22: in boxes so large that d_max 2^-10 no longer covers the fp32 rounding of cell_of the cells get wider, not the box refused
+    gi = hb.GridInfo()
+    import math
+    for L, n in ((4096.0, 4092), (8192.0, 8180), (65536.0, 64776)):
+        rc, h = _create(lib, 2, (L, 8.0), hb.KIND_POLYGON, 4, verts=wl.regular_polygon(5, 0.5))
+        assert rc == 0 and lib.hpmc_get_grid(h, C.byref(gi)) == 0 and gi.n[0] == n, (L, gi.n[0])
+        ulp = math.ldexp(1.0, math.frexp(math.nextafter(L, 0.0))[1] - 24)        # fp32 ulp of coordinate differences just below L
+        assert gi.w[0] - 1.0 >= max(2.0 ** -10, 3 * ulp) and gi.n[0] % 2 == 0
+        lib.hpmc_destroy(h)
 
 def test_binding_fails_loudly_without_gpu():
     import torch

@@ -430,3 +430,39 @@ def test_polygon_test_variants_lockstep_with_oracle(shape, path):
     assert all(gc[k] == oc[k] for k in oc)
     assert gc["trans_rej_overlap"] + gc["rot_rej_overlap"] > 0.05 * gc["trials"]          # the narrow phase decides many trials
     assert g.count_overlaps() == 0 and o.count_overlaps_cells() == 0 and marginal <= 3
+
+
+def test_lockstep_in_a_box_of_edge_20000():
+    """R11/R22: fp32 coordinates of magnitude 10^4 (spacing 1e-3).  The cell width carries 3 ulp(L) of slack there; the CUDA path
+    and the oracle must still agree on every cell index and decision, also for the particles at the seam."""
+    L = (20000.0, 8.0)
+    xs = np.concatenate([np.arange(-10000.0 + 0.6, -10000.0 + 150, 1.05), np.arange(10000.0 - 150, 10000.0 - 0.6, 1.05)])
+    ys = np.array([-3.0, -1.9, -0.8, 0.3, 1.4, 2.5])
+    P = np.array([[x, y] for x in xs for y in ys])
+    N = P.shape[0]
+    pos = np.zeros((N, 4), np.float32); pos[:, :2] = P
+    rng = np.random.default_rng(2)
+    th = rng.uniform(0, 2 * np.pi, N)
+    quat = np.zeros((N, 4), np.float32); quat[:, 0] = np.cos(th / 2); quat[:, 3] = np.sin(th / 2)
+    w = wl.Workload(name="long_box", dim=2, N=N, L=L, kind=wl.KIND_POLYGON, diameter=0.0, verts=wl.regular_polygon(5, 0.5), d=0.3, a=0.5,
+                    n_select=4, sweeps=1, pos4=pos, quat4=quat)
+    for path in (2, 3):
+        from paper_1509_04692_b200 import binding as hb
+        g, o = hb.from_workload(w, seed=4), orc(w, seed=4)
+        assert list(g.n[:2]) == [19882, 6] and np.array_equal(g.n, o.n)
+        g.set_option("path", path)
+        g.enable_trace(True)
+        marginal = 0
+        for s in range(8):
+            cid, cst, mem, shift, perm = g.cell_list(s)
+            oshift, _ = o.sweep_header(s)
+            ocid, ocst, omem = o.cell_list(oshift)
+            assert np.array_equal(cid, ocid) and np.array_equal(cst, ocst) and np.array_equal(mem, omem)
+            g.sweep(1)
+            f = o.sweep(follow=g.read_trace(), follow_tol=MARGIN_TOL)["follow"]
+            assert f["hard_mismatch"] == 0, (path, s, f)
+            marginal += f["marginal"]
+            gp, gq = g.get_state(); op, oq = o.get_state()
+            assert np.array_equal(gp, op) and np.max(np.abs(gq.astype(np.float64) - oq)) < 1e-5
+            o.set_state(op, gq)
+        assert g.count_overlaps() == 0 and o.count_overlaps_bruteforce() == 0 and marginal <= 3

@@ -227,3 +227,31 @@ def test_textbook_metropolis_keeps_zero_overlaps_and_moves_everything():
     assert o.count_overlaps_bruteforce() == 0
     c = o.counters()
     assert c["trans_rej_cell"] == 0 and c["trials"] == 20 * w.N and c["rot_acc"] > 0 and c["trans_acc"] > 0
+
+
+def test_large_box_grid_keeps_same_colour_cells_apart():
+    # R11/R22: in a box of edge 20 000 the fp32 cell function misplaces boundaries by ~1e-3; the cell width then carries a slack
+    # of 3 ulp(L) instead of d_max 2^-10, so that particles of different same-colour cells still cannot come within d_max (P4)
+    L = (20000.0, 8.0)
+    pent = wl.regular_polygon(5, 0.5)
+    o = ho.Oracle(2, L, ho.KIND_POLYGON, 0, 1, verts=pent)
+    assert list(o.n[:2]) == [19882, 6] and o.w[0] - 1.0 >= 3 * 2.0 ** -9          # ulp of differences in [16384, 32768) is 2^-9
+    # a dense row of pentagons at both ends of the box (largest coordinates: coarsest fp32 spacing) and across the seam
+    xs = np.concatenate([np.arange(-10000.0 + 0.6, -10000.0 + 150, 1.05), np.arange(10000.0 - 150, 10000.0 - 0.6, 1.05)])
+    ys = np.array([-3.0, -1.9, -0.8, 0.3, 1.4, 2.5])
+    P = np.array([[x, y] for x in xs for y in ys])
+    N = P.shape[0]
+    pos = np.zeros((N, 4), np.float32); pos[:, :2] = P
+    rng = np.random.default_rng(2)
+    th = rng.uniform(0, 2 * np.pi, N)
+    quat = np.zeros((N, 4), np.float32); quat[:, 0] = np.cos(th / 2); quat[:, 3] = np.sin(th / 2)
+    o = ho.Oracle(2, L, ho.KIND_POLYGON, N, 3, verts=pent)
+    o.set_moves(0.3, 0.5, 4); o.set_state(pos, quat)
+    assert o.count_overlaps_bruteforce() == 0
+    for t in range(25):
+        shift, _ = o.sweep_header(t)
+        assert o.min_same_colour_distance(shift) >= 1.0
+        o.sweep()
+    assert o.count_overlaps_bruteforce() == 0
+    c = o.counters()
+    assert c["trans_acc"] > 0 and c["trans_rej_overlap"] > 0
