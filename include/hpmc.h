@@ -155,7 +155,10 @@ int hpmc_sweep_host(hpmc_ctx* ctx, const float* h_pos4, const float* h_quat4, in
  *   "small_build" 1 (default): a system with at most 11 500 cells and 8192 particles builds its cell list in one CTA
  *              (one launch instead of three); 0: always the multi-launch build.
  *   "graph"    1 (default): hpmc_sweep(n >= 3) replays a captured CUDA graph of two sweeps; 0: plain launches.
- *              Needs a real stream: contexts created on the legacy default stream (NULL) always use plain launches.  */
+ *              Needs a real stream: contexts created on the legacy default stream (NULL) always use plain launches.
+ *   "pdl"      1 (default): the kernels of a sweep are launched with programmatic stream serialisation: a kernel may start
+ *              while its predecessor drains, and every kernel waits (griddepcontrol.wait) before it reads or writes anything
+ *              a predecessor touches; 0: plain stream order.  */
 int hpmc_set_option(hpmc_ctx* ctx, const char* name, int64_t value);
 
 /* Per-kernel device timing for the roofline report (S:8(d)).  While on, CUDA events on the context's stream

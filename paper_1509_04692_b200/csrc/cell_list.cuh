@@ -29,6 +29,8 @@ __global__ void k_hist(const __grid_constant__ GridParams g, Control* __restrict
                        int* __restrict__ counts, int2* __restrict__ key_rank, uint32_t k0, uint32_t k1, int mode,
                        unsigned long long t_override)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     __shared__ SweepHeader sh;
     if (threadIdx.x == 0) {
         const unsigned long long t = (mode == 0) ? ctrl->t : t_override;
@@ -101,6 +103,8 @@ __device__ __forceinline__ int block_exclusive_scan(int v, int& total)
 // wavefront advances 32 tiles per L2 round trip, 0.77 TB/s on 16.7 M counts.)
 __global__ void __launch_bounds__(kScanThreads) k_scan_reduce(const int* __restrict__ counts, int n, int* __restrict__ tile_sums)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     __shared__ int s_wsum[kScanThreads / 32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int wbase = blockIdx.x * kScanTile + warp * (32 * kScanItems) + lane;
@@ -124,6 +128,8 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_reduce(const int* __restr
 // exclusive scan of the tile totals by ONE block; also advances the sweep counter of a real sweep (mode 0)
 __global__ void __launch_bounds__(kScanThreads) k_scan_spine(int* __restrict__ tile_sums, int ntiles, Control* __restrict__ ctrl, int mode)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     __shared__ int carry_s;
     if (threadIdx.x == 0) {
         carry_s = 0;
@@ -153,6 +159,8 @@ __global__ void __launch_bounds__(kScanThreads)
 k_scan_final(int* __restrict__ counts, int n, int* __restrict__ cell_start, const int* __restrict__ tile_sums, int single,
              Control* __restrict__ ctrl, int mode)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     __shared__ int s_wsum[kScanThreads / 32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int wbase = blockIdx.x * kScanTile + warp * (32 * kScanItems) + lane;
@@ -211,6 +219,8 @@ __global__ void k_scatter(int N, int dim, const float4* __restrict__ src_pos, co
                           const int* __restrict__ src_tag, const int2* __restrict__ key_rank, const int* __restrict__ cell_start,
                           float4* __restrict__ dst_pos, float4* __restrict__ dst_quat, int* __restrict__ dst_tag)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= N) return;
     const int2 kr = key_rank[p];
@@ -235,6 +245,8 @@ __global__ void k_scatter(int N, int dim, const float4* __restrict__ src_pos, co
 // (measured on 1 M pentagons: scatter + sort 9.8 + ~5 us against 25 us for the scatter whose last arrival sorted the cell).
 __global__ void k_sort_cells(int C, int dim, const int* __restrict__ cell_start, float4* pos, float4* quat, int* tag)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= C) return;
     const int s = cell_start[c], e = cell_start[c + 1];
@@ -271,6 +283,8 @@ k_build_small(const __grid_constant__ GridParams g, Control* __restrict__ ctrl, 
               const int* __restrict__ src_tag, int2* __restrict__ key_rank, int* __restrict__ cell_start, float4* dst_pos,
               float4* dst_quat, int* dst_tag)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     extern __shared__ int s_off[];            // counts, then exclusive offsets, C + 1 entries
     __shared__ SweepHeader sh;
     __shared__ int s_part[kSmallBuildThreads / 32];

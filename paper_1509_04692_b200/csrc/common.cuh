@@ -56,6 +56,14 @@ struct Control {
     SweepHeader hdr;
 };
 
+// Programmatic dependent launch (sm_90+): a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may start
+// while its predecessor in the stream still runs; it must not touch anything the predecessor writes (or reads and it writes)
+// before pdl_wait(), which returns once the predecessor grid has completed and its memory operations are visible.
+// pdl_launch_dependents() lets the successor's launch begin: called at the top, it takes the launch latency (~2 us, a third
+// of a colour pass of a 4096-particle system) off the critical path.  Both are no-ops in a kernel launched the plain way.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // Cell-sorted state.  3-D: pos = (x, y, z, 0) and quat = (w, x, y, z), two arrays.  2-D: ONE array of
 // poses (x, y, qw, qz) in `pos` (R30: z = 0 and qx = qy = 0 always), `quat` is not allocated -- half the bytes per particle.
 __device__ __forceinline__ void load_state(int dim, const float4* __restrict__ pos, const float4* __restrict__ quat, int i,

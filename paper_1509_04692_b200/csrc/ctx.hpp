@@ -49,6 +49,8 @@ struct hpmc_ctx {
     int num_sms = 0;
     int device = 0;                      // CUDA device of the context (the one current at hpmc_create); every entry point switches to it
     uint32_t attr_done = 0;              // cudaFuncSetAttribute(MaxDynamicSharedMemorySize) done for this context: bit per tile shape / flow
+    bool after_colour = false;           // the last launch on the stream was a colour pass of the current cell list (PDL: its successor may
+                                         // read the cell list before waiting)
     bool flow_now = false;               // this sweep's colour passes go out as one dataflow launch
     Control* ctrl = nullptr;
 
@@ -66,6 +68,7 @@ struct hpmc_ctx {
     int opt_flow = -1;                // 2-D tile pass as one dataflow launch per sweep: -1 = when it pays (auto), 0 = never, 1 = always
     int opt_small_build = 1;          // 1: systems with few cells build their cell list in one CTA (k_build_small)
     int opt_graph = 1;                // 1: hpmc_sweep(n >= 3) replays a captured two-sweep CUDA graph
+    int opt_pdl = 1;                  // 1: the kernels of a sweep are launched with programmatic stream serialization (common.cuh)
 
     // CUDA graph of two consecutive sweeps (the ping-pong buffers return to where they started), one per parity of `cur`
     cudaGraphExec_t graph_exec[2] = {nullptr, nullptr};
@@ -100,6 +103,24 @@ inline bool cuda_ok(hpmc_ctx* c, cudaError_t e, const char* what)
     return false;
 }
 
+
+// Kernel launch on the context's stream, as a programmatic dependent launch when the option is on (every kernel launched
+// through here starts with pdl_launch_dependents(); pdl_wait();).
+template <typename... KArgs, typename... Args>
+inline cudaError_t hpmc_launch(hpmc_ctx* c, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, Args&&... args)
+{
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = c->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = c->opt_pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
 
 constexpr int kTileWHost = 32;   // active cells per tile row (= kTileW of sweep_tile2d.cuh)
 

@@ -255,6 +255,7 @@ struct ProfileScope {
 int build_cell_list(hpmc_ctx* c, int mode, unsigned long long t_override)
 {
     ProfileScope prof(c, 0);
+    c->after_colour = false;
     const GridParams& g = c->g;
     const int TB = 256;
     const float4* src_pos = c->state_in_bound ? c->d_pos_bound : c->pos[c->cur];
@@ -262,7 +263,7 @@ int build_cell_list(hpmc_ctx* c, int mode, unsigned long long t_override)
     const int* src_tag = c->state_in_bound ? nullptr : c->tag[c->cur];
     const int dst = c->state_in_bound ? 0 : 1 - c->cur;
     if (c->opt_small_build && g.C <= kSmallBuildMaxCells && g.N <= kSmallBuildMaxN) {   // one CTA does the whole build
-        k_build_small<<<1, kSmallBuildThreads, ((size_t)g.C + 2) * sizeof(int), c->stream>>>(
+        hpmc_launch(c, k_build_small, 1, kSmallBuildThreads, ((size_t)g.C + 2) * sizeof(int),
             g, c->ctrl, c->k0, c->k1, mode, t_override, src_pos, src_quat, src_tag, c->key_rank, c->cell_start, c->pos[dst], c->quat[dst],
             c->tag[dst]);
         LAUNCH_CHECK(c, "k_build_small");
@@ -273,25 +274,25 @@ int build_cell_list(hpmc_ctx* c, int mode, unsigned long long t_override)
     }
     const int nblk_part = (g.N + TB - 1) / TB;
     const int nblk_hist = (g.N + TB * kHistItems - 1) / (TB * kHistItems);
-    k_hist<<<nblk_hist > 0 ? nblk_hist : 1, TB, 0, c->stream>>>(g, c->ctrl, src_pos, c->counts, c->key_rank, c->k0, c->k1, mode, t_override);
+    hpmc_launch(c, k_hist, nblk_hist > 0 ? nblk_hist : 1, TB, 0, g, c->ctrl, src_pos, c->counts, c->key_rank, c->k0, c->k1, mode, t_override);
     LAUNCH_CHECK(c, "k_hist");
     const int tiles = scan_tiles(c);
     const bool fused = tiles > 1 && tiles <= kFusedSpineMax;
     if (tiles > 1) {
-        k_scan_reduce<<<tiles, kScanThreads, 0, c->stream>>>(c->counts, g.C, c->tile_sums);
+        hpmc_launch(c, k_scan_reduce, tiles, kScanThreads, 0, c->counts, g.C, c->tile_sums);
         LAUNCH_CHECK(c, "k_scan_reduce");
         if (!fused) {
-            k_scan_spine<<<1, kScanThreads, 0, c->stream>>>(c->tile_sums, tiles, c->ctrl, mode);
+            hpmc_launch(c, k_scan_spine, 1, kScanThreads, 0, c->tile_sums, tiles, c->ctrl, mode);
             LAUNCH_CHECK(c, "k_scan_spine");
         }
     }
-    k_scan_final<<<tiles, kScanThreads, 0, c->stream>>>(c->counts, g.C, c->cell_start, c->tile_sums, tiles == 1 ? 1 : fused ? 2 : 0, c->ctrl, mode);
+    hpmc_launch(c, k_scan_final, tiles, kScanThreads, 0, c->counts, g.C, c->cell_start, c->tile_sums, tiles == 1 ? 1 : fused ? 2 : 0, c->ctrl, mode);
     LAUNCH_CHECK(c, "k_scan_final");
     if (g.N > 0) {
-        k_scatter<<<nblk_part, TB, 0, c->stream>>>(g.N, g.dim, src_pos, src_quat, src_tag, c->key_rank, c->cell_start, c->pos[dst], c->quat[dst],
+        hpmc_launch(c, k_scatter, nblk_part, TB, 0, g.N, g.dim, src_pos, src_quat, src_tag, c->key_rank, c->cell_start, c->pos[dst], c->quat[dst],
                                                   c->tag[dst]);
         LAUNCH_CHECK(c, "k_scatter");
-        k_sort_cells<<<(g.C + TB - 1) / TB, TB, 0, c->stream>>>(g.C, g.dim, c->cell_start, c->pos[dst], c->quat[dst], c->tag[dst]);
+        hpmc_launch(c, k_sort_cells, (g.C + TB - 1) / TB, TB, 0, g.C, g.dim, c->cell_start, c->pos[dst], c->quat[dst], c->tag[dst]);
         LAUNCH_CHECK(c, "k_sort_cells");
     }
     c->cur = dst;
@@ -394,6 +395,7 @@ int launch_colour_dispatch(hpmc_ctx* c, int ci)
     else ok = hpmc_launch_tile2d(c, ci, kind, nv, pick_tile_shape(c));
     if (!ok) return HPMC_E_CUDA;
     LAUNCH_CHECK(c, "colour pass");
+    c->after_colour = !c->profile;   // an event record between the launches makes the next one an ordinary successor anyway
     return HPMC_OK;
 }
 
@@ -802,6 +804,8 @@ int hpmc_set_option(hpmc_ctx* c, const char* name, int64_t value)
         c->opt_tile_cap = value > (1 << 30) ? (1 << 30) : (int)value;
     } else if (n == "small_build") {
         c->opt_small_build = value != 0;
+    } else if (n == "pdl") {
+        c->opt_pdl = value != 0;
     } else if (n == "flow") {
         if (value < -1 || value > 1) return fail(c, HPMC_E_ARG, "flow must be -1 (auto), 0 or 1");
         c->opt_flow = (int)value;

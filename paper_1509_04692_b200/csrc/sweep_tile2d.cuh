@@ -125,7 +125,7 @@ template <int KIND, int NV, int WARPS, int R, bool FLOW>
 __device__ __forceinline__ void tile2d_body(const GridParams& g, const MoveParams& mv, const ShapeF& S, const ShapeD& SD,
                                             Control* __restrict__ ctrl, int gamma, int tile, int cap_limit, float4* __restrict__ pose,
                                             const int* __restrict__ tag, const int* __restrict__ cell_start, uint32_t k0, uint32_t k1,
-                                            uint2* __restrict__ trace, unsigned char* smem_raw)
+                                            uint2* __restrict__ trace, unsigned char* smem_raw, bool late_wait = false)
 {
     using TL = Tile2D<WARPS, R>;
     // staged poses, positions and orientations apart: the broad phase reads only (x, y), and 8-byte elements halve the
@@ -225,6 +225,7 @@ __device__ __forceinline__ void tile2d_body(const GridParams& g, const MoveParam
     }
     const bool staged = ntot <= min(cap_limit, TL::CAP);   // block-uniform
     CellCounters cc;
+    if (late_wait) pdl_wait();   // the segment table came from the cell list alone; the poses need the previous colour pass complete
 
     if (!staged) {
         // overflow: more particles around this tile than the staging buffers hold -> per-thread global path
@@ -426,12 +427,17 @@ __global__ void __launch_bounds__(32 * WARPS, MINB)
 k_sweep_tile2d(const __grid_constant__ GridParams g, const __grid_constant__ MoveParams mv, const __grid_constant__ ShapeF S,
                const __grid_constant__ ShapeD SD, Control* __restrict__ ctrl, int colour_index, int cap_limit,
                float4* __restrict__ pose, const int* __restrict__ tag, const int* __restrict__ cell_start, uint32_t k0,
-               uint32_t k1, uint2* __restrict__ trace, int tile0)
+               uint32_t k1, uint2* __restrict__ trace, int tile0, int after_colour)
 {
+    // programmatic dependent launch: see k_sweep_warpcell for the rule (first colour pass: wait, then let the next one launch;
+    // later passes: launch the next at once and wait only in front of the pose staging)
+    const bool late_wait = after_colour != 0;
+    if (!late_wait) pdl_wait();
+    pdl_launch_dependents();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     // tile0: first tile of this launch (0 unless the context runs a partition of the tile rows, hpmc_set_partition)
     tile2d_body<KIND, NV, WARPS, R, false>(g, mv, S, SD, ctrl, ctrl->hdr.perm[colour_index], tile0 + (int)blockIdx.x, cap_limit, pose, tag,
-                                           cell_start, k0, k1, trace, smem_raw);
+                                           cell_start, k0, k1, trace, smem_raw, late_wait);
 }
 
 // One launch = all four colours of a sweep, as a dataflow over (colour, tile) tickets.  A colour pass ends with a tail in
@@ -449,6 +455,7 @@ k_sweep_tile2d_flow(const __grid_constant__ GridParams g, const __grid_constant_
                     uint2* __restrict__ trace, unsigned int* __restrict__ done)
 {
     using TL = Tile2D<WARPS, R>;
+    pdl_wait();   // no early launch of the successor: this persistent grid fills every SM
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int s_ticket;
     const int nax = g.n[0] >> 1, nay = g.n[1] >> 1;

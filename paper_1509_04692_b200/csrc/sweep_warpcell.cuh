@@ -42,8 +42,16 @@ __global__ void __launch_bounds__(32 * kW3Warps)
 k_sweep_warpcell(const __grid_constant__ GridParams g, const __grid_constant__ MoveParams mv, const __grid_constant__ ShapeF S,
                const __grid_constant__ ShapeD SD, Control* __restrict__ ctrl, int colour_index, int cap_limit,
                float4* __restrict__ pos, float4* __restrict__ quat, const int* __restrict__ tag,
-               const int* __restrict__ cell_start, uint32_t k0, uint32_t k1, uint2* __restrict__ trace)
+               const int* __restrict__ cell_start, uint32_t k0, uint32_t k1, uint2* __restrict__ trace, int after_colour)
 {
+    // Programmatic dependent launch (common.cuh).  A colour pass that follows the cell-list build (or anything else): nothing can be
+    // read before that has completed, and only then may the next pass be launched.  A later pass starts while the pass
+    // before it still runs (which itself started only after the build was complete): header, cell offsets, Philox blocks and
+    // the empty-cell exits do not depend on that pass; the poses do, so the wait sits in front of the staging loads.
+    // after_colour: the launch before this one in the stream was a colour pass of the same sweep (set by the host)
+    const bool late_wait = after_colour != 0;
+    if (!late_wait) pdl_wait();
+    pdl_launch_dependents();
     __shared__ Warp3dSmem sm_all[kW3Warps];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     Warp3dSmem& sm = sm_all[warp];
@@ -92,12 +100,20 @@ k_sweep_warpcell(const __grid_constant__ GridParams g, const __grid_constant__ M
         return;
     }
     if (total > min(cap_limit, kW3Cap)) {   // warp-uniform: neighbourhood does not fit the staging buffers
+        if (late_wait) pdl_wait();
         if (lane == 0)
             sweep_cell_global<KIND, NV>(g, mv, S, SD, gamma, t_lo, t_hi16, shift, cx, cy, cz, pos, quat, tag, cell_start, k0, k1, trace, cc);
         flush_counters(ctrl, cc);
         return;
     }
     if (lane <= NNB) { sm.off[lane] = incl - my_cnt; sm.start[lane] = my_start; }   // lane 3^d: off = total
+    // a0: the Philox blocks of the first 32 trials, one trial per lane, off the critical path of the sequential trials (a trial
+    // is a chain of dependent instructions; ten Philox rounds are a quarter of it) -- and in front of the wait
+    const uint32_t c3 = (kTagTrial << 24) | ((uint32_t)gamma << 16) | t_hi16;
+    U4 blk = philox4x32_10((uint32_t)cell, t_lo, (uint32_t)lane, c3, k0, k1);
+    uint32_t blk_uc = 0u;
+    if (DIM == 3) blk_uc = philox4x32_10((uint32_t)cell, t_lo, (uint32_t)lane | (1u << 16), c3, k0, k1).x;
+    if (late_wait) pdl_wait();   // the previous colour pass is complete: its poses can be staged
     __syncwarp();
     for (int e = lane; e < total; e += 32) {
         int j = 0;   // largest j with off[j] <= e (off is non-decreasing, off[3^d] = total > e)
@@ -113,13 +129,9 @@ k_sweep_warpcell(const __grid_constant__ GridParams g, const __grid_constant__ M
     }
     __syncwarp();
 
-    const uint32_t c3 = (kTagTrial << 24) | ((uint32_t)gamma << 16) | t_hi16;
-    U4 blk{0u, 0u, 0u, 0u};
-    uint32_t blk_uc = 0u;
     for (int k = 0; k < mv.n_select; ++k) {
-        // ---- a0: the Philox blocks of the next 32 trials, one trial per lane, off the critical path of the sequential trials
-        // (a trial is a chain of dependent instructions; ten Philox rounds are a quarter of it); trial k broadcasts its block
-        if ((k & 31) == 0) {
+        // ---- a0: the blocks of the next 32 trials (the first batch was drawn above); trial k broadcasts its block
+        if ((k & 31) == 0 && k > 0) {
             blk = philox4x32_10((uint32_t)cell, t_lo, (uint32_t)(k + lane), c3, k0, k1);
             if (DIM == 3) blk_uc = philox4x32_10((uint32_t)cell, t_lo, (uint32_t)(k + lane) | (1u << 16), c3, k0, k1).x;
         }
