@@ -532,6 +532,7 @@ struct orc_sys {
     int mut_no_shift, mut_fixed_order, mut_no_leave;
     int work_detail; /* O7: also count separating axes / GJK support calls (costs extra narrow-phase work) */
     int nthreads;    /* 1 = serial (the definition); > 1 = same-colour cells as an OpenMP parallel-for */
+    uint8_t* inactive;   /* P:136-138 inactive region: layers of cells along the last axis that make no trials this sweep; NULL = none */
     int64_t probe_slot;      /* O8 "FAIL with a dump": trial slot whose pose and candidates are recorded, -1 = none */
     orc_probe probe;
     int32_t *cell_id, *cell_start, *members;
@@ -589,7 +590,7 @@ orc_sys* orc_create(int dim, const double L[3], int kind, double diameter, int n
 void orc_destroy(orc_sys* s)
 {
     if (!s) return;
-    free(s->pos); free(s->quat); free(s->cell_id); free(s->members); free(s->cell_start);
+    free(s->pos); free(s->quat); free(s->cell_id); free(s->members); free(s->cell_start); free(s->inactive);
     orc_shape_destroy(s->shape);
     free(s);
 }
@@ -626,6 +627,17 @@ int64_t orc_num_cells(const orc_sys* s) { return s->C; }
 void orc_set_mutations(orc_sys* s, int a, int b, int c) { s->mut_no_shift = a; s->mut_fixed_order = b; s->mut_no_leave = c; }
 void orc_set_work_detail(orc_sys* s, int on) { s->work_detail = on; }
 void orc_set_threads(orc_sys* s, int n) { s->nthreads = n > 1 ? n : 1; }
+int orc_set_inactive_layers(orc_sys* s, const uint8_t* mask, int32_t n)
+{
+    free(s->inactive);
+    s->inactive = NULL;
+    if (!mask) return 0;
+    if (n != s->n[s->dim - 1]) return -1;
+    s->inactive = (uint8_t*)malloc((size_t)n);
+    if (!s->inactive) return -2;
+    memcpy(s->inactive, mask, (size_t)n);
+    return 0;
+}
 void orc_set_probe(orc_sys* s, int64_t slot) { s->probe_slot = slot; memset(&s->probe, 0, sizeof s->probe); s->probe.slot = -1; }
 void orc_get_probe(const orc_sys* s, orc_probe* out) { *out = s->probe; }
 int orc_get_threads(const orc_sys* s) { return s->nthreads; }
@@ -957,6 +969,7 @@ int orc_sweep(orc_sys* s, int neighbour_mode, int reverse_cells, const uint32_t*
                 cc[2] = (int32_t)(cell / ((int64_t)s->n[0] * s->n[1]));
                 int colour = (cc[0] & 1) | ((cc[1] & 1) << 1) | ((cc[2] & 1) << 2);
                 if (colour != x.gamma) continue;
+                if (s->inactive && s->inactive[cc[s->dim - 1]]) continue;   /* inactive region: no trials, particles stay */
                 sweep_cell(s, &x, cell, cc, &lc, &lw, &lf);
             }
 #pragma omp critical

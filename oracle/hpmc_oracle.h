@@ -147,6 +147,14 @@ void orc_set_work_detail(orc_sys*, int on);
 void orc_set_threads(orc_sys*, int n);
 int orc_get_threads(const orc_sys*);
 
+/* P:134-138 (domain decomposition): "we modify the checkerboard scheme to have only two regions (active and inactive) ...
+ * these particles do not move during substeps".  Reading R-strip: the inactive region is a set of whole layers
+ * of cells along the LAST axis (rows in 2-D, z-layers in 3-D) of the sweep's shifted grid -- a cell is at least d_max wide,
+ * the paper's strip width -- and it moves with the grid shift from sweep to sweep.  mask[k] != 0: the cells of layer k make
+ * no trials (and draw no random numbers; every other cell's Philox keys are unchanged).  n must equal the grid's extent
+ * along that axis; mask = NULL clears it.  Returns 0, or < 0 on a size mismatch. */
+int orc_set_inactive_layers(orc_sys*, const uint8_t* mask, int32_t n);
+
 /* O8 dump: record the trial of `slot` (-1 = off) during the following sweeps; read it back with orc_get_probe */
 void orc_set_probe(orc_sys*, int64_t slot);
 void orc_get_probe(const orc_sys*, orc_probe* out);

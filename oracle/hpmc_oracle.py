@@ -94,6 +94,7 @@ def lib():
     L.orc_set_work_detail.argtypes = [vp, C.c_int]
     L.orc_set_threads.argtypes = [vp, C.c_int]
     L.orc_get_threads.argtypes = [vp]; L.orc_get_threads.restype = C.c_int
+    L.orc_set_inactive_layers.argtypes = [vp, C.c_void_p, C.c_int32]; L.orc_set_inactive_layers.restype = C.c_int
     L.orc_set_probe.argtypes = [vp, C.c_int64]
     L.orc_get_probe.argtypes = [vp, C.POINTER(Probe)]
     L.orc_textbook_trials.argtypes = [vp, C.c_int64]; L.orc_textbook_trials.restype = C.c_int
@@ -292,6 +293,14 @@ class Oracle:
     def set_threads(self, n):
         """n > 1: same-colour cells as an OpenMP parallel-for (identical results, P4); 1 = serial (default)."""
         lib().orc_set_threads(self._h, int(n))
+
+    def set_inactive_layers(self, mask):
+        """layers of cells along the last axis that make no trials (mask: n[dim-1] bytes; None clears)."""
+        if mask is None:
+            assert lib().orc_set_inactive_layers(self._h, None, 0) == 0
+            return
+        m = np.ascontiguousarray(mask, dtype=np.uint8)
+        assert lib().orc_set_inactive_layers(self._h, m.ctypes.data_as(C.c_void_p), int(m.size)) == 0, "mask size != grid extent"
 
     def set_probe(self, slot):
         """O8 dump: record the trial pose and candidates of `slot` during the following sweeps (-1 = off)."""
