@@ -341,12 +341,14 @@ def run_reference(args):
 
 
 def run_partitioned(args, D):
-    """--partition: ONE system on all ranks (paper_1509_04692_b200/partition.py): replicated state, the colour-pass tiles of a
-    slab of cell rows per rank, boundary rows after every colour and the slabs after the last over NCCL.  Same step, metric
-    and timing rules as the default arm; "scaling": "strong"."""
+    """--partition: ONE system on all ranks (paper_1509_04692_b200/partition.py).  "replicated": every rank holds the whole
+    state and runs the colour-pass tiles of a slab of cell rows, boundary rows after every colour and the slabs after the last
+    over NCCL.  "distributed": every rank holds its slab and one ghost row, the last row of a slab is the inactive region of
+    the sweep, particles are routed between neighbouring ranks once per sweep.  Same step, metric and timing rules
+    as the default arm; "scaling": "strong"."""
     import torch
     from paper_1509_04692_b200 import binding as hb
-    from paper_1509_04692_b200.partition import DistributedRank, LocalRanks
+    from paper_1509_04692_b200.partition import DistributedRank, DistributedState, pose_of
     device = f"cuda:{D.local}"
     torch.cuda.set_device(D.local)
     w = wl.config(args.config, seed=1)               # the SAME system and Philox seed on every rank
@@ -355,9 +357,15 @@ def run_partitioned(args, D):
     g.set_option("path", 2); g.set_option("flow", 0)
     assert g.count_overlaps() == 0
     g.sweep(w.warmup_sweeps)                         # melt: every rank on its own (identical trajectories)
-    runner = DistributedRank(g, D.dist) if D.on else None
-    if runner is None:                               # one rank: the same phase calls, nothing to exchange
+    distributed = args.partition == "distributed"
+    if not D.on:                                     # one rank: the same phase calls, nothing to exchange
+        runner = None
         g.set_partition(0, 1)
+    elif distributed:                                # hand every rank the melted state; it keeps its slab and ghost row
+        p, q = g.get_state()
+        runner = DistributedState(g, D.dist, torch.from_numpy(pose_of(p, q)).to(device), torch.arange(w.N, dtype=torch.int32, device=device))
+    else:
+        runner = DistributedRank(g, D.dist)
 
     def one_step():
         if runner is not None:
@@ -394,8 +402,10 @@ def run_partitioned(args, D):
                           "warmup": args.warmup, "ms_per_step": 1e3 * t_max / args.steps, "higher_is_better": True, "scaling": "strong",
                           "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                           "config": {"workload": w.name, "N": w.N, "cells": g.C,
-                                     "parallelism": f"{args.gpus} ranks: partitioned colour passes over a replicated state, boundary rows "
-                                                    "exchanged after every colour, slabs after the last (NCCL)",
+                                     "parallelism": (f"{args.gpus} ranks: distributed state (slab + ghost row per rank), last cell row of every "
+                                                     "slab inactive during the sweep, particles routed once per sweep (NCCL)") if distributed else
+                                                    (f"{args.gpus} ranks: partitioned colour passes over a replicated state, boundary rows "
+                                                     "exchanged after every colour, slabs after the last (NCCL)"),
                                      "l2": "flushed between steps" if fbuf is not None else "not flushed"},
                           "particle_sweeps_per_sec": w.N * args.steps / t_max, "trials_per_step": trials_all / args.steps,
                           "gpu_launches": int(D.reduce(g.launch_count(), "SUM")), "roofline": None, "clocks": clocks}), flush=True)
@@ -442,9 +452,11 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-flush", action="store_true", help="do not evict L2 between steps (L2-resident number)")
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, cpu_baseline and the small-system line")
-    ap.add_argument("--partition", action="store_true",
-                    help="--gpus N as ONE system: every rank holds the whole state and runs the colour-pass tiles of its own slab of "
-                         "cell rows, boundary rows exchanged after every colour (strong scaling; 2-D configs; default: N replicas)")
+    ap.add_argument("--partition", nargs="?", const="replicated", default=None, choices=["replicated", "distributed"],
+                    help="--gpus N as ONE system (strong scaling; 2-D configs; default: N replicas).  replicated: every rank holds the "
+                         "whole state and runs the colour-pass tiles of its own slab of cell rows, boundary rows exchanged after every "
+                         "colour.  distributed: every rank holds its slab and a ghost row, the last row of a slab is inactive during the "
+                         "sweep (the paper's scheme, P:128-151), particles are routed once per sweep")
     ap.add_argument("--paper-states", action="store_true",
                     help="also prepare and time the paper's own benchmark states (65 536 pentagons at phi = 0.676 with tuned moves, "
                          "32 768 dodecahedra at phi = 0.5; P:183, P:237): about two more minutes")

@@ -195,6 +195,43 @@ int hpmc_partition_rows(const hpmc_ctx* ctx, int rank, int nranks, int32_t* h_ro
 int hpmc_row_offsets(hpmc_ctx* ctx, const int32_t* h_rows, int n, int64_t* h_offsets);
 int hpmc_sorted_pose(hpmc_ctx* ctx, void** d_pose);
 
+/* ---- One system on several GPUs: distributed state with an inactive region -----------------
+ * "Each rank covers a portion of the simulation box and owns all of the particles in that region"; "we modify the
+ * checkerboard scheme to have only two regions (active and inactive) ... these particles do not move during substeps.
+ * Communication between ranks only occurs at the end of the step".
+ *
+ *   hpmc_set_inactive_layers  h_mask: n = (grid extent along the LAST axis) bytes, host; layer k of cells (a cell row in 2-D, a
+ *                        z-layer in 3-D) makes no trials while h_mask[k] != 0 (reading R-strip: the strip is whole cells of the
+ *                        sweep's shifted grid, >= d_max wide, and moves with the grid shift).  NULL clears.  Works for every
+ *                        colour-pass kernel but the cluster pass, with or without a partition; results match the oracle's
+ *                        orc_set_inactive_layers.  The mask is copied; synchronises.
+ *
+ * With hpmc_set_partition(rank, nranks >= 2) and a mask that flags the LAST cell row of every slab, a context no longer needs
+ * the whole state: during a sweep its tiles read rows [r0 - 1, r1) only, and row r0 - 1 -- the inactive last row of the slab
+ * below -- does not change.  Such a context holds its own slab plus that ghost row, under GLOBAL tags (the members of a cell
+ * are ordered by tag, so the trajectory equals the single-context one with the same mask), and once per sweep the caller
+ * moves particles between the contexts (the paper's stage 9).  2-D, tile pass, no trace; N of hpmc_create is the capacity.
+ *   hpmc_dist_load     n <= capacity particles as device arrays: poses (x, y, qw, qz) and int32 global tags, any order; they
+ *                      become the context's state (hpmc_get_state no longer applies: read hpmc_sorted_pose / hpmc_sorted_tags)
+ *   hpmc_dist_route    classify the particles for the grid of the NEXT sweep (header of the current sweep counter) with the
+ *                      pinned cell function: keep rows r0 - 1 .. r1 - 1; copy rows r1 - 1 and r1 to the `up` buffers (for the
+ *                      context above) and row r0 - 1 to the `down` buffers (for the one below); drop the rest.
+ *                      owned_only = 1: after a sweep -- only the own slab is classified (the old ghost row is dropped) and a
+ *                      particle that fits no class is an error; 0: after hpmc_dist_load of a superset -- foreign particles are
+ *                      dropped silently.  h_counts4 (host) = kept, up, down, unclassified.  Synchronises.  HPMC_E_ARG when a
+ *                      send buffer is too small (counts are still returned; the state is then undefined).
+ *   hpmc_dist_append   n received particles behind the kept ones
+ *   hpmc_local_count   particles the context holds now
+ *   hpmc_sorted_tags   device pointer of the tags that go with hpmc_sorted_pose
+ * One sweep of a distributed system: phase -1, phases 0..3 (no exchange in between), hpmc_dist_route, exchange, hpmc_dist_append. */
+int hpmc_set_inactive_layers(hpmc_ctx* ctx, const uint8_t* h_mask, int32_t n);
+int hpmc_dist_load(hpmc_ctx* ctx, const float* d_pose4, const int32_t* d_tags, int64_t n);
+int hpmc_dist_route(hpmc_ctx* ctx, int owned_only, float* d_up_pose4, int32_t* d_up_tags, int64_t cap_up, float* d_down_pose4,
+                    int32_t* d_down_tags, int64_t cap_down, int64_t* h_counts4);
+int hpmc_dist_append(hpmc_ctx* ctx, const float* d_pose4, const int32_t* d_tags, int64_t n);
+int64_t hpmc_local_count(const hpmc_ctx* ctx);
+int hpmc_sorted_tags(hpmc_ctx* ctx, void** d_tags);
+
 /* Diagnostic tallies kept on the device (synchronises).  Names:
  *   "gjk_f64_reruns"  polyhedron pairs whose fp32 GJK verdict was "unsure" (near contact, or a degenerate simplex) and that
  *                     were decided by the fp64 re-run from the raw fp32 state -- the mixed-precision path of P:106-108,

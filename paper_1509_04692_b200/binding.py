@@ -18,7 +18,8 @@ ABI_SYMBOLS = ["hpmc_create", "hpmc_destroy", "hpmc_last_error", "hpmc_get_grid"
                "hpmc_set_moves", "hpmc_sweep", "hpmc_count_overlaps", "hpmc_get_state", "hpmc_set_sweep_counter",
                "hpmc_reset_counters", "hpmc_set_trace", "hpmc_get_cell_list", "hpmc_sweep_host", "hpmc_set_option", "hpmc_set_profile",
                "hpmc_get_profile", "hpmc_launch_count", "hpmc_describe_pass", "hpmc_get_stat", "hpmc_measure_fp32_peak", "hpmc_set_partition", "hpmc_sweep_phase",
-               "hpmc_partition_rows", "hpmc_row_offsets", "hpmc_sorted_pose"]
+               "hpmc_partition_rows", "hpmc_row_offsets", "hpmc_sorted_pose", "hpmc_set_inactive_layers", "hpmc_dist_load",
+               "hpmc_dist_route", "hpmc_dist_append", "hpmc_local_count", "hpmc_sorted_tags"]
 
 
 class HpmcError(RuntimeError):
@@ -85,9 +86,15 @@ def load_library():
     L.hpmc_partition_rows.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     L.hpmc_row_offsets.argtypes = [vp, C.POINTER(C.c_int32), C.c_int, C.POINTER(C.c_int64)]
     L.hpmc_sorted_pose.argtypes = [vp, C.POINTER(vp)]
+    L.hpmc_sorted_tags.argtypes = [vp, C.POINTER(vp)]
+    L.hpmc_set_inactive_layers.argtypes = [vp, vp, C.c_int32]
+    L.hpmc_dist_load.argtypes = [vp, vp, vp, C.c_int64]
+    L.hpmc_dist_route.argtypes = [vp, C.c_int, vp, vp, C.c_int64, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
+    L.hpmc_dist_append.argtypes = [vp, vp, vp, C.c_int64]
+    L.hpmc_local_count.argtypes = [vp]; L.hpmc_local_count.restype = C.c_int64
     L.hpmc_describe_pass.argtypes = [vp, C.c_char_p, C.c_size_t]
     for name in ABI_SYMBOLS:
-        if name not in ("hpmc_last_error", "hpmc_workspace_bytes", "hpmc_launch_count"):
+        if name not in ("hpmc_last_error", "hpmc_workspace_bytes", "hpmc_launch_count", "hpmc_local_count"):
             getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -277,12 +284,52 @@ class Hpmc:
         return [int(x) for x in o]
 
     def sorted_pose(self):
-        """The current cell-sorted pose array as a torch view (N, 4) into the workspace (valid until the next build)."""
+        """The current cell-sorted pose array as a torch view (local count, 4) into the workspace (valid until the next build)."""
         p = C.c_void_p()
         self._check(self._lib.hpmc_sorted_pose(self._h, C.byref(p)))
+        n = self.local_count()
         off = int(p.value) - self.workspace.data_ptr()
-        assert 0 <= off and off + 16 * self.N <= self.workspace.numel()
-        return self.workspace[off:off + 16 * self.N].view(self._torch.float32).view(self.N, 4)
+        assert 0 <= off and off + 16 * n <= self.workspace.numel()
+        return self.workspace[off:off + 16 * n].view(self._torch.float32).view(n, 4)
+
+    def sorted_tags(self):
+        """The tags that go with sorted_pose(), as a torch int32 view into the workspace."""
+        p = C.c_void_p()
+        self._check(self._lib.hpmc_sorted_tags(self._h, C.byref(p)))
+        n = self.local_count()
+        off = int(p.value) - self.workspace.data_ptr()
+        assert 0 <= off and off + 4 * n <= self.workspace.numel()
+        return self.workspace[off:off + 4 * n].view(self._torch.int32)
+
+    def local_count(self):
+        return int(self._lib.hpmc_local_count(self._h))
+
+    def set_inactive_layers(self, mask):
+        """layers of cells along the last axis that make no trials (n[dim-1] bytes; None clears)."""
+        if mask is None:
+            self._check(self._lib.hpmc_set_inactive_layers(self._h, None, 0))
+            return
+        m = np.ascontiguousarray(mask, dtype=np.uint8)
+        self._check(self._lib.hpmc_set_inactive_layers(self._h, m.ctypes.data_as(C.c_void_p), int(m.size)))
+
+    def dist_load(self, pose4, tags):
+        """Distributed state: `pose4` (n, 4) float32 (x, y, qw, qz) and `tags` (n,) int32 global ids, device tensors."""
+        assert pose4.is_cuda and tags.is_cuda and pose4.dtype == self._torch.float32 and tags.dtype == self._torch.int32
+        pose4, tags = pose4.contiguous(), tags.contiguous()
+        with self._torch.cuda.stream(self.stream):
+            self._check(self._lib.hpmc_dist_load(self._h, pose4.data_ptr(), tags.data_ptr(), int(tags.numel())))
+        self.stream.synchronize()            # the sources may be temporaries
+
+    def dist_route(self, owned_only, up_pose, up_tags, down_pose, down_tags):
+        """Classify for the next sweep's grid; fills the caller's send buffers; returns (kept, up, down, unclassified)."""
+        cnt = (C.c_int64 * 4)()
+        self._check(self._lib.hpmc_dist_route(self._h, int(bool(owned_only)), up_pose.data_ptr(), up_tags.data_ptr(), int(up_tags.numel()),
+                                              down_pose.data_ptr(), down_tags.data_ptr(), int(down_tags.numel()), cnt))
+        return tuple(int(x) for x in cnt)
+
+    def dist_append(self, pose4, tags, n):
+        if n:
+            self._check(self._lib.hpmc_dist_append(self._h, pose4.data_ptr(), tags.data_ptr(), int(n)))
 
     def get_stat(self, name):
         v = C.c_int64()

@@ -23,7 +23,13 @@ struct GridParams {
     float inv_w[3];   // (float)(n/L), R13
     float w_f[3];     // (float)(L/n), scale of the grid shift, R10
     double Ld[3];     // (double)L for the fp64 seam subtraction, R21
+    // P:134-138 inactive region (R-strip): n[dim-1] bytes, one per layer of cells along the last axis; the cells of a flagged
+    // layer make no trials this sweep.  nullptr = none.  Static between hpmc_set_inactive_layers calls: any kernel may read
+    // it in front of its programmatic-launch wait.
+    const unsigned char* inactive;
 };
+
+__device__ __forceinline__ bool layer_inactive(const GridParams& g, int layer) { return g.inactive != nullptr && g.inactive[layer] != 0; }
 
 struct MoveParams {
     float d, a;       // R5, R6
@@ -53,6 +59,7 @@ struct Control {
     unsigned long long overlaps;     // validator result
     unsigned int flow_ticket, flow_exited;   // k_sweep_tile2d_flow: next (colour, tile) ticket; CTAs that have left
     unsigned int bad_coords, pad_bc;         // particles whose coordinates were not finite or not in [-L/2, L/2) when a cell list was built
+    unsigned int route[4];                   // k_route: particles kept / sent up / sent down / fitting no class
     SweepHeader hdr;
 };
 

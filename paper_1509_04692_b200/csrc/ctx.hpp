@@ -53,6 +53,11 @@ struct hpmc_ctx {
                                          // read the cell list before waiting)
     bool flow_now = false;               // this sweep's colour passes go out as one dataflow launch
     Control* ctrl = nullptr;
+    int n_cap = 0;                                  // particles the workspace holds (N of hpmc_create); g.N <= n_cap varies with a distributed state
+    bool cell_valid = false;                        // cell_start describes the arrays of `cur` (false after a route / append / load)
+    bool dist = false;                              // distributed state: tags are global ids, the bound arrays are not used
+    unsigned char* d_inactive = nullptr;            // workspace slot of the inactive-region mask (g.inactive points here while any layer is flagged)
+    std::vector<unsigned char> inactive_h;          // host copy (survives a re-bind)
 
     uint2* trace = nullptr;
     int64_t trace_words = 0;

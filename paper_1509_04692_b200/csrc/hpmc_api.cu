@@ -11,6 +11,7 @@
 #include "../../include/hpmc.h"
 #include "cell_list.cuh"
 #include "common.cuh"
+#include "dist.cuh"
 #include "overlap.cuh"
 #include "sweep.cuh"
 #include "ctx.hpp"
@@ -70,14 +71,14 @@ size_t flow_words(const hpmc_ctx* c)
 }
 
 struct Layout {
-    size_t pos[2], quat[2], tag[2], key_rank, cell_start, counts, arrived, tile_sums, flow_done, ctrl, total;
+    size_t pos[2], quat[2], tag[2], key_rank, cell_start, counts, arrived, tile_sums, flow_done, ctrl, inactive, total;
 };
 
 Layout layout_of(const hpmc_ctx* c)
 {
     Layout L{};
     Carve cv;
-    const size_t N = (size_t)(c->g.N > 0 ? c->g.N : 1);
+    const size_t N = (size_t)(c->n_cap > 0 ? c->n_cap : 1);
     for (int b = 0; b < 2; ++b) {
         L.pos[b] = cv.take(N * sizeof(float4));
         L.quat[b] = cv.take(c->g.dim == 3 ? N * sizeof(float4) : 0);   // 2-D keeps one pose array
@@ -90,6 +91,7 @@ Layout layout_of(const hpmc_ctx* c)
     L.tile_sums = cv.take((size_t)(scan_tiles(c) + 1) * sizeof(int));
     L.flow_done = cv.take(flow_words(c) * sizeof(unsigned int));
     L.ctrl = cv.take(sizeof(Control));
+    L.inactive = cv.take((size_t)c->g.n[c->g.dim - 1]);   // inactive-region mask, one byte per layer of cells along the last axis
     L.total = cv.off;
     return L;
 }
@@ -270,6 +272,7 @@ int build_cell_list(hpmc_ctx* c, int mode, unsigned long long t_override)
         c->cur = dst;
         c->state_in_bound = false;
         c->have_sorted = true;
+        c->cell_valid = true;
         return HPMC_OK;
     }
     const int nblk_part = (g.N + TB - 1) / TB;
@@ -298,6 +301,7 @@ int build_cell_list(hpmc_ctx* c, int mode, unsigned long long t_override)
     c->cur = dst;
     c->state_in_bound = false;
     c->have_sorted = true;
+    c->cell_valid = true;
     return HPMC_OK;
 }
 
@@ -337,7 +341,7 @@ constexpr int kClusterMaxCtas = 16, kClusterThreads = 1024, kClusterMaxCells = 1
 bool cluster_eligible(const hpmc_ctx* c)
 {
     const GridParams& g = c->g;
-    if (g.dim != 2 || c->sf.kind == kKindPolyhedron || c->cluster_ctas == 0 || c->part_n > 1) return false;
+    if (g.dim != 2 || c->sf.kind == kKindPolyhedron || c->cluster_ctas == 0 || c->part_n > 1 || g.inactive) return false;
     if (g.N < 1 || g.N > kClusterMaxCtas * kClusterThreads || g.C + 2 > kClusterMaxCells) return false;
     // measured on B200 (profiles/r2_cluster.md): 58 us per sweep of 4096 pentagons against 39 us for the graph of five launches --
     // a trial is a ~2 us dependent chain either way and seven cluster barriers do not beat four launch gaps -- so the pass is
@@ -446,6 +450,7 @@ int hpmc_create(const hpmc_box* box, const hpmc_shape* shape, int64_t N, uint64_
     GridParams& g = c->g;
     g.dim = box->dim;
     g.N = (int)N;
+    c->n_cap = (int)N;
     double cells = 1.0;
     for (int k = 0; k < 3; ++k) {
         if (k < g.dim) {
@@ -514,6 +519,20 @@ int hpmc_get_grid(const hpmc_ctx* c, hpmc_grid_info* o)
     return HPMC_OK;
 }
 
+// the host copy of the inactive-region mask -> its slot in the workspace; g.inactive stays NULL while no layer is flagged
+static int upload_inactive(hpmc_ctx* c)
+{
+    bool any = false;
+    for (unsigned char b : c->inactive_h) any = any || b != 0;
+    c->g.inactive = nullptr;
+    if (!any || !c->d_inactive) return HPMC_OK;
+    if (!cuda_ok(c, cudaMemcpyAsync(c->d_inactive, c->inactive_h.data(), c->inactive_h.size(), cudaMemcpyHostToDevice, c->stream), "inactive/memcpy"))
+        return HPMC_E_CUDA;
+    if (!cuda_ok(c, cudaStreamSynchronize(c->stream), "inactive/sync")) return HPMC_E_CUDA;
+    c->g.inactive = c->d_inactive;
+    return HPMC_OK;
+}
+
 size_t hpmc_workspace_bytes(const hpmc_ctx* c) { return c ? layout_of(c).total : 0; }
 
 int hpmc_bind(hpmc_ctx* c, float* d_pos4, float* d_quat4, void* d_workspace, size_t bytes)
@@ -544,6 +563,8 @@ int hpmc_bind(hpmc_ctx* c, float* d_pos4, float* d_quat4, void* d_workspace, siz
     c->tile_sums = (int*)(c->d_ws + L.tile_sums);
     c->flow_done = (unsigned int*)(c->d_ws + L.flow_done);
     c->ctrl = (Control*)(c->d_ws + L.ctrl);
+    c->d_inactive = (unsigned char*)(c->d_ws + L.inactive);
+    if (upload_inactive(c) != HPMC_OK) return HPMC_E_CUDA;
     if (first) {  // a new workspace: zero the builder's scratch, (re)create the control block, keeping the host-side sweep counter
         if (!cuda_ok(c, cudaMemsetAsync(c->d_ws + L.counts, 0, L.ctrl - L.counts, c->stream), "bind/memset")) return HPMC_E_CUDA;
         Control& init = c->h_ctrl;
@@ -557,6 +578,8 @@ int hpmc_bind(hpmc_ctx* c, float* d_pos4, float* d_quat4, void* d_workspace, siz
     c->state_in_bound = true;
     c->have_sorted = false;
     c->cur = 0;
+    c->dist = false;          // a bound state is a whole state in tag order
+    c->g.N = c->n_cap;
     return HPMC_OK;
 }
 
@@ -577,6 +600,7 @@ int hpmc_sweep(hpmc_ctx* c, int64_t n)
     int rc = check_ready(c);
     if (rc != HPMC_OK) return rc;
     if (n < 0) return fail(c, HPMC_E_ARG, "n must be >= 0");
+    if (c->dist) return fail(c, HPMC_E_ARG, "distributed state: sweeps go through hpmc_sweep_phase and hpmc_dist_route");
     if (c->trace && c->trace_words < 2 * (int64_t)c->g.C * c->mv.n_select) return fail(c, HPMC_E_TRACE, "trace buffer too small");
     int64_t s = 0;
     // Small 2-D systems: whole sweeps inside one thread-block cluster, any number per launch (sweep_cluster2d.cuh)
@@ -664,6 +688,8 @@ int hpmc_get_state(hpmc_ctx* c, float* d_pos4_out, float* d_quat4_out, hpmc_coun
     DeviceGuard dev_guard(c);
     int rc = check_ready(c);
     if (rc != HPMC_OK) return rc;
+    if ((d_pos4_out || d_quat4_out) && c->dist)
+        return fail(c, HPMC_E_ARG, "distributed state: tags are global ids; read hpmc_sorted_pose / hpmc_sorted_tags");
     if ((d_pos4_out || d_quat4_out) && c->g.N > 0) {
         if (c->state_in_bound) {  // nothing ran since bind: the bound arrays are the state
             const size_t bytes = (size_t)c->g.N * sizeof(float4);
@@ -774,6 +800,8 @@ int hpmc_sweep_host(hpmc_ctx* c, const float* h_pos4, const float* h_quat4, int6
     if (!cuda_ok(c, cudaMemcpyAsync(c->d_quat_bound, h_quat4, bytes, cudaMemcpyHostToDevice, c->stream), "sweep_host/h2d")) return HPMC_E_CUDA;
     c->state_in_bound = true;
     c->have_sorted = false;
+    c->dist = false;
+    c->g.N = c->n_cap;
     int rc = hpmc_sweep(c, n);
     if (rc != HPMC_OK) return rc;
     rc = hpmc_get_state(c, (float*)c->d_pos_bound, (float*)c->d_quat_bound, nullptr, nullptr);
@@ -889,6 +917,18 @@ int hpmc_set_partition(hpmc_ctx* c, int rank, int nranks)
     return HPMC_OK;
 }
 
+int hpmc_set_inactive_layers(hpmc_ctx* c, const uint8_t* h_mask, int32_t n)
+{
+    DeviceGuard dev_guard(c);
+    if (!c) return HPMC_E_ARG;
+    if (c->cuda_failed) return HPMC_E_CUDA;
+    if (h_mask && n != c->g.n[c->g.dim - 1]) return fail(c, HPMC_E_ARG, "mask length must be the grid extent along the last axis");
+    graph_reset(c);   // a captured sweep carries the old grid parameters
+    if (h_mask) c->inactive_h.assign(h_mask, h_mask + n);
+    else c->inactive_h.clear();
+    return upload_inactive(c);
+}
+
 int hpmc_sweep_phase(hpmc_ctx* c, int phase)
 {
     DeviceGuard dev_guard(c);
@@ -900,7 +940,7 @@ int hpmc_sweep_phase(hpmc_ctx* c, int phase)
         return rc;
     }
     if (phase < 0 || phase >= (1 << c->g.dim)) return fail(c, HPMC_E_ARG, "phase must be -1 (build) or a colour index");
-    if (!c->have_sorted) return fail(c, HPMC_E_UNBOUND, "no cell list: run phase -1 first");
+    if (!c->have_sorted || (c->dist && !c->cell_valid)) return fail(c, HPMC_E_UNBOUND, "no cell list: run phase -1 first");
     return launch_colour_dispatch(c, phase);
 }
 
@@ -928,6 +968,102 @@ int hpmc_row_offsets(hpmc_ctx* c, const int32_t* h_rows, int n, int64_t* h_offse
     }
     if (!cuda_ok(c, cudaStreamSynchronize(c->stream), "rows/sync")) return HPMC_E_CUDA;
     for (int i = 0; i < n; ++i) h_offsets[i] = vals[i];
+    return HPMC_OK;
+}
+
+int hpmc_sorted_tags(hpmc_ctx* c, void** d_tags)
+{
+    int rc = check_ready(c);
+    if (rc != HPMC_OK) return rc;
+    if (!d_tags) return fail(c, HPMC_E_ARG, "d_tags is NULL");
+    if (!c->have_sorted) return fail(c, HPMC_E_UNBOUND, "no cell-sorted state yet");
+    *d_tags = c->tag[c->cur];
+    return HPMC_OK;
+}
+
+int64_t hpmc_local_count(const hpmc_ctx* c) { return c ? c->g.N : 0; }
+
+static int dist_ready(hpmc_ctx* c)
+{
+    int rc = check_ready(c);
+    if (rc != HPMC_OK) return rc;
+    if (c->g.dim != 2 || c->part_n < 2) return fail(c, HPMC_E_ARG, "distributed state: 2-D, after hpmc_set_partition with nranks >= 2");
+    if (c->trace) return fail(c, HPMC_E_ARG, "distributed state keeps no trace");
+    return HPMC_OK;
+}
+
+int hpmc_dist_load(hpmc_ctx* c, const float* d_pose4, const int32_t* d_tags, int64_t n)
+{
+    DeviceGuard dev_guard(c);
+    int rc = dist_ready(c);
+    if (rc != HPMC_OK) return rc;
+    if (n < 0 || n > c->n_cap) return fail(c, HPMC_E_ARG, "more particles than the context was created for");
+    if (n > 0 && (!d_pose4 || !d_tags)) return fail(c, HPMC_E_ARG, "NULL device pointer");
+    graph_reset(c);
+    c->cur = 0;
+    if (n > 0) {
+        if (!cuda_ok(c, cudaMemcpyAsync(c->pos[0], d_pose4, (size_t)n * sizeof(float4), cudaMemcpyDeviceToDevice, c->stream), "dist_load/copy")) return HPMC_E_CUDA;
+        if (!cuda_ok(c, cudaMemcpyAsync(c->tag[0], d_tags, (size_t)n * sizeof(int), cudaMemcpyDeviceToDevice, c->stream), "dist_load/copy")) return HPMC_E_CUDA;
+    }
+    c->g.N = (int)n;
+    c->dist = true;
+    c->state_in_bound = false;
+    c->have_sorted = true;     // "sorted" arrays hold the state (no cell list yet: cell_valid is false until phase -1)
+    c->cell_valid = false;
+    c->after_colour = false;
+    return HPMC_OK;
+}
+
+int hpmc_dist_route(hpmc_ctx* c, int owned_only, float* d_up_pose4, int32_t* d_up_tags, int64_t cap_up, float* d_down_pose4,
+                    int32_t* d_down_tags, int64_t cap_down, int64_t* h_counts4)
+{
+    DeviceGuard dev_guard(c);
+    int rc = dist_ready(c);
+    if (rc != HPMC_OK) return rc;
+    if (!c->dist) return fail(c, HPMC_E_UNBOUND, "no distributed state: hpmc_dist_load first");
+    if (!h_counts4 || cap_up < 0 || cap_down < 0 || (cap_up > 0 && (!d_up_pose4 || !d_up_tags)) || (cap_down > 0 && (!d_down_pose4 || !d_down_tags)))
+        return fail(c, HPMC_E_ARG, "NULL buffer");
+    if (owned_only && !c->cell_valid) return fail(c, HPMC_E_UNBOUND, "owned_only needs the cell list of the sweep just made");
+    int r0, r1;
+    slab_rows(c, c->part_rank, c->part_n, r0, r1);
+    if (r1 - r0 < 2) return fail(c, HPMC_E_ARG, "a slab needs at least two cell rows");
+    if (!cuda_ok(c, cudaMemsetAsync(c->ctrl->route, 0, sizeof(unsigned int) * 4, c->stream), "route/memset")) return HPMC_E_CUDA;
+    const int dst = c->cur ^ 1;
+    if (c->g.N > 0) {
+        const int TB = 256;
+        k_route<<<(c->g.N + TB - 1) / TB, TB, 0, c->stream>>>(c->g, c->ctrl, c->k0, c->k1, owned_only ? 1 : 0, r0, r1, c->pos[c->cur], c->tag[c->cur],
+                                                              c->cell_start, c->pos[dst], c->tag[dst], (float4*)d_up_pose4, d_up_tags,
+                                                              (int)std::min<int64_t>(cap_up, 2147483647), (float4*)d_down_pose4, d_down_tags,
+                                                              (int)std::min<int64_t>(cap_down, 2147483647), c->ctrl->route);
+        ++c->launches;
+        if (!cuda_ok(c, cudaGetLastError(), "k_route")) return HPMC_E_CUDA;
+    }
+    unsigned int h[4] = {0, 0, 0, 0};
+    if (!cuda_ok(c, cudaMemcpyAsync(h, c->ctrl->route, sizeof h, cudaMemcpyDeviceToHost, c->stream), "route/memcpy")) return HPMC_E_CUDA;
+    if (!cuda_ok(c, cudaStreamSynchronize(c->stream), "route/sync")) return HPMC_E_CUDA;
+    for (int k = 0; k < 4; ++k) h_counts4[k] = h[k];
+    c->cur = dst;
+    c->g.N = (int)h[0];
+    c->cell_valid = false;
+    c->after_colour = false;
+    if ((int64_t)h[1] > cap_up || (int64_t)h[2] > cap_down) return fail(c, HPMC_E_ARG, "send buffer too small (counts returned)");
+    if (owned_only && h[3] != 0) return fail(c, HPMC_E_ARG, "a particle moved more than one cell row between two sweeps");
+    return HPMC_OK;
+}
+
+int hpmc_dist_append(hpmc_ctx* c, const float* d_pose4, const int32_t* d_tags, int64_t n)
+{
+    DeviceGuard dev_guard(c);
+    int rc = dist_ready(c);
+    if (rc != HPMC_OK) return rc;
+    if (!c->dist) return fail(c, HPMC_E_UNBOUND, "no distributed state: hpmc_dist_load first");
+    if (n < 0 || (int64_t)c->g.N + n > c->n_cap) return fail(c, HPMC_E_ARG, "more particles than the context was created for");
+    if (n == 0) return HPMC_OK;
+    if (!d_pose4 || !d_tags) return fail(c, HPMC_E_ARG, "NULL device pointer");
+    if (!cuda_ok(c, cudaMemcpyAsync(c->pos[c->cur] + c->g.N, d_pose4, (size_t)n * sizeof(float4), cudaMemcpyDeviceToDevice, c->stream), "dist_append/copy")) return HPMC_E_CUDA;
+    if (!cuda_ok(c, cudaMemcpyAsync(c->tag[c->cur] + c->g.N, d_tags, (size_t)n * sizeof(int), cudaMemcpyDeviceToDevice, c->stream), "dist_append/copy")) return HPMC_E_CUDA;
+    c->g.N += (int)n;
+    c->cell_valid = false;
     return HPMC_OK;
 }
 

@@ -176,7 +176,7 @@ __device__ void sweep_cell_global(const GridParams& g, const MoveParams& mv, con
         const int cell = cx + g.n[0] * (cy + g.n[1] * cz);
         const int start = cell_start[cell], nmem = cell_start[cell + 1] - start;
         const long long slot0 = (long long)cell * mv.n_select;
-        if (nmem == 0) {
+        if (nmem == 0 || layer_inactive(g, g.dim == 3 ? cz : cy)) {
             if (trace)
                 for (int k = 0; k < mv.n_select; ++k) trace[slot0 + k] = make_uint2(0u, 0u);
         } else {

@@ -273,7 +273,7 @@ __device__ __forceinline__ void tile2d_body(const GridParams& g, const MoveParam
         int nmem = 0;
         if (valid) {
             const int lc = (2 * ay + 1) * RW + 2 * lane + 1;
-            nmem = (int)sm_lstart[lc + 1] - (int)sm_lstart[lc];
+            nmem = layer_inactive(g, cy0 + 2 * ay) ? 0 : (int)sm_lstart[lc + 1] - (int)sm_lstart[lc];   // an inactive row makes no trials
             if (nmem == 0 && trace) {
                 const long long slot0 = (long long)((cx0 + 2 * lane) + n0 * (cy0 + 2 * ay)) * mv.n_select;
                 for (int k = 0; k < mv.n_select; ++k) trace[slot0 + k] = make_uint2(0u, 0u);

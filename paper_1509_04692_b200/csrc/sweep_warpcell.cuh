@@ -94,7 +94,7 @@ k_sweep_warpcell(const __grid_constant__ GridParams g, const __grid_constant__ M
     const int own_s = __shfl_sync(0xffffffffu, incl - my_cnt, OWN);
     const int nmem = __shfl_sync(0xffffffffu, my_cnt, OWN);
     CellCounters cc;
-    if (nmem == 0) {
+    if (nmem == 0 || layer_inactive(g, DIM == 3 ? cz : cy)) {   // empty, or in the inactive region: no trials
         if (trace && lane == 0)
             for (int k = 0; k < mv.n_select; ++k) trace[slot0 + k] = make_uint2(0u, 0u);
         return;

@@ -77,3 +77,59 @@ def test_exchange_and_gather_with_two_gloo_ranks(tmp_path):
                             "--master-port", str(29640 + world), str(script), ROOT], capture_output=True, text=True, timeout=300)
         assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
         assert r.stdout.count("ok") == world
+
+
+MIGRANT_WORKER = r'''
+import os, sys
+import numpy as np, torch, torch.distributed as dist
+sys.path.insert(0, sys.argv[1])
+from paper_1509_04692_b200 import partition as pt
+dist.init_process_group("gloo")
+rank, n = dist.get_rank(), dist.get_world_size()
+slabs = pt.reference_rows(26, 2, n)
+below, above = pt.neighbours(rank, slabs)
+assert below == (rank - 1) % n and above == (rank + 1) % n
+
+def payload(r, which, step):                       # what rank r sends up (which = 0) / down (1) in `step`: sizes vary, some empty
+    k = (3 * r + 5 * which + 2 * step) % 7
+    tags = (1000 * r + 500 * which + 10 * step + torch.arange(k)).to(torch.int32)
+    pose = tags.to(torch.float32)[:, None] * torch.tensor([1.0, -1.0, 0.5, 0.25])
+    return pose, tags
+
+cap = 16
+for step in range(4):
+    up = (torch.zeros(cap, 4), torch.zeros(cap, dtype=torch.int32)); down = (torch.zeros(cap, 4), torch.zeros(cap, dtype=torch.int32))
+    pu, tu = payload(rank, 0, step); pd, td = payload(rank, 1, step)
+    up[0][:len(tu)] = pu; up[1][:len(tu)] = tu; down[0][:len(td)] = pd; down[1][:len(td)] = td
+    got_below, got_above = pt.exchange_migrants(dist, below, above, up, len(tu), down, len(td))
+    eb = payload(below, 0, step); ea = payload(above, 1, step)        # the rank below sends UP to me, the rank above DOWN
+    assert torch.equal(got_below[1], eb[1]) and torch.equal(got_below[0], eb[0]), (rank, step)
+    assert torch.equal(got_above[1], ea[1]) and torch.equal(got_above[0], ea[0]), (rank, step)
+dist.destroy_process_group()
+print("rank", rank, "ok")
+'''
+
+
+def test_inactive_mask_and_neighbours():
+    slabs = pt.reference_rows(26, 2, 3)
+    mask = pt.inactive_mask(slabs, 26)
+    assert mask.sum() == 3 and all(mask[b - 1] == 1 for _, b in slabs)
+    assert pt.neighbours(0, slabs) == (2, 1) and pt.neighbours(2, slabs) == (1, 0)
+    slabs = pt.reference_rows(4, 2, 3)                     # more ranks than tile rows: empty slabs own nothing
+    owners = [r for r, (a, b) in enumerate(slabs) if b > a]
+    assert pt.inactive_mask(slabs, 4).sum() == len(owners)
+    for r in owners:
+        lo, hi = pt.neighbours(r, slabs)
+        assert lo in owners and hi in owners
+    pos = np.arange(12, dtype=np.float32).reshape(3, 4); quat = np.arange(12, 24, dtype=np.float32).reshape(3, 4)
+    assert np.array_equal(pt.pose_of(pos, quat), np.array([[0, 1, 12, 15], [4, 5, 16, 19], [8, 9, 20, 23]], dtype=np.float32))
+
+
+def test_migrant_exchange_with_gloo_ranks(tmp_path):
+    script = tmp_path / "migrants.py"
+    script.write_text(MIGRANT_WORKER)
+    for world in (2, 3):
+        r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={world}", "--master-addr", "127.0.0.1",
+                            "--master-port", str(29650 + world), str(script), ROOT], capture_output=True, text=True, timeout=300)
+        assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
+        assert r.stdout.count("ok") == world
