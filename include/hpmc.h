@@ -145,7 +145,9 @@ int hpmc_sweep_host(hpmc_ctx* ctx, const float* h_pos4, const float* h_quat4, in
  *   "path"     0 = automatic, 1 = per-thread global-memory colour pass, 2 = shared-memory tile colour pass (2-D; in 3-D
  *              the warp-per-cell pass), 3 = warp-per-cell colour pass (automatic in 3-D and for small 2-D systems),
  *              4 = whole sweeps (cell list + the four colours) inside ONE launch of one thread-block cluster of up to 16 CTAs,
- *              separated by hardware cluster barriers (2-D, at most 16 384 particles and 11 498 cells; never automatic)
+ *              separated by hardware cluster barriers (2-D, at most 16 384 particles and 11 498 cells; never automatic),
+ *              5 = warp-per-cell pass that evaluates the decision tree of four consecutive trials of a cell at once (2-D;
+ *              never automatic: measured no faster than 3)
  *   "tile_cap" upper limit on the particles a tile may stage; tiles above it take the per-thread path
  *              (tests set 0 to force that fallback everywhere).
  *   "tile_shape" 2-D tile kernel shape: 0 = chosen by grid size, 1 = 8 warps per CTA x 2 rows of 32 active cells per warp,

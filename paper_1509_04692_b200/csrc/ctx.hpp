@@ -66,7 +66,7 @@ struct hpmc_ctx {
     int part_rank = 0, part_n = 1;
 
     // tuning / test knobs (hpmc_set_option)
-    int opt_path = 0;                 // 0 auto, 1 per-thread global path, 2 tile path (2-D only), 3 warp per cell, 4 cluster (small 2-D)
+    int opt_path = 0;                 // 0 auto, 1 per-thread global path, 2 tile path (2-D only), 3 warp per cell, 4 cluster (small 2-D), 5 speculative warp per cell (2-D)
     int cluster_ctas = -1;            // CTAs per cluster of the whole-sweep pass: -1 = not probed yet, 0 = unavailable on this device
     int opt_tile_cap = 1 << 30;       // staging capacity limit of the tile kernel (tests force the overflow path)
     int opt_tile_shape = 0;           // 0 = by grid size, 1..3 = fixed (see pick_tile_shape)
@@ -133,6 +133,7 @@ constexpr int kTileWHost = 32;   // active cells per tile row (= kTileW of sweep
 //   kind: kKindDisk / kKindPolygon / kKindPolyhedron; nv: unrolled vertex count (5 pentagons, 8 cubes) or 0 = runtime count
 bool hpmc_launch_tile2d(hpmc_ctx* c, int ci, int kind, int nv, int shape);       // pass_tile2d_*.cu (2-D, not polyhedra)
 bool hpmc_launch_warpcell(hpmc_ctx* c, int ci, int kind, int nv, int nactive);   // pass_warpcell_*.cu
+bool hpmc_launch_spec2d(hpmc_ctx* c, int ci, int kind, int nv, int nactive);     // pass_spec2d.cu
 bool hpmc_launch_colour(hpmc_ctx* c, int ci, int kind, int nv, int nactive);     // pass_colour.cu
 // whole sweeps of a small 2-D system in one cluster launch (pass_cluster2d.cu): sweeps enqueued, 0 = cluster size unavailable, -1 = error
 int hpmc_launch_cluster2d(hpmc_ctx* c, int64_t n_sweeps, int ncta, int kind, int nv);

@@ -319,11 +319,21 @@ int pick_tile_shape(const hpmc_ctx* c)
 // kernel would leave most SMs idle (config 1: 961 active cells = 31 warps) and each warp round would be a long serial chain
 constexpr int kWarpCellMax2d = 148 * 48;
 
+// 2-D systems: the speculative warp-per-cell pass (sweep_spec2d.cuh), on request only.  Measured on B200 (4096 pentagons): a
+// batch of four trials takes 4.4 us against 4 x 1.05 us for the sequential warp-per-cell pass -- every phase of the decision
+// tree (replay, 15 x candidates broad phase, queue, tree walk) is itself a few hundred dependent instructions on a lone warp
+bool use_spec(const hpmc_ctx* c)
+{
+    const GridParams& g = c->g;
+    if (g.dim != 2 || c->sf.kind == kKindPolyhedron || c->part_n > 1) return false;
+    return c->opt_path == 5;
+}
+
 // does the 2-D tile pass apply (not the warp-per-cell pass, not the per-thread path), and as a dataflow launch?
 bool use_flow(const hpmc_ctx* c)
 {
     const GridParams& g = c->g;
-    if (g.dim != 2 || c->sf.kind == kKindPolyhedron || c->opt_path == 1 || c->opt_path == 3 || c->opt_flow == 0) return false;
+    if (g.dim != 2 || c->sf.kind == kKindPolyhedron || c->opt_path == 1 || c->opt_path == 3 || c->opt_path == 5 || c->opt_flow == 0) return false;
     if (c->part_n > 1) return false;   // the ranks exchange boundary rows between the colours: one launch per colour
     const int nactive = (g.n[0] / 2) * (g.n[1] / 2);
     if (c->opt_path == 0 && c->opt_tile_shape == 0 && nactive <= kWarpCellMax2d) return false;
@@ -394,6 +404,7 @@ int launch_colour_dispatch(hpmc_ctx* c, int ci)
     bool ok = true;
     if (c->part_n > 1) ok = hpmc_launch_tile2d(c, ci, kind, nv, pick_tile_shape(c));
     else if (c->opt_path == 1 || (g.dim == 2 && kind == kKindPolyhedron)) ok = hpmc_launch_colour(c, ci, kind, nv, nactive);
+    else if (use_spec(c)) ok = hpmc_launch_spec2d(c, ci, kind, nv, nactive);
     else if (g.dim == 3 || c->opt_path == 3 || (c->opt_path == 0 && c->opt_tile_shape == 0 && nactive <= kWarpCellMax2d))
         ok = hpmc_launch_warpcell(c, ci, kind, nv, nactive);
     else ok = hpmc_launch_tile2d(c, ci, kind, nv, pick_tile_shape(c));
@@ -825,7 +836,7 @@ int hpmc_set_option(hpmc_ctx* c, const char* name, int64_t value)
     if (n == "graph") {
         c->opt_graph = value != 0;
     } else if (n == "path") {
-        if (value < 0 || value > 4) return fail(c, HPMC_E_ARG, "path must be 0 (auto), 1 (per-thread), 2 (tile), 3 (warp per cell) or 4 (cluster)");
+        if (value < 0 || value > 5) return fail(c, HPMC_E_ARG, "path must be 0 (auto), 1 (per-thread), 2 (tile), 3 (warp per cell), 4 (cluster) or 5 (speculative warp per cell)");
         c->opt_path = (int)value;
     } else if (n == "tile_cap") {
         if (value < 0) return fail(c, HPMC_E_ARG, "tile_cap must be >= 0");
@@ -880,6 +891,7 @@ int hpmc_describe_pass(const hpmc_ctx* c, char* h_buf, size_t n)
         d = "k_sweep_cluster2d: whole sweeps (build + 4 colour passes) in one launch of one thread-block cluster of " +
             std::to_string(c->cluster_ctas > 0 ? c->cluster_ctas : kClusterMaxCtas) + " CTAs";
     else if (c->opt_path == 1) d = "k_sweep_colour: one thread per active cell";
+    else if (use_spec(c)) d = "k_sweep_spec2d: one warp per active cell, the decision tree of 4 trials evaluated at once, 1 colour pass per launch";
     else if (g.dim == 3 || c->opt_path == 3 || (c->opt_path == 0 && c->opt_tile_shape == 0 && nactive <= kWarpCellMax2d))
         d = "k_sweep_warpcell: one warp per active cell, 1 colour pass per launch";
     else {

@@ -74,6 +74,17 @@ __device__ __forceinline__ void small_sincos(float h, float a, float& sn, float&
     }
 }
 
+// R6, 2-D: q' = normalise(q (x) dq) for q = (qw, 0, 0, qz), dq = (cs, 0, 0, sn).  Explicit roundings: one definition for
+// make_trial and for the speculative pass, which replays accepted rotations (sweep_spec2d.cuh)
+__device__ __forceinline__ void rotate_2d(float qw, float qz, float sn, float cs, float& ow, float& oz)
+{
+    const float w = __fmaf_rn(qw, cs, -__fmul_rn(qz, sn));
+    const float z = __fmaf_rn(qw, sn, __fmul_rn(qz, cs));
+    const float inv = rsqrtf(__fmaf_rn(w, w, __fmul_rn(z, z)));
+    ow = __fmul_rn(w, inv);
+    oz = __fmul_rn(z, inv);
+}
+
 // a5 + a6: the trial pose of one move (R5-R7) and the leave-cell test (R13).  b0 = (select, type, ua, ub), uc = first
 // word of block 1 (3-D only).  Returns false iff a translation left `cell`.  One definition for every colour-pass
 // variant, so that they produce bit-identical trials.
@@ -93,9 +104,8 @@ __device__ __forceinline__ bool make_trial(const GridParams& g, const MoveParams
     if (dim == 2) {                                   // R6, 2-D: angle about z
         float sn, cs;
         small_sincos(0.5f * __fmul_rn(mv.a, usym(b0.z)), mv.a, sn, cs);
-        const float w = qp.x * cs - qp.w * sn, z = qp.x * sn + qp.w * cs;
-        const float inv = rsqrtf(w * w + z * z);
-        A.qw = w * inv; A.qx = 0.0f; A.qy = 0.0f; A.qz = z * inv;
+        rotate_2d(qp.x, qp.w, sn, cs, A.qw, A.qz);
+        A.qx = 0.0f; A.qy = 0.0f;
     } else {                                          // R6, 3-D: uniform axis, angle in [-a,a)
         const float zz = usym(b0.z);
         float sphi, cphi, sn, cs;

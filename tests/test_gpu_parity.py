@@ -144,6 +144,7 @@ def test_colour_pass_variants_agree_bit_for_bit(name):
                {"path": 2, "flow": 1, "tile_cap": some}] if w.dim == 2 else []
     warp = [{"path": 3}, {"path": 3, "tile_cap": 6}] if w.dim == 2 else []        # 2-D warp-per-cell pass and its fallback
     warp += [{"path": 4}] if w.dim == 2 else []                                   # whole sweeps in one thread-block cluster
+    warp += [{"path": 5}, {"path": 5, "tile_cap": 6}] if w.dim == 2 else []       # speculative warp-per-cell pass and its fallback
     builds = [{"small_build": 0}, {"small_build": 0, "path": 2}]                   # the multi-launch cell-list build
     for opts in [{"path": 2}, {"path": 2, "tile_cap": 0}, {"path": 1}, {"path": 2, "tile_cap": some}] + shapes + warp + builds:
         g = gpu(w)
@@ -466,3 +467,53 @@ def test_lockstep_in_a_box_of_edge_20000():
             assert np.array_equal(gp, op) and np.max(np.abs(gq.astype(np.float64) - oq)) < 1e-5
             o.set_state(op, gq)
         assert g.count_overlaps() == 0 and o.count_overlaps_bruteforce() == 0 and marginal <= 3
+
+
+@pytest.mark.parametrize("case", ["pentagons_ns1", "pentagons_ns3", "pentagons_ns6", "pentagons_ns9", "disks_ns5", "needles_crowded",
+                                  "needles_overfull"])
+def test_speculative_pass_lockstep_with_oracle(case):
+    """k_sweep_spec2d evaluates the decision tree of four trials of a cell at once (sweep_spec2d.cuh).  Against the oracle in lock
+    step: batches that are not full (n_select 1, 3), several batches (6, 9), cells with several members -- where a node's
+    state differs from the staged one for OTHER members too -- and cells with more members than the tree handles (fallback)."""
+    opts = {"path": 5}
+    pent = wl.regular_polygon(5, 0.5)
+    if case.startswith("pentagons_ns"):
+        w = _lattice_workload(2, (26, 30), (1.06, 1.04), wl.KIND_POLYGON, verts=pent, d=0.12, a=0.3, n_select=int(case[-1]), seed=11)
+    elif case == "disks_ns5":
+        w = _lattice_workload(2, (30, 26), (1.08, 1.1), wl.KIND_DISK, diameter=1.0, d=0.2, n_select=5)
+    else:
+        # thin rectangles 1.0 x 0.16 stacked at a pitch of 0.5 (crowded: mostly 2-4 per cell) or 0.2 (overfull: most cells above
+        # kSpecMaxMem = 4), all nearly parallel: many members per cell, and the moved particle's cell mates are its closest neighbours
+        pitch = 0.5 if case == "needles_crowded" else 0.2
+        verts = np.array([[0.5, -0.08], [0.5, 0.08], [-0.5, 0.08], [-0.5, -0.08]])
+        w = _lattice_workload(2, (20, int(round(20.8 / pitch))), (1.08, pitch), wl.KIND_POLYGON, verts=verts, d=0.03, a=0.05, n_select=4, seed=12)
+        rng = np.random.default_rng(13)
+        th = rng.uniform(-0.03, 0.03, w.N)
+        w.quat4[:, 0], w.quat4[:, 3] = np.cos(th / 2), np.sin(th / 2)
+    from paper_1509_04692_b200 import binding as hb
+    g, o = hb.from_workload(w, seed=9), orc(w, seed=9)
+    for k, v in opts.items():
+        g.set_option(k, v)
+    assert "spec2d" in g.describe_pass()
+    assert g.count_overlaps() == 0 and o.count_overlaps_cells() == 0
+    g.enable_trace(True)
+    marginal, multi, share = 0, 0, 1.0
+    for s in range(8):
+        cid, cst, mem, shift, perm = g.cell_list(s)
+        cnt = np.diff(cst)
+        multi = max(multi, int(cnt.max()))
+        share = min(share, float(np.mean((cnt[cnt > 0] >= 2) & (cnt[cnt > 0] <= 4))))
+        g.sweep(1)
+        f = o.sweep(follow=g.read_trace(), follow_tol=MARGIN_TOL)["follow"]
+        assert f["hard_mismatch"] == 0, (case, s, f)
+        marginal += f["marginal"]
+        gp, gq = g.get_state(); op, oq = o.get_state()
+        assert np.array_equal(gp, op) and np.max(np.abs(gq.astype(np.float64) - oq)) < 1e-5
+        o.set_state(op, gq)
+    gc, oc = g.counters(), o.counters()
+    assert all(gc[k] == oc[k] for k in oc)
+    assert gc["trans_acc"] > 0.1 * gc["trials"] and g.count_overlaps() == 0 and marginal <= 5
+    if case == "needles_crowded":
+        assert share > 0.5, share            # most occupied cells hold 2-4 members: the tree runs with cell mates in its states
+    if case == "needles_overfull":
+        assert multi >= 5
