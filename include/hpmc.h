@@ -246,6 +246,29 @@ int hpmc_get_stat(hpmc_ctx* ctx, const char* name, int64_t* h_value);
  * launches in TFLOP/s (FMA = 2 flops).  Synchronises.  Nominal on B200: 148 SMs x 128 lanes x 2 x 1.965 GHz = 74.4.   */
 int hpmc_measure_fp32_peak(hpmc_ctx* ctx, double* h_tflops);
 
+/* The overlap count of P:247 without any allocation and without a workspace: for callers that cannot call cudaMalloc (code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid it).  Same result as hpmc_bind + hpmc_count_overlaps --
+ * the number of pairs whose interiors intersect, strict margin < 0, fp64 narrow phase -- for the n particles given here in
+ * the box and with the shape of `ctx` (n need not be the N of hpmc_create; the context needs no hpmc_bind and its own state
+ * is not touched).
+ *   d_pos4, d_quat4  DEVICE, n x float4 each, tag order, the layout of hpmc_bind (d_quat4 may be NULL for disks / spheres);
+ *                    16-byte aligned; read only
+ *   d_count_out      DEVICE, one int64, 8-byte aligned: the pair count, or -1 if a coordinate was not finite or not in
+ *                    [-L/2, L/2) (the particle is then binned into a clamped cell; nothing is read out of bounds)
+ * The cell list it needs lives in ONE static device array inside the library (1.25 MB on every GPU that loads libhpmc.so,
+ * held until the process exits), so:
+ *   - limits: n <= HPMC_NOALLOC_MAX_N and at most HPMC_NOALLOC_MAX_CELLS cells in the context's grid; beyond them the call
+ *     returns HPMC_E_ARG with a message and launches nothing;
+ *   - the call makes no cudaMalloc / cudaFree and calls no allocating routine: six kernel launches on the context's stream;
+ *     it is asynchronous and never synchronises (read d_count_out after synchronising the stream).  The first call on a
+ *     device also resolves the array's device address (cudaGetSymbolAddress): make that first call outside graph capture;
+ *   - all calls on a device share the array, which keeps the previous call's contents; each call clears what it needs at
+ *     zero.  Calls whose kernels can overlap on the GPU (contexts on different streams, several host threads) RACE on it:
+ *     keep them on one stream or order them with events.                                                          */
+#define HPMC_NOALLOC_MAX_N 65536
+#define HPMC_NOALLOC_MAX_CELLS 131072
+int hpmc_count_overlaps_noalloc(hpmc_ctx* ctx, const float* d_pos4, const float* d_quat4, int64_t n, int64_t* d_count_out);
+
 /* Launch bookkeeping for bench.py: kernels launched by this context so far.                        */
 int64_t hpmc_launch_count(const hpmc_ctx* ctx);
 

@@ -19,7 +19,7 @@ ABI_SYMBOLS = ["hpmc_create", "hpmc_destroy", "hpmc_last_error", "hpmc_get_grid"
                "hpmc_reset_counters", "hpmc_set_trace", "hpmc_get_cell_list", "hpmc_sweep_host", "hpmc_set_option", "hpmc_set_profile",
                "hpmc_get_profile", "hpmc_launch_count", "hpmc_describe_pass", "hpmc_get_stat", "hpmc_measure_fp32_peak", "hpmc_set_partition", "hpmc_sweep_phase",
                "hpmc_partition_rows", "hpmc_row_offsets", "hpmc_sorted_pose", "hpmc_set_inactive_layers", "hpmc_dist_load",
-               "hpmc_dist_route", "hpmc_dist_append", "hpmc_local_count", "hpmc_sorted_tags"]
+               "hpmc_dist_route", "hpmc_dist_append", "hpmc_local_count", "hpmc_sorted_tags", "hpmc_count_overlaps_noalloc"]
 
 
 class HpmcError(RuntimeError):
@@ -92,6 +92,7 @@ def load_library():
     L.hpmc_dist_route.argtypes = [vp, C.c_int, vp, vp, C.c_int64, vp, vp, C.c_int64, C.POINTER(C.c_int64)]
     L.hpmc_dist_append.argtypes = [vp, vp, vp, C.c_int64]
     L.hpmc_local_count.argtypes = [vp]; L.hpmc_local_count.restype = C.c_int64
+    L.hpmc_count_overlaps_noalloc.argtypes = [vp, vp, vp, C.c_int64, vp]
     L.hpmc_describe_pass.argtypes = [vp, C.c_char_p, C.c_size_t]
     for name in ABI_SYMBOLS:
         if name not in ("hpmc_last_error", "hpmc_workspace_bytes", "hpmc_launch_count", "hpmc_local_count"):
@@ -330,6 +331,19 @@ class Hpmc:
     def dist_append(self, pose4, tags, n):
         if n:
             self._check(self._lib.hpmc_dist_append(self._h, pose4.data_ptr(), tags.data_ptr(), int(n)))
+
+    def count_overlaps_noalloc(self, pos4, quat4, out):
+        """Overlapping pairs among the particles of the CUDA tensors pos4 / quat4 ((n, 4) float32, tag order) in this context's
+        box, through the entry point that allocates nothing (static scratch inside the library; n <= 65 536).  `out`: a CUDA
+        int64 tensor of one element that receives the count (-1: a coordinate outside the box).  No bind is needed.
+        Asynchronous on the context's stream: synchronise it before reading `out`."""
+        torch = self._torch
+        assert pos4.is_cuda and pos4.dtype == torch.float32 and pos4.is_contiguous() and pos4.shape[1] == 4
+        assert quat4 is None or (quat4.is_cuda and quat4.dtype == torch.float32 and quat4.is_contiguous() and quat4.shape == pos4.shape)
+        assert out.is_cuda and out.dtype == torch.int64 and out.numel() == 1
+        torch.cuda.current_stream(self.device).synchronize()      # the caller's tensors are ready
+        self._check(self._lib.hpmc_count_overlaps_noalloc(self._h, pos4.data_ptr(), quat4.data_ptr() if quat4 is not None else None,
+                                                          int(pos4.shape[0]), out.data_ptr()))
 
     def get_stat(self, name):
         v = C.c_int64()
