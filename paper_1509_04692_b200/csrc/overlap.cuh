@@ -180,7 +180,7 @@ __device__ __forceinline__ bool polygon_separated(const ShapeT<float>& S, float 
 // ---------------------------------------------------------------------------------------------
 // NVP > 0: compile-time vertex count (the loop unrolls and the vertices become constant-bank operands); 0: runtime count.
 template <typename T, int NVP = 0>
-__device__ __forceinline__ V3<T> support_minkowski(const ShapeT<T>& S, const T* Rm, const V3<T>& r, const V3<T>& dir)
+__device__ __forceinline__ V3<T> support_minkowski(const ShapeT<T>& S, const T* Rm, const V3<T>& r, const V3<T>& dir, int& pair)
 {
     // R^-1 dir = R^T dir
     const V3<T> db{Rm[0] * dir.x + Rm[3] * dir.y + Rm[6] * dir.z, Rm[1] * dir.x + Rm[4] * dir.y + Rm[7] * dir.z,
@@ -195,6 +195,7 @@ __device__ __forceinline__ V3<T> support_minkowski(const ShapeT<T>& S, const T* 
         if (da > bestA) { bestA = da; ia = i; }
         if (dbv > bestB) { bestB = dbv; ib = i; }
     }
+    pair = ia | (ib << 8);   // the vertices of A and of B behind this point of B (-) A
     const T bx = S.vx[ib], by = S.vy[ib], bz = S.vz[ib];
     return V3<T>{Rm[0] * bx + Rm[1] * by + Rm[2] * bz + r.x - S.vx[ia], Rm[3] * bx + Rm[4] * by + Rm[5] * bz + r.y - S.vy[ia],
                  Rm[6] * bx + Rm[7] * by + Rm[8] * bz + r.z - S.vz[ia]};
@@ -242,7 +243,8 @@ __device__ int gjk_classify(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T e
     V3<T> W[4];
     int nW = 0;
     for (int iter = 0; iter < 40; ++iter) {
-        const V3<T> w = support_minkowski<T, NVP>(S, Rm, r, V3<T>{-v.x, -v.y, -v.z});
+        int wpair;
+        const V3<T> w = support_minkowski<T, NVP>(S, Rm, r, V3<T>{-v.x, -v.y, -v.z}, wpair);
         const T vw = dot(v, w);
         if (vw >= 0 && vw * vw >= eps * eps * vv) return kGjkSeparated;   // certificate: v^.w >= eps
         if (iter > 0 && vv - vw <= reltol * vv) return kGjkUnsure;           // converged: distance |v| < eps
@@ -323,6 +325,107 @@ __device__ int gjk_classify(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T e
     return kGjkUnsure;
 }
 
+// Is the origin inside the tetrahedron (a, b, c, d), farther than `deep` from each of its faces, and is the tetrahedron
+// solid enough for fp32 to vouch for that (every face has a real area and the opposite vertex stands well clear of it)?
+template <typename T>
+__device__ __forceinline__ bool origin_deep_inside(const V3<T>& a, const V3<T>& b, const V3<T>& c, const V3<T>& d, T dmax2, T deep)
+{
+    const T area_min2 = (T)1e-3 * dmax2 * dmax2, height_min = (T)10 * deep;
+    bool ok = true;
+#pragma unroll
+    for (int f = 0; f < 4; ++f) {
+        const V3<T> p = (f == 3) ? b : a;
+        const V3<T> q = (f == 0) ? b : (f == 1) ? c : d;
+        const V3<T> s3 = (f == 0) ? c : (f == 1) ? d : (f == 2) ? b : c;
+        const V3<T> o = (f == 0) ? d : (f == 1) ? b : (f == 2) ? c : a;
+        const V3<T> nn = cross(q - p, s3 - p);
+        const T sp = -dot(nn, p);          // origin side
+        const T sd = dot(nn, o - p);       // opposite-vertex side
+        const T nn2 = dot(nn, nn);
+        const T inv = rsqrt(nn2);
+        ok = ok && sp * sd > 0 && fabs(sp) * inv > deep && nn2 >= area_min2 && fabs(sd) * inv >= height_min;
+    }
+    return ok;
+}
+
+// Minkowski portal refinement -- XenoCollide, the paper's GPU overlap check for convex polyhedra ("XenoCollide [32] is faster
+// on the GPU"; "implemented as a single loop") -- on the Minkowski difference B (-) A with the support function
+// of Eq. (2), same verdicts as gjk_classify:
+//   kGjkSeparated  some direction n was found with max_{x in B(-)A} n^ . x <= -eps: a separating plane, evaluated directly
+//                  from a support point (the same kind of certificate as in gjk_classify);
+//   kGjkOverlap    the origin lies inside a tetrahedron (v0, v1, v2, v3) of points of B (-) A -- v0 = r, the difference of
+//                  the two body origins, an interior point -- deeper than `deep` and the tetrahedron is solid
+//                  (origin_deep_inside): the interiors intersect by more than `deep` >> eps;
+//   kGjkUnsure     everything else (the origin within `deep` of the boundary, a separating direction with less than eps of
+//                  clearance, degenerate portals, iteration cap): the fp32 caller decides such a pair in fp64.
+// Why not GJK in fp32: the loop body is the same for every lane whatever the state of its simplex (one support call, a few
+// cross products and selects), where GJK's case analysis (line / triangle / four faces of a tetrahedron, each with a
+// closest-point-on-triangle) makes the lanes of a warp -- one pair each -- execute the union of all cases; and the
+// tetrahedron that certifies an overlap has the deep interior point v0 as a vertex, so it is rarely a sliver (GJK's simplex
+// of nearby support points often is, which sent those pairs to fp64).
+template <typename T, int NVP = 0>
+__device__ int mpr_classify(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T eps, T deep)
+{
+    const T tiny = (T)1e-14;
+    int unused;
+    const V3<T> v0 = r;
+    const T v00 = dot(v0, v0);
+    if (v00 < tiny) return kGjkUnsure;
+    // verdict of a support point w found along n (not normalised): is the whole of B (-) A at n^ . x <= -eps ?
+#define HPMC_MPR_MISS(w, n)                                                   \
+    {                                                                         \
+        const T h_ = dot(w, n);                                               \
+        if (h_ <= 0) return (h_ * h_ >= eps * eps * dot(n, n)) ? kGjkSeparated : kGjkUnsure; \
+    }
+    V3<T> n{-v0.x, -v0.y, -v0.z};
+    V3<T> v1 = support_minkowski<T, NVP>(S, Rm, r, n, unused);
+    HPMC_MPR_MISS(v1, n)
+    n = cross(v1, v0);
+    if (dot(n, n) < tiny * v00) return kGjkUnsure;   // v0, v1 and the origin on one line
+    V3<T> v2 = support_minkowski<T, NVP>(S, Rm, r, n, unused);
+    HPMC_MPR_MISS(v2, n)
+    n = cross(v1 - v0, v2 - v0);
+    if (dot(n, v0) > 0) {   // the origin on the positive side of (v0, v1, v2)
+        const V3<T> t = v1; v1 = v2; v2 = t;
+        n = V3<T>{-n.x, -n.y, -n.z};
+    }
+    // ---- portal discovery: a triangle (v1, v2, v3) that the ray from v0 through the origin crosses ------------------------
+    V3<T> v3;
+    int it = 0;
+    for (;; ++it) {
+        if (it >= 12 || dot(n, n) < tiny) return kGjkUnsure;
+        v3 = support_minkowski<T, NVP>(S, Rm, r, n, unused);
+        HPMC_MPR_MISS(v3, n)
+        if (dot(cross(v1, v3), v0) < 0) { v2 = v3; n = cross(v1 - v0, v3 - v0); continue; }
+        if (dot(cross(v3, v2), v0) < 0) { v1 = v3; n = cross(v3 - v0, v2 - v0); continue; }
+        break;
+    }
+    // ---- portal refinement: push the portal outward until it passes the origin, or a support plane excludes it --------------
+    for (it = 0; it < 24; ++it) {
+        n = cross(v2 - v1, v3 - v1);
+        const T nn = dot(n, n);
+        if (nn < tiny) return kGjkUnsure;
+        const T inv = rsqrt(nn);
+        if (dot(n, v1) * inv > deep)   // the origin is behind the portal by more than `deep`: inside (v0, v1, v2, v3) ?
+            return origin_deep_inside(v0, v1, v2, v3, S.dmax2, deep) ? kGjkOverlap : kGjkUnsure;
+        const V3<T> v4 = support_minkowski<T, NVP>(S, Rm, r, n, unused);
+        HPMC_MPR_MISS(v4, n)
+        if (dot(v4 - v3, n) * inv <= (T)1e-6) return kGjkUnsure;   // the portal has reached the surface: origin within ~deep of it
+        const V3<T> c4 = cross(v4, v0);
+        if (dot(v1, c4) > 0) {
+            if (dot(v2, c4) > 0) v1 = v4; else v3 = v4;
+        } else {
+            if (dot(v3, c4) > 0) v2 = v4; else v1 = v4;
+        }
+    }
+#undef HPMC_MPR_MISS
+    return kGjkUnsure;
+}
+
+// which fp32 classifier the colour passes use (the fp64 decisions are always GJK): one switch for every variant, so that
+// they stay bit-identical to each other
+constexpr bool kFp32UseMpr = true;
+
 // rotation matrix (row major) of the unit quaternion (w,x,y,z)
 template <typename T>
 __device__ __forceinline__ void quat_to_matrix(T w, T x, T y, T z, T* M)
@@ -344,6 +447,7 @@ __device__ __forceinline__ int polyhedron_classify(const ShapeT<T>& S, const T* 
         for (int j = 0; j < 3; ++j) Rm[3 * i + j] = MA[i] * MB[j] + MA[3 + i] * MB[3 + j] + MA[6 + i] * MB[6 + j];
     const V3<T> r{MA[0] * rw.x + MA[3] * rw.y + MA[6] * rw.z, MA[1] * rw.x + MA[4] * rw.y + MA[7] * rw.z,
                   MA[2] * rw.x + MA[5] * rw.y + MA[8] * rw.z};
+    if (sizeof(T) == 4 && kFp32UseMpr) return mpr_classify<T, NVP>(S, Rm, r, eps, deep);
     return gjk_classify<T, NVP>(S, Rm, r, eps, deep);
 }
 
