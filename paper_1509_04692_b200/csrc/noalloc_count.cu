@@ -178,7 +178,8 @@ k_na_count(const __grid_constant__ GridParams g, const __grid_constant__ ShapeD 
                             } else {
                                 double MB[9];
                                 quat_to_matrix<double>(w, x, y, z, MB);
-                                ov = polyhedron_classify<double>(S, MA, MB, V3<double>{r[0], r[1], r[2]}, 0.0, 0.0) != kGjkSeparated;
+                                int unused[3];
+                                ov = polyhedron_classify<double>(S, MA, MB, V3<double>{r[0], r[1], r[2]}, 0.0, 0.0, unused) != kGjkSeparated;
                             }
                         }
                         if (ov) ++found;

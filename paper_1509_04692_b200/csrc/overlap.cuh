@@ -364,62 +364,74 @@ __device__ __forceinline__ bool origin_deep_inside(const V3<T>& a, const V3<T>& 
 // tetrahedron that certifies an overlap has the deep interior point v0 as a vertex, so it is rarely a sliver (GJK's simplex
 // of nearby support points often is, which sent those pairs to fp64).
 template <typename T, int NVP = 0>
-__device__ int mpr_classify(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T eps, T deep)
+__device__ int mpr_classify(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T eps, T deep, int* portal)
 {
+    // portal[0..2]: on kGjkUnsure from the refinement stage, the vertex pairs (index in A | index in B << 8) behind the last
+    // portal (v1, v2, v3) -- exact data from which the fp64 re-run rebuilds the tetrahedron (r, v1, v2, v3); else portal[0] = -1
+    //
+    // ONE loop with ONE support call for all stages ("implemented as a single loop"): the lanes of a warp, one pair
+    // each, are in different stages -- first point, second point, portal discovery, portal refinement -- and the support
+    // function is nine tenths of an iteration; what differs per stage is a few cross products behind it.
     const T tiny = (T)1e-14;
-    int unused;
+    portal[0] = -1;
     const V3<T> v0 = r;
     const T v00 = dot(v0, v0);
     if (v00 < tiny) return kGjkUnsure;
-    // verdict of a support point w found along n (not normalised): is the whole of B (-) A at n^ . x <= -eps ?
-#define HPMC_MPR_MISS(w, n)                                                   \
-    {                                                                         \
-        const T h_ = dot(w, n);                                               \
-        if (h_ <= 0) return (h_ * h_ >= eps * eps * dot(n, n)) ? kGjkSeparated : kGjkUnsure; \
-    }
+    V3<T> v1{0, 0, 0}, v2{0, 0, 0}, v3{0, 0, 0};
+    int p1 = -1, p2 = -1, p3 = -1;
     V3<T> n{-v0.x, -v0.y, -v0.z};
-    V3<T> v1 = support_minkowski<T, NVP>(S, Rm, r, n, unused);
-    HPMC_MPR_MISS(v1, n)
-    n = cross(v1, v0);
-    if (dot(n, n) < tiny * v00) return kGjkUnsure;   // v0, v1 and the origin on one line
-    V3<T> v2 = support_minkowski<T, NVP>(S, Rm, r, n, unused);
-    HPMC_MPR_MISS(v2, n)
-    n = cross(v1 - v0, v2 - v0);
-    if (dot(n, v0) > 0) {   // the origin on the positive side of (v0, v1, v2)
-        const V3<T> t = v1; v1 = v2; v2 = t;
-        n = V3<T>{-n.x, -n.y, -n.z};
-    }
-    // ---- portal discovery: a triangle (v1, v2, v3) that the ray from v0 through the origin crosses ------------------------
-    V3<T> v3;
-    int it = 0;
-    for (;; ++it) {
-        if (it >= 12 || dot(n, n) < tiny) return kGjkUnsure;
-        v3 = support_minkowski<T, NVP>(S, Rm, r, n, unused);
-        HPMC_MPR_MISS(v3, n)
-        if (dot(cross(v1, v3), v0) < 0) { v2 = v3; n = cross(v1 - v0, v3 - v0); continue; }
-        if (dot(cross(v3, v2), v0) < 0) { v1 = v3; n = cross(v3 - v0, v2 - v0); continue; }
-        break;
-    }
-    // ---- portal refinement: push the portal outward until it passes the origin, or a support plane excludes it --------------
-    for (it = 0; it < 24; ++it) {
-        n = cross(v2 - v1, v3 - v1);
+    int stage = 0;   // 0: v1 along -v0; 1: v2 along v1 x v0; 2: discovery of v3; 3: refinement
+    int verdict = kGjkUnsure;
+    bool have_portal = false;
+    for (int it = 0; it < 40; ++it) {
         const T nn = dot(n, n);
-        if (nn < tiny) return kGjkUnsure;
-        const T inv = rsqrt(nn);
-        if (dot(n, v1) * inv > deep)   // the origin is behind the portal by more than `deep`: inside (v0, v1, v2, v3) ?
-            return origin_deep_inside(v0, v1, v2, v3, S.dmax2, deep) ? kGjkOverlap : kGjkUnsure;
-        const V3<T> v4 = support_minkowski<T, NVP>(S, Rm, r, n, unused);
-        HPMC_MPR_MISS(v4, n)
-        if (dot(v4 - v3, n) * inv <= (T)1e-6) return kGjkUnsure;   // the portal has reached the surface: origin within ~deep of it
-        const V3<T> c4 = cross(v4, v0);
-        if (dot(v1, c4) > 0) {
-            if (dot(v2, c4) > 0) v1 = v4; else v3 = v4;
-        } else {
-            if (dot(v3, c4) > 0) v2 = v4; else v1 = v4;
+        if (nn < tiny * (stage == 1 ? v00 : (T)1)) break;             // degenerate direction (stage 1: v0, v1, origin on one line)
+        if (stage == 3) {
+            // the origin is behind the portal by more than `deep`: inside the tetrahedron (v0, v1, v2, v3) ?
+            if (dot(n, v1) * rsqrt(nn) > deep) {
+                if (origin_deep_inside(v0, v1, v2, v3, S.dmax2, deep)) verdict = kGjkOverlap;
+                break;
+            }
+        }
+        int pw;
+        const V3<T> w = support_minkowski<T, NVP>(S, Rm, r, n, pw);
+        const T h = dot(w, n);
+        if (h <= 0) {   // the whole of B (-) A lies at n^ . x <= h / |n|: a separating plane if that is <= -eps
+            if (h * h >= eps * eps * nn) verdict = kGjkSeparated;
+            else have_portal = false;   // a weak separating plane: the portal is of no use to the re-run
+            break;
+        }
+        if (stage == 0) {
+            v1 = w; p1 = pw;
+            n = cross(v1, v0);
+            stage = 1;
+        } else if (stage == 1) {
+            v2 = w; p2 = pw;
+            n = cross(v1 - v0, v2 - v0);
+            if (dot(n, v0) > 0) {   // the origin on the positive side of (v0, v1, v2)
+                const V3<T> t = v1; v1 = v2; v2 = t;
+                const int tp = p1; p1 = p2; p2 = tp;
+                n = V3<T>{-n.x, -n.y, -n.z};
+            }
+            stage = 2;
+        } else if (stage == 2) {   // discovery: a triangle (v1, v2, v3) that the ray from v0 through the origin crosses
+            v3 = w; p3 = pw;
+            if (dot(cross(v1, v3), v0) < 0) { v2 = v3; p2 = p3; n = cross(v1 - v0, v3 - v0); }
+            else if (dot(cross(v3, v2), v0) < 0) { v1 = v3; p1 = p3; n = cross(v3 - v0, v2 - v0); }
+            else { stage = 3; have_portal = true; n = cross(v2 - v1, v3 - v1); }
+        } else {                   // refinement: push the portal outward
+            if (dot(w - v3, n) <= (T)1e-6 * sqrt(nn)) break;   // the portal has reached the surface: origin within ~deep of it
+            const V3<T> c4 = cross(w, v0);
+            if (dot(v1, c4) > 0) {
+                if (dot(v2, c4) > 0) { v1 = w; p1 = pw; } else { v3 = w; p3 = pw; }
+            } else {
+                if (dot(v3, c4) > 0) { v2 = w; p2 = pw; } else { v1 = w; p1 = pw; }
+            }
+            n = cross(v2 - v1, v3 - v1);
         }
     }
-#undef HPMC_MPR_MISS
-    return kGjkUnsure;
+    if (verdict == kGjkUnsure && have_portal) { portal[0] = p1; portal[1] = p2; portal[2] = p3; }
+    return verdict;
 }
 
 // which fp32 classifier the colour passes use (the fp64 decisions are always GJK): one switch for every variant, so that
@@ -438,7 +450,7 @@ __device__ __forceinline__ void quat_to_matrix(T w, T x, T y, T z, T* M)
 
 // polyhedron pair in A's frame: MA, MB = world rotation matrices of A and B, rw = r_AB (world).  GJK verdict.
 template <typename T, int NVP = 0>
-__device__ __forceinline__ int polyhedron_classify(const ShapeT<T>& S, const T* MA, const T* MB, const V3<T>& rw, T eps, T deep)
+__device__ __forceinline__ int polyhedron_classify(const ShapeT<T>& S, const T* MA, const T* MB, const V3<T>& rw, T eps, T deep, int* portal)
 {
     T Rm[9];  // R = MA^T MB takes B's frame into A's frame (q = q_A* q_B)
 #pragma unroll
@@ -447,19 +459,59 @@ __device__ __forceinline__ int polyhedron_classify(const ShapeT<T>& S, const T* 
         for (int j = 0; j < 3; ++j) Rm[3 * i + j] = MA[i] * MB[j] + MA[3 + i] * MB[3 + j] + MA[6 + i] * MB[6 + j];
     const V3<T> r{MA[0] * rw.x + MA[3] * rw.y + MA[6] * rw.z, MA[1] * rw.x + MA[4] * rw.y + MA[7] * rw.z,
                   MA[2] * rw.x + MA[5] * rw.y + MA[8] * rw.z};
-    if (sizeof(T) == 4 && kFp32UseMpr) return mpr_classify<T, NVP>(S, Rm, r, eps, deep);
+    portal[0] = -1;
+    if (sizeof(T) == 4 && kFp32UseMpr) return mpr_classify<T, NVP>(S, Rm, r, eps, deep, portal);
     return gjk_classify<T, NVP>(S, Rm, r, eps, deep);
 }
 
-// fp64 narrow phase from the raw fp32 state: normalised quaternions, exact separation rd (already minimum image)
-static __device__ __noinline__ bool polyhedron_overlap_f64(const ShapeD& S, float4 qA, float4 qB, double rx, double ry, double rz, double eps)
+// fp64 narrow phase from the raw fp32 state: normalised quaternions, exact separation rd (already minimum image).
+// portal: what the fp32 XenoCollide run left (mpr_classify), or portal[0] < 0.  With a portal the vertices v1, v2, v3 of
+// B (-) A are rebuilt in fp64 from their vertex indices, and if the origin lies strictly inside the tetrahedron (r, v1, v2, v3)
+// -- four points of the convex set B (-) A -- the interiors intersect: overlap, decided with ~300 fp64 operations.  Otherwise (no
+// portal, or the origin is not inside that tetrahedron) the fp64 GJK decides as before.  The shortcut only ever answers
+// "overlap" and only when that is a fact, so the decision is the same with and without it.
+template <int NVP = 0>
+static __device__ __noinline__ bool polyhedron_overlap_f64(const ShapeD& S, float4 qA, float4 qB, double rx, double ry, double rz, double eps,
+                                                           const int* portal)
 {
     double MA[9], MB[9];
     const double na = 1.0 / sqrt((double)qA.x * qA.x + (double)qA.y * qA.y + (double)qA.z * qA.z + (double)qA.w * qA.w);
     const double nb = 1.0 / sqrt((double)qB.x * qB.x + (double)qB.y * qB.y + (double)qB.z * qB.z + (double)qB.w * qB.w);
     quat_to_matrix<double>(qA.x * na, qA.y * na, qA.z * na, qA.w * na, MA);
     quat_to_matrix<double>(qB.x * nb, qB.y * nb, qB.z * nb, qB.w * nb, MB);
-    return polyhedron_classify<double>(S, MA, MB, V3<double>{rx, ry, rz}, eps, 0.0) != kGjkSeparated;
+    if (portal[0] >= 0) {
+        double Rm[9];
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+            for (int j = 0; j < 3; ++j) Rm[3 * i + j] = MA[i] * MB[j] + MA[3 + i] * MB[3 + j] + MA[6 + i] * MB[6 + j];
+        const V3<double> r{MA[0] * rx + MA[3] * ry + MA[6] * rz, MA[1] * rx + MA[4] * ry + MA[7] * rz, MA[2] * rx + MA[5] * ry + MA[8] * rz};
+        V3<double> v[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const int ia = portal[k] & 255, ib = portal[k] >> 8;
+            const double bx = S.vx[ib], by = S.vy[ib], bz = S.vz[ib];
+            v[k] = V3<double>{Rm[0] * bx + Rm[1] * by + Rm[2] * bz + r.x - S.vx[ia], Rm[3] * bx + Rm[4] * by + Rm[5] * bz + r.y - S.vy[ia],
+                              Rm[6] * bx + Rm[7] * by + Rm[8] * bz + r.z - S.vz[ia]};
+        }
+        // strictly inside: on the inner side of all four faces by more than 1e-9 (fp64 rounding here is ~1e-15)
+        const V3<double> a = r, b = v[0], c = v[1], d = v[2];
+        bool inside = true;
+#pragma unroll
+        for (int f = 0; f < 4; ++f) {
+            const V3<double> p = (f == 3) ? b : a;
+            const V3<double> q = (f == 0) ? b : (f == 1) ? c : d;
+            const V3<double> s3 = (f == 0) ? c : (f == 1) ? d : (f == 2) ? b : c;
+            const V3<double> o = (f == 0) ? d : (f == 1) ? b : (f == 2) ? c : a;
+            const V3<double> nn = cross(q - p, s3 - p);
+            const double sp = -dot(nn, p), sd = dot(nn, o - p), nn2 = dot(nn, nn);
+            // sp, sd of one sign; |sp| / |nn| > 1e-9 and the face not degenerate
+            inside = inside && sp * sd > 0.0 && sp * sp > 1e-18 * nn2 && nn2 > 1e-20;
+        }
+        if (inside) return true;
+    }
+    int unused[3];
+    return polyhedron_classify<double, NVP>(S, MA, MB, V3<double>{rx, ry, rz}, eps, 0.0, unused) != kGjkSeparated;
 }
 
 }  // namespace hpmc

@@ -137,10 +137,11 @@ __device__ __forceinline__ bool narrow_overlap(const ShapeF& S, const ShapeD& SD
     } else {
         float MB[9];
         quat_to_matrix<float>(qB.x, qB.y, qB.z, qB.w, MB);
-        const int verdict = polyhedron_classify<float>(S, MA, MB, V3<float>{rx, ry, rz}, eps, kGjkDeepF);
+        int portal[3];
+        const int verdict = polyhedron_classify<float>(S, MA, MB, V3<float>{rx, ry, rz}, eps, kGjkDeepF, portal);
         if (verdict != kGjkUnsure) return verdict == kGjkOverlap;
         // near contact: decide in fp64 from the raw fp32 state (mixed precision)
-        return polyhedron_overlap_f64(SD, make_float4(A.qw, A.qx, A.qy, A.qz), qB, rd[0], rd[1], rd[2], (double)eps);
+        return polyhedron_overlap_f64(SD, make_float4(A.qw, A.qx, A.qy, A.qz), qB, rd[0], rd[1], rd[2], (double)eps, portal);
     }
 }
 
@@ -350,7 +351,8 @@ k_count_overlaps(const __grid_constant__ GridParams g, const __grid_constant__ S
                             } else {
                                 double MB[9];
                                 quat_to_matrix<double>(w, x, y, z, MB);
-                                ov = polyhedron_classify<double>(S, MA, MB, V3<double>{r[0], r[1], r[2]}, 0.0, 0.0) != kGjkSeparated;
+                                int unused[3];
+                                ov = polyhedron_classify<double>(S, MA, MB, V3<double>{r[0], r[1], r[2]}, 0.0, 0.0, unused) != kGjkSeparated;
                             }
                         }
                         if (ov) ++found;

@@ -195,11 +195,12 @@ k_sweep_warpcell(const __grid_constant__ GridParams g, const __grid_constant__ M
                         const float rz = seam ? min_image(xq.z, A.z, g.hi[2], g.Ld[2]) : xq.z - A.z;
                         float MB[9];
                         quat_to_matrix<float>(qq.x, qq.y, qq.z, qq.w, MB);
-                        const int verdict = polyhedron_classify<float, NV>(S, MA, MB, V3<float>{rx, ry, rz}, mv.eps_g, kGjkDeepF);
+                        int portal[3];
+                        const int verdict = polyhedron_classify<float, NV>(S, MA, MB, V3<float>{rx, ry, rz}, mv.eps_g, kGjkDeepF, portal);
                         if (verdict == kGjkUnsure) {   // near contact: decide in fp64 from the raw fp32 state
                             ++cc.f64;
-                            ov = polyhedron_overlap_f64(SD, make_float4(A.qw, A.qx, A.qy, A.qz), qq, min_image_d(xq.x, A.x, g.Ld[0]),
-                                                        min_image_d(xq.y, A.y, g.Ld[1]), min_image_d(xq.z, A.z, g.Ld[2]), (double)mv.eps_g);
+                            ov = polyhedron_overlap_f64<NV>(SD, make_float4(A.qw, A.qx, A.qy, A.qz), qq, min_image_d(xq.x, A.x, g.Ld[0]),
+                                                            min_image_d(xq.y, A.y, g.Ld[1]), min_image_d(xq.z, A.z, g.Ld[2]), (double)mv.eps_g, portal);
                         } else
                             ov = verdict == kGjkOverlap;
                     }
