@@ -100,6 +100,10 @@ struct orc_shape {
     double face_c[ORC_MAX_FACES];        /* n . v on the face                     */
     int nedgedirs;                       /* distinct edge directions (polyhedron) */
     double edge_d[ORC_MAX_EDGES][3];
+    int nedges;                          /* all edges of the polyhedron as vertex pairs (core distance of rounded shapes) */
+    int edge_v[ORC_MAX_EDGES][2];
+    double sweep_r;                      /* P:89 spheropolygon / spheropolyhedron: radius of the disk / sphere swept over
+                                            the polygon / polyhedron (the "core"); 0 = the sharp shape */
 };
 
 static int derive_polygon(orc_shape* s)
@@ -175,6 +179,7 @@ static int derive_polyhedron(orc_shape* s)
     }
     /* edges: vertex pairs sharing >= 2 faces; keep distinct directions (up to sign) */
     s->nedgedirs = 0;
+    s->nedges = 0;
     for (int i = 0; i < n; ++i)
         for (int j = i + 1; j < n; ++j) {
             int shared = 0;
@@ -183,6 +188,10 @@ static int derive_polyhedron(orc_shape* s)
                     fabs(dot3(s->face_n[f], s->verts[j]) - s->face_c[f]) < tol)
                     ++shared;
             if (shared < 2) continue;
+            if (s->nedges >= ORC_MAX_EDGES) return -1;
+            s->edge_v[s->nedges][0] = i;
+            s->edge_v[s->nedges][1] = j;
+            ++s->nedges;
             double e[3];
             sub3(s->verts[j], s->verts[i], e);
             double len = norm3(e);
@@ -198,7 +207,19 @@ static int derive_polyhedron(orc_shape* s)
     return 0;
 }
 
+static orc_shape* shape_create(int dim, int kind, double diameter, int nverts, const double* verts, double sweep_r);
 orc_shape* orc_shape_create(int dim, int kind, double diameter, int nverts, const double* verts)
+{
+    return shape_create(dim, kind, diameter, nverts, verts, 0.0);
+}
+/* P:89 "spheropolygons ... convex spheropolyhedra": the polygon / polyhedron swept by a disk / sphere of radius sweep_r */
+orc_shape* orc_shape_create_rounded(int dim, int kind, double sweep_r, int nverts, const double* verts)
+{
+    if (kind != ORC_KIND_POLYGON && kind != ORC_KIND_POLYHEDRON) return NULL;
+    if (!(sweep_r >= 0.0)) return NULL;
+    return shape_create(dim, kind, 0.0, nverts, verts, sweep_r);
+}
+static orc_shape* shape_create(int dim, int kind, double diameter, int nverts, const double* verts, double sweep_r)
 {
     if (dim != 2 && dim != 3) return NULL;
     orc_shape* s = (orc_shape*)calloc(1, sizeof *s);
@@ -222,7 +243,8 @@ orc_shape* orc_shape_create(int dim, int kind, double diameter, int nverts, cons
                 double r = norm3(s->verts[i]);
                 if (r > rmax) rmax = r;
             }
-            s->dmax = 2.0 * rmax; /* "diameter of the sphere that encloses particle i, centered on r_i" P:59 */
+            s->sweep_r = sweep_r;
+            s->dmax = 2.0 * (rmax + sweep_r); /* "diameter of the sphere that encloses particle i, centered on r_i" P:59 */
             rc = (kind == ORC_KIND_POLYGON) ? derive_polygon(s) : derive_polyhedron(s);
         }
     } else
@@ -233,6 +255,7 @@ orc_shape* orc_shape_create(int dim, int kind, double diameter, int nverts, cons
 
 void orc_shape_destroy(orc_shape* s) { free(s); }
 double orc_shape_dmax(const orc_shape* s) { return s->dmax; }
+double orc_shape_sweep_radius(const orc_shape* s) { return s->sweep_r; }
 int orc_shape_nfaces(const orc_shape* s) { return s->nfaces; }
 int orc_shape_nedgedirs(const orc_shape* s) { return s->nedgedirs; }
 void orc_shape_faces(const orc_shape* s, double* normals3, double* offsets)
@@ -262,7 +285,125 @@ static double axis_separation(const double nhat[3], const double r_ab[3], double
     return dot3(nhat, r_ab) - support_height(wa, nv, nhat) - support_height(wb, nv, neg);
 }
 
+/* ---- Euclidean distance between two DISJOINT convex cores, by brute force over feature pairs (rounded shapes) ----
+ * The closest points of two disjoint convex polygons are a vertex of one and a point of an edge of the other; of two
+ * disjoint convex polyhedra, a vertex of one and a point of a face of the other, or points of two edges.  A vertex whose
+ * foot on a face plane falls outside the face is closer to one of the face's edges, which the edge-edge pairs cover (every
+ * vertex is the end of an edge). */
+static double point_segment_distance(const double p[3], const double a[3], const double b[3])
+{
+    double ab[3], ap[3], c[3];
+    sub3(b, a, ab);
+    sub3(p, a, ap);
+    double t = dot3(ap, ab) / dot3(ab, ab);
+    if (t < 0.0) t = 0.0;
+    if (t > 1.0) t = 1.0;
+    for (int k = 0; k < 3; ++k) c[k] = a[k] + t * ab[k] - p[k];
+    return norm3(c);
+}
+
+/* min over (s, t) in [0,1]^2 of |a0 + s (a1-a0) - b0 - t (b1-b0)|: a convex function on a square has its minimum at an
+ * interior stationary point or on one of the four sides, and each side is a point-segment problem */
+static double segment_segment_distance(const double a0[3], const double a1[3], const double b0[3], const double b1[3])
+{
+    double best = point_segment_distance(a0, b0, b1);
+    double d = point_segment_distance(a1, b0, b1);
+    if (d < best) best = d;
+    d = point_segment_distance(b0, a0, a1);
+    if (d < best) best = d;
+    d = point_segment_distance(b1, a0, a1);
+    if (d < best) best = d;
+    double u[3], v[3], w[3];
+    sub3(a1, a0, u);
+    sub3(b1, b0, v);
+    sub3(a0, b0, w);
+    double uu = dot3(u, u), uv = dot3(u, v), vv = dot3(v, v), uw = dot3(u, w), vw = dot3(v, w);
+    double den = uu * vv - uv * uv;
+    if (den > 1e-14 * uu * vv) { /* not parallel: the stationary point of the two infinite lines */
+        double sc = (uv * vw - vv * uw) / den, tc = (uu * vw - uv * uw) / den;
+        if (sc > 0.0 && sc < 1.0 && tc > 0.0 && tc < 1.0) {
+            double c[3];
+            for (int k = 0; k < 3; ++k) c[k] = w[k] + sc * u[k] - tc * v[k];
+            d = norm3(c);
+            if (d < best) best = d;
+        }
+    }
+    return best;
+}
+
+/* wa, wb: world-oriented vertices about each body origin; B's origin sits at r_ab from A's */
+static double core_distance(const orc_shape* s, const double r_ab[3], const double qa[4], const double qb[4], double (*wa)[3],
+                            double (*wb)[3])
+{
+    int nv = s->nverts;
+    double pb[ORC_MAX_VERTS][3]; /* B's vertices seen from A's origin */
+    for (int i = 0; i < nv; ++i)
+        for (int k = 0; k < 3; ++k) pb[i][k] = wb[i][k] + r_ab[k];
+    double best = INFINITY;
+    if (s->kind == ORC_KIND_POLYGON) {
+        for (int i = 0; i < nv; ++i)
+            for (int e = 0; e < nv; ++e) {
+                double d1 = point_segment_distance(pb[i], wa[e], wa[(e + 1) % nv]);
+                double d2 = point_segment_distance(wa[i], pb[e], pb[(e + 1) % nv]);
+                if (d1 < best) best = d1;
+                if (d2 < best) best = d2;
+            }
+        return best;
+    }
+    for (int e = 0; e < s->nedges; ++e)
+        for (int f = 0; f < s->nedges; ++f) {
+            double d = segment_segment_distance(wa[s->edge_v[e][0]], wa[s->edge_v[e][1]], pb[s->edge_v[f][0]], pb[s->edge_v[f][1]]);
+            if (d < best) best = d;
+        }
+    /* vertex above the inside of a face: the foot p - (n.p - c) n satisfies every other face inequality of that body */
+    for (int side = 0; side < 2; ++side) {
+        const double* q = side == 0 ? qa : qb;
+        for (int f = 0; f < s->nfaces; ++f) {
+            double n[3];
+            quat_rotate(q, s->face_n[f], n);
+            for (int i = 0; i < nv; ++i) {
+                double p[3]; /* the other body's vertex relative to this body's origin */
+                for (int k = 0; k < 3; ++k) p[k] = side == 0 ? pb[i][k] : wa[i][k] - r_ab[k];
+                double h = dot3(n, p) - s->face_c[f];
+                if (h < 0.0) continue;
+                double foot[3];
+                for (int k = 0; k < 3; ++k) foot[k] = p[k] - h * n[k];
+                int inside = 1;
+                for (int g = 0; g < s->nfaces && inside; ++g) {
+                    if (g == f) continue;
+                    double ng[3];
+                    quat_rotate(q, s->face_n[g], ng);
+                    if (dot3(ng, foot) > s->face_c[g]) inside = 0;
+                }
+                if (inside && h < best) best = h;
+            }
+        }
+    }
+    return best;
+}
+
+static double sharp_margin(const orc_shape* s, const double r_ab[3], const double qa[4], const double qb[4]);
+
+/* margin of the pair: < 0 iff the interiors intersect.  Sharp shapes: the separating-axis margin (O4).  Rounded shapes
+ * (sweep_r > 0): A (+) ball(r) and B (+) ball(r) intersect iff the cores are closer than 2 r, so
+ * m = D(core A, core B) - 2 r with D the Euclidean distance of disjoint cores and the (non-positive) separating-axis margin
+ * of cores that touch or intersect (continuous: both vanish at contact). */
 double orc_shape_margin(const orc_shape* s, const double r_ab[3], const double qa[4], const double qb[4])
+{
+    double m = sharp_margin(s, r_ab, qa, qb);
+    if (s->kind == ORC_KIND_DISK || !(s->sweep_r > 0.0)) return m;
+    if (m > 0.0) {
+        double wa[ORC_MAX_VERTS][3], wb[ORC_MAX_VERTS][3];
+        for (int i = 0; i < s->nverts; ++i) {
+            quat_rotate(qa, s->verts[i], wa[i]);
+            quat_rotate(qb, s->verts[i], wb[i]);
+        }
+        m = core_distance(s, r_ab, qa, qb, wa, wb);
+    }
+    return m - 2.0 * s->sweep_r;
+}
+
+static double sharp_margin(const orc_shape* s, const double r_ab[3], const double qa[4], const double qb[4])
 {
     if (s->kind == ORC_KIND_DISK) return norm3(r_ab) - s->diameter; /* P:89, P5 */
 
@@ -324,6 +465,16 @@ static void touch_axis(const double nhat[3], const double r_ab[3], double (*wa)[
 double orc_shape_touch_scale(const orc_shape* s, const double r_ab[3], const double qa[4], const double qb[4])
 {
     if (s->kind == ORC_KIND_DISK) return s->diameter / norm3(r_ab);
+    if (s->sweep_r > 0.0) {
+        /* rounded shapes: m(lambda r) is not piecewise linear in lambda; the pair overlaps iff lambda r lies inside the
+         * convex set B (-) A, which contains the origin, so m changes sign once on the ray: bisection on [0, d_max / |r|] */
+        double lo = 0.0, hi = s->dmax / norm3(r_ab);
+        for (int it = 0; it < 100; ++it) {
+            double mid = 0.5 * (lo + hi), rr[3] = {mid * r_ab[0], mid * r_ab[1], mid * r_ab[2]};
+            if (orc_shape_margin(s, rr, qa, qb) < 0.0) lo = mid; else hi = mid;
+        }
+        return 0.5 * (lo + hi);
+    }
     double wa[ORC_MAX_VERTS][3], wb[ORC_MAX_VERTS][3];
     int nv = s->nverts;
     for (int i = 0; i < nv; ++i) {
@@ -482,6 +633,7 @@ static int gjk_run(const orc_shape* s, const double r_ab[3], const double qa[4],
 
 int orc_shape_gjk(const orc_shape* s, const double r_ab[3], const double qa[4], const double qb[4])
 {
+    if (s->sweep_r > 0.0) return -1; /* the cross-check GJK runs on vertex sets only */
     return gjk_run(s, r_ab, qa, qb, NULL);
 }
 
@@ -538,10 +690,19 @@ struct orc_sys {
     int32_t *cell_id, *cell_start, *members;
 };
 
+static orc_sys* sys_create(orc_shape* sh, int dim, const double L[3], int64_t N, uint64_t seed);
 orc_sys* orc_create(int dim, const double L[3], int kind, double diameter, int nverts, const double* verts,
                     int64_t N, uint64_t seed)
 {
-    orc_shape* sh = orc_shape_create(dim, kind, diameter, nverts, verts);
+    return sys_create(orc_shape_create(dim, kind, diameter, nverts, verts), dim, L, N, seed);
+}
+orc_sys* orc_create_rounded(int dim, const double L[3], int kind, double sweep_r, int nverts, const double* verts,
+                            int64_t N, uint64_t seed)
+{
+    return sys_create(orc_shape_create_rounded(dim, kind, sweep_r, nverts, verts), dim, L, N, seed);
+}
+static orc_sys* sys_create(orc_shape* sh, int dim, const double L[3], int64_t N, uint64_t seed)
+{
     if (!sh) return NULL;
     orc_sys* s = (orc_sys*)calloc(1, sizeof *s);
     s->dim = dim;
@@ -769,7 +930,7 @@ static double scan_candidates(const orc_sys* s, orc_work* wk, orc_probe* probe, 
                         for (int k = 0; k < 3; ++k) probe->r[c][k] = r[k];
                         for (int k = 0; k < 4; ++k) probe->qb[c][k] = s->quat[4 * j + k];
                     }
-                    if (!found && s->work_detail) { /* O7: what an early-exit narrow phase would have evaluated */
+                    if (!found && s->work_detail && !(sh->sweep_r > 0.0)) { /* O7: what an early-exit narrow phase would have evaluated */
                         if (sh->kind == ORC_KIND_POLYGON)
                             wk->polygon_axes_early += (uint64_t)polygon_axes_until_separation(sh, r, qa, qb, s->eps_g);
                         else if (sh->kind == ORC_KIND_POLYHEDRON)

@@ -92,6 +92,11 @@ float orc_usym(uint32_t r); /* ((int)(r>>8) - 2^23) * 2^-23 in [-1,1) */
 
 /* ---- shapes and margins (O4) ------------------------------------------- */
 orc_shape* orc_shape_create(int dim, int kind, double diameter, int nverts, const double* verts);
+/* P:89 spheropolygon (dim 2, ORC_KIND_POLYGON) / convex spheropolyhedron (dim 3, ORC_KIND_POLYHEDRON): the polygon /
+ * polyhedron ("core") swept by a disk / sphere of radius sweep_radius >= 0; d_max = 2 (circumradius + sweep_radius).
+ * margin = distance between the cores - 2 sweep_radius (brute force over vertex/edge/face pairs). */
+orc_shape* orc_shape_create_rounded(int dim, int kind, double sweep_radius, int nverts, const double* verts);
+double orc_shape_sweep_radius(const orc_shape*);
 void orc_shape_destroy(orc_shape*);
 double orc_shape_dmax(const orc_shape*);
 int orc_shape_nfaces(const orc_shape*);
@@ -107,6 +112,8 @@ int orc_shape_gjk(const orc_shape*, const double r_ab[3], const double qa[4], co
 /* ---- system -------------------------------------------------------------- */
 orc_sys* orc_create(int dim, const double L[3], int kind, double diameter, int nverts,
                     const double* verts, int64_t N, uint64_t seed);
+orc_sys* orc_create_rounded(int dim, const double L[3], int kind, double sweep_radius, int nverts, const double* verts,
+                            int64_t N, uint64_t seed);
 void orc_destroy(orc_sys*);
 const orc_shape* orc_sys_shape(const orc_sys*);
 int orc_set_moves(orc_sys*, double d, double a, int n_select);

@@ -60,6 +60,10 @@ def lib():
     L.orc_u01.argtypes = [C.c_uint32]; L.orc_u01.restype = C.c_float
     L.orc_usym.argtypes = [C.c_uint32]; L.orc_usym.restype = C.c_float
     L.orc_shape_create.argtypes = [C.c_int, C.c_int, C.c_double, C.c_int, dp]; L.orc_shape_create.restype = vp
+    L.orc_shape_create_rounded.argtypes = [C.c_int, C.c_int, C.c_double, C.c_int, dp]; L.orc_shape_create_rounded.restype = vp
+    L.orc_shape_sweep_radius.argtypes = [vp]; L.orc_shape_sweep_radius.restype = C.c_double
+    L.orc_create_rounded.argtypes = [C.c_int, dp, C.c_int, C.c_double, C.c_int, dp, C.c_int64, C.c_uint64]
+    L.orc_create_rounded.restype = vp
     L.orc_shape_destroy.argtypes = [vp]
     L.orc_shape_dmax.argtypes = [vp]; L.orc_shape_dmax.restype = C.c_double
     L.orc_shape_nfaces.argtypes = [vp]; L.orc_shape_nfaces.restype = C.c_int
@@ -139,13 +143,17 @@ def usym(r):
 
 
 class Shape:
-    """One hard shape (O1): disk/sphere, convex polygon (CCW) or convex polyhedron (vertex list)."""
+    """One hard shape (O1): disk/sphere, convex polygon (CCW) or convex polyhedron (vertex list); sweep_radius > 0 rounds
+    the polygon / polyhedron (spheropolygon / spheropolyhedron)."""
 
-    def __init__(self, dim, kind, diameter=0.0, verts=None):
+    def __init__(self, dim, kind, diameter=0.0, verts=None, sweep_radius=0.0):
         self.dim, self.kind = dim, kind
         v = np.zeros(1) if verts is None else np.ascontiguousarray(verts, dtype=np.float64)
         nv = 0 if verts is None else v.shape[0]
-        self._h = lib().orc_shape_create(dim, kind, float(diameter), nv, _dp(v))
+        if sweep_radius:
+            self._h = lib().orc_shape_create_rounded(dim, kind, float(sweep_radius), nv, _dp(v))
+        else:
+            self._h = lib().orc_shape_create(dim, kind, float(diameter), nv, _dp(v))
         if not self._h:
             raise ValueError("oracle rejected the shape (non-convex, not CCW, too many vertices, bad dim)")
 
@@ -157,6 +165,10 @@ class Shape:
     @property
     def dmax(self):
         return lib().orc_shape_dmax(self._h)
+
+    @property
+    def sweep_radius(self):
+        return lib().orc_shape_sweep_radius(self._h)
 
     @property
     def nfaces(self):
@@ -192,12 +204,15 @@ class Shape:
 class Oracle:
     """The serial checkerboard-sweep oracle (O1-O8, O11)."""
 
-    def __init__(self, dim, L, kind, N, seed, diameter=0.0, verts=None):
+    def __init__(self, dim, L, kind, N, seed, diameter=0.0, verts=None, sweep_radius=0.0):
         Ld = np.ones(3); Ld[:dim] = np.asarray(L, dtype=np.float64)[:dim]
         v = np.zeros(1) if verts is None else np.ascontiguousarray(verts, dtype=np.float64)
         nv = 0 if verts is None else v.shape[0]
         self.dim, self.N, self.kind = dim, int(N), kind
-        self._h = lib().orc_create(dim, _dp(Ld), kind, float(diameter), nv, _dp(v), int(N), int(seed))
+        if sweep_radius:
+            self._h = lib().orc_create_rounded(dim, _dp(Ld), kind, float(sweep_radius), nv, _dp(v), int(N), int(seed))
+        else:
+            self._h = lib().orc_create(dim, _dp(Ld), kind, float(diameter), nv, _dp(v), int(N), int(seed))
         if not self._h:
             raise ValueError("oracle rejected the system (shape invalid or fewer than 4 cells per side)")
         n = np.zeros(3, np.int32); w = np.zeros(3); wf = np.zeros(3, np.float32)
