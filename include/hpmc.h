@@ -60,6 +60,10 @@ typedef struct {
     double diameter;     /* kind 0 */
     int nverts;          /* kind 1: 3..32 vertices (x,y); kind 2: 4..32 vertices (x,y,z) */
     const double* verts; /* h_: nverts*2 or nverts*3 doubles, body frame; read during the call only */
+    double sweep_radius; /* kinds 1, 2: >= 0.  > 0 makes the shape a spheropolygon / convex spheropolyhedron: the polygon /
+                            polyhedron swept by a disk / sphere of this radius; two of them overlap iff their cores are
+                            closer than 2 sweep_radius, and d_max = 2 (circumradius + sweep_radius).  0 = the sharp shape.
+                            Ignored for kind 0.  Negative or non-finite: HPMC_E_SHAPE.                                    */
 } hpmc_shape;
 
 /* P:47 "percentage of the trial moves are accepted": accepted / attempted per type (R26) */

@@ -31,7 +31,8 @@ class Box(C.Structure):
 
 
 class ShapeDesc(C.Structure):
-    _fields_ = [("kind", C.c_int), ("diameter", C.c_double), ("nverts", C.c_int), ("verts", C.POINTER(C.c_double))]
+    _fields_ = [("kind", C.c_int), ("diameter", C.c_double), ("nverts", C.c_int), ("verts", C.POINTER(C.c_double)),
+                ("sweep_radius", C.c_double)]
 
 
 class Counters(C.Structure):
@@ -104,7 +105,7 @@ def load_library():
 class Hpmc:
     """One NVT hard-particle system on one GPU.  Mirrors the C-ABI names one to one."""
 
-    def __init__(self, dim, L, kind, N, seed, diameter=0.0, verts=None, device="cuda:0", stream=None):
+    def __init__(self, dim, L, kind, N, seed, diameter=0.0, verts=None, device="cuda:0", stream=None, sweep_radius=0.0):
         import torch  # device memory + streams only
         self._torch = torch
         self._lib = load_library()
@@ -115,7 +116,7 @@ class Hpmc:
         box = Box(); box.dim = self.dim
         for k in range(3):
             box.L[k] = float(L[k]) if k < self.dim else 1.0
-        sd = ShapeDesc(); sd.kind = self.kind; sd.diameter = float(diameter)
+        sd = ShapeDesc(); sd.kind = self.kind; sd.diameter = float(diameter); sd.sweep_radius = float(sweep_radius)
         self._verts = None
         if verts is not None:
             self._verts = np.ascontiguousarray(verts, dtype=np.float64)
@@ -353,7 +354,7 @@ class Hpmc:
 
 def from_workload(w, seed=1, device="cuda:0"):
     """Create + bind + set_moves for a workloads.Workload."""
-    h = Hpmc(w.dim, w.L, w.kind, w.N, seed, diameter=w.diameter, verts=w.verts, device=device)
+    h = Hpmc(w.dim, w.L, w.kind, w.N, seed, diameter=w.diameter, verts=w.verts, device=device, sweep_radius=w.sweep_radius)
     h.set_moves(w.d, w.a, w.n_select)
     h.bind(w.pos4, w.quat4)
     return h

@@ -120,7 +120,10 @@ int build_shape(hpmc_ctx* c, const hpmc_shape* s, int dim)
             D.vz[i] = poly2 ? 0.0 : s->verts[i * vd + 2];
             rmax = std::fmax(rmax, std::sqrt(D.vx[i] * D.vx[i] + D.vy[i] * D.vy[i] + D.vz[i] * D.vz[i]));
         }
-        c->d_max = 2.0 * rmax;  // circumsphere centred on the particle position
+        const double rho = s->sweep_radius;   // rounded shapes (spheropolygons / spheropolyhedra)
+        if (!(rho >= 0.0) || !std::isfinite(rho)) return fail(c, HPMC_E_SHAPE, "sweep_radius must be finite and >= 0");
+        D.sweep = 2.0 * rho;
+        c->d_max = 2.0 * (rmax + rho);  // circumsphere centred on the particle position
         double r_in = 1e300;    // inscribed radius about the body origin = smallest face/edge offset
         if (poly2) {
             // regular n-gon centred on the origin: equal radii and equal angular steps (see polygon_separated)
@@ -180,7 +183,7 @@ int build_shape(hpmc_ctx* c, const hpmc_shape* s, int dim)
             for (int l = 0; l < nv; ++l)
                 if (on_hull[l] < 3) return fail(c, HPMC_E_SHAPE, "every vertex must be a hull vertex (convex polyhedron)");
         }
-        const double din = std::fmax(0.0, 2.0 * r_in - 1e-5);
+        const double din = std::fmax(0.0, 2.0 * (r_in + rho) - 1e-5);   // the rounded shape holds the ball of radius r_in + rho
         D.din2 = din * din;
         D.rin = r_in;
     } else
@@ -194,6 +197,7 @@ int build_shape(hpmc_ctx* c, const hpmc_shape* s, int dim)
     F.din2 = (float)D.din2;
     F.rin = (float)(D.rin * (1.0 - 1e-6));   // rounded DOWN: the candidate-axis test of polygon_separated must never exclude an axis that separates
     F.regular = D.regular;
+    F.sweep = (float)D.sweep;
     for (int i = 0; i < kMaxVerts; ++i) {
         F.vx[i] = (float)D.vx[i]; F.vy[i] = (float)D.vy[i]; F.vz[i] = (float)D.vz[i];
         F.nx[i] = (float)D.nx[i]; F.ny[i] = (float)D.ny[i]; F.fc[i] = (float)D.fc[i];
@@ -363,7 +367,7 @@ bool cluster_eligible(const hpmc_ctx* c)
 int64_t sweep_cluster(hpmc_ctx* c, int64_t n)
 {
     const int kind = c->sf.kind;
-    const int nv = (kind == kKindPolygon && c->sf.nverts == 5 && c->sf.regular) ? 5 : 0;
+    const int nv = (kind == kKindPolygon && c->sf.nverts == 5 && c->sf.regular && c->sd.sweep == 0.0) ? 5 : 0;
     int64_t done = 0;
     while (done < n) {
         const int64_t want = std::min<int64_t>(n - done, 1 << 20);   // sweeps per launch
@@ -398,7 +402,8 @@ int launch_colour_dispatch(hpmc_ctx* c, int ci)
     ProfileScope prof(c, 1, c->flow_now ? 4 : 1);
     // the (kind, unrolled vertex count) variants of each pass are compiled in separate translation units (pass_*.cu)
     const int kind = c->sf.kind;
-    const int nv = (kind == kKindPolygon && c->sf.nverts == 5 && c->sf.regular) ? 5 : (kind == kKindPolyhedron && c->sf.nverts == 8) ? 8 : 0;
+    const bool sharp = c->sd.sweep == 0.0;   // rounded shapes take the runtime-vertex-count kernels (overlap.cuh)
+    const int nv = (kind == kKindPolygon && c->sf.nverts == 5 && c->sf.regular && sharp) ? 5 : (kind == kKindPolyhedron && c->sf.nverts == 8 && sharp) ? 8 : 0;
     const GridParams& g = c->g;
     const int nactive = (g.n[0] / 2) * (g.n[1] / 2) * (g.dim == 3 ? g.n[2] / 2 : 1);
     bool ok = true;

@@ -4,6 +4,9 @@
 //   convex polygon     : separating axes over the edge normals of both, in A's frame
 //   convex polyhedron  : GJK separating-axis search on the Minkowski difference B (-) A with the support
 //                        function of Eq. (2): S(n) = R S_B(R^-1 n) + r_AB - S_A(-n), in A's frame.
+//   rounded shapes     : spheropolygons / convex spheropolyhedra, the polygon / polyhedron ("core") swept by a disk /
+//                        sphere of radius rho: two of them overlap iff their cores are closer than 2 rho = S.sweep.  Runtime
+//                        vertex count only (NV == 0 instantiations), so the unrolled pentagon / cube paths do not carry it.
 // Every test answers "is the pair separated by at least eps?"; "no" means overlap (R15, R-poly).
 #pragma once
 #include "common.cuh"
@@ -18,6 +21,7 @@ struct ShapeT {
     T din2;               // (2 r_in - 1e-5)^2: centres closer than this certainly overlap (r_in = inscribed radius about
                           // the body origin); 0 for disks (the broad phase is the whole test)
     T rin;                // inscribed radius about the body origin (polygons: min_k fc[k]); every support height h(u) >= rin
+    T sweep;              // rounded shapes: 2 x sweep radius, the distance below which two cores mean overlap; 0 = sharp
     int regular;          // polygon: regular n-gon centred on the body origin (all |v| equal, equal angles): see polygon_separated
     T vx[kMaxVerts], vy[kMaxVerts], vz[kMaxVerts];
     T nx[kMaxVerts], ny[kMaxVerts], fc[kMaxVerts];  // polygon: outward unit edge normals and offsets n.v
@@ -56,6 +60,60 @@ __device__ __forceinline__ V3<T> operator*(T s, const V3<T>& a)
 }
 
 // ---------------------------------------------------------------------------------------------
+// spheropolygons: is the distance between the two core polygons at least S.sweep + eps?  In A's body frame.
+//   1. the largest separation of the cores over the edge normals of both (the separating-axis margin, a lower bound of the
+//      distance): at least S.sweep + eps -> separated; negative -> the cores themselves intersect -> overlap;
+//   2. otherwise the cores are disjoint and closer than their axis separation can tell (vertex against vertex): the
+//      distance of two disjoint convex polygons is attained between a vertex of one and an edge of the other, so take the
+//      minimum point-segment distance over all such pairs.
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+__device__ __forceinline__ T point_segment_dist2(T px, T py, T ax, T ay, T bx, T by)
+{
+    const T ex = bx - ax, ey = by - ay, wx = px - ax, wy = py - ay;
+    T t = (wx * ex + wy * ey) / (ex * ex + ey * ey);
+    t = min(max(t, (T)0), (T)1);
+    const T dx = wx - t * ex, dy = wy - t * ey;
+    return dx * dx + dy * dy;
+}
+
+template <typename T>
+__device__ __noinline__ bool spheropolygon_separated(const ShapeT<T>& S, T rx, T ry, T cA, T sA, T cB, T sB, T eps)
+{
+    const int nv = S.nverts;
+    const T need = S.sweep + eps;
+    const T lx = cA * rx + sA * ry, ly = -sA * rx + cA * ry;   // R_A^T r_AB
+    const T c = cA * cB + sA * sB, s = cA * sB - sA * cB;      // R = R_A^T R_B
+    T px[kMaxVerts], py[kMaxVerts];                            // B's vertices in A's frame
+    for (int j = 0; j < nv; ++j) {
+        px[j] = c * S.vx[j] - s * S.vy[j] + lx;
+        py[j] = s * S.vx[j] + c * S.vy[j] + ly;
+    }
+    T msat = -(T)3.0e38;
+    for (int k = 0; k < nv; ++k) {
+        // A's edge normal k against B's vertices; B's edge normal k (rotated into A's frame) against A's vertices
+        const T nxk = c * S.nx[k] - s * S.ny[k], nyk = s * S.nx[k] + c * S.ny[k];
+        T ma = S.nx[k] * px[0] + S.ny[k] * py[0];
+        T mb = nxk * (S.vx[0] - lx) + nyk * (S.vy[0] - ly);
+        for (int j = 1; j < nv; ++j) {
+            ma = min(ma, S.nx[k] * px[j] + S.ny[k] * py[j]);
+            mb = min(mb, nxk * (S.vx[j] - lx) + nyk * (S.vy[j] - ly));
+        }
+        msat = max(msat, max(ma, mb) - S.fc[k]);
+    }
+    if (msat >= need) return true;
+    if (msat < (T)0) return false;
+    T d2 = (T)3.0e38;
+    for (int i = 0; i < nv; ++i)
+        for (int k = 0; k < nv; ++k) {
+            const int k1 = (k + 1 == nv) ? 0 : k + 1;
+            d2 = min(d2, point_segment_dist2(px[i], py[i], S.vx[k], S.vy[k], S.vx[k1], S.vy[k1]));
+            d2 = min(d2, point_segment_dist2(S.vx[i], S.vy[i], px[k], py[k], px[k1], py[k1]));
+        }
+    return d2 >= need * need;
+}
+
+// ---------------------------------------------------------------------------------------------
 // convex polygons: in A's body frame A's vertices/normals are the stored constants, so only B has to
 // be rotated ("a local coordinate system centered on particle A").
 // (rx, ry) = r_AB in the world frame; (cA,sA), (cB,sB) = cos/sin of the orientation angles.
@@ -66,6 +124,7 @@ __device__ __forceinline__ V3<T> operator*(T s, const V3<T>& a)
 template <typename T, int NV>
 __device__ __forceinline__ bool polygon_overlap(const ShapeT<T>& S, T rx, T ry, T cA, T sA, T cB, T sB, T eps)
 {
+    if (NV == 0 && S.sweep > (T)0) return !spheropolygon_separated<T>(S, rx, ry, cA, sA, cB, sB, eps);
     const int nv = (NV > 0) ? NV : S.nverts;
     const T lx = cA * rx + sA * ry;    // R_A^T r_AB
     const T ly = -sA * rx + cA * ry;
@@ -129,6 +188,7 @@ __device__ __forceinline__ bool polygon_overlap(const ShapeT<T>& S, T rx, T ry, 
 template <int NV>
 __device__ __forceinline__ bool polygon_separated(const ShapeT<float>& S, float rx, float ry, float cA, float sA, float cB, float sB, float eps)
 {
+    if (NV == 0 && S.sweep > 0.0f) return spheropolygon_separated<float>(S, rx, ry, cA, sA, cB, sB, eps);
     const int nv = (NV > 0) ? NV : S.nverts;
     const float lAx = cA * rx + sA * ry, lAy = cA * ry - sA * rx;      // R_A^T r
     const float lBx = cB * rx + sB * ry, lBy = cB * ry - sB * rx;      // R_B^T r
@@ -394,7 +454,10 @@ __device__ int mpr_classify(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T e
             }
         }
         int pw;
-        const V3<T> w = support_minkowski<T, NVP>(S, Rm, r, n, pw);
+        V3<T> w = support_minkowski<T, NVP>(S, Rm, r, n, pw);
+        // rounded shapes: B (-) A is the difference of the cores swept by a ball of radius 2 rho = S.sweep, whose support point
+        // along n lies S.sweep further out (every certificate below then speaks about the rounded bodies)
+        if (NVP == 0 && S.sweep > (T)0) w = w + (S.sweep * rsqrt(nn)) * n;
         const T h = dot(w, n);
         if (h <= 0) {   // the whole of B (-) A lies at n^ . x <= h / |n|: a separating plane if that is <= -eps
             if (h * h >= eps * eps * nn) verdict = kGjkSeparated;
@@ -461,7 +524,8 @@ __device__ __forceinline__ int polyhedron_classify(const ShapeT<T>& S, const T* 
                   MA[2] * rw.x + MA[5] * rw.y + MA[8] * rw.z};
     portal[0] = -1;
     if (sizeof(T) == 4 && kFp32UseMpr) return mpr_classify<T, NVP>(S, Rm, r, eps, deep, portal);
-    return gjk_classify<T, NVP>(S, Rm, r, eps, deep);
+    // GJK runs on the cores (finite for polytopes): rounded shapes are separated by eps iff the cores are by S.sweep + eps
+    return gjk_classify<T, NVP>(S, Rm, r, (NVP == 0) ? eps + S.sweep : eps, deep);
 }
 
 // fp64 narrow phase from the raw fp32 state: normalised quaternions, exact separation rd (already minimum image).

@@ -35,6 +35,7 @@ class Workload:
     warmup_sweeps: int = 0     # sweeps to melt the lattice before timing
     notes: str = ""
     extra: dict = field(default_factory=dict)
+    sweep_radius: float = 0.0  # > 0: spheropolygon / spheropolyhedron, `verts` is the core
 
 
 def regular_polygon(nv: int, circumradius: float) -> np.ndarray:
@@ -149,8 +150,28 @@ def pentagons(n_lat: int = 64, seed: int = 1, name: str = None, sweeps: int = No
                     extra={"seed": seed, "phi": N * area / (L * L)})
 
 
+def rounded_polygons(n_lat: int = 64, seed: int = 1, nv: int = 5, circumradius: float = 0.35, sweep_radius: float = 0.1,
+                     spacing: float = 1.0, d: float = 0.1, a: float = 0.3, name: str = None) -> Workload:
+    """Spheropolygons: regular nv-gons of the given circumradius swept by a disk of `sweep_radius`, on a square lattice
+    with uniform-random orientations.  The caller keeps d_max = 2 (circumradius + sweep_radius) below `spacing`, so that every
+    orientation is overlap-free."""
+    assert 2.0 * (circumradius + sweep_radius) < spacing
+    N = n_lat * n_lat
+    pos4 = _lattice(2, n_lat, spacing)
+    theta = 2.0 * np.pi * _rng(seed, 404).random(N)
+    quat4 = np.zeros((N, 4), dtype=np.float32)
+    quat4[:, 0] = np.cos(0.5 * theta).astype(np.float32)
+    quat4[:, 3] = np.sin(0.5 * theta).astype(np.float32)
+    L = n_lat * spacing
+    side = 2.0 * circumradius * np.sin(np.pi / nv)
+    area = 0.5 * nv * circumradius ** 2 * np.sin(2.0 * np.pi / nv) + nv * side * sweep_radius + np.pi * sweep_radius ** 2
+    return Workload(name=name or f"rounded_{nv}gons_{N}", dim=2, N=N, L=(L, L), kind=KIND_POLYGON, diameter=0.0,
+                    verts=regular_polygon(nv, circumradius), sweep_radius=sweep_radius, d=d, a=a, n_select=4, sweeps=100,
+                    pos4=pos4, quat4=quat4, warmup_sweeps=50, extra={"seed": seed, "phi": N * area / (L * L)})
+
+
 def cubes(n_lat: int = 32, seed: int = 1, max_tilt: float = 0.15, name: str = "k3_cubes", spacing: float = 1.25,
-          d: float = 0.1, a: float = 0.1) -> Workload:
+          d: float = 0.1, a: float = 0.1, edge: float = 1.0, sweep_radius: float = 0.0) -> Workload:
     """I3: configs[3]; unit cubes as generic 8-vertex polyhedra on a simple-cubic lattice, spacing 1.25.
 
     DEVIATION (R27): uniform-random orientations at spacing 1.25 overlap with probability 0.877 per
@@ -160,6 +181,8 @@ def cubes(n_lat: int = 32, seed: int = 1, max_tilt: float = 0.15, name: str = "k
 
     Other `spacing` / `max_tilt` / move sizes give test cases (the caller keeps 0.5 (1 + sqrt 2 sin(max_tilt)) below
     spacing / 2): e.g. spacing 1.0006 with tilts of 2e-4 rad is a crystal of nearly parallel, nearly touching faces.
+    `edge` and `sweep_radius` make rounded cubes (spheropolyhedra): a cube of that edge swept by a sphere of that
+    radius; the caller keeps 0.61 edge + sweep_radius below spacing / 2.
     """
     N = n_lat ** 3
     pos4 = _lattice(3, n_lat, spacing)
@@ -175,7 +198,8 @@ def cubes(n_lat: int = 32, seed: int = 1, max_tilt: float = 0.15, name: str = "k
     q = _qmul(g, tau)
     q /= np.linalg.norm(q, axis=1, keepdims=True)
     L = n_lat * spacing
-    return Workload(name=name, dim=3, N=N, L=(L, L, L), kind=KIND_POLYHEDRON, diameter=0.0, verts=cube_vertices(1.0),
+    return Workload(name=name, dim=3, N=N, L=(L, L, L), kind=KIND_POLYHEDRON, diameter=0.0, verts=cube_vertices(edge),
+                    sweep_radius=sweep_radius,
                     d=d, a=a, n_select=4, sweeps=1000, pos4=pos4, quat4=q.astype(np.float32), warmup_sweeps=200,
                     notes="initial orientations: cube-group element x tilt<=0.15 rad (BASELINE.json's uniform-random "
                           "orientations are infeasible at spacing 1.25)",

@@ -28,11 +28,11 @@ def test_header_symbols_all_exported(lib):
         assert getattr(lib, name) is not None
 
 
-def _create(lib, dim, L, kind, N, diameter=0.0, verts=None):
+def _create(lib, dim, L, kind, N, diameter=0.0, verts=None, sweep_radius=0.0):
     box = hb.Box(); box.dim = dim
     for k in range(3):
         box.L[k] = L[k] if k < len(L) else 1.0
-    sd = hb.ShapeDesc(); sd.kind = kind; sd.diameter = diameter
+    sd = hb.ShapeDesc(); sd.kind = kind; sd.diameter = diameter; sd.sweep_radius = sweep_radius
     keep = None
     if verts is not None:
         keep = np.ascontiguousarray(verts, dtype=np.float64)
@@ -65,6 +65,22 @@ def test_create_validation_and_grid(lib):
     assert rc == 0 and lib.hpmc_get_grid(h, C.byref(gi)) == 0 and list(gi.n) == [22, 22, 22]
     assert gi.d_max == pytest.approx(3 ** 0.5)
     lib.hpmc_destroy(h)
+
+
+def test_rounded_shapes_grid_and_validation(lib):
+    """Spheropolygons / spheropolyhedra: d_max = 2 (circumradius + sweep_radius) sets the grid (R11)."""
+    gi = hb.GridInfo()
+    rc, h = _create(lib, 2, (64.0, 64.0), hb.KIND_POLYGON, 16, verts=wl.regular_polygon(5, 0.35), sweep_radius=0.1)
+    assert rc == 0 and lib.hpmc_get_grid(h, C.byref(gi)) == 0
+    assert gi.d_max == pytest.approx(0.9, abs=1e-15) and list(gi.n)[:2] == [70, 70]        # 2 floor(64 / (2 x 0.9 (1 + 2^-10)))
+    lib.hpmc_destroy(h)
+    rc, h = _create(lib, 3, (40.0,) * 3, hb.KIND_POLYHEDRON, 8, verts=wl.cube_vertices(0.7), sweep_radius=0.15)
+    assert rc == 0 and lib.hpmc_get_grid(h, C.byref(gi)) == 0
+    assert gi.d_max == pytest.approx(2 * (0.35 * 3 ** 0.5 + 0.15)) and list(gi.n) == [26, 26, 26]
+    lib.hpmc_destroy(h)
+    for bad in (-0.1, float("nan"), float("inf")):
+        assert _create(lib, 2, (64.0, 64.0), hb.KIND_POLYGON, 16, verts=wl.regular_polygon(5, 0.35), sweep_radius=bad)[0] == -2
+    assert _create(lib, 2, (64.0, 64.0), hb.KIND_DISK, 16, diameter=1.0, sweep_radius=-1.0)[0] == 0     # ignored for disks
 
 
 def test_create_rejects_bad_input(lib):
