@@ -254,6 +254,43 @@ def polyhedra(verts: np.ndarray, n_lat: int = 6, spacing: float = 1.05, seed: in
                     extra={"seed": seed})
 
 
+def fcc_spheres(m: int = 32, phi: float = 0.60, d: float = 0.06, name: str = "fcc_spheres") -> Workload:
+    """4 m^3 hard spheres of diameter 1 on a face-centred cubic lattice at volume fraction `phi`: the paper's sphere validation
+    state is 131 072 = 4 x 32^3 spheres at phi = 0.60, started "on the known self-assembled FCC" lattice."""
+    A = (4.0 * (np.pi / 6.0) / phi) ** (1.0 / 3.0)
+    basis = np.array([[0.0, 0.0, 0.0], [0.5, 0.5, 0.0], [0.5, 0.0, 0.5], [0.0, 0.5, 0.5]])
+    idx = np.stack(np.meshgrid(np.arange(m), np.arange(m), np.arange(m), indexing="ij"), axis=-1).reshape(-1, 3)
+    p = (idx[:, None, :] + basis[None, :, :] + 0.25).reshape(-1, 3) * A - 0.5 * m * A
+    N = p.shape[0]
+    pos4 = np.zeros((N, 4), dtype=np.float32)
+    pos4[:, :3] = p.astype(np.float32)
+    L = m * A
+    return Workload(name=name, dim=3, N=N, L=(L, L, L), kind=KIND_DISK, diameter=1.0, verts=None, d=d, a=0.0, n_select=4,
+                    sweeps=100, pos4=pos4, quat4=_identity_quats(N), warmup_sweeps=50, notes=f"FCC crystal start at phi = {phi}",
+                    extra={"phi": phi})
+
+
+def bcc_polyhedra(verts: np.ndarray, m: int = 20, phi: float = 0.7, volume: float = None, name: str = "bcc_polyhedra",
+                  d: float = 0.04, a: float = 0.05) -> Workload:
+    """2 m^3 identical convex polyhedra on a body-centred cubic lattice at volume fraction `phi`, all in the body orientation:
+    the paper's third validation state is 16 000 = 2 x 20^3 truncated octahedra at phi = 0.7 on "the known self-assembled ...
+    BCC" lattice (P:253); truncated octahedra with the vertices of `truncated_octahedron_vertices` tile space on it at phi = 1."""
+    if volume is None:
+        from scipy.spatial import ConvexHull
+        volume = float(ConvexHull(np.asarray(verts, dtype=np.float64)).volume)
+    A = (2.0 * volume / phi) ** (1.0 / 3.0)
+    basis = np.array([[0.0, 0.0, 0.0], [0.5, 0.5, 0.5]])
+    idx = np.stack(np.meshgrid(np.arange(m), np.arange(m), np.arange(m), indexing="ij"), axis=-1).reshape(-1, 3)
+    p = (idx[:, None, :] + basis[None, :, :] + 0.25).reshape(-1, 3) * A - 0.5 * m * A
+    N = p.shape[0]
+    pos4 = np.zeros((N, 4), dtype=np.float32)
+    pos4[:, :3] = p.astype(np.float32)
+    L = m * A
+    return Workload(name=name, dim=3, N=N, L=(L, L, L), kind=KIND_POLYHEDRON, diameter=0.0, verts=np.asarray(verts, dtype=np.float64),
+                    d=d, a=a, n_select=4, sweeps=100, pos4=pos4, quat4=_identity_quats(N), warmup_sweeps=50,
+                    notes=f"BCC crystal start at phi = {phi}", extra={"phi": phi, "volume": volume})
+
+
 def config(k: int, seed: int = 1) -> Workload:
     """BASELINE.json configs[k], k = 0..4."""
     if k == 0:
