@@ -243,13 +243,58 @@ __global__ void k_scatter(int N, int dim, const float4* __restrict__ src_pos, co
 // the atomics of k_hist produced.  A launch of its own: the scatter's stores are then visible without fences, the cells of
 // neighbouring threads are neighbours in memory, and no thread spins through dependent L2 loads while its warp waits
 // (measured on 1 M pentagons: scatter + sort 9.8 + ~5 us against 25 us for the scatter whose last arrival sorted the cell).
-__global__ void k_sort_cells(int C, int dim, const int* __restrict__ cell_start, float4* pos, float4* quat, int* tag)
+// Cells of up to kSortRegs members (all but freak cells) are sorted in registers: every tag is loaded at once, the rank of a
+// member is the number of smaller tags in its cell, then every pose is loaded at once and stored at its rank -- two rounds of
+// independent loads instead of an insertion sort's chain of dependent global loads and stores (config 3, ~3 members per cell:
+// 17 -> 6 us under ncu).
+template <int M>
+__device__ __forceinline__ void sort_cell_in_registers(int s, int n, int dim, float4* pos, float4* quat, int* tag)
 {
+    int t[M], r[M];
+#pragma unroll
+    for (int k = 0; k < M; ++k) t[k] = (k < n) ? tag[s + k] : 0x7fffffff;   // padding ranks behind every member
+    bool sorted = true;
+#pragma unroll
+    for (int k = 0; k < M; ++k) {
+        int rk = 0;
+#pragma unroll
+        for (int j = 0; j < M; ++j) rk += (j != k && t[j] < t[k]) ? 1 : 0;   // tags are distinct
+        r[k] = rk;
+        sorted = sorted && (k >= n || rk == k);
+    }
+    if (sorted) return;
+    float4 P[M];
+#pragma unroll
+    for (int k = 0; k < M; ++k)
+        if (k < n) P[k] = pos[s + k];
+#pragma unroll
+    for (int k = 0; k < M; ++k)
+        if (k < n) { pos[s + r[k]] = P[k]; tag[s + r[k]] = t[k]; }
+    if (dim == 3) {
+#pragma unroll
+        for (int k = 0; k < M; ++k)
+            if (k < n) P[k] = quat[s + k];
+#pragma unroll
+        for (int k = 0; k < M; ++k)
+            if (k < n) quat[s + r[k]] = P[k];
+    }
+}
+
+// DIM = 3 only takes the register path: 2-D cells hold one particle, sometimes two (the insertion sort is then one compare
+// and one swap), and the 1 M-thread launch of config 2 is 5 us slower with the 78 registers of the register path.
+template <int DIM>
+__global__ void k_sort_cells(int C, const int* __restrict__ cell_start, float4* pos, float4* quat, int* tag)
+{
+    constexpr int dim = DIM;
     pdl_launch_dependents();
     pdl_wait();
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= C) return;
     const int s = cell_start[c], e = cell_start[c + 1];
+    const int n = e - s;
+    if (n < 2) return;
+    if (DIM == 3 && n <= 4) { sort_cell_in_registers<4>(s, n, dim, pos, quat, tag); return; }
+    if (DIM == 3 && n <= 8) { sort_cell_in_registers<8>(s, n, dim, pos, quat, tag); return; }
     for (int i = s + 1; i < e; ++i) {
         const int ti = tag[i];
         int j = i - 1;

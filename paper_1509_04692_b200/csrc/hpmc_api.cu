@@ -299,7 +299,8 @@ int build_cell_list(hpmc_ctx* c, int mode, unsigned long long t_override)
         hpmc_launch(c, k_scatter, nblk_part, TB, 0, g.N, g.dim, src_pos, src_quat, src_tag, c->key_rank, c->cell_start, c->pos[dst], c->quat[dst],
                                                   c->tag[dst]);
         LAUNCH_CHECK(c, "k_scatter");
-        hpmc_launch(c, k_sort_cells, (g.C + TB - 1) / TB, TB, 0, g.C, g.dim, c->cell_start, c->pos[dst], c->quat[dst], c->tag[dst]);
+        if (g.dim == 3) hpmc_launch(c, k_sort_cells<3>, (g.C + TB - 1) / TB, TB, 0, g.C, c->cell_start, c->pos[dst], c->quat[dst], c->tag[dst]);
+        else hpmc_launch(c, k_sort_cells<2>, (g.C + TB - 1) / TB, TB, 0, g.C, c->cell_start, c->pos[dst], c->quat[dst], c->tag[dst]);
         LAUNCH_CHECK(c, "k_sort_cells");
     }
     c->cur = dst;
