@@ -446,18 +446,17 @@ __device__ int mpr_classify(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T e
     for (int it = 0; it < 40; ++it) {
         const T nn = dot(n, n);
         if (nn < tiny * (stage == 1 ? v00 : (T)1)) break;             // degenerate direction (stage 1: v0, v1, origin on one line)
-        if (stage == 3) {
-            // the origin is behind the portal by more than `deep`: inside the tetrahedron (v0, v1, v2, v3) ?
-            if (dot(n, v1) * rsqrt(nn) > deep) {
-                if (origin_deep_inside(v0, v1, v2, v3, S.dmax2, deep)) verdict = kGjkOverlap;
-                break;
-            }
+        const T inv_n = rsqrt(nn);
+        // refinement: the origin is behind the portal by more than `deep`: inside the tetrahedron (v0, v1, v2, v3) ?
+        if (stage == 3 && dot(n, v1) * inv_n > deep) {
+            if (origin_deep_inside(v0, v1, v2, v3, S.dmax2, deep)) verdict = kGjkOverlap;
+            break;
         }
         int pw;
         V3<T> w = support_minkowski<T, NVP>(S, Rm, r, n, pw);
         // rounded shapes: B (-) A is the difference of the cores swept by a ball of radius 2 rho = S.sweep, whose support point
         // along n lies S.sweep further out (every certificate below then speaks about the rounded bodies)
-        if (NVP == 0 && S.sweep > (T)0) w = w + (S.sweep * rsqrt(nn)) * n;
+        if (NVP == 0 && S.sweep > (T)0) w = w + (S.sweep * inv_n) * n;
         const T h = dot(w, n);
         if (h <= 0) {   // the whole of B (-) A lies at n^ . x <= h / |n|: a separating plane if that is <= -eps
             if (h * h >= eps * eps * nn) verdict = kGjkSeparated;
@@ -477,20 +476,28 @@ __device__ int mpr_classify(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T e
                 n = V3<T>{-n.x, -n.y, -n.z};
             }
             stage = 2;
-        } else if (stage == 2) {   // discovery: a triangle (v1, v2, v3) that the ray from v0 through the origin crosses
-            v3 = w; p3 = pw;
-            if (dot(cross(v1, v3), v0) < 0) { v2 = v3; p2 = p3; n = cross(v1 - v0, v3 - v0); }
-            else if (dot(cross(v3, v2), v0) < 0) { v1 = v3; p1 = p3; n = cross(v3 - v0, v2 - v0); }
-            else { stage = 3; have_portal = true; n = cross(v2 - v1, v3 - v1); }
-        } else {                   // refinement: push the portal outward
-            if (dot(w - v3, n) <= (T)1e-6 * sqrt(nn)) break;   // the portal has reached the surface: origin within ~deep of it
+        } else {
+            // Discovery (stage 2) and refinement (stage 3) are ONE body, so that lanes in either stage -- from the third
+            // iteration on a warp holds both kinds -- run the same instructions: with c4 = w x v0 the signs of
+            // d_k = v_k . c4 = det(v_k, w, v0) say which of v1, v2, v3 the new point w replaces in either stage, and the next
+            // direction is (a - c) x (b - c) for a stage-dependent choice of (a, b, c): selects, not two divergent branches.
+            // refinement only: the portal has reached the surface, the origin is within ~deep of it
+            if (stage == 3 && dot(w - v3, n) <= (T)1e-6 * (nn * inv_n)) break;
             const V3<T> c4 = cross(w, v0);
-            if (dot(v1, c4) > 0) {
-                if (dot(v2, c4) > 0) { v1 = w; p1 = pw; } else { v3 = w; p3 = pw; }
-            } else {
-                if (dot(v3, c4) > 0) { v2 = w; p2 = pw; } else { v1 = w; p1 = pw; }
-            }
-            n = cross(v2 - v1, v3 - v1);
+            const T d1 = dot(v1, c4), d2 = dot(v2, c4), d3 = dot(v3, c4);
+            // discovery (a triangle (v1, v2, v3) that the ray from v0 through the origin crosses): w replaces v2 if the origin
+            // is outside the plane (v0, v1, w), else v1 if outside (v0, w, v2), else it closes the portal as v3.
+            // refinement (push the portal outward): w replaces the vertex that keeps the ray inside the new triangle.
+            int slot;
+            if (stage == 2) slot = (d1 < 0) ? 2 : (d2 > 0) ? 1 : 3;
+            else slot = (d1 > 0) ? ((d2 > 0) ? 1 : 3) : ((d3 > 0) ? 2 : 1);
+            if (slot == 1) { v1 = w; p1 = pw; }
+            if (slot == 2) { v2 = w; p2 = pw; }
+            if (slot == 3) { v3 = w; p3 = pw; }
+            const bool discovering = stage == 2 && slot != 3;
+            if (!discovering) { stage = 3; have_portal = true; }
+            const V3<T> a = discovering ? v1 : v2, b = discovering ? v2 : v3, c = discovering ? v0 : v1;
+            n = cross(a - c, b - c);
         }
     }
     if (verdict == kGjkUnsure && have_portal) { portal[0] = p1; portal[1] = p2; portal[2] = p3; }
