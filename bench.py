@@ -420,8 +420,8 @@ def paper_states(device):
     out = {}
     for label, make, sweeps, paper in (("pentagons_65536_phi0.676", lambda: sp.pentagons_paper_state(256, device=device), 1000,
                                         "3.89e7 trial moves/s per K20X at 65 536 per GPU (P:237)"),
-                                       ("dodecahedra_32768_phi0.5", lambda: sp.dodecahedra_paper_state(32, device=device), 200,
-                                        "8.16e6 trial moves/s per K20X (P:239)"),
+                                       ("dodecahedra_110592_phi0.5", lambda: sp.dodecahedra_paper_state(48, device=device), 100,
+                                        "8.16e6 trial moves/s per K20X at 131 072 per GPU (P:237-239)"),
                                        # the paper's two 3-D validation states (Table 1), lattice starts as in the paper
                                        ("spheres_131072_fcc_phi0.60", lambda: (wl.fcc_spheres(32, 0.60), (None, None)), 1000,
                                         "validation state of Table 1 (P* = 9.3135); no throughput printed"),

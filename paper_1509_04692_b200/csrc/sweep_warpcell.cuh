@@ -38,11 +38,10 @@ struct Warp3dSmem {
 };
 
 template <int KIND, int NV, int DIM>
-__global__ void __launch_bounds__(32 * kW3Warps)
-k_sweep_warpcell(const __grid_constant__ GridParams g, const __grid_constant__ MoveParams mv, const __grid_constant__ ShapeF S,
-               const __grid_constant__ ShapeD SD, Control* __restrict__ ctrl, int colour_index, int cap_limit,
-               float4* __restrict__ pos, float4* __restrict__ quat, const int* __restrict__ tag,
-               const int* __restrict__ cell_start, uint32_t k0, uint32_t k1, uint2* __restrict__ trace, int after_colour)
+__device__ __forceinline__ void warpcell_body(const GridParams& g, const MoveParams& mv, const ShapeF& S, const ShapeD& SD,
+                                              Control* __restrict__ ctrl, int colour_index, int cap_limit, float4* __restrict__ pos,
+                                              float4* __restrict__ quat, const int* __restrict__ tag, const int* __restrict__ cell_start,
+                                              uint32_t k0, uint32_t k1, uint2* __restrict__ trace, int after_colour)
 {
     // Programmatic dependent launch (common.cuh).  A colour pass that follows the cell-list build (or anything else): nothing can be
     // read before that has completed, and only then may the next pass be launched.  A later pass starts while the pass
@@ -237,5 +236,29 @@ k_sweep_warpcell(const __grid_constant__ GridParams g, const __grid_constant__ M
     }
     flush_counters(ctrl, cc);
 }
+
+#define HPMC_WARPCELL_PARAMS                                                                                                        \
+    const __grid_constant__ GridParams g, const __grid_constant__ MoveParams mv, const __grid_constant__ ShapeF S,                  \
+        const __grid_constant__ ShapeD SD, Control *__restrict__ ctrl, int colour_index, int cap_limit, float4 *__restrict__ pos,   \
+        float4 *__restrict__ quat, const int *__restrict__ tag, const int *__restrict__ cell_start, uint32_t k0, uint32_t k1,       \
+        uint2 *__restrict__ trace, int after_colour
+
+// The pass as the compiler sizes it (polyhedra: 168 registers, 12 warps per SM): a system of up to a wave or two of active
+// cells is a latency chain per warp, and fewer registers would put spills on that chain (config 3: -14 % at 128 registers).
+template <int KIND, int NV, int DIM>
+__global__ void __launch_bounds__(32 * kW3Warps) k_sweep_warpcell(HPMC_WARPCELL_PARAMS)
+{
+    warpcell_body<KIND, NV, DIM>(g, mv, S, SD, ctrl, colour_index, cap_limit, pos, quat, tag, cell_start, k0, k1, trace, after_colour);
+}
+
+// The same pass held to 96 registers (20 warps per SM) for systems with many waves of active cells, where the pass is bound by
+// instruction issue and the extra warps fill the slots a dependent chain leaves empty: 96^3 cubes 3.18e8 -> 3.77e8 trial
+// moves/s, 131 072 dodecahedra (the paper's per-GPU size) 1.51e8 -> 1.69e8.  Same code, same results.
+template <int KIND, int NV, int DIM>
+__global__ void __launch_bounds__(32 * kW3Warps, 5) k_sweep_warpcell_occ(HPMC_WARPCELL_PARAMS)
+{
+    warpcell_body<KIND, NV, DIM>(g, mv, S, SD, ctrl, colour_index, cap_limit, pos, quat, tag, cell_start, k0, k1, trace, after_colour);
+}
+#undef HPMC_WARPCELL_PARAMS
 
 }  // namespace hpmc
