@@ -423,8 +423,40 @@ __device__ __forceinline__ bool origin_deep_inside(const V3<T>& a, const V3<T>& 
 // closest-point-on-triangle) makes the lanes of a warp -- one pair each -- execute the union of all cases; and the
 // tetrahedron that certifies an overlap has the deep interior point v0 as a vertex, so it is rarely a sliver (GJK's simplex
 // of nearby support points often is, which sent those pairs to fp64).
-template <typename T, int NVP = 0>
-__device__ int mpr_classify(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T eps, T deep, int* portal)
+// G = lanes per pair.  G = 1: the lane evaluates both support maxima.  G = 2 (the warp-per-cell pass): the two lanes of an
+// aligned pair hold the SAME pair of particles and run the same instructions; in the support call lane `sub` = 0 scans the
+// vertices for S_A(-n), lane 1 for S_B(R^-1 n), they exchange the two vertex indices with one shuffle each and both form the
+// same point of B (-) A.  Same arithmetic per vertex and the same first-maximum rule as G = 1, so the verdicts -- and the
+// trajectories of the passes that use one or the other -- are bit-identical.  ~10 pairs pass the broad phase of a trial, so the
+// second lane is free, and the vertex scans are most of an iteration (more so with 20 or 24 vertices).
+template <typename T, int NVP, int G>
+__device__ __forceinline__ V3<T> support_mpr(const ShapeT<T>& S, const T* Rm, const V3<T>& r, const V3<T>& dir, int& pair, int sub, unsigned pair_mask)
+{
+    if (G == 1) return support_minkowski<T, NVP>(S, Rm, r, dir, pair);
+    // R^-1 dir = R^T dir
+    const V3<T> db{Rm[0] * dir.x + Rm[3] * dir.y + Rm[6] * dir.z, Rm[1] * dir.x + Rm[4] * dir.y + Rm[7] * dir.z,
+                   Rm[2] * dir.x + Rm[5] * dir.y + Rm[8] * dir.z};
+    // support_minkowski's two scans are da = -(dir . v) and dbv = db . v; this lane runs one of them.  -(a + b + c) with the
+    // contraction fma(z, vz, fma(y, vy, x vx)) equals the same expression of the negated direction bit for bit
+    const V3<T> d = sub ? db : V3<T>{-dir.x, -dir.y, -dir.z};
+    T best = -(T)3.0e38;
+    int ibest = 0;
+    const int nv = (NVP > 0) ? NVP : S.nverts;
+#pragma unroll
+    for (int i = 0; i < nv; ++i) {
+        const T t = d.x * S.vx[i] + d.y * S.vy[i] + d.z * S.vz[i];
+        if (t > best) { best = t; ibest = i; }
+    }
+    const int lane0 = (threadIdx.x & 31) & ~1;
+    const int ia = __shfl_sync(pair_mask, ibest, lane0), ib = __shfl_sync(pair_mask, ibest, lane0 + 1);
+    pair = ia | (ib << 8);
+    const T bx = S.vx[ib], by = S.vy[ib], bz = S.vz[ib];
+    return V3<T>{Rm[0] * bx + Rm[1] * by + Rm[2] * bz + r.x - S.vx[ia], Rm[3] * bx + Rm[4] * by + Rm[5] * bz + r.y - S.vy[ia],
+                 Rm[6] * bx + Rm[7] * by + Rm[8] * bz + r.z - S.vz[ia]};
+}
+
+template <typename T, int NVP = 0, int G = 1>
+__device__ int mpr_classify(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T eps, T deep, int* portal, int sub = 0, unsigned pair_mask = 0u)
 {
     // portal[0..2]: on kGjkUnsure from the refinement stage, the vertex pairs (index in A | index in B << 8) behind the last
     // portal (v1, v2, v3) -- exact data from which the fp64 re-run rebuilds the tetrahedron (r, v1, v2, v3); else portal[0] = -1
@@ -453,7 +485,7 @@ __device__ int mpr_classify(const ShapeT<T>& S, const T* Rm, const V3<T>& r, T e
             break;
         }
         int pw;
-        V3<T> w = support_minkowski<T, NVP>(S, Rm, r, n, pw);
+        V3<T> w = support_mpr<T, NVP, G>(S, Rm, r, n, pw, sub, pair_mask);
         // rounded shapes: B (-) A is the difference of the cores swept by a ball of radius 2 rho = S.sweep, whose support point
         // along n lies S.sweep further out (every certificate below then speaks about the rounded bodies)
         if (NVP == 0 && S.sweep > (T)0) w = w + (S.sweep * inv_n) * n;
@@ -519,8 +551,10 @@ __device__ __forceinline__ void quat_to_matrix(T w, T x, T y, T z, T* M)
 }
 
 // polyhedron pair in A's frame: MA, MB = world rotation matrices of A and B, rw = r_AB (world).  GJK verdict.
-template <typename T, int NVP = 0>
-__device__ __forceinline__ int polyhedron_classify(const ShapeT<T>& S, const T* MA, const T* MB, const V3<T>& rw, T eps, T deep, int* portal)
+// G, sub, pair_mask: two lanes per pair in the fp32 XenoCollide run (support_mpr); G = 1 everywhere else.
+template <typename T, int NVP = 0, int G = 1>
+__device__ __forceinline__ int polyhedron_classify(const ShapeT<T>& S, const T* MA, const T* MB, const V3<T>& rw, T eps, T deep, int* portal,
+                                                   int sub = 0, unsigned pair_mask = 0u)
 {
     T Rm[9];  // R = MA^T MB takes B's frame into A's frame (q = q_A* q_B)
 #pragma unroll
@@ -530,7 +564,7 @@ __device__ __forceinline__ int polyhedron_classify(const ShapeT<T>& S, const T* 
     const V3<T> r{MA[0] * rw.x + MA[3] * rw.y + MA[6] * rw.z, MA[1] * rw.x + MA[4] * rw.y + MA[7] * rw.z,
                   MA[2] * rw.x + MA[5] * rw.y + MA[8] * rw.z};
     portal[0] = -1;
-    if (sizeof(T) == 4 && kFp32UseMpr) return mpr_classify<T, NVP>(S, Rm, r, eps, deep, portal);
+    if (sizeof(T) == 4 && kFp32UseMpr) return mpr_classify<T, NVP, G>(S, Rm, r, eps, deep, portal, sub, pair_mask);
     // GJK runs on the cores (finite for polytopes): rounded shapes are separated by eps iff the cores are by S.sweep + eps
     return gjk_classify<T, NVP>(S, Rm, r, (NVP == 0) ? eps + S.sweep : eps, deep);
 }

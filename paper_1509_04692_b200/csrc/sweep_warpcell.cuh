@@ -37,7 +37,8 @@ struct Warp3dSmem {
     int start[28];
 };
 
-template <int KIND, int NV, int DIM>
+// G: lanes per narrow-phase pair of the polyhedron pass (1 or 2, see support_mpr)
+template <int KIND, int NV, int DIM, int G>
 __device__ __forceinline__ void warpcell_body(const GridParams& g, const MoveParams& mv, const ShapeF& S, const ShapeD& SD,
                                               Control* __restrict__ ctrl, int colour_index, int cap_limit, float4* __restrict__ pos,
                                               float4* __restrict__ quat, const int* __restrict__ tag, const int* __restrict__ cell_start,
@@ -183,8 +184,12 @@ __device__ __forceinline__ void warpcell_body(const GridParams& g, const MovePar
                 }
             }
             if (KIND == kKindPolyhedron) {
-                for (int base = 0; base < nq && !overlap; base += 32) {
-                    const int e = base + lane;
+                // G = 2: two lanes per queue entry (support_mpr), the support scans of a XenoCollide iteration split into their A
+                // half and their B half
+                const int sub = lane & (G - 1);
+                const unsigned pair_mask = ((1u << G) - 1u) << (lane & ~(G - 1));
+                for (int base = 0; base < nq && !overlap; base += 32 / G) {
+                    const int e = base + lane / G;
                     bool ov = false;
                     if (e < nq) {
                         const int q = sm.queue[e];
@@ -195,9 +200,9 @@ __device__ __forceinline__ void warpcell_body(const GridParams& g, const MovePar
                         float MB[9];
                         quat_to_matrix<float>(qq.x, qq.y, qq.z, qq.w, MB);
                         int portal[3];
-                        const int verdict = polyhedron_classify<float, NV>(S, MA, MB, V3<float>{rx, ry, rz}, mv.eps_g, kGjkDeepF, portal);
+                        const int verdict = polyhedron_classify<float, NV, G>(S, MA, MB, V3<float>{rx, ry, rz}, mv.eps_g, kGjkDeepF, portal, sub, pair_mask);
                         if (verdict == kGjkUnsure) {   // near contact: decide in fp64 from the raw fp32 state
-                            ++cc.f64;
+                            if (sub == 0) ++cc.f64;
                             ov = polyhedron_overlap_f64<NV>(SD, make_float4(A.qw, A.qx, A.qy, A.qz), qq, min_image_d(xq.x, A.x, g.Ld[0]),
                                                             min_image_d(xq.y, A.y, g.Ld[1]), min_image_d(xq.z, A.z, g.Ld[2]), (double)mv.eps_g, portal);
                         } else
@@ -245,19 +250,22 @@ __device__ __forceinline__ void warpcell_body(const GridParams& g, const MovePar
 
 // The pass as the compiler sizes it (polyhedra: 168 registers, 12 warps per SM): a system of up to a wave or two of active
 // cells is a latency chain per warp, and fewer registers would put spills on that chain (config 3: -14 % at 128 registers).
+// One lane per pair for the unrolled 8-vertex shape (config 3: two lanes are 1 % slower, the pair shuffle inside the divergent
+// loop costs what the halved scan saves), two for runtime vertex counts (20, 24 vertices: the scans are most of an iteration).
 template <int KIND, int NV, int DIM>
 __global__ void __launch_bounds__(32 * kW3Warps) k_sweep_warpcell(HPMC_WARPCELL_PARAMS)
 {
-    warpcell_body<KIND, NV, DIM>(g, mv, S, SD, ctrl, colour_index, cap_limit, pos, quat, tag, cell_start, k0, k1, trace, after_colour);
+    warpcell_body<KIND, NV, DIM, (NV == 0) ? 2 : 1>(g, mv, S, SD, ctrl, colour_index, cap_limit, pos, quat, tag, cell_start, k0, k1, trace, after_colour);
 }
 
 // The same pass held to 96 registers (20 warps per SM) for systems with many waves of active cells, where the pass is bound by
 // instruction issue and the extra warps fill the slots a dependent chain leaves empty: 96^3 cubes 3.18e8 -> 3.77e8 trial
-// moves/s, 131 072 dodecahedra (the paper's per-GPU size) 1.51e8 -> 1.69e8.  Same code, same results.
+// moves/s, 131 072 dodecahedra (the paper's per-GPU size) 1.51e8 -> 1.69e8, and with two lanes per pair (instruction
+// count is what binds here) 3.86e8 and 1.93e8.  Same arithmetic, same results.
 template <int KIND, int NV, int DIM>
 __global__ void __launch_bounds__(32 * kW3Warps, 5) k_sweep_warpcell_occ(HPMC_WARPCELL_PARAMS)
 {
-    warpcell_body<KIND, NV, DIM>(g, mv, S, SD, ctrl, colour_index, cap_limit, pos, quat, tag, cell_start, k0, k1, trace, after_colour);
+    warpcell_body<KIND, NV, DIM, 2>(g, mv, S, SD, ctrl, colour_index, cap_limit, pos, quat, tag, cell_start, k0, k1, trace, after_colour);
 }
 #undef HPMC_WARPCELL_PARAMS
 
