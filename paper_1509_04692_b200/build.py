@@ -12,7 +12,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "_obj")
 LIB = os.path.join(HERE, "libhpmc.so")
 UNITS = ["hpmc_api", "pass_colour", "pass_tile2d_disk", "pass_tile2d_pentagon", "pass_tile2d_polygon", "pass_warpcell_2d",
-         "pass_warpcell_3d", "pass_cluster2d", "pass_spec2d", "noalloc_count"]
+         "pass_warpcell_3d", "pass_warpcell_3d_nv", "pass_cluster2d", "pass_spec2d", "noalloc_count"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
 

@@ -404,7 +404,9 @@ int launch_colour_dispatch(hpmc_ctx* c, int ci)
     // the (kind, unrolled vertex count) variants of each pass are compiled in separate translation units (pass_*.cu)
     const int kind = c->sf.kind;
     const bool sharp = c->sd.sweep == 0.0;   // rounded shapes take the runtime-vertex-count kernels (overlap.cuh)
-    const int nv = (kind == kKindPolygon && c->sf.nverts == 5 && c->sf.regular && sharp) ? 5 : (kind == kKindPolyhedron && c->sf.nverts == 8 && sharp) ? 8 : 0;
+    const int nvp = c->sf.nverts;             // polyhedra with 8, 20 or 24 vertices have unrolled support functions
+    const int nv = (kind == kKindPolygon && nvp == 5 && c->sf.regular && sharp) ? 5
+                   : (kind == kKindPolyhedron && sharp && (nvp == 8 || nvp == 20 || nvp == 24)) ? nvp : 0;
     const GridParams& g = c->g;
     const int nactive = (g.n[0] / 2) * (g.n[1] / 2) * (g.dim == 3 ? g.n[2] / 2 : 1);
     bool ok = true;

@@ -1,4 +1,4 @@
-// Colour-pass translation unit: the warp-per-cell kernels of one dimension.  See sweep_warpcell.cuh.
+// Colour-pass translation unit: the 3-D warp-per-cell kernels with 20 and 24 unrolled vertices.  See sweep_warpcell.cuh.
 #include "ctx.hpp"
 #include "sweep_warpcell.cuh"
 
@@ -26,12 +26,9 @@ bool launch_warpcell(hpmc_ctx* c, int ci, int nactive)
 
 }  // namespace
 
-bool hpmc_launch_warpcell_3d_nv(hpmc_ctx* c, int ci, int nv, int nactive);
-
-bool hpmc_launch_warpcell_3d(hpmc_ctx* c, int ci, int kind, int nv, int nactive)
+// Unrolled support functions for the paper's two benchmark polyhedra: 20 vertices (dodecahedra) and 24 (truncated
+// octahedra, Fig. 4 and Table 1).  A translation unit of its own so that it compiles beside pass_warpcell_3d.cu.
+bool hpmc_launch_warpcell_3d_nv(hpmc_ctx* c, int ci, int nv, int nactive)
 {
-    if (kind == kKindDisk) return launch_warpcell<kKindDisk, 0, 3>(c, ci, nactive);
-    // polyhedra: 8 vertices (cubes, config 3), 20 and 24 (pass_warpcell_3d_nv.cu) have unrolled support functions
-    if (nv == 20 || nv == 24) return hpmc_launch_warpcell_3d_nv(c, ci, nv, nactive);
-    return (nv == 8) ? launch_warpcell<kKindPolyhedron, 8, 3>(c, ci, nactive) : launch_warpcell<kKindPolyhedron, 0, 3>(c, ci, nactive);
+    return (nv == 20) ? launch_warpcell<kKindPolyhedron, 20, 3>(c, ci, nactive) : launch_warpcell<kKindPolyhedron, 24, 3>(c, ci, nactive);
 }

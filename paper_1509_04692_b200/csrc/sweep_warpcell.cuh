@@ -203,7 +203,7 @@ __device__ __forceinline__ void warpcell_body(const GridParams& g, const MovePar
                         const int verdict = polyhedron_classify<float, NV, G>(S, MA, MB, V3<float>{rx, ry, rz}, mv.eps_g, kGjkDeepF, portal, sub, pair_mask);
                         if (verdict == kGjkUnsure) {   // near contact: decide in fp64 from the raw fp32 state
                             if (sub == 0) ++cc.f64;
-                            ov = polyhedron_overlap_f64<NV>(SD, make_float4(A.qw, A.qx, A.qy, A.qz), qq, min_image_d(xq.x, A.x, g.Ld[0]),
+                            ov = polyhedron_overlap_f64<(NV == 8) ? 8 : 0>(SD, make_float4(A.qw, A.qx, A.qy, A.qz), qq, min_image_d(xq.x, A.x, g.Ld[0]),
                                                             min_image_d(xq.y, A.y, g.Ld[1]), min_image_d(xq.z, A.z, g.Ld[2]), (double)mv.eps_g, portal);
                         } else
                             ov = verdict == kGjkOverlap;
@@ -251,11 +251,11 @@ __device__ __forceinline__ void warpcell_body(const GridParams& g, const MovePar
 // The pass as the compiler sizes it (polyhedra: 168 registers, 12 warps per SM): a system of up to a wave or two of active
 // cells is a latency chain per warp, and fewer registers would put spills on that chain (config 3: -14 % at 128 registers).
 // One lane per pair for the unrolled 8-vertex shape (config 3: two lanes are 1 % slower, the pair shuffle inside the divergent
-// loop costs what the halved scan saves), two for runtime vertex counts (20, 24 vertices: the scans are most of an iteration).
+// loop costs what the halved scan saves), two for the other counts (20, 24 vertices: the scans are most of an iteration).
 template <int KIND, int NV, int DIM>
 __global__ void __launch_bounds__(32 * kW3Warps) k_sweep_warpcell(HPMC_WARPCELL_PARAMS)
 {
-    warpcell_body<KIND, NV, DIM, (NV == 0) ? 2 : 1>(g, mv, S, SD, ctrl, colour_index, cap_limit, pos, quat, tag, cell_start, k0, k1, trace, after_colour);
+    warpcell_body<KIND, NV, DIM, (NV == 8) ? 1 : 2>(g, mv, S, SD, ctrl, colour_index, cap_limit, pos, quat, tag, cell_start, k0, k1, trace, after_colour);
 }
 
 // The same pass held to 96 registers (20 warps per SM) for systems with many waves of active cells, where the pass is bound by
