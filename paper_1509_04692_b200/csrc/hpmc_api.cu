@@ -316,9 +316,15 @@ int pick_tile_shape(const hpmc_ctx* c)
     if (c->opt_tile_shape) return c->opt_tile_shape;
     const int nax = c->g.n[0] / 2, nay = c->g.n[1] / 2;
     const long long cols = (nax + kTileWHost - 1) / kTileWHost;
-    if (cols * ((nay + 3) / 4) >= 2 * 148) return 2;     // 4 warps x 1 row, 64 registers: 8 CTAs per SM
+    // 4 warps x 1 row (64 registers, 8 CTAs per SM) once its tiles of one colour nearly fill the machine; below that the 2-warp
+    // tile spreads a colour over twice as many CTAs (measured on B200, pentagons, n x n lattice: 448 / 512 / 640 -> 2 warps
+    // +11 / +16 / +7 %; 768 and above -> 4 warps +13 % and more)
+    if (cols * ((nay + 3) / 4) * 32 >= (long long)c->num_sms * 8 * 27) return 2;
     return 3;                                            // 2 warps x 1 row
 }
+
+// active rows of cells per tile of each shape (Tile2D<WARPS, R>::TH)
+int tile_rows(int shape) { return shape == 1 ? 16 : shape == 2 ? 4 : 2; }
 
 // 2-D systems with fewer active cells per colour than this run one warp per cell instead of one lane per cell: the tile
 // kernel would leave most SMs idle (config 1: 961 active cells = 31 warps) and each warp round would be a long serial chain
@@ -346,7 +352,8 @@ bool use_flow(const hpmc_ctx* c)
     // auto: the dataflow launch pays when a colour is one to a few waves of tiles (measured on B200: +9 % at 1M pentagons,
     // 1.7 waves; slower below one wave, where the stamps only add latency; no difference from 4M up)
     const long long slots = (long long)c->num_sms * 8;
-    const long long tiles = (long long)((g.n[0] / 2 + kTileWHost - 1) / kTileWHost) * ((g.n[1] / 2 + 3) / 4);
+    const int rows = tile_rows(pick_tile_shape(c));
+    const long long tiles = (long long)((g.n[0] / 2 + kTileWHost - 1) / kTileWHost) * ((g.n[1] / 2 + rows - 1) / rows);
     return c->opt_tile_shape == 0 && tiles > slots && tiles <= 4 * slots;
 }
 
@@ -914,10 +921,9 @@ int hpmc_describe_pass(const hpmc_ctx* c, char* h_buf, size_t n)
 
 // ---- compute partition across contexts / GPUs --------------------------------------------------------
 namespace {
-int tile_rows_of_shape(int shape) { return shape == 1 ? 16 : shape == 2 ? 4 : 2; }   // active rows per tile (WARPS x R)
 void slab_rows(const hpmc_ctx* c, int rank, int nranks, int& r0, int& r1)
 {
-    const int TH = tile_rows_of_shape(pick_tile_shape(c));
+    const int TH = tile_rows(pick_tile_shape(c));
     const int nay = c->g.n[1] / 2, tiles_y = (nay + TH - 1) / TH;
     const int ty0 = (int)((long long)tiles_y * rank / nranks), ty1 = (int)((long long)tiles_y * (rank + 1) / nranks);
     r0 = std::min(2 * TH * ty0, c->g.n[1]);
