@@ -128,9 +128,12 @@ inline cudaError_t hpmc_launch(hpmc_ctx* c, void (*kern)(KArgs...), dim3 grid, d
 }
 
 constexpr int kTileWHost = 32;   // active cells per tile row (= kTileW of sweep_tile2d.cuh)
+// 3-D polyhedron systems with more active cells per colour than two waves of the 168-register warp-per-cell kernel (12 warps per
+// SM) are bound by instruction issue and run k_sweep_warpcell_occ (sweep_warpcell.cuh)
+constexpr int kOccMinActive3d = 2 * 148 * 12;
 
 // Colour-pass launchers; each returns false after recording a CUDA error in the context.
-//   kind: kKindDisk / kKindPolygon / kKindPolyhedron; nv: unrolled vertex count (5 pentagons, 8 cubes) or 0 = runtime count
+//   kind: kKindDisk / kKindPolygon / kKindPolyhedron; nv: unrolled vertex count (5 pentagons; 8, 20, 24 polyhedra) or 0 = runtime count
 bool hpmc_launch_tile2d(hpmc_ctx* c, int ci, int kind, int nv, int shape);       // pass_tile2d_*.cu (2-D, not polyhedra)
 bool hpmc_launch_warpcell(hpmc_ctx* c, int ci, int kind, int nv, int nactive);   // pass_warpcell_*.cu
 bool hpmc_launch_spec2d(hpmc_ctx* c, int ci, int kind, int nv, int nactive);     // pass_spec2d.cu

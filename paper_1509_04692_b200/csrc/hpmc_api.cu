@@ -908,7 +908,9 @@ int hpmc_describe_pass(const hpmc_ctx* c, char* h_buf, size_t n)
     else if (c->opt_path == 1) d = "k_sweep_colour: one thread per active cell";
     else if (use_spec(c)) d = "k_sweep_spec2d: one warp per active cell, the decision tree of 4 trials evaluated at once, 1 colour pass per launch";
     else if (g.dim == 3 || c->opt_path == 3 || (c->opt_path == 0 && c->opt_tile_shape == 0 && nactive <= kWarpCellMax2d))
-        d = "k_sweep_warpcell: one warp per active cell, 1 colour pass per launch";
+        d = (g.dim == 3 && c->sf.kind == kKindPolyhedron && nactive > kOccMinActive3d)
+                ? "k_sweep_warpcell_occ: one warp per active cell at 96 registers (20 warps/SM), two lanes per narrow-phase pair, 1 colour pass per launch"
+                : "k_sweep_warpcell: one warp per active cell, 1 colour pass per launch";
     else {
         static const char* shapes[4] = {"", "8 warps x 2 rows, 2 CTAs/SM", "4 warps x 1 row, 8 CTAs/SM", "2 warps x 1 row, 8 CTAs/SM"};
         const bool flow = use_flow(c);

@@ -4,14 +4,12 @@
 
 namespace {
 
-// more active cells than two waves of the 168-register kernel (12 warps per SM): the pass is throughput-bound
-constexpr int kOccMinActive = 2 * 148 * 12;
 
 template <int KIND, int NV, int DIM>
 bool launch_warpcell(hpmc_ctx* c, int ci, int nactive)
 {
     if constexpr (KIND == kKindPolyhedron) {
-        if (nactive > kOccMinActive) {
+        if (nactive > kOccMinActive3d) {
             hpmc_launch(c, k_sweep_warpcell_occ<KIND, NV, DIM>, (nactive + kW3Warps - 1) / kW3Warps, 32 * kW3Warps, 0,
                 c->g, c->mv, c->sf, c->sd, c->ctrl, ci, c->opt_tile_cap, c->pos[c->cur], c->quat[c->cur], c->tag[c->cur], c->cell_start, c->k0,
                 c->k1, c->trace, c->after_colour ? 1 : 0);

@@ -101,3 +101,45 @@ def test_config3_cubes_32768_lockstep_and_invariants():
 @pytest.mark.skipif(os.environ.get("HPMC_SKIP_16M") == "1", reason="HPMC_SKIP_16M=1")
 def test_config4_pentagons_16M_lockstep_and_invariants():
     _lockstep_full(4, 3, 2)
+
+
+@pytest.mark.parametrize("name", ["cubes_48", "dodecahedra_fcc_55296"])
+def test_many_wave_polyhedron_pass_lockstep(name):
+    """Polyhedron systems with more than two waves of active cells per colour run the warp-per-cell pass held to 96 registers
+    with two lanes per narrow-phase pair (k_sweep_warpcell_occ; 20 unrolled vertices for the dodecahedra): 110 592 cubes at the
+    state point of config 3 and 55 296 dodecahedra at phi = 0.5 (FCC start) in lock-step with the oracle, and bit-identical to
+    the per-thread pass."""
+    from paper_1509_04692_b200 import binding as hb
+    if name == "cubes_48":
+        w, n_lock = wl.cubes(48, name=name), 3
+    else:
+        w, n_lock = wl.fcc_polyhedra(wl.dodecahedron_vertices(0.5), 24, 0.5, name=name), 2
+    g = hb.from_workload(w, seed=1)
+    assert g.C // 8 > 2 * 148 * 12                      # the many-wave kernel is the one launched
+    o = ho.Oracle(w.dim, w.L, w.kind, w.N, 1, diameter=w.diameter, verts=w.verts)
+    o.set_moves(w.d, w.a, w.n_select)
+    o.set_state(w.pos4, w.quat4)
+    o.set_threads(min(os.cpu_count() or 1, 16))
+    assert g.count_overlaps() == 0
+    g.enable_trace(True)
+    marginal = 0
+    for s in range(n_lock):
+        g.sweep(1)
+        f = o.sweep(follow=g.read_trace(), follow_tol=1e-5)["follow"]
+        assert f["hard_mismatch"] == 0, (name, s, f)
+        marginal += f["marginal"]
+        gp, gq = g.get_state()
+        op, oq = o.get_state()
+        assert np.array_equal(gp, op) and np.max(np.abs(gq - oq)) < 1e-5
+        o.set_state(op, gq)
+    gc, oc = g.counters(), o.counters()
+    for key in ("trans_acc", "trans_rej_overlap", "trans_rej_cell", "rot_acc", "rot_rej_overlap", "trials", "sweeps"):
+        assert gc[key] == oc[key], (key, gc, oc)
+    assert marginal <= max(3, 2e-4 * gc["trials"]), (marginal, gc["trials"])
+    g1 = hb.from_workload(w, seed=1)
+    g1.set_option("path", 1)
+    g1.sweep(n_lock)
+    p1, q1 = g1.get_state()
+    assert np.array_equal(p1, gp) and np.array_equal(q1, gq) and g1.counters() == gc
+    assert g.count_overlaps() == 0
+    print(name, g.describe_pass(), "trials", gc["trials"], "marginal", marginal, "fp64 re-runs", g.get_stat("gjk_f64_reruns"))
