@@ -244,25 +244,34 @@ def time_gpu(w, seed, device, steps, warmup, flush, dist_ctx):
 
 
 def time_e2e(g, w, steps, device):
-    """The same step through hpmc_sweep_host: pinned HOST state in, one sweep, state + counters out."""
+    """The same step through the host-buffer call: pinned HOST state in, one sweep, state + counters out.  2-D systems use
+    hpmc_sweep_host_pose2d (one pose (x, y, qw, qz) per particle, 16 N bytes each way), 3-D systems hpmc_sweep_host (pos4 +
+    quat4, 32 N bytes each way)."""
     import torch
     p, q = g.get_state()
-    hp = [torch.from_numpy(p.copy()).pin_memory(), torch.empty(w.N, 4).pin_memory()]
-    hq = [torch.from_numpy(q.copy()).pin_memory(), torch.empty(w.N, 4).pin_memory()]
-    g.sweep_host(hp[0], hq[0], 1, hp[1], hq[1])      # warm
+    if w.dim == 2:
+        pose = np.concatenate([p[:, :2], q[:, [0, 3]]], axis=1).astype(np.float32)
+        hp = [torch.from_numpy(np.ascontiguousarray(pose)).pin_memory(), torch.empty(w.N, 4).pin_memory()]
+        step = lambda cur: g.sweep_host_pose2d(hp[cur], 1, hp[1 - cur])
+        nbytes, call = w.N * 16, "hpmc_sweep_host_pose2d(n=1), pinned host buffers"
+    else:
+        hp = [torch.from_numpy(p.copy()).pin_memory(), torch.empty(w.N, 4).pin_memory()]
+        hq = [torch.from_numpy(q.copy()).pin_memory(), torch.empty(w.N, 4).pin_memory()]
+        step = lambda cur: g.sweep_host(hp[cur], hq[cur], 1, hp[1 - cur], hq[1 - cur])
+        nbytes, call = 2 * w.N * 16, "hpmc_sweep_host(n=1), pinned host buffers"
+    step(0)                                           # warm
     g.reset_counters()
     torch.cuda.synchronize(device)
     t = time.perf_counter()
     trials = 0
     cur = 1
     for _ in range(steps):
-        c = g.sweep_host(hp[cur], hq[cur], 1, hp[1 - cur], hq[1 - cur])
+        c = step(cur)
         cur = 1 - cur
     torch.cuda.synchronize(device)
     t = time.perf_counter() - t
     trials = c["trials"]                              # counters accumulate over the calls
-    nbytes = 2 * w.N * 16
-    return dict(seconds=t, trials=trials, h2d=nbytes, d2h=nbytes + 56)
+    return dict(seconds=t, trials=trials, h2d=nbytes, d2h=nbytes + 56, call=call)
 
 
 def sample_of(k, n_lat):
@@ -525,7 +534,7 @@ def main():
         e_t = D.reduce(e["seconds"], "MAX")
         e_trials = D.reduce(e["trials"], "SUM")
         line["e2e"] = {"value": e_trials / e_t, "unit": UNIT, "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"],
-                       "steps": min(args.steps, 20), "call": "hpmc_sweep_host(n=1), pinned host buffers"}
+                       "steps": min(args.steps, 20), "call": e["call"]}
     fp32_peak_run = r["fp32_peak"]
     del g, r
     if not args.no_extras and D.rank == 0:

@@ -145,6 +145,13 @@ int hpmc_get_cell_list(hpmc_ctx* ctx, uint64_t t, int32_t* d_cell_start, int32_t
 int hpmc_sweep_host(hpmc_ctx* ctx, const float* h_pos4, const float* h_quat4, int64_t n,
                     float* h_pos4_out, float* h_quat4_out, hpmc_counters* h_counters);
 
+/* The same for 2-D systems with the state as ONE host array of poses, N x (x, y, qw, qz) fp32 in tag order: a 2-D particle is
+ * its position r_i and one rotation angle (R30: z = 0 and q = (cos t/2, 0, 0, sin t/2)), so half of the pos4 + quat4
+ * layout is zeros and this call moves half the bytes over the host link (16 N each way).  Copies the poses host->device into
+ * the bound arrays (their device staging), expands them to pos4 / quat4 there, runs n sweeps, packs the result and copies
+ * poses and counters back.  h_pose4_out may be NULL.  Synchronises.  dim != 2: HPMC_E_ARG.                                 */
+int hpmc_sweep_host_pose2d(hpmc_ctx* ctx, const float* h_pose4, int64_t n, float* h_pose4_out, hpmc_counters* h_counters);
+
 /* Tuning and test knobs; results never depend on them (only speed does).
  *   "path"     0 = automatic, 1 = per-thread global-memory colour pass, 2 = shared-memory tile colour pass (2-D; in 3-D
  *              the warp-per-cell pass), 3 = warp-per-cell colour pass (automatic in 3-D and for small 2-D systems),

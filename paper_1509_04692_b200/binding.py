@@ -16,7 +16,7 @@ KIND_DISK, KIND_POLYGON, KIND_POLYHEDRON = 0, 1, 2
 # every symbol include/hpmc.h declares (checked by tests/test_abi.py)
 ABI_SYMBOLS = ["hpmc_create", "hpmc_destroy", "hpmc_last_error", "hpmc_get_grid", "hpmc_workspace_bytes", "hpmc_bind",
                "hpmc_set_moves", "hpmc_sweep", "hpmc_count_overlaps", "hpmc_get_state", "hpmc_set_sweep_counter",
-               "hpmc_reset_counters", "hpmc_set_trace", "hpmc_get_cell_list", "hpmc_sweep_host", "hpmc_set_option", "hpmc_set_profile",
+               "hpmc_reset_counters", "hpmc_set_trace", "hpmc_get_cell_list", "hpmc_sweep_host", "hpmc_sweep_host_pose2d", "hpmc_set_option", "hpmc_set_profile",
                "hpmc_get_profile", "hpmc_launch_count", "hpmc_describe_pass", "hpmc_get_stat", "hpmc_measure_fp32_peak", "hpmc_set_partition", "hpmc_sweep_phase",
                "hpmc_partition_rows", "hpmc_row_offsets", "hpmc_sorted_pose", "hpmc_set_inactive_layers", "hpmc_dist_load",
                "hpmc_dist_route", "hpmc_dist_append", "hpmc_local_count", "hpmc_sorted_tags", "hpmc_count_overlaps_noalloc"]
@@ -76,6 +76,7 @@ def load_library():
     L.hpmc_set_trace.argtypes = [vp, vp, C.c_int64]
     L.hpmc_get_cell_list.argtypes = [vp, C.c_uint64, vp, vp, vp, C.POINTER(C.c_float), C.POINTER(C.c_int32)]
     L.hpmc_sweep_host.argtypes = [vp, vp, vp, C.c_int64, vp, vp, C.POINTER(Counters)]
+    L.hpmc_sweep_host_pose2d.argtypes = [vp, vp, C.c_int64, vp, C.POINTER(Counters)]
     L.hpmc_set_option.argtypes = [vp, C.c_char_p, C.c_int64]
     L.hpmc_set_profile.argtypes = [vp, C.c_int]
     L.hpmc_get_profile.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64), C.POINTER(C.c_double), C.POINTER(C.c_int64)]
@@ -236,6 +237,14 @@ class Hpmc:
         c = Counters()
         self._check(self._lib.hpmc_sweep_host(self._h, h_pos4.data_ptr(), h_quat4.data_ptr(), int(n),
                                               h_pos4_out.data_ptr(), h_quat4_out.data_ptr(), C.byref(c)))
+        return c.as_dict()
+
+    def sweep_host_pose2d(self, h_pose4, n, h_pose4_out):
+        """End-to-end call for 2-D systems with HOST poses (N, 4) = (x, y, qw, qz) (torch CPU tensors, ideally pinned): half the
+        bytes of sweep_host each way.  h_pose4_out may be None."""
+        c = Counters()
+        self._check(self._lib.hpmc_sweep_host_pose2d(self._h, h_pose4.data_ptr(), int(n),
+                                                     h_pose4_out.data_ptr() if h_pose4_out is not None else None, C.byref(c)))
         return c.as_dict()
 
     def set_option(self, name, value):

@@ -839,6 +839,60 @@ int hpmc_sweep_host(hpmc_ctx* c, const float* h_pos4, const float* h_quat4, int6
     return rc;
 }
 
+namespace {
+// tag-order pose (x, y, qw, qz) <-> pos4 (x, y, 0, 0) + quat4 (qw, 0, 0, qz) over the bound arrays, element by element in place
+__global__ void k_pose_expand(int N, float4* __restrict__ pos, float4* __restrict__ quat)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const float4 P = pos[i];
+    quat[i] = make_float4(P.z, 0.0f, 0.0f, P.w);
+    pos[i] = make_float4(P.x, P.y, 0.0f, 0.0f);
+}
+__global__ void k_pose_pack(int N, float4* __restrict__ pos, const float4* __restrict__ quat)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const float4 P = pos[i], Q = quat[i];
+    pos[i] = make_float4(P.x, P.y, Q.x, Q.w);
+}
+}  // namespace
+
+int hpmc_sweep_host_pose2d(hpmc_ctx* c, const float* h_pose4, int64_t n, float* h_pose4_out, hpmc_counters* h_counters)
+{
+    DeviceGuard dev_guard(c);
+    if (!c) return HPMC_E_ARG;
+    if (c->cuda_failed) return HPMC_E_CUDA;
+    if (c->g.dim != 2) return fail(c, HPMC_E_ARG, "hpmc_sweep_host_pose2d needs a 2-D system");
+    if (!c->d_ws || !c->d_pos_bound) return fail(c, HPMC_E_UNBOUND, "state/workspace not bound");
+    if (!h_pose4) return fail(c, HPMC_E_ARG, "NULL host pointer");
+    const int N = c->n_cap, TB = 256;
+    const size_t bytes = (size_t)N * sizeof(float4);
+    if (!cuda_ok(c, cudaMemsetAsync(&c->ctrl->bad_coords, 0, sizeof(unsigned int), c->stream), "sweep_host_pose2d/memset")) return HPMC_E_CUDA;
+    if (!cuda_ok(c, cudaMemcpyAsync(c->d_pos_bound, h_pose4, bytes, cudaMemcpyHostToDevice, c->stream), "sweep_host_pose2d/h2d")) return HPMC_E_CUDA;
+    if (N > 0) k_pose_expand<<<(N + TB - 1) / TB, TB, 0, c->stream>>>(N, (float4*)c->d_pos_bound, (float4*)c->d_quat_bound);
+    c->launches += 1;
+    c->state_in_bound = true;
+    c->have_sorted = false;
+    c->dist = false;
+    c->g.N = c->n_cap;
+    int rc = hpmc_sweep(c, n);
+    if (rc != HPMC_OK) return rc;
+    rc = hpmc_get_state(c, (float*)c->d_pos_bound, (float*)c->d_quat_bound, nullptr, nullptr);
+    if (rc != HPMC_OK) return rc;
+    if (h_pose4_out) {
+        if (N > 0) k_pose_pack<<<(N + TB - 1) / TB, TB, 0, c->stream>>>(N, (float4*)c->d_pos_bound, (const float4*)c->d_quat_bound);
+        c->launches += 1;
+        if (!cuda_ok(c, cudaMemcpyAsync(h_pose4_out, c->d_pos_bound, bytes, cudaMemcpyDeviceToHost, c->stream), "sweep_host_pose2d/d2h")) return HPMC_E_CUDA;
+        // the bound arrays are the caller's: leave them in the documented pos4 / quat4 layout
+        if (N > 0) k_pose_expand<<<(N + TB - 1) / TB, TB, 0, c->stream>>>(N, (float4*)c->d_pos_bound, (float4*)c->d_quat_bound);
+        c->launches += 1;
+    }
+    hpmc_counters tmp;
+    rc = hpmc_get_state(c, nullptr, nullptr, h_counters ? h_counters : &tmp, nullptr);  // also synchronises
+    return rc;
+}
+
 int hpmc_set_option(hpmc_ctx* c, const char* name, int64_t value)
 {
     DeviceGuard dev_guard(c);

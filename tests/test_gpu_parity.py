@@ -517,3 +517,29 @@ def test_speculative_pass_lockstep_with_oracle(case):
         assert share > 0.5, share            # most occupied cells hold 2-4 members: the tree runs with cell mates in its states
     if case == "needles_overfull":
         assert multi >= 5
+
+
+def test_sweep_host_pose2d_equals_sweep_host():
+    """The 2-D host-buffer call with one pose (x, y, qw, qz) per particle makes the trajectory of hpmc_sweep_host (pos4 + quat4)
+    bit for bit, returns the same counters, leaves the bound device arrays in the pos4 / quat4 layout, and refuses 3-D systems."""
+    import torch
+    from paper_1509_04692_b200 import binding as hb
+    w = wl.pentagons(48)
+    a, b = gpu(w), gpu(w)
+    hp, hq = torch.from_numpy(w.pos4.copy()).pin_memory(), torch.from_numpy(w.quat4.copy()).pin_memory()
+    op, oq = torch.empty(w.N, 4).pin_memory(), torch.empty(w.N, 4).pin_memory()
+    pose = torch.from_numpy(np.ascontiguousarray(np.concatenate([w.pos4[:, :2], w.quat4[:, [0, 3]]], axis=1))).pin_memory()
+    out = torch.empty(w.N, 4).pin_memory()
+    for step in range(3):
+        ca = a.sweep_host(hp, hq, 2, op, oq)
+        cb = b.sweep_host_pose2d(pose, 2, out)
+        assert ca == cb
+        assert torch.equal(out[:, :2], op[:, :2]) and torch.equal(out[:, 2], oq[:, 0]) and torch.equal(out[:, 3], oq[:, 3])
+        hp.copy_(op); hq.copy_(oq); pose.copy_(out)
+    pb, qb = b.get_state()
+    assert np.array_equal(pb, op.numpy()) and np.array_equal(qb, oq.numpy())
+    assert b.count_overlaps() == 0
+    assert b.sweep_host_pose2d(pose, 1, None)["trials"] > ca["trials"]          # no output buffer: counters only
+    c3 = gpu(wl.cubes(6))
+    with pytest.raises(hb.HpmcError):
+        c3.sweep_host_pose2d(pose, 1, out)
