@@ -24,7 +24,7 @@ EVERY = 10
 
 
 def _analysis_oracle(w):
-    o = ho.Oracle(w.dim, w.L, w.kind, w.N, 0, diameter=w.diameter, verts=w.verts)
+    o = ho.Oracle(w.dim, w.L, w.kind, w.N, 0, diameter=w.diameter, verts=w.verts, sweep_radius=w.sweep_radius)
     return o
 
 
@@ -35,8 +35,8 @@ def _summ(counters0, counters1):
     return d["trans_acc"] / max(nt, 1), (d["rot_acc"] / nr if nr else 0.0)
 
 
-def run_oracle(w, seed, sweeps):
-    o = ho.Oracle(w.dim, w.L, w.kind, w.N, seed, diameter=w.diameter, verts=w.verts)
+def run_oracle(w, seed, sweeps, pressure=True):
+    o = ho.Oracle(w.dim, w.L, w.kind, w.N, seed, diameter=w.diameter, verts=w.verts, sweep_radius=w.sweep_radius)
     o.set_moves(w.d, w.a, w.n_select)
     o.set_state(w.pos4, w.quat4)
     o.sweeps(sweeps // 10)
@@ -44,14 +44,15 @@ def run_oracle(w, seed, sweeps):
     hist, ns = np.zeros(pr.NBINS), 0
     for _ in range((sweeps - sweeps // 10) // EVERY):
         o.sweeps(EVERY)
-        hist += o.scale_histogram(pr.S_MAX, pr.NBINS)
+        if pressure:
+            hist += o.scale_histogram(pr.S_MAX, pr.NBINS)
         ns += 1
     ta, ra = _summ(c0, o.counters())
     assert o.count_overlaps_cells() == 0
-    return ta, ra, pr.compressibility(hist, ns, w.N, w.dim)
+    return ta, ra, (pr.compressibility(hist, ns, w.N, w.dim) if pressure else 0.0)
 
 
-def run_gpu(w, seed, sweeps):
+def run_gpu(w, seed, sweeps, pressure=True):
     from paper_1509_04692_b200 import binding as hb
     g = hb.from_workload(w, seed=seed)
     an = _analysis_oracle(w)
@@ -60,30 +61,36 @@ def run_gpu(w, seed, sweeps):
     hist, ns = np.zeros(pr.NBINS), 0
     for _ in range((sweeps - sweeps // 10) // EVERY):
         g.sweep(EVERY)
-        p, q = g.get_state()
-        an.set_state(p, q)
-        hist += an.scale_histogram(pr.S_MAX, pr.NBINS)
+        if pressure:
+            p, q = g.get_state()
+            an.set_state(p, q)
+            hist += an.scale_histogram(pr.S_MAX, pr.NBINS)
         ns += 1
     ta, ra = _summ(c0, g.counters())
     assert g.count_overlaps() == 0
-    return ta, ra, pr.compressibility(hist, ns, w.N, w.dim)
+    return ta, ra, (pr.compressibility(hist, ns, w.N, w.dim) if pressure else 0.0)
 
 
 CASES = {
     "k0_disks": (lambda s: wl.config(0, seed=s), 400),
     "k1_pentagons": (lambda s: wl.config(1, seed=s), 600),
     "cubes_12": (lambda s: wl.cubes(12, seed=s), 200),
+    # rounded shapes: acceptance only -- the touch scale of a rounded pair is a bisection (oracle), too slow for the
+    # snapshots of 24 runs; the pressure estimator itself is shape-independent and pinned on the other cases
+    "rounded_pentagons_24": (lambda s: wl.rounded_polygons(24, seed=s), 400),
+    "rounded_cubes_6": (lambda s: wl.cubes(6, seed=s, edge=0.7, sweep_radius=0.15, d=0.15, a=0.3), 200),
 }
 
 
 @pytest.mark.parametrize("name", list(CASES))
 def test_acceptance_and_pressure_within_3_standard_errors(name):
     make, sweeps = CASES[name]
+    pressure = not name.startswith("rounded")
     seeds = list(range(1, 9))
     with ThreadPoolExecutor(8) as ex:       # the oracle is serial C; ctypes releases the GIL, one thread per seed
-        fut = [ex.submit(run_oracle, make(s), s, sweeps) for s in seeds]
-        gpu_same = np.array([run_gpu(make(s), s, sweeps) for s in seeds])
-        gpu_indep = np.array([run_gpu(make(100 + s), 100 + s, sweeps) for s in seeds])
+        fut = [ex.submit(run_oracle, make(s), s, sweeps, pressure) for s in seeds]
+        gpu_same = np.array([run_gpu(make(s), s, sweeps, pressure) for s in seeds])
+        gpu_indep = np.array([run_gpu(make(100 + s), 100 + s, sweeps, pressure) for s in seeds])
         orc = np.array([f.result() for f in fut])
     report = {}
     for label, gp in (("same seeds", gpu_same), ("independent seeds", gpu_indep)):
@@ -91,6 +98,8 @@ def test_acceptance_and_pressure_within_3_standard_errors(name):
             mg, sg = pr.mean_and_se(gp[:, col])
             mo, so = pr.mean_and_se(orc[:, col])
             report[(label, q)] = (mg, sg, mo, so)
+            if q == "beta P / rho" and not pressure:
+                continue
             if q == "rotate acceptance" and mo == 0.0:
                 assert mg == 0.0
                 continue
