@@ -95,11 +95,16 @@ template <int KIND, bool SEAM>
 __device__ __forceinline__ void broad_slots(const GridParams& g, const ShapeF& S, const float2* sm_xy, const int (&rs)[3], int p,
                                             const float4& T, unsigned& mask, bool& sure)
 {
+    // The two comparisons of a slot as sign bits: d2 < c  <=>  d2 - c < 0 (the difference of two distinct floats is never -0, and
+    // x - x is +0), shifted into the masks with one funnel shift each -- an FADD (fma pipe) and an SHF instead of a compare and a
+    // predicated OR, both on the half-rate alu pipe, which this pass keeps busier than the fma pipe (profiles/r2_final.md).
+    // Slots run from the last to the first so that slot (dy, j) ends on bit kRowSlots dy + j.
     unsigned smask = 0u;
+    mask = 0u;
 #pragma unroll
-    for (int dy = 0; dy < 3; ++dy) {
+    for (int dy = 2; dy >= 0; --dy) {
 #pragma unroll
-        for (int j = 0; j < kRowSlots; ++j) {
+        for (int j = kRowSlots - 1; j >= 0; --j) {
             const float2 B = sm_xy[rs[dy] + j];
             float rx = B.x - T.x, ry = B.y - T.y;
             if (SEAM) {
@@ -107,8 +112,8 @@ __device__ __forceinline__ void broad_slots(const GridParams& g, const ShapeF& S
                 ry = min_image(B.y, T.y, g.hi[1], g.Ld[1]);
             }
             const float d2 = rx * rx + ry * ry;
-            if (d2 < S.dmax2) mask |= 1u << (kRowSlots * dy + j);                        // R16
-            if (KIND != kKindDisk && d2 < S.din2) smask |= 1u << (kRowSlots * dy + j);
+            mask = __funnelshift_l(__float_as_uint(__fsub_rn(d2, S.dmax2)), mask, 1);                               // R16
+            if (KIND != kKindDisk) smask = __funnelshift_l(__float_as_uint(__fsub_rn(d2, S.din2)), smask, 1);
         }
     }
     // the particle itself: slot p - rs[1] of the middle run, and -- when the cells between are empty, so that the slots of
