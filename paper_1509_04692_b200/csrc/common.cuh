@@ -27,6 +27,9 @@ struct GridParams {
     // layer make no trials this sweep.  nullptr = none.  Static between hpmc_set_inactive_layers calls: any kernel may read
     // it in front of its programmatic-launch wait.
     const unsigned char* inactive;
+    // the ten round keys of Philox4x32-10 for this system's seed, (k0 + r W0, k1 + r W1): operands straight from the constant
+    // bank in the tile pass instead of 18 vector adds per block (philox4x32_10_rk)
+    uint32_t philox_rk[20];
 };
 
 __device__ __forceinline__ bool layer_inactive(const GridParams& g, int layer) { return g.inactive != nullptr && g.inactive[layer] != 0; }

@@ -509,6 +509,10 @@ int hpmc_create(const hpmc_box* box, const hpmc_shape* shape, int64_t N, uint64_
     c->seed = seed;
     c->k0 = (uint32_t)seed;
     c->k1 = (uint32_t)(seed >> 32);
+    for (uint32_t r = 0; r < 10; ++r) {   // Philox round keys (philox4x32_10_rk)
+        g.philox_rk[2 * r] = c->k0 + r * kPhiloxW0;
+        g.philox_rk[2 * r + 1] = c->k1 + r * kPhiloxW1;
+    }
     c->stream = (cudaStream_t)cuda_stream;
     {
         int dev = 0, sms = 0;

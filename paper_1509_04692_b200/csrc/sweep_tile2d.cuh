@@ -313,7 +313,7 @@ __device__ __forceinline__ void tile2d_body(const GridParams& g, const MoveParam
                     const int cell = (cx0 + 2 * al) + n0 * (cy0 + 2 * ay);
                     const int lc = ryl * RW + rxl;
                     const int own_s = sm_lstart[lc], nmem = (int)sm_lstart[lc + 1] - own_s;
-                    const U4 b0 = philox4x32_10((uint32_t)cell, t_lo, (uint32_t)k, c3, k0, k1);
+                    const U4 b0 = philox4x32_10_rk((uint32_t)cell, t_lo, (uint32_t)k, c3, g.philox_rk);
                     p = own_s + (int)mulhi32(b0.x, (uint32_t)nmem);                 // R8
                     const float4 P = ld_pose(p);
                     TrialState A;
