@@ -402,7 +402,9 @@ __device__ __forceinline__ void tile2d_body(const GridParams& g, const MoveParam
                     const int gi = sm_seg_g[seg] + (p - sm_seg_l[seg]);
                     if (acc) {
                         float4 T = my_trial[slot];
-                        if (!rotate) {   // R-wrap: at most one add per axis (x + (-L) is the same fp32 operation as x - L)
+                        // R-wrap: at most one add per axis (x + (-L) is the same fp32 operation as x - L).  Only a cell on the box
+                        // edge can hold a position outside [-L/2, L/2), and its tile is a seam tile (block-uniform)
+                        if (!rotate && seam) {
                             T.x = __fadd_rn(T.x, (T.x >= g.hi[0]) ? -g.L[0] : (T.x < g.lo[0]) ? g.L[0] : 0.0f);
                             T.y = __fadd_rn(T.y, (T.y >= g.hi[1]) ? -g.L[1] : (T.y < g.lo[1]) ? g.L[1] : 0.0f);
                         }
