@@ -253,10 +253,15 @@ __device__ __forceinline__ void tile2d_body(const GridParams& g, const MoveParam
         const int* row_start = cell_start + cy * n0;
         const int g0 = sm_seg_g[2 * ry], g1 = sm_seg_g[2 * ry + 1];
         const int l0 = sm_seg_l[2 * ry], l1 = sm_seg_l[2 * ry + 1], l2 = sm_seg_l[2 * ry + 2];
-        for (int rx = lane; rx < RW; rx += 32) {
-            const bool second = rx >= split;
-            const int cx = second ? rx - split : xs + rx;
-            sm_lstart[ry * RW + rx] = (unsigned short)(row_start[cx] - (second ? g1 : g0) + (second ? l1 : l0));
+        if (split == RW) {   // block-uniform: the row does not wrap in x (every tile but those on the box edge): one segment
+            const int delta = l0 - g0;
+            for (int rx = lane; rx < RW; rx += 32) sm_lstart[ry * RW + rx] = (unsigned short)(row_start[xs + rx] + delta);
+        } else {
+            for (int rx = lane; rx < RW; rx += 32) {
+                const bool second = rx >= split;
+                const int cx = second ? rx - split : xs + rx;
+                sm_lstart[ry * RW + rx] = (unsigned short)(row_start[cx] - (second ? g1 : g0) + (second ? l1 : l0));
+            }
         }
         for (int e = lane; e < l1 - l0; e += 32) st_pose(l0 + e, FLOW ? __ldcg(&pose[g0 + e]) : pose[g0 + e]);
         for (int e = lane; e < l2 - l1; e += 32) st_pose(l1 + e, FLOW ? __ldcg(&pose[g1 + e]) : pose[g1 + e]);
