@@ -50,8 +50,10 @@ __device__ __forceinline__ U4 philox4x32_10_rk(uint32_t c0, uint32_t c1, uint32_
 {
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
-        const uint32_t hi0 = mulhi32(kPhiloxM0, c0), lo0 = kPhiloxM0 * c0;
-        const uint32_t hi1 = mulhi32(kPhiloxM1, c2), lo1 = kPhiloxM1 * c2;
+        // one 32 x 32 -> 64 bit product per multiplier (IMAD.WIDE) instead of a high and a low multiply
+        const uint64_t p0 = (uint64_t)kPhiloxM0 * (uint64_t)c0, p1 = (uint64_t)kPhiloxM1 * (uint64_t)c2;
+        const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+        const uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
         c0 = hi1 ^ c1 ^ rk[2 * r];
         c1 = lo1;
         c2 = hi0 ^ c3 ^ rk[2 * r + 1];
