@@ -194,15 +194,36 @@ __device__ __forceinline__ bool polygon_separated(const ShapeT<float>& S, float 
     const float lBx = cB * rx + sB * ry, lBy = cB * ry - sB * rx;      // R_B^T r
     const float c = cA * cB + sA * sB, s = cA * sB - sA * cB;          // R = R_A^T R_B: (x, y) -> (c x - s y, s x + c y)
     if (NV > 0 || S.regular) {
-        // the normal of A closest to l_A and the normal of B closest to -l_B
+        // the normal of A closest to l_A and the normal of B closest to -l_B (the first of equal maxima)
         float gA = -3.0e38f, nAx = 0.f, nAy = 0.f, gB = -3.0e38f, nBx = 0.f, nBy = 0.f;
+        if constexpr (NV > 0) {
+            // compile-time count: the maxima with max instructions, then the normals by equality from the last to the first --
+            // 14 operations of the half-rate alu pipe per side instead of a compare and three selects per normal (20)
+            float a[NV], b[NV];
 #pragma unroll
-        for (int k = 0; k < nv; ++k) {
-            const float a = fmaf(S.nx[k], lAx, fmaf(S.ny[k], lAy, -S.fc[k]));
-            const float b = -fmaf(S.nx[k], lBx, fmaf(S.ny[k], lBy, S.fc[k]));
-            const bool pa = a > gA, pb = b > gB;
-            gA = pa ? a : gA; nAx = pa ? S.nx[k] : nAx; nAy = pa ? S.ny[k] : nAy;
-            gB = pb ? b : gB; nBx = pb ? S.nx[k] : nBx; nBy = pb ? S.ny[k] : nBy;
+            for (int k = 0; k < NV; ++k) {
+                a[k] = fmaf(S.nx[k], lAx, fmaf(S.ny[k], lAy, -S.fc[k]));
+                b[k] = -fmaf(S.nx[k], lBx, fmaf(S.ny[k], lBy, S.fc[k]));
+                gA = fmaxf(gA, a[k]);
+                gB = fmaxf(gB, b[k]);
+            }
+            nAx = nBx = S.nx[NV - 1];
+            nAy = nBy = S.ny[NV - 1];
+#pragma unroll
+            for (int k = NV - 2; k >= 0; --k) {
+                const bool pa = a[k] == gA, pb = b[k] == gB;
+                nAx = pa ? S.nx[k] : nAx; nAy = pa ? S.ny[k] : nAy;
+                nBx = pb ? S.nx[k] : nBx; nBy = pb ? S.ny[k] : nBy;
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < nv; ++k) {
+                const float a = fmaf(S.nx[k], lAx, fmaf(S.ny[k], lAy, -S.fc[k]));
+                const float b = -fmaf(S.nx[k], lBx, fmaf(S.ny[k], lBy, S.fc[k]));
+                const bool pa = a > gA, pb = b > gB;
+                gA = pa ? a : gA; nAx = pa ? S.nx[k] : nAx; nAy = pa ? S.ny[k] : nAy;
+                gB = pb ? b : gB; nBx = pb ? S.nx[k] : nBx; nBy = pb ? S.ny[k] : nBy;
+            }
         }
         const float uAx = -(c * nAx + s * nAy), uAy = s * nAx - c * nAy;     // -R^T n_A, in B's frame
         const float uBx = s * nBy - c * nBx, uBy = -(s * nBx + c * nBy);     // -R n_B, in A's frame

@@ -469,21 +469,29 @@ k_sweep_tile2d_flow(const __grid_constant__ GridParams g, const __grid_constant_
     using TL = Tile2D<WARPS, R>;
     pdl_wait();   // no early launch of the successor: this persistent grid fills every SM
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ int s_ticket;
-    const int nax = g.n[0] >> 1, nay = g.n[1] >> 1;
-    const int tiles_x = (nax + kTileW - 1) / kTileW, tiles_y = (nay + TL::TH - 1) / TL::TH;
-    const int ntiles = tiles_x * tiles_y;
-    // stamp of this sweep: 1 + (t mod (2^32 - 1)).  Never 0 (the cleared state), and different from the stamp of the sweep
-    // before, which is what every entry holds when the sweep starts -- also across the 2^32 wrap of the counter
-    const unsigned stamp = (unsigned)((((unsigned long long)ctrl->hdr.t_hi16 << 32) | ctrl->hdr.t_lo) % 0xFFFFFFFFull) + 1u;
+    // launch constants live in shared memory, not in registers across the tile body (64 registers: every one counts there)
+    __shared__ int s_ticket, s_ntiles, s_tiles_x, s_tiles_y;
+    __shared__ unsigned s_stamp;
     volatile unsigned int* vdone = done;
-    if (threadIdx.x == 0) s_ticket = (int)atomicAdd(&ctrl->flow_ticket, 1u);
+    if (threadIdx.x == 0) {
+        const int nax = g.n[0] >> 1, nay = g.n[1] >> 1;
+        s_tiles_x = (nax + kTileW - 1) / kTileW;
+        s_tiles_y = (nay + TL::TH - 1) / TL::TH;
+        s_ntiles = s_tiles_x * s_tiles_y;
+        // stamp of this sweep: 1 + (t mod (2^32 - 1)).  Never 0 (the cleared state), and different from the stamp of the sweep
+        // before, which is what every entry holds when the sweep starts -- also across the 2^32 wrap of the counter
+        s_stamp = (unsigned)((((unsigned long long)ctrl->hdr.t_hi16 << 32) | ctrl->hdr.t_lo) % 0xFFFFFFFFull) + 1u;
+        s_ticket = (int)atomicAdd(&ctrl->flow_ticket, 1u);
+    }
     __syncthreads();
     for (;;) {
         const int ticket = s_ticket;                       // written before the barrier that ends the previous iteration
+        const int ntiles = s_ntiles;
         if (ticket >= 4 * ntiles) break;
         const int ci = ticket / ntiles, tile = ticket - ci * ntiles;
         if (ci > 0 && threadIdx.x < 9) {                   // the nine tiles of the previous colour around this one
+            const int tiles_x = s_tiles_x, tiles_y = s_tiles_y;
+            const unsigned stamp = s_stamp;
             const int tx = tile % tiles_x, ty = tile / tiles_x;
             int nx = tx + (int)(threadIdx.x % 3) - 1, ny = ty + (int)(threadIdx.x / 3) - 1;
             nx += (nx < 0) ? tiles_x : 0; nx -= (nx >= tiles_x) ? tiles_x : 0;
@@ -502,7 +510,7 @@ k_sweep_tile2d_flow(const __grid_constant__ GridParams g, const __grid_constant_
         __threadfence();                                   // this thread's pose write-backs are visible device-wide ...
         __syncthreads();                                   // ... and the tile's shared memory is no longer in use
         if (threadIdx.x == 0) {
-            vdone[ci * ntiles + tile] = stamp;             // ... before the tile is announced
+            vdone[ticket] = s_stamp;                       // ... before the tile is announced (ticket = ci * ntiles + tile)
             s_ticket = (int)atomicAdd(&ctrl->flow_ticket, 1u);
         }
         __syncthreads();
