@@ -874,8 +874,10 @@ int hpmc_sweep_host_pose2d(hpmc_ctx* c, const float* h_pose4, int64_t n, float* 
     const size_t bytes = (size_t)N * sizeof(float4);
     if (!cuda_ok(c, cudaMemsetAsync(&c->ctrl->bad_coords, 0, sizeof(unsigned int), c->stream), "sweep_host_pose2d/memset")) return HPMC_E_CUDA;
     if (!cuda_ok(c, cudaMemcpyAsync(c->d_pos_bound, h_pose4, bytes, cudaMemcpyHostToDevice, c->stream), "sweep_host_pose2d/h2d")) return HPMC_E_CUDA;
-    if (N > 0) k_pose_expand<<<(N + TB - 1) / TB, TB, 0, c->stream>>>(N, (float4*)c->d_pos_bound, (float4*)c->d_quat_bound);
-    c->launches += 1;
+    if (N > 0) {
+        k_pose_expand<<<(N + TB - 1) / TB, TB, 0, c->stream>>>(N, (float4*)c->d_pos_bound, (float4*)c->d_quat_bound);
+        LAUNCH_CHECK(c, "k_pose_expand");
+    }
     c->state_in_bound = true;
     c->have_sorted = false;
     c->dist = false;
@@ -884,13 +886,13 @@ int hpmc_sweep_host_pose2d(hpmc_ctx* c, const float* h_pose4, int64_t n, float* 
     if (rc != HPMC_OK) return rc;
     rc = hpmc_get_state(c, (float*)c->d_pos_bound, (float*)c->d_quat_bound, nullptr, nullptr);
     if (rc != HPMC_OK) return rc;
-    if (h_pose4_out) {
-        if (N > 0) k_pose_pack<<<(N + TB - 1) / TB, TB, 0, c->stream>>>(N, (float4*)c->d_pos_bound, (const float4*)c->d_quat_bound);
-        c->launches += 1;
+    if (h_pose4_out && N > 0) {
+        k_pose_pack<<<(N + TB - 1) / TB, TB, 0, c->stream>>>(N, (float4*)c->d_pos_bound, (const float4*)c->d_quat_bound);
+        LAUNCH_CHECK(c, "k_pose_pack");
         if (!cuda_ok(c, cudaMemcpyAsync(h_pose4_out, c->d_pos_bound, bytes, cudaMemcpyDeviceToHost, c->stream), "sweep_host_pose2d/d2h")) return HPMC_E_CUDA;
         // the bound arrays are the caller's: leave them in the documented pos4 / quat4 layout
-        if (N > 0) k_pose_expand<<<(N + TB - 1) / TB, TB, 0, c->stream>>>(N, (float4*)c->d_pos_bound, (float4*)c->d_quat_bound);
-        c->launches += 1;
+        k_pose_expand<<<(N + TB - 1) / TB, TB, 0, c->stream>>>(N, (float4*)c->d_pos_bound, (float4*)c->d_quat_bound);
+        LAUNCH_CHECK(c, "k_pose_expand");
     }
     hpmc_counters tmp;
     rc = hpmc_get_state(c, nullptr, nullptr, h_counters ? h_counters : &tmp, nullptr);  // also synchronises
