@@ -66,7 +66,7 @@ def algo_flops_per_trial(k, w):
 
 # ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per colour pass of the dominant kernel, round-2 kernels
 # (profiles/r2_final.md lists the captures; a dataflow / whole-sweep launch is divided by the passes it covers)
-NCU_TRAFFIC = {"k2_pentagons_1M": 21.06e6 / 4, "k4_pentagons_16M": 425.0e6, "k3_cubes": 1.92e6, "k1_pentagons_4096": 0.13e6,
+NCU_TRAFFIC = {"k2_pentagons_1M": 21.34e6 / 4, "k4_pentagons_16M": 425.0e6, "k3_cubes": 1.20e6, "k1_pentagons_4096": 0.13e6,
                "k0_disks": 0.12e6}
 
 
